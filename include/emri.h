@@ -1,0 +1,174 @@
+/* emri.h -- C ABI of the B200-native (sm_100a) hot path of EMRI_MC (arXiv 2311.17174).
+ *
+ * The library evaluates, for a whole MCMC ensemble of K walkers at once (PAPER.md:57, :122, :146:
+ * "a matrix (n_walkers x n_dim) ... computed in a vectorised manner"), the Analytic-Kludge EMRI
+ * waveform (Eqs. 1-2), its projection on the two LISA channels,
+ * the modified-gravity propagation factors (Eqs. 4-6), its discrete Fourier
+ * transform and the noise-weighted Gaussian log-likelihood (PAPER.md:112-116,
+ * Eq. 8).  The equations the paper defers to Barack & Cutler 2004 and Peters & Mathews 1963 are
+ * restated in DESIGN.md section 3.
+ *
+ * Conventions
+ *  - "DEV" pointers are CUDA device pointers on the plan's device, "HOST" pointers are host memory.
+ *    The caller owns every pointer it passes; the plan owns its workspace.
+ *  - Every call that takes `cuda_stream` (a cudaStream_t passed as void*; NULL = legacy default
+ *    stream) only ENQUEUES work on that stream and returns; it never synchronises.  Results are
+ *    valid after the stream reaches the end of the enqueued work.  The *_host variants copy with
+ *    cudaMemcpyAsync on the same stream and DO synchronise the stream before returning.
+ *  - One plan must not be used from two streams concurrently (the workspace is shared).
+ *  - All functions return EMRI_OK (0) or a negative error code; they never throw or exit.
+ *
+ * Parameter row, P = EMRI_NPAR = 17 doubles per walker, row-major params[K][17]
+ * (first three are M, mu, S/M^2 as PAPER.md:149 prescribes):
+ *    0 M      central mass, detector frame [Msun]     9  theta_S  source colatitude [rad]
+ *    1 mu     small mass [Msun]                       10 phi_S    source azimuth    [rad]
+ *    2 a      spin S/M^2, |a| <= 1                    11 theta_K  spin colatitude   [rad]
+ *    3 e0     eccentricity at t = 0, [0,1)            12 phi_K    spin azimuth      [rad]
+ *    4 nu0    orbital frequency at t = 0 [Hz]         13 D_L      EM luminosity distance [Gpc]
+ *    5 Phi0   mean anomaly at t = 0 [rad]             14 Xi0      Eq. 6
+ *    6 gam0   gamma~ at t = 0 [rad]                   15 n_Xi     Eq. 6
+ *    7 alp0   alpha at t = 0 [rad]                    16 delta_T  c_T - 1 (GW speed excess)
+ *    8 lambda angle between L and S [rad]
+ *
+ * Per-walker status bits (not errors; written to `status[K]` when it is not NULL):
+ *    1 EMRI_ST_BADPARAM  non-finite or out-of-domain parameter (M, mu, D_L, nu0 <= 0, e0 not in
+ *                        [0,1), |a| > 1, Xi(z) <= 0)
+ *    2 EMRI_ST_PLUNGE    nu reached nu_LSO(e) inside the window; the waveform is
+ *                        zero from the first plunged coarse node on; logL uses the truncated wave
+ *    4 EMRI_ST_DELAY     |Delta T| exceeds one coarse interval (the guard)
+ *    8 EMRI_ST_STATE     e left [0,1) or the state became non-finite during the integration
+ * For bits 1, 4, 8 the waveform rows are zero and logL = -inf.
+ */
+#ifndef EMRI_H
+#define EMRI_H
+
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+#define EMRI_NPAR 17
+#define EMRI_NMAX_CAP 48 /* largest n_max a plan accepts */
+
+enum {
+  EMRI_OK = 0,
+  EMRI_EINVAL = -1, /* bad argument (NULL pointer, K > K_max, N odd or < 4, n_max out of range ...) */
+  EMRI_ENOMEM = -2, /* host or device allocation failed */
+  EMRI_ECUDA = -3,  /* a CUDA runtime call failed; see emri_plan_last_cuda_error */
+  EMRI_ECUFFT = -4  /* a cuFFT call failed; see emri_plan_last_cuda_error */
+};
+
+enum { EMRI_ST_BADPARAM = 1, EMRI_ST_PLUNGE = 2, EMRI_ST_DELAY = 4, EMRI_ST_STATE = 8 };
+
+typedef struct emri_plan emri_plan;
+
+/* Static description of an error code. */
+const char* emri_strerror(int code);
+
+/* Create a plan for N samples at spacing dt [s], harmonics n = 1..n_max (Eq. 2), at
+ * most K_max walkers per call.  psd: HOST, N/2+1 values of the one-sided noise PSD S_n(f_m) [1/Hz]
+ * at f_m = m/(N dt) (Eq. 8's S_noise); entries that are <= 0, NaN or +inf mask
+ * their bin (weight 0); pass +inf at m = 0 and m = N/2 to exclude DC and Nyquist.  psd may be NULL
+ * (all weights 0; only emri_waveform / emri_data_fft are then meaningful).
+ * Requirements: N even, N >= 4; dt > 0; 1 <= n_max <= EMRI_NMAX_CAP; K_max >= 1.
+ * Uses the current CUDA device; synchronises it.  Defaults: flat LambdaCDM H0 = 67.4 km/s/Mpc,
+ * Omega_m = 0.315 (the paper's dL() leaves the cosmology open); coarse stride
+ * S = 256 samples. */
+int emri_plan_create(emri_plan** out, int64_t N, double dt, int n_max, int K_max, const double* psd);
+
+/* Free everything the plan owns (synchronises the device). */
+int emri_plan_destroy(emri_plan* p);
+
+/* Background cosmology behind z(D_L) and the look-back time. */
+int emri_plan_set_cosmology(emri_plan* p, double H0_km_s_Mpc, double Omega_m);
+
+/* Coarse-grid stride S in samples (power of two, 2 <= S <= 65536): the RK4 step of the orbital
+ * ODEs (Eq. 1) is S*dt.  Reallocates the orbit workspace; synchronises. */
+int emri_plan_set_coarse_stride(emri_plan* p, int S);
+
+/* Number of walkers processed per internal chunk (bounds the workspace: 2*chunk*(N+2) doubles
+ * plus the cuFFT work area).  Default min(K_max, 128).  Reallocates; synchronises. */
+int emri_plan_set_chunk(emri_plan* p, int walkers_per_chunk);
+
+/* Stage (a): coarse orbit of Eq. 1 by fixed-step RK4 (S3).
+ * params: DEV [K][17].  nodes: DEV, K * n_nodes * 16 doubles, n_nodes = ceil(N/S) + 3 (node j at
+ * row j+1, j = -1 .. ceil(N/S)+1); each node row is
+ *   {Phi_c, nu, gam_c, e, alp_c,  d/dt of those five,  increment of those five over [j, j+1], 0}
+ * with the three angles in cycles wrapped to [0,1) and their increments unwrapped.
+ * status: DEV [K] or NULL.  Mainly for stage-wise parity tests. */
+int emri_orbit(emri_plan* p, const double* params, int K, double* nodes, int32_t* status,
+               void* cuda_stream);
+int64_t emri_plan_num_nodes(const emri_plan* p);
+
+/* Stages (a)+(b): observed strain of both LISA channels, h_alpha(t_i), i = 0..N-1, t_i = i dt
+ * (Eq. 2 with the response of PAPER.md:79/:118 and the factors of Eqs. 4-6 folded in).
+ * params: DEV [K][17]; h_I, h_II: DEV [K][N] each (row k = walker k); status: DEV [K] or NULL. */
+int emri_waveform(emri_plan* p, const double* params, int K, double* h_I, double* h_II,
+                  int32_t* status, void* cuda_stream);
+
+/* Stages (a)+(b)+(c): un-normalised forward DFT  H[m] = sum_i h[i] exp(-2 pi i i m / N),
+ * m = 0..N/2.  spectra: DEV [K][2][N/2+1] complex128 (re, im interleaved),
+ * channel I then II.  For stage-wise parity tests and for building data. */
+int emri_waveform_fft(emri_plan* p, const double* params, int K, double* spectra, int32_t* status,
+                      void* cuda_stream);
+
+/* Transform a measured / mock time series of both channels into the `data_fft` argument of
+ * emri_loglike (the paper's h[theta_0](f)).  d_I, d_II: DEV [N] each;
+ * data_fft: DEV [2][N/2+1] complex128, same convention as emri_waveform_fft. */
+int emri_data_fft(emri_plan* p, const double* d_I, const double* d_II, double* data_fft,
+                  void* cuda_stream);
+
+/* Stages (a)..(d): Gaussian log-likelihood of Eq. 8 for every walker,
+ *   logL[k] = -(1/2) <d - h_k | d - h_k> = -(2 dt / N) sum_{chan} sum_m |D[m] - H_k[m]|^2 / S_n(f_m)
+ * over the unmasked bins.  params: DEV [K][17], K <= K_max; data_fft: DEV [2][N/2+1] complex128;
+ * logL: DEV [K]; status: DEV [K] or NULL. */
+int emri_loglike(emri_plan* p, const double* params, int K, const double* data_fft, double* logL,
+                 int32_t* status, void* cuda_stream);
+
+/* Same as emri_loglike with HOST buffers: copies params (and data_fft, unless it is NULL, in which
+ * case the data uploaded by the previous non-NULL call is reused) to the device, runs the path,
+ * copies logL and status back and synchronises the stream.  This is the end-to-end entry point
+ * bench.py times as "e2e". */
+int emri_loglike_host(emri_plan* p, const double* params, int K, const double* data_fft,
+                      double* logL, int32_t* status, void* cuda_stream);
+
+/* Device milliseconds of stages (a) orbit, (b) synthesis, (c) cuFFT, (d) likelihood reduction of
+ * the last emri_loglike / emri_waveform(_fft) call, summed over chunks.  Timing events are only
+ * recorded after emri_plan_enable_timings(p, 1).  Synchronises on the recorded events. */
+int emri_plan_enable_timings(emri_plan* p, int on);
+int emri_plan_get_timings(emri_plan* p, double ms[4]);
+
+/* Raw cudaError_t / cufftResult of the last failing CUDA / cuFFT call on this plan (0 if none). */
+int emri_plan_last_cuda_error(const emri_plan* p);
+
+/* Bytes of device memory the plan currently owns. */
+int64_t emri_plan_workspace_bytes(const emri_plan* p);
+
+/* ---- ensemble sampler step (BASELINE.json configs[4]; emcee's affine-invariant
+ * stretch move [Goodman & Weare], run on the device so that parameters and logL never visit the
+ * host).  Walkers are split in two fixed halves; `emri_stretch_step` updates half `half` (0 or 1)
+ * given the other:  for walker k in the active half, partner j uniform in the other half,
+ * z = ((a-1) u + 1)^2 / a, Y = X_j + z (X_k - X_j), accept iff
+ * ln u' < (P_free - 1) ln z + lnp(Y) - lnp(X_k), lnp = logL + uniform box prior.
+ * Random numbers: Philox4x32-10 keyed by `seed`, counter (step, half, walker).
+ *   X: DEV [K][17] in/out; logL: DEV [K] in/out (must hold logL of X on entry; use
+ *   emri_loglike first); lo, hi: DEV [17] box prior (a column with lo == hi is held fixed and
+ *   does not count in P_free); accepted: DEV int32 [K] or NULL, set to 1/0 for the active half;
+ *   log_buf: DEV [K/2][EMRI_NPAR+4] doubles or NULL: per active walker {proposal[17], z, ln u',
+ *   logL(Y), partner} for the teacher-forced parity protocol. K must be even, K/2 <= K_max. */
+int emri_stretch_step(emri_plan* p, double* X, double* logL, int K, const double* data_fft,
+                      const double* lo, const double* hi, double a_stretch, uint64_t seed,
+                      int64_t step, int half, int32_t* accepted, double* log_buf,
+                      void* cuda_stream);
+
+/* ---- measurement helpers (bench.py): peak probes on the current device.
+ * emri_probe_fp64_peak: runs a dependent-chain-free DFMA kernel and returns TFLOP/s (FMA = 2).
+ * emri_probe_hbm_read: streams `bytes` of device memory once and returns GB/s. */
+int emri_probe_fp64_peak(double* tflops, void* cuda_stream);
+int emri_probe_hbm_read(int64_t bytes, double* gbs, void* cuda_stream);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* EMRI_H */

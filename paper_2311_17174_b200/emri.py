@@ -1,0 +1,245 @@
+"""Thin ctypes binding of include/emri.h -- argument marshalling only.
+
+Every step of the path runs in the CUDA library (csrc/emri.cu).  PyTorch supplies device memory
+(`tensor.data_ptr()`) and the stream (`torch.cuda.current_stream()`); nothing is computed here and
+there is no CPU fallback: `load()` raises if libemri_b200.so is missing or does not load.
+"""
+import ctypes as C
+import os
+
+import numpy as np
+
+NPAR = 17
+NODE_STRIDE = 16
+ST_BADPARAM, ST_PLUNGE, ST_DELAY, ST_STATE = 1, 2, 4, 8
+_LIB_PATH = os.path.join(os.path.dirname(os.path.abspath(__file__)), "libemri_b200.so")
+_lib = None
+
+EXPORTS = (
+    "emri_strerror", "emri_plan_create", "emri_plan_destroy", "emri_plan_set_cosmology",
+    "emri_plan_set_coarse_stride", "emri_plan_set_chunk", "emri_orbit", "emri_plan_num_nodes", "emri_waveform",
+    "emri_waveform_fft", "emri_data_fft", "emri_loglike", "emri_loglike_host", "emri_plan_enable_timings",
+    "emri_plan_get_timings", "emri_plan_last_cuda_error", "emri_plan_workspace_bytes", "emri_stretch_step",
+    "emri_probe_fp64_peak", "emri_probe_hbm_read",
+)
+
+
+class EmriError(RuntimeError):
+    pass
+
+
+def load():
+    """dlopen libemri_b200.so and declare the prototypes of include/emri.h.  Fails loudly."""
+    global _lib
+    if _lib is not None:
+        return _lib
+    if not os.path.exists(_LIB_PATH):
+        raise EmriError(f"{_LIB_PATH} is missing: build it with `python -m paper_2311_17174_b200.build` "
+                        "(there is no CPU fallback)")
+    L = C.CDLL(_LIB_PATH)
+    vp, i32, i64, dbl, u64 = C.c_void_p, C.c_int, C.c_int64, C.c_double, C.c_uint64
+    L.emri_strerror.restype = C.c_char_p
+    L.emri_strerror.argtypes = [i32]
+    L.emri_plan_create.argtypes = [C.POINTER(vp), i64, dbl, i32, i32, vp]
+    L.emri_plan_destroy.argtypes = [vp]
+    L.emri_plan_set_cosmology.argtypes = [vp, dbl, dbl]
+    L.emri_plan_set_coarse_stride.argtypes = [vp, i32]
+    L.emri_plan_set_chunk.argtypes = [vp, i32]
+    L.emri_orbit.argtypes = [vp, vp, i32, vp, vp, vp]
+    L.emri_plan_num_nodes.restype = i64
+    L.emri_plan_num_nodes.argtypes = [vp]
+    L.emri_waveform.argtypes = [vp, vp, i32, vp, vp, vp, vp]
+    L.emri_waveform_fft.argtypes = [vp, vp, i32, vp, vp, vp]
+    L.emri_data_fft.argtypes = [vp, vp, vp, vp, vp]
+    L.emri_loglike.argtypes = [vp, vp, i32, vp, vp, vp, vp]
+    L.emri_loglike_host.argtypes = [vp, vp, i32, vp, vp, vp, vp]
+    L.emri_plan_enable_timings.argtypes = [vp, i32]
+    L.emri_plan_get_timings.argtypes = [vp, C.POINTER(dbl)]
+    L.emri_plan_last_cuda_error.argtypes = [vp]
+    L.emri_plan_workspace_bytes.restype = i64
+    L.emri_plan_workspace_bytes.argtypes = [vp]
+    L.emri_stretch_step.argtypes = [vp, vp, vp, i32, vp, vp, vp, dbl, u64, i64, i32, vp, vp, vp]
+    L.emri_probe_fp64_peak.argtypes = [C.POINTER(dbl), vp]
+    L.emri_probe_hbm_read.argtypes = [i64, C.POINTER(dbl), vp]
+    for name in EXPORTS:
+        if name not in ("emri_strerror", "emri_plan_num_nodes", "emri_plan_workspace_bytes"):
+            getattr(L, name).restype = i32
+    _lib = L
+    return L
+
+
+def _stream():
+    import torch
+    return C.c_void_p(torch.cuda.current_stream().cuda_stream)
+
+
+def _ptr(t, dtype=None, shape=None):
+    """device pointer of a contiguous CUDA tensor (None -> NULL)"""
+    if t is None:
+        return None
+    import torch
+    if not (isinstance(t, torch.Tensor) and t.is_cuda and t.is_contiguous()):
+        raise TypeError("expected a contiguous CUDA tensor")
+    if dtype is not None and t.dtype != dtype:
+        raise TypeError(f"expected dtype {dtype}, got {t.dtype}")
+    if shape is not None and tuple(t.shape) != tuple(shape):
+        raise TypeError(f"expected shape {tuple(shape)}, got {tuple(t.shape)}")
+    return C.c_void_p(t.data_ptr())
+
+
+def probe_fp64_peak():
+    """TFLOP/s of a chain-free DFMA kernel on the current device (roofline denominator of stage b)."""
+    v = C.c_double()
+    rc = load().emri_probe_fp64_peak(C.byref(v), _stream())
+    if rc:
+        raise EmriError(f"fp64 probe failed ({rc})")
+    return v.value
+
+
+def probe_hbm_read(nbytes=4 << 30):
+    """GB/s of a streaming read of `nbytes` of device memory."""
+    v = C.c_double()
+    rc = load().emri_probe_hbm_read(int(nbytes), C.byref(v), _stream())
+    if rc:
+        raise EmriError(f"hbm probe failed ({rc})")
+    return v.value
+
+
+class Plan:
+    """emri_plan_create(N, dt, n_max, K_max, psd) and the calls that use it (include/emri.h)."""
+
+    def __init__(self, N, dt, n_max, K_max, psd=None):
+        self._L = load()
+        self._h = C.c_void_p()
+        self.N, self.dt, self.n_max, self.K_max = int(N), float(dt), int(n_max), int(K_max)
+        self.Nf = self.N // 2 + 1
+        if psd is not None:
+            psd = np.ascontiguousarray(psd, dtype=np.float64)
+            if psd.shape != (self.Nf,):
+                raise ValueError("psd must have N/2+1 entries")
+        self._check(self._L.emri_plan_create(C.byref(self._h), self.N, self.dt, self.n_max, self.K_max,
+                                              psd.ctypes.data_as(C.c_void_p) if psd is not None else None))
+
+    def _check(self, rc):
+        if rc != 0:
+            raw = self._L.emri_plan_last_cuda_error(self._h) if self._h else 0
+            raise EmriError(f"{self._L.emri_strerror(rc).decode()} (code {rc}, raw {raw})")
+
+    def close(self):
+        if getattr(self, "_h", None):
+            self._L.emri_plan_destroy(self._h)
+            self._h = C.c_void_p()
+
+    def __del__(self):
+        try:
+            self.close()
+        except Exception:
+            pass
+
+    # ---- settings
+    def set_cosmology(self, H0, Om):
+        self._check(self._L.emri_plan_set_cosmology(self._h, H0, Om))
+
+    def set_coarse_stride(self, S):
+        self._check(self._L.emri_plan_set_coarse_stride(self._h, S))
+
+    def set_chunk(self, c):
+        self._check(self._L.emri_plan_set_chunk(self._h, c))
+
+    def num_nodes(self):
+        return int(self._L.emri_plan_num_nodes(self._h))
+
+    def workspace_bytes(self):
+        return int(self._L.emri_plan_workspace_bytes(self._h))
+
+    def enable_timings(self, on=True):
+        self._check(self._L.emri_plan_enable_timings(self._h, 1 if on else 0))
+
+    def timings(self):
+        ms = (C.c_double * 4)()
+        self._check(self._L.emri_plan_get_timings(self._h, ms))
+        return dict(orbit=ms[0], synth=ms[1], fft=ms[2], like=ms[3])
+
+    # ---- the path (device tensors; results are valid once the current stream has caught up)
+    def orbit(self, params, nodes=None, status=None):
+        import torch
+        K = params.shape[0]
+        if nodes is None:
+            nodes = torch.empty((K, self.num_nodes(), NODE_STRIDE), dtype=torch.float64, device=params.device)
+        self._check(self._L.emri_orbit(self._h, _ptr(params, torch.float64, (K, NPAR)), K,
+                                       _ptr(nodes, torch.float64, (K, self.num_nodes(), NODE_STRIDE)),
+                                       _ptr(status, torch.int32, (K,)), _stream()))
+        return nodes
+
+    def waveform(self, params, h_I=None, h_II=None, status=None):
+        import torch
+        K = params.shape[0]
+        if h_I is None:
+            h_I = torch.empty((K, self.N), dtype=torch.float64, device=params.device)
+        if h_II is None:
+            h_II = torch.empty((K, self.N), dtype=torch.float64, device=params.device)
+        self._check(self._L.emri_waveform(self._h, _ptr(params, torch.float64, (K, NPAR)), K,
+                                          _ptr(h_I, torch.float64, (K, self.N)), _ptr(h_II, torch.float64, (K, self.N)),
+                                          _ptr(status, torch.int32, (K,)), _stream()))
+        return h_I, h_II
+
+    def waveform_fft(self, params, spectra=None, status=None):
+        import torch
+        K = params.shape[0]
+        if spectra is None:
+            spectra = torch.empty((K, 2, self.Nf), dtype=torch.complex128, device=params.device)
+        self._check(self._L.emri_waveform_fft(self._h, _ptr(params, torch.float64, (K, NPAR)), K,
+                                              _ptr(spectra, torch.complex128, (K, 2, self.Nf)),
+                                              _ptr(status, torch.int32, (K,)), _stream()))
+        return spectra
+
+    def data_fft(self, d_I, d_II, out=None):
+        import torch
+        if out is None:
+            out = torch.empty((2, self.Nf), dtype=torch.complex128, device=d_I.device)
+        self._check(self._L.emri_data_fft(self._h, _ptr(d_I, torch.float64, (self.N,)),
+                                          _ptr(d_II, torch.float64, (self.N,)),
+                                          _ptr(out, torch.complex128, (2, self.Nf)), _stream()))
+        return out
+
+    def loglike(self, params, data_fft, logL=None, status=None):
+        import torch
+        K = params.shape[0]
+        if logL is None:
+            logL = torch.empty((K,), dtype=torch.float64, device=params.device)
+        self._check(self._L.emri_loglike(self._h, _ptr(params, torch.float64, (K, NPAR)), K,
+                                         _ptr(data_fft, torch.complex128, (2, self.Nf)),
+                                         _ptr(logL, torch.float64, (K,)), _ptr(status, torch.int32, (K,)), _stream()))
+        return logL
+
+    def loglike_host(self, params, data_fft=None, logL=None, status=None):
+        """HOST numpy arrays in and out (pinned or pageable); synchronises.  data_fft=None reuses the
+        spectrum uploaded by the previous call."""
+        params = np.ascontiguousarray(params, dtype=np.float64)
+        K = params.shape[0]
+        if data_fft is not None:
+            data_fft = np.ascontiguousarray(data_fft, dtype=np.complex128)
+            if data_fft.shape != (2, self.Nf):
+                raise ValueError("data_fft must be complex [2][N/2+1]")
+        logL = np.empty(K) if logL is None else logL
+        self._check(self._L.emri_loglike_host(
+            self._h, params.ctypes.data_as(C.c_void_p), K,
+            data_fft.ctypes.data_as(C.c_void_p) if data_fft is not None else None,
+            logL.ctypes.data_as(C.c_void_p),
+            status.ctypes.data_as(C.c_void_p) if status is not None else None, _stream()))
+        return logL
+
+    def loglike_host_ptr(self, params_ptr, K, data_ptr, logL_ptr, status_ptr=None):
+        """same, with raw host addresses (pinned torch tensors' data_ptr())"""
+        self._check(self._L.emri_loglike_host(
+            self._h, C.c_void_p(params_ptr), K, C.c_void_p(data_ptr) if data_ptr else None,
+            C.c_void_p(logL_ptr), C.c_void_p(status_ptr) if status_ptr else None, _stream()))
+
+    def stretch_step(self, X, logL, data_fft, lo, hi, a, seed, step, half, accepted=None, log_buf=None):
+        import torch
+        K = X.shape[0]
+        self._check(self._L.emri_stretch_step(
+            self._h, _ptr(X, torch.float64, (K, NPAR)), _ptr(logL, torch.float64, (K,)), K,
+            _ptr(data_fft, torch.complex128, (2, self.Nf)), _ptr(lo, torch.float64, (NPAR,)),
+            _ptr(hi, torch.float64, (NPAR,)), float(a), int(seed), int(step), int(half),
+            _ptr(accepted, torch.int32, (K,)), _ptr(log_buf, torch.float64, (K // 2, NPAR + 4)), _stream()))
