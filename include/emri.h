@@ -87,6 +87,19 @@ int emri_plan_set_cosmology(emri_plan* p, double H0_km_s_Mpc, double Omega_m);
  * ODEs (Eq. 1) is S*dt.  Reallocates the orbit workspace; synchronises. */
 int emri_plan_set_coarse_stride(emri_plan* p, int S);
 
+/* How stage (a) is scheduled on the device.  1 (default): parallel in time -- multiple shooting
+ * over segments of the coarse grid with a Newton correction and verification, which reproduces the
+ * sequential RK4 recursion to ~1e-18 relative in (nu, e).  0: the plain
+ * sequential recursion, one thread per walker (latency-bound; kept as the in-library reference of
+ * the schedule and used by the tests).  Both evaluate the same scheme (S3). */
+int emri_plan_set_orbit_schedule(emri_plan* p, int schedule);
+
+/* Diagnostics of the last parallel-in-time orbit evaluation: modes[k] (HOST int32 [K]) is 1 if
+ * walker k's segments were all verified after a Newton round, 2 if a sequential tail was needed
+ * from the first unverified boundary, 3 if its node rows are zero (invalid parameters, plunge at
+ * t = 0, bad guard step).  Synchronises the device. */
+int emri_plan_orbit_report(emri_plan* p, int K, int32_t* modes);
+
 /* Number of walkers processed per internal chunk (bounds the workspace: 2*chunk*(N+2) doubles
  * plus the cuFFT work area).  Default min(K_max, 128).  Reallocates; synchronises. */
 int emri_plan_set_chunk(emri_plan* p, int walkers_per_chunk);

@@ -7,6 +7,7 @@ import sys
 HERE = os.path.dirname(os.path.abspath(__file__))
 SRC = os.path.join(HERE, "csrc", "emri.cu")
 HDR = os.path.join(os.path.dirname(HERE), "include", "emri.h")
+CSRC = os.path.join(HERE, "csrc")
 LIB = os.path.join(HERE, "libemri_b200.so")
 NVCC_FLAGS = ["-O3", "-std=c++17", "-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo",
               "-Xcompiler", "-fPIC", "-shared", "-diag-suppress", "550"]
@@ -23,7 +24,8 @@ def stale():
     if not os.path.exists(LIB):
         return True
     t = os.path.getmtime(LIB)
-    return any(os.path.getmtime(f) > t for f in (SRC, HDR))
+    deps = [HDR] + [os.path.join(CSRC, f) for f in os.listdir(CSRC) if f.endswith((".cu", ".cuh"))]
+    return any(os.path.getmtime(f) > t for f in deps)
 
 
 def build(force=False, verbose=False):

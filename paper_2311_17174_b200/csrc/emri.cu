@@ -16,6 +16,7 @@
 #include <cmath>
 #include <cstdint>
 #include <cstdio>
+#include <cstdlib>
 #include <cstring>
 #include <map>
 #include <new>
@@ -23,757 +24,12 @@
 
 #include "../../include/emri.h"
 
-namespace {
-
-// ------------------------------------------------------------------ constants (S0)
-constexpr double kPi = 3.14159265358979323846;
-constexpr double kTwoPi = 6.28318530717958647692;
-constexpr double kMsunSec = 4.925490947e-6;
-constexpr double kGpcSec = 1.0292712503e17;
-constexpr double kAuSec = 499.004783836;
-constexpr double kYearSec = 31557600.0;
-constexpr double kMpcMetre = 3.0856775814913673e22;
-constexpr double kSqrt3 = 1.7320508075688772935;
-constexpr double kHalfSqrt3 = 0.86602540378443864676;
-
-constexpr int NODE_STRIDE = 16;   // doubles per coarse node: 5 values, 5 slopes, 5 increments, 1 spare
-constexpr int WC_STRIDE = 48;     // doubles of per-walker constants
-constexpr int MCAP = 48;          // largest number of Bessel series terms kept per (n, order)
-constexpr int NCOEF = 12;         // per-harmonic constants
-constexpr int SYNTH_THREADS = 128;
-constexpr int TILE = 2 * SYNTH_THREADS;   // samples per tile (2 per thread)
-constexpr int LL_THREADS = 256;
-constexpr int LL_BINS_PER_THREAD = 4;
-constexpr int LL_TILE = LL_THREADS * LL_BINS_PER_THREAD;
-constexpr int LL_WARPS = LL_THREADS / 32;
-
-// per-walker constant block
-enum {
-  WC_TWOPIMS = 0, WC_CNU, WC_CE, WC_A, WC_SP, WC_AMP, WC_DT, WC_SIGMA, WC_DOP,
-  WC_CPHS, WC_SPHS, WC_CS, WC_SS, WC_LN0, WC_LN1, WC_LN2, WC_CL, WC_SN, WC_B1, WC_B2,
-  WC_A0X, WC_A0Y, WC_A0Z, WC_A1X, WC_A1Y, WC_A1Z, WC_A2X, WC_A2Y,
-  WC_Z, WC_XI, WC_EMAX, WC_COUNT
-};
-static_assert(WC_COUNT <= WC_STRIDE, "constant block too small");
-
-enum { P_M = 0, P_MU, P_A, P_E0, P_NU0, P_PHI0, P_GAM0, P_ALP0, P_LAM, P_THS, P_PHS, P_THK, P_PHK,
-       P_DL, P_XI0, P_NXI, P_DELT };
-
-#define DEVINL __device__ __forceinline__
-
-DEVINL double frac(double x) { return x - floor(x); }
-
-// cube root polished by one Newton step on an exactly computed residual: CUDA's cbrt is faithful
-// (1 ulp) and, for a slowly drifting argument, its error is systematic from step to step, which
-// would bias gamma~ over ~1e4 steps (reading D3)
-DEVINL double cbrt_polished(double x) {
-  double c = cbrt(x);
-  double p = c * c;
-  double ep = fma(c, c, -p);
-  double r = fma(-p, c, x) - ep * c;
-  return fma(r, (double)__frcp_rn((float)(3.0 * p)), c);
-}
-
-// ------------------------------------------------------------------ (a0) cosmology, per walker
-// 16-point Gauss-Legendre on panels of width <= 0.75 in z.
-__constant__ double c_glx[8] = {0.0950125098376374401853193, 0.2816035507792589132304605,
-                                0.4580167776572273863424194, 0.6178762444026437484466718,
-                                0.7554044083550030338951012, 0.8656312023878317438804679,
-                                0.9445750230732325760779884, 0.9894009349916499325961542};
-__constant__ double c_glw[8] = {0.1894506104550684962853967, 0.1826034150449235888667637,
-                                0.1691565193950025381893121, 0.1495959888165767320815017,
-                                0.1246289712555338720524763, 0.0951585116824927848099251,
-                                0.0622535239386478928628438, 0.0271524594117540948517806};
-
-DEVINL double Ez(double z, double Om) {
-  double a = 1.0 + z;
-  return sqrt(fma(Om * a, a * a, 1.0 - Om));
-}
-// I1 = int_0^z dz'/E, I2 = int_0^z dz'/((1+z')E)
-DEVINL void cosmo_integrals(double z, double Om, double* I1, double* I2) {
-  int np = (int)ceil(z / 0.75);
-  if (np < 1) np = 1;
-  double h = z / np, s1 = 0.0, s2 = 0.0;
-  for (int p = 0; p < np; ++p) {
-    double mid = (p + 0.5) * h;
-    for (int i = 0; i < 8; ++i) {
-      double dx = 0.5 * h * c_glx[i];
-      double za = mid - dx, zb = mid + dx;
-      double fa = 1.0 / Ez(za, Om), fb = 1.0 / Ez(zb, Om);
-      s1 += c_glw[i] * (fa + fb);
-      s2 += c_glw[i] * (fa / (1.0 + za) + fb / (1.0 + zb));
-    }
-  }
-  *I1 = 0.5 * h * s1;
-  *I2 = 0.5 * h * s2;
-}
-// solve (1+z) tH I1(z) = D for z in [0, 20]: safeguarded Newton
-DEVINL double z_of_dL(double D, double tH, double Om) {
-  double lo = 0.0, hi = 20.0;
-  double z = fmin(D / tH, 1.0);
-  for (int it = 0; it < 60; ++it) {
-    double I1, I2;
-    cosmo_integrals(z, Om, &I1, &I2);
-    double f = (1.0 + z) * tH * I1 - D;
-    if (f > 0.0) hi = z; else lo = z;
-    double fp = tH * (I1 + (1.0 + z) / Ez(z, Om));
-    double zn = z - f / fp;
-    if (!(zn > lo && zn < hi)) zn = 0.5 * (lo + hi);
-    if (fabs(zn - z) <= 4e-16 * fmax(zn, 1e-300)) { z = zn; break; }
-    z = zn;
-  }
-  return z;
-}
-
-// ------------------------------------------------------------------ (a1) right-hand side, BC Eqs. 27-31
-struct OrbitConst { double twoPiMs, Cnu, Ce, a, sp; };
-
-// rates of (nu, gam_c, e, alp_c); Phi_c' = nu.  Angles in cycles (reading D2).
-DEVINL void rhs(const OrbitConst& w, double nu, double e, double* fnu, double* fgam, double* fe, double* falp) {
-  const double x = w.twoPiMs * nu;
-  const double cb = cbrt_polished(x);
-  const double u = cb * cb;
-  const double e2 = e * e;
-  const double q = 1.0 - e2;
-  const double rq = 1.0 / q;
-  const double sq = sqrt(q);
-  const double rsq = sq * rq;          // q^{-1/2}
-  const double x2 = x * x;
-  const double x83 = x2 * u, x113 = x83 * x;
-  const double rq2 = rq * rq;
-  // nu'
-  {
-    double t0 = fma(e2, fma(e2, 37.0 / 96.0, 73.0 / 24.0), 1.0) * q;
-    double t1 = u * fma(e2, fma(e2, fma(e2, -13147.0 / 5376.0, -3885.0 / 128.0), -2561.0 / 224.0), 1273.0 / 336.0);
-    double t2 = x * w.sp * rsq * fma(e2, fma(e2, fma(e2, 65.0 / 64.0, 3143.0 / 96.0), 1211.0 / 24.0), 73.0 / 12.0);
-    *fnu = w.Cnu * x113 * (rq2 * rq2 * rsq) * (t0 + t1 - t2);
-  }
-  // gamma~'/2pi
-  {
-    double uq = u * rq;
-    *fgam = 3.0 * nu * uq * fma(uq, 0.25 * fma(e2, -15.0, 26.0), 1.0) - 6.0 * nu * w.sp * x * (rq * rsq);
-  }
-  // e'
-  {
-    double t0 = fma(e2, 121.0, 304.0) * q * fma(u, 12.0, 1.0);
-    double t1 = u * fma(e2, fma(e2, -25211.0, 12.0 * 9082.0), 8.0 * 16705.0) * (1.0 / 56.0);
-    double t2 = w.sp * x113 * (rq2 * rq2) * fma(e2, fma(e2, 263.0 / 10.0, 5032.0 / 15.0), 1364.0 / 5.0);
-    *fe = e * w.Ce * (t2 - (1.0 / 15.0) * x83 * (rq2 * rq * rsq) * (t0 - t1));
-  }
-  *falp = 2.0 * nu * w.a * x * (rq * rsq);
-}
-
-DEVINL bool plunged(const OrbitConst& w, double nu, double e) {
-  // nu >= nu_LSO(e) = ((1-e^2)/(6+2e))^{3/2} / (2 pi M), division- and root-free
-  double x = w.twoPiMs * nu, q = 1.0 - e * e, d = 6.0 + 2.0 * e;
-  return !(x * x * d * d * d < q * q * q);
-}
-
-struct RkOut { double d[5]; double k1[5]; };
-
-DEVINL void rk4_increment(const OrbitConst& w, const double y[5], double h, RkOut& o) {
-  double k2[5], k3[5], k4[5];
-  o.k1[0] = y[1];
-  rhs(w, y[1], y[3], &o.k1[1], &o.k1[2], &o.k1[3], &o.k1[4]);
-  double hh = 0.5 * h;
-  double nu = fma(hh, o.k1[1], y[1]), e = fma(hh, o.k1[3], y[3]);
-  k2[0] = nu;
-  rhs(w, nu, e, &k2[1], &k2[2], &k2[3], &k2[4]);
-  nu = fma(hh, k2[1], y[1]); e = fma(hh, k2[3], y[3]);
-  k3[0] = nu;
-  rhs(w, nu, e, &k3[1], &k3[2], &k3[3], &k3[4]);
-  nu = fma(h, k3[1], y[1]); e = fma(h, k3[3], y[3]);
-  k4[0] = nu;
-  rhs(w, nu, e, &k4[1], &k4[2], &k4[3], &k4[4]);
-#pragma unroll
-  for (int q = 0; q < 5; ++q) o.d[q] = (h / 6.0) * (o.k1[q] + 2.0 * k2[q] + 2.0 * k3[q] + k4[q]);
-}
-
-struct OrbitArgs {
-  const double* params;   // [K][17]
-  int K;
-  int64_t N;
-  double dt;
-  int S;
-  int64_t Nc, Nn;
-  int n_max;
-  double tH, Om;          // Hubble time [s], Omega_m
-  double* wc;             // [K][WC_STRIDE]
-  double* nodes;          // [K][Nn][NODE_STRIDE]
-  int32_t* jpl;           // [K] first plunged node (index j), Nn if none
-  int32_t* status;        // [K]
-  uint8_t* mterms;        // [K][EMRI_NMAX_CAP+1] Bessel series lengths per harmonic
-};
-
-DEVINL void store_node(double* row, const double y[5], const double k1[5], const double d[5]) {
-  double2* r = reinterpret_cast<double2*>(row);
-  r[0] = make_double2(y[0], y[1]);
-  r[1] = make_double2(y[2], y[3]);
-  r[2] = make_double2(y[4], k1[0]);
-  r[3] = make_double2(k1[1], k1[2]);
-  r[4] = make_double2(k1[3], k1[4]);
-  r[5] = make_double2(d[0], d[1]);
-  r[6] = make_double2(d[2], d[3]);
-  r[7] = make_double2(d[4], 0.0);
-}
-
-__global__ void __launch_bounds__(32) orbit_kernel(OrbitArgs a) {
-  const int k = blockIdx.x * blockDim.x + threadIdx.x;
-  if (k >= a.K) return;
-  const double* p = a.params + (size_t)k * EMRI_NPAR;
-  double* wc = a.wc + (size_t)k * WC_STRIDE;
-  double* nodes = a.nodes + (size_t)k * a.Nn * NODE_STRIDE;
-  const double Delta = a.S * a.dt;
-  int status = 0;
-  int32_t jpl = (int32_t)a.Nn;
-
-  // ---- (a0) validity and per-walker scalars
-  bool ok = true;
-#pragma unroll
-  for (int i = 0; i < EMRI_NPAR; ++i) ok = ok && isfinite(p[i]);
-  ok = ok && p[P_M] > 0.0 && p[P_MU] > 0.0 && p[P_DL] > 0.0 && p[P_E0] >= 0.0 && p[P_E0] < 1.0 &&
-       fabs(p[P_A]) <= 1.0 && p[P_NU0] > 0.0;
-  double Xi = 1.0, z = 0.0, dT = 0.0, amp = 0.0;
-  const double Ms = p[P_M] * kMsunSec, mus = p[P_MU] * kMsunSec;
-  if (ok) {
-    const double Ds = p[P_DL] * kGpcSec;
-    z = z_of_dL(Ds, a.tH, a.Om);
-    Xi = p[P_XI0] + (1.0 - p[P_XI0]) * pow(1.0 + z, -p[P_NXI]);     // Eq. 6
-    ok = (Xi > 0.0) && isfinite(Xi);
-    if (ok) {
-      double I1, I2;
-      cosmo_integrals(z, a.Om, &I1, &I2);
-      dT = -p[P_DELT] * (a.tH * I2);                                 // reading R9
-      amp = mus / (Xi * Ds);                                         // d_GW = Xi d_EM (Eq. 5)
-    }
-  }
-  if (!ok) status |= EMRI_ST_BADPARAM;
-
-  OrbitConst oc;
-  oc.twoPiMs = kTwoPi * Ms;
-  oc.Cnu = 96.0 / (10.0 * kPi) * (mus / (Ms * Ms * Ms));
-  oc.Ce = mus / (Ms * Ms);
-  oc.a = p[P_A];
-  double sl, cl;
-  sincos(p[P_LAM], &sl, &cl);
-  oc.sp = p[P_A] * cl;
-  {
-    double sS, cS, sK, cK, sphS, cphS, sphK, cphK;
-    sincos(p[P_THS], &sS, &cS);
-    sincos(p[P_THK], &sK, &cK);
-    sincos(p[P_PHS], &sphS, &cphS);
-    sincos(p[P_PHK], &sphK, &cphK);
-    // L^(alpha) = A0 + A1 cos(alpha) + A2 sin(alpha)   (BC Eqs. 19-21)
-    const double A0x = sK * cphK * cl, A0y = sK * sphK * cl, A0z = cK * cl;
-    const double A1x = -cphK * cK * sl, A1y = -sphK * cK * sl, A1z = sK * sl;
-    const double A2x = sphK * sl, A2y = -cphK * sl;
-    const double nx = sS * cphS, ny = sS * sphS, nz = cS;
-    const double Sn = cS * cK + sS * sK * (cphS * cphK + sphS * sphK);
-    wc[WC_TWOPIMS] = oc.twoPiMs; wc[WC_CNU] = oc.Cnu; wc[WC_CE] = oc.Ce; wc[WC_A] = oc.a; wc[WC_SP] = oc.sp;
-    wc[WC_AMP] = amp; wc[WC_DT] = dT; wc[WC_SIGMA] = dT / Delta; wc[WC_DOP] = kAuSec * sS;
-    wc[WC_CPHS] = cphS; wc[WC_SPHS] = sphS; wc[WC_CS] = cS; wc[WC_SS] = sS;
-    wc[WC_LN0] = A0x * nx + A0y * ny + A0z * nz;
-    wc[WC_LN1] = A1x * nx + A1y * ny + A1z * nz;
-    wc[WC_LN2] = A2x * nx + A2y * ny;
-    wc[WC_CL] = cl; wc[WC_SN] = Sn;
-    wc[WC_B1] = sS * (sphK * cphS - cphK * sphS) * sl;               // sin(thS) sin(phK - phS) sin(lam)
-    wc[WC_B2] = (Sn * cK - cS) / sK * sl;
-    wc[WC_A0X] = A0x; wc[WC_A0Y] = A0y; wc[WC_A0Z] = A0z;
-    wc[WC_A1X] = A1x; wc[WC_A1Y] = A1y; wc[WC_A1Z] = A1z;
-    wc[WC_A2X] = A2x; wc[WC_A2Y] = A2y;
-    wc[WC_Z] = z; wc[WC_XI] = Xi;
-  }
-  if (ok && !(fabs(dT) <= Delta)) status |= EMRI_ST_DELAY;          // reading R20
-
-  // ---- (a1) RK4 on the coarse grid
-  double y[5] = {frac(p[P_PHI0] / kTwoPi), p[P_NU0], frac(p[P_GAM0] / kTwoPi), p[P_E0], frac(p[P_ALP0] / kTwoPi)};
-  double emax = ok ? y[3] : 0.0;
-  const double zero5[5] = {0, 0, 0, 0, 0};
-  bool run = ok;
-  if (run && plunged(oc, y[1], y[3])) { status |= EMRI_ST_PLUNGE; jpl = 0; run = false; }
-  if (!run) {
-    for (int64_t m = 0; m < a.Nn; ++m) store_node(nodes + m * NODE_STRIDE, zero5, zero5, zero5);
-  } else {
-    RkOut r;
-    // backward guard step: node -1
-    rk4_increment(oc, y, -Delta, r);
-    double ym[5] = {frac(y[0] + r.d[0]), y[1] + r.d[1], frac(y[2] + r.d[2]), y[3] + r.d[3], frac(y[4] + r.d[4])};
-    bool okm = isfinite(ym[0]) && isfinite(ym[1]) && isfinite(ym[2]) && isfinite(ym[3]) && isfinite(ym[4]) &&
-               ym[3] >= 0.0 && ym[3] < 1.0 && ym[1] > 0.0;
-    if (!okm) {
-      status |= EMRI_ST_STATE;
-      for (int64_t m = 0; m < a.Nn; ++m) store_node(nodes + m * NODE_STRIDE, zero5, zero5, zero5);
-    } else {
-      double km[5], dm[5];
-      km[0] = ym[1];
-      rhs(oc, ym[1], ym[3], &km[1], &km[2], &km[3], &km[4]);
-#pragma unroll
-      for (int q = 0; q < 5; ++q) dm[q] = -r.d[q];
-      store_node(nodes, ym, km, dm);
-      emax = fmax(emax, ym[3]);
-      // forward sweep; nu and e are Kahan-compensated (reading D3)
-      double comp_nu = 0.0, comp_e = 0.0;
-      const int64_t last = a.Nc + 1;          // node index j of the last node (G = 1)
-      for (int64_t j = 0; j <= last; ++j) {
-        double* row = nodes + (j + 1) * NODE_STRIDE;
-        if (j == last) {
-          double k1[5];
-          k1[0] = y[1];
-          rhs(oc, y[1], y[3], &k1[1], &k1[2], &k1[3], &k1[4]);
-          store_node(row, y, k1, zero5);
-          break;
-        }
-        rk4_increment(oc, y, Delta, r);
-        store_node(row, y, r.k1, r.d);
-        double yn[5];
-        yn[0] = frac(y[0] + r.d[0]);
-        yn[2] = frac(y[2] + r.d[2]);
-        yn[4] = frac(y[4] + r.d[4]);
-        { double t = r.d[1] - comp_nu, s = y[1] + t; comp_nu = (s - y[1]) - t; yn[1] = s; }
-        { double t = r.d[3] - comp_e, s = y[3] + t; comp_e = (s - y[3]) - t; yn[3] = s; }
-        bool okn = isfinite(yn[0]) && isfinite(yn[1]) && isfinite(yn[2]) && isfinite(yn[3]) && isfinite(yn[4]) &&
-                   yn[3] >= 0.0 && yn[3] < 1.0 && yn[1] > 0.0;
-        bool pl = okn && plunged(oc, yn[1], yn[3]);
-        if (!okn || pl) {
-          status |= okn ? EMRI_ST_PLUNGE : EMRI_ST_STATE;
-          jpl = (int32_t)(j + 1);
-          // nodes from j_pl on are copies of node j_pl - 1 with zero increments
-          for (int64_t m = j + 1; m <= last; ++m) store_node(nodes + (m + 1) * NODE_STRIDE, y, r.k1, zero5);
-          break;
-        }
-#pragma unroll
-        for (int q = 0; q < 5; ++q) y[q] = yn[q];
-      }
-    }
-  }
-  wc[WC_EMAX] = emax;
-  a.jpl[k] = jpl;
-  a.status[k] = status;
-  // Bessel series lengths: smallest M with prod_{i<=M} y/(i(i+n+1)) < 2^-58, y = (n emax/2)^2
-  uint8_t* mt = a.mterms + (size_t)k * (EMRI_NMAX_CAP + 1);
-  for (int n = 1; n <= a.n_max; ++n) {
-    double yy = 0.25 * n * n * emax * emax, term = 1.0;
-    int M = 1;
-    while (M < MCAP) {
-      term *= yy / ((double)M * (double)(M + n + 1));
-      ++M;                      // M coefficients cover powers 0..M-1; `term` is the size of power M-1
-      if (term < 3.5e-18) break;
-    }
-    mt[n] = (uint8_t)M;
-  }
-}
-
-// ------------------------------------------------------------------ (b) synthesis
-struct SynthArgs {
-  const double* wc;
-  const double* nodes;
-  const int32_t* jpl;
-  const int32_t* status;
-  const uint8_t* mterms;
-  const double2* series;   // [n_max+1][MCAP] {coef for order n+1, coef for order n+2} in powers of e^2
-  const double* ncoef;     // [n_max+1][NCOEF]
-  int k0, K;               // walkers k0 .. k0+K-1
-  int64_t N;
-  double dt;
-  int S, logS;
-  int64_t Nn;
-  int n_max;
-  double* outI;            // row of walker k0+i at outI + i*pitch
-  double* outII;
-  int64_t pitch;
-  int64_t tiles_per_walker;
-};
-
-struct Sample {
-  double e2, e4, c1, s1;     // e^2, e^4, cos/sin of Phi_tot
-  double cn, sn;             // cos/sin(n Phi_tot)
-  double Sa, Sb, Sc;
-};
-
-// cubic Hermite of the five orbital quantities at fraction s of interval j (node row jj = j+1)
-DEVINL void hermite5(const double* __restrict__ nodes, int64_t jj, double s, double Delta, double out[5]) {
-  const double2* r0 = reinterpret_cast<const double2*>(nodes + jj * NODE_STRIDE);
-  const double2* r1 = r0 + NODE_STRIDE / 2;
-  double2 v01 = __ldg(r0), v23 = __ldg(r0 + 1), v4m0 = __ldg(r0 + 2), m12 = __ldg(r0 + 3), m34 = __ldg(r0 + 4),
-          d01 = __ldg(r0 + 5), d23 = __ldg(r0 + 6), d4 = __ldg(r0 + 7);
-  double2 n4m0 = __ldg(r1 + 2), n12 = __ldg(r1 + 3), n34 = __ldg(r1 + 4);
-  const double s2 = s * s, s3 = s2 * s;
-  const double b = 3.0 * s2 - 2.0 * s3;
-  const double c0 = Delta * (s3 - 2.0 * s2 + s), c1 = Delta * (s3 - s2);
-  out[0] = v01.x + fma(b, d01.x, fma(c0, v4m0.y, c1 * n4m0.y));
-  out[1] = v01.y + fma(b, d01.y, fma(c0, m12.x, c1 * n12.x));
-  out[2] = v23.x + fma(b, d23.x, fma(c0, m12.y, c1 * n12.y));
-  out[3] = v23.y + fma(b, d23.y, fma(c0, m34.x, c1 * n34.x));
-  out[4] = v4m0.x + fma(b, d4.x, fma(c0, m34.y, c1 * n34.y));
-}
-
-struct Projection { double FIp, FIx, FIIp, FIIx, c2g, s2g, sq, A, Ln, e; };
-
-// everything of one sample that does not depend on the harmonic index
-DEVINL void sample_setup(const double* __restrict__ w, const double* __restrict__ nodes, int64_t i, int S, int logS,
-                         double dt, int32_t jpl, bool* live, Sample* sm, Projection* pr) {
-  // source-time split (reading D4)
-  int64_t j = i >> logS;
-  double s = (double)(i & (S - 1)) * (1.0 / (double)S) - w[WC_SIGMA];
-  if (s < 0.0) { s += 1.0; j -= 1; } else if (s >= 1.0) { s -= 1.0; j += 1; }
-  *live = (j + 1 < (int64_t)jpl);
-  double orb[5];
-  hermite5(nodes, j + 1, s, S * dt, orb);
-  const double Phic = orb[0], nu = orb[1], gamc = orb[2], e = orb[3], alpc = orb[4];
-  double sa, ca, s2gt, c2gt, spb, cpb;
-  sincospi(2.0 * alpc, &sa, &ca);
-  sincospi(4.0 * gamc, &s2gt, &c2gt);
-  sincospi(2.0 * frac(((double)i * dt) / kYearSec), &spb, &cpb);
-  // orbital-plane normal and its projections (BC 19-21)
-  const double Lx = fma(w[WC_A2X], sa, fma(w[WC_A1X], ca, w[WC_A0X]));
-  const double Ly = fma(w[WC_A2Y], sa, fma(w[WC_A1Y], ca, w[WC_A0Y]));
-  const double Lz = fma(w[WC_A1Z], ca, w[WC_A0Z]);
-  const double Ln = fma(w[WC_LN2], sa, fma(w[WC_LN1], ca, w[WC_LN0]));
-  // beta (BC 22-24): tan(beta) = Ns/Nc
-  const double Ns = fma(w[WC_CL], Ln, -w[WC_SN]);
-  const double Nc = fma(w[WC_B2], sa, w[WC_B1] * ca);
-  const double den_b = fma(Nc, Nc, Ns * Ns);
-  // detector time quantities
-  const double cphS = w[WC_CPHS], sphS = w[WC_SPHS], cS = w[WC_CS], sS = w[WC_SS];
-  const double cd = fma(cpb, cphS, spb * sphS), sd = fma(spb, cphS, -cpb * sphS);
-  const double cthd = fma(-kHalfSqrt3 * sS, cd, 0.5 * cS);
-  const double Pq = fma(sS, cd, kSqrt3 * cS), Qq = 2.0 * sS * sd;
-  const double den_a = fma(Pq, Pq, Qq * Qq);
-  const double Npsi = fma(-cthd, Ln, fma(-kHalfSqrt3, fma(Lx, cpb, Ly * spb), 0.5 * Lz));
-  const double Dpsi = 0.5 * sS * fma(Ly, cphS, -Lx * sphS)
-                      - kHalfSqrt3 * (cpb * fma(Lz * sS, sphS, -cS * Ly) + spb * fma(cS, Lx, -Lz * sS * cphS));
-  const double den_p = fma(Npsi, Npsi, Dpsi * Dpsi);
-  // one division for the three normalisations
-  const double bp = den_b * den_p;
-  const double inv = 1.0 / (bp * den_a);
-  const double ib = (den_b > 0.0) ? inv * (den_a * den_p) : 0.0;
-  const double ia = inv * bp;
-  const double ip = (den_p > 0.0) ? inv * (den_a * den_b) : 0.0;
-  double c2b = fma(Nc, Nc, -Ns * Ns) * ib, s2b = 2.0 * Ns * Nc * ib;
-  if (!(den_b > 0.0)) { c2b = 1.0; s2b = 0.0; }                     // reading R16: beta = 0
-  const double c2a = fma(Qq, Qq, -Pq * Pq) * ia, s2a = 2.0 * Pq * Qq * ia;
-  double c2s = fma(Dpsi, Dpsi, -Npsi * Npsi) * ip, s2s = 2.0 * Npsi * Dpsi * ip;
-  if (!(den_p > 0.0)) { c2s = 1.0; s2s = 0.0; }
-  const double c2g = fma(c2gt, c2b, -s2gt * s2b), s2g = fma(s2gt, c2b, c2gt * s2b);
-  const double c2pb = fma(cpb, cpb, -spb * spb), s2pb = 2.0 * cpb * spb;
-  const double c2p = fma(c2pb, c2a, -s2pb * s2a), s2p = fma(s2pb, c2a, c2pb * s2a);
-  const double hh = 0.5 * fma(cthd, cthd, 1.0);
-  pr->FIp = fma(hh * c2p, c2s, -cthd * s2p * s2s);
-  pr->FIx = fma(hh * c2p, s2s, cthd * s2p * c2s);
-  pr->FIIp = fma(hh * s2p, c2s, cthd * c2p * s2s);
-  pr->FIIx = fma(hh * s2p, s2s, -cthd * c2p * c2s);
-  // amplitude A = (2 pi M nu)^{2/3} mu / (Xi D)   (BC 10 with Eqs. 4-6 folded in)
-  const double cb = cbrt(w[WC_TWOPIMS] * nu);
-  pr->A = cb * cb * w[WC_AMP];
-  pr->Ln = Ln;
-  pr->sq = sqrt(fma(-e, e, 1.0));
-  pr->c2g = c2g; pr->s2g = s2g; pr->e = e;
-  // Doppler-shifted phase in cycles (BC 25)
-  const double Phit = frac(fma(nu * w[WC_DOP], cd, Phic));
-  sincospi(2.0 * Phit, &sm->s1, &sm->c1);
-  sm->e2 = e * e;
-  sm->e4 = sm->e2 * sm->e2;
-  sm->cn = sm->c1; sm->sn = sm->s1;
-  sm->Sa = 0.0; sm->Sb = 0.0; sm->Sc = 0.0;
-}
-
-DEVINL void sample_finish(const Sample& sm, const Projection& pr, bool live, double* hI, double* hII) {
-  const double Ln2 = pr.Ln * pr.Ln;
-  const double sb = pr.sq * sm.Sb;
-  // A+ = A {(1+Ln^2)(c2g Sa - s2g sq Sb) + 2 (1-Ln^2) Sc},  Ax = -2 A Ln (sq Sb c2g + Sa s2g)   (BC 7-9 summed over n)
-  const double Ap = pr.A * fma(1.0 + Ln2, fma(pr.c2g, sm.Sa, -pr.s2g * sb), 2.0 * (1.0 - Ln2) * sm.Sc);
-  const double Ax = -2.0 * pr.A * pr.Ln * fma(sb, pr.c2g, sm.Sa * pr.s2g);
-  *hI = live ? kHalfSqrt3 * fma(pr.FIp, Ap, pr.FIx * Ax) : 0.0;
-  *hII = live ? kHalfSqrt3 * fma(pr.FIIp, Ap, pr.FIIx * Ax) : 0.0;
-}
-
-__global__ void __launch_bounds__(SYNTH_THREADS, 4) synth_kernel(SynthArgs a) {
-  extern __shared__ __align__(16) unsigned char smem_raw[];
-  double2* s_series = reinterpret_cast<double2*>(smem_raw);                         // [(n_max+1)*MCAP]
-  double* s_ncoef = reinterpret_cast<double*>(s_series + (size_t)(a.n_max + 1) * MCAP);   // [(n_max+1)*NCOEF]
-  double* s_wc = s_ncoef + (size_t)(a.n_max + 1) * NCOEF;                           // [WC_STRIDE]
-  __shared__ uint8_t s_mt[EMRI_NMAX_CAP + 1];
-
-  for (int i = threadIdx.x; i < (a.n_max + 1) * MCAP; i += blockDim.x) s_series[i] = a.series[i];
-  for (int i = threadIdx.x; i < (a.n_max + 1) * NCOEF; i += blockDim.x) s_ncoef[i] = a.ncoef[i];
-
-  const int64_t total = (int64_t)a.K * a.tiles_per_walker;
-  int cur_k = -1;
-  for (int64_t t = blockIdx.x; t < total; t += gridDim.x) {
-    const int kl = (int)(t / a.tiles_per_walker);
-    const int64_t tile = t - (int64_t)kl * a.tiles_per_walker;
-    const int k = a.k0 + kl;
-    if (k != cur_k) {
-      __syncthreads();
-      if (threadIdx.x < WC_STRIDE) s_wc[threadIdx.x] = a.wc[(size_t)k * WC_STRIDE + threadIdx.x];
-      if (threadIdx.x <= EMRI_NMAX_CAP) s_mt[threadIdx.x] = a.mterms[(size_t)k * (EMRI_NMAX_CAP + 1) + threadIdx.x];
-      cur_k = k;
-      __syncthreads();
-    }
-    const int64_t i0 = tile * TILE + 2 * threadIdx.x;
-    if (i0 >= a.N) continue;
-    double* oI = a.outI + (size_t)kl * a.pitch + i0;
-    double* oII = a.outII + (size_t)kl * a.pitch + i0;
-    const int32_t st = a.status[k];
-    if (st & (EMRI_ST_BADPARAM | EMRI_ST_DELAY | EMRI_ST_STATE)) {
-      *reinterpret_cast<double2*>(oI) = make_double2(0.0, 0.0);
-      *reinterpret_cast<double2*>(oII) = make_double2(0.0, 0.0);
-      continue;
-    }
-    const double* nodes = a.nodes + (size_t)k * a.Nn * NODE_STRIDE;
-    const int32_t jpl = a.jpl[k];
-    Sample A, B;
-    Projection pa, pb;
-    bool la, lb;
-    sample_setup(s_wc, nodes, i0, a.S, a.logS, a.dt, jpl, &la, &A, &pa);
-    sample_setup(s_wc, nodes, i0 + 1, a.S, a.logS, a.dt, jpl, &lb, &B, &pb);
-
-    // ---- harmonic n = 1 (brackets odd in e; J_{-1} = -J_1)
-    {
-      const int M = s_mt[1];
-      const double2* tab = s_series + MCAP;
-      double2 c = tab[M - 1];
-      double j2a = c.x, j3a = c.y, j2b = c.x, j3b = c.y;     // scaled J_2, J_3
-      for (int m = M - 2; m >= 0; --m) {
-        c = tab[m];
-        j2a = fma(j2a, A.e2, c.x); j3a = fma(j3a, A.e2, c.y);
-        j2b = fma(j2b, B.e2, c.x); j3b = fma(j3b, B.e2, c.y);
-      }
-      const double* kc = s_ncoef + NCOEF;
-#pragma unroll
-      for (int h = 0; h < 2; ++h) {
-        Sample& s = h ? B : A;
-        const double e = h ? pb.e : pa.e;
-        const double j2 = h ? j2b : j2a, j3 = h ? j3b : j3a;
-        const double j1 = fma(-s.e2 * kc[8], j3, j2);
-        const double j0 = fma(-s.e2 * kc[9], j2, j1);
-        const double ba = fma(s.e2, fma(-1.0 / 48.0, j3, 0.25 * j2), fma(0.5, j1, -2.0 * j0));
-        const double bb = fma(s.e2 * (1.0 / 48.0), j3, -1.5 * j1);
-        const double tc = e * s.cn, ts = e * s.sn;
-        s.Sa = ba * tc; s.Sb = bb * ts; s.Sc = 0.5 * j1 * tc;
-        const double cn = fma(s.cn, s.c1, -s.sn * s.s1), sn = fma(s.sn, s.c1, s.cn * s.s1);
-        s.cn = cn; s.sn = sn;
-      }
-    }
-    // ---- harmonics n = 2 .. n_max
-    double ta = 1.0, tb = 1.0;     // t'_n = (n e/2)^{n-2}/(n-2)!
-    for (int n = 2; n <= a.n_max; ++n) {
-      const int M = s_mt[n];
-      const double2* tab = s_series + n * MCAP;
-      double2 c = tab[M - 1];
-      double p1a = c.x, p2a = c.y, p1b = c.x, p2b = c.y;     // scaled J_{n+1}, J_{n+2}
-      for (int m = M - 2; m >= 0; --m) {
-        c = tab[m];
-        p1a = fma(p1a, A.e2, c.x); p2a = fma(p2a, A.e2, c.y);
-        p1b = fma(p1b, B.e2, c.x); p2b = fma(p2b, B.e2, c.y);
-      }
-      const double* kc = s_ncoef + n * NCOEF;
-#pragma unroll
-      for (int h = 0; h < 2; ++h) {
-        Sample& s = h ? B : A;
-        const double p1 = h ? p1b : p1a, p2 = h ? p2b : p2a;
-        double& t = h ? tb : ta;
-        const double j0 = fma(-s.e2 * kc[8], p2, p1);        // scaled J_n
-        const double jm1 = fma(-s.e2 * kc[9], p1, j0);       // scaled J_{n-1}
-        const double jm2 = fma(-s.e2 * kc[10], j0, jm1);     // scaled J_{n-2}
-        const double ba = fma(s.e4, fma(kc[4], p2, kc[3] * p1), fma(s.e2, fma(kc[2], j0, kc[1] * jm1), kc[0] * jm2));
-        const double bb = fma(s.e4 * kc[6], p2, fma(s.e2 * kc[5], j0, kc[0] * jm2));
-        const double bc = s.e2 * kc[7] * j0;
-        const double tc = t * s.cn, ts = t * s.sn;
-        s.Sa = fma(ba, tc, s.Sa); s.Sb = fma(bb, ts, s.Sb); s.Sc = fma(bc, tc, s.Sc);
-        const double cn = fma(s.cn, s.c1, -s.sn * s.s1), sn = fma(s.sn, s.c1, s.cn * s.s1);
-        s.cn = cn; s.sn = sn;
-        t *= (h ? pb.e : pa.e) * kc[11];
-      }
-    }
-    double hIa, hIIa, hIb, hIIb;
-    sample_finish(A, pa, la, &hIa, &hIIa);
-    sample_finish(B, pb, lb, &hIb, &hIIb);
-    *reinterpret_cast<double2*>(oI) = make_double2(hIa, hIb);
-    *reinterpret_cast<double2*>(oII) = make_double2(hIIa, hIIb);
-  }
-}
-
-// ------------------------------------------------------------------ (d) likelihood reduction
-struct LikeArgs {
-  const double2* H;        // [2*K][Nf] complex (row pitch Nf)
-  const double2* D;        // [2][Nf]
-  const double* w;         // [Nf] 1/S_n or 0
-  double* partial;         // [K_total][n_part], this chunk starts at row k0
-  int k0, K;
-  int64_t Nf;
-  int n_part;              // partial sums per walker = tiles * LL_WARPS
-};
-
-__global__ void __launch_bounds__(LL_THREADS) loglike_kernel(LikeArgs a) {
-  const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
-  const int64_t base = (int64_t)blockIdx.x * LL_TILE + threadIdx.x;
-  double2 dI[LL_BINS_PER_THREAD], dII[LL_BINS_PER_THREAD];
-  double wt[LL_BINS_PER_THREAD];
-#pragma unroll
-  for (int b = 0; b < LL_BINS_PER_THREAD; ++b) {
-    const int64_t m = base + (int64_t)b * LL_THREADS;
-    const bool in = m < a.Nf;
-    dI[b] = in ? __ldg(a.D + m) : make_double2(0.0, 0.0);
-    dII[b] = in ? __ldg(a.D + a.Nf + m) : make_double2(0.0, 0.0);
-    wt[b] = in ? __ldg(a.w + m) : 0.0;
-  }
-  for (int kl = 0; kl < a.K; ++kl) {
-    const double2* HI = a.H + (size_t)(2 * kl) * a.Nf;
-    const double2* HII = HI + a.Nf;
-    double2 hI[LL_BINS_PER_THREAD], hII[LL_BINS_PER_THREAD];
-#pragma unroll
-    for (int b = 0; b < LL_BINS_PER_THREAD; ++b) {
-      const int64_t m = base + (int64_t)b * LL_THREADS;
-      const bool in = m < a.Nf;
-      hI[b] = in ? __ldcs(HI + m) : make_double2(0.0, 0.0);
-      hII[b] = in ? __ldcs(HII + m) : make_double2(0.0, 0.0);
-    }
-    double acc = 0.0;
-#pragma unroll
-    for (int b = 0; b < LL_BINS_PER_THREAD; ++b) {
-      const double ar = dI[b].x - hI[b].x, ai = dI[b].y - hI[b].y;
-      const double br = dII[b].x - hII[b].x, bi = dII[b].y - hII[b].y;
-      const double pw = fma(ar, ar, ai * ai) + fma(br, br, bi * bi);
-      acc = fma(wt[b], pw, acc);
-    }
-#pragma unroll
-    for (int off = 16; off > 0; off >>= 1) acc += __shfl_xor_sync(0xffffffffu, acc, off);
-    if (lane == 0) a.partial[(size_t)(a.k0 + kl) * a.n_part + (size_t)blockIdx.x * LL_WARPS + warp] = acc;
-  }
-}
-
-// fixed-order final sum: one warp per walker, lane-strided partial sums then a shuffle tree
-__global__ void loglike_final_kernel(const double* partial, int n_part, int K, double scale, const int32_t* status,
-                                     double* logL, int32_t* status_out) {
-  const int k = blockIdx.x * (blockDim.x >> 5) + (threadIdx.x >> 5);
-  const int lane = threadIdx.x & 31;
-  if (k >= K) return;
-  const double* p = partial + (size_t)k * n_part;
-  double acc = 0.0;
-  for (int i = lane; i < n_part; i += 32) acc += p[i];
-#pragma unroll
-  for (int off = 16; off > 0; off >>= 1) acc += __shfl_xor_sync(0xffffffffu, acc, off);
-  if (lane == 0) {
-    const int32_t st = status[k];
-    logL[k] = (st & (EMRI_ST_BADPARAM | EMRI_ST_DELAY | EMRI_ST_STATE)) ? -INFINITY : -scale * acc;
-    if (status_out) status_out[k] = st;
-  }
-}
-
-__global__ void copy_status_kernel(const int32_t* in, int32_t* out, int K) {
-  int k = blockIdx.x * blockDim.x + threadIdx.x;
-  if (k < K) out[k] = in[k];
-}
-
-// ------------------------------------------------------------------ stretch move (configs[4])
-DEVINL uint32_t mulhilo(uint32_t a, uint32_t b, uint32_t* hi) {
-  uint64_t p = (uint64_t)a * b;
-  *hi = (uint32_t)(p >> 32);
-  return (uint32_t)p;
-}
-// Philox4x32-10 (Salmon et al. 2011)
-DEVINL void philox4x32(uint32_t c[4], uint32_t k0, uint32_t k1) {
-#pragma unroll
-  for (int r = 0; r < 10; ++r) {
-    uint32_t hi0, hi1;
-    uint32_t lo0 = mulhilo(0xD2511F53u, c[0], &hi0);
-    uint32_t lo1 = mulhilo(0xCD9E8D57u, c[2], &hi1);
-    uint32_t n0 = hi1 ^ c[1] ^ k0, n1 = lo1, n2 = hi0 ^ c[3] ^ k1, n3 = lo0;
-    c[0] = n0; c[1] = n1; c[2] = n2; c[3] = n3;
-    k0 += 0x9E3779B9u; k1 += 0xBB67AE85u;
-  }
-}
-DEVINL double u53(uint32_t hi, uint32_t lo) {      // uniform in (0,1): (53-bit integer + 0.5) / 2^53
-  uint64_t v = (((uint64_t)hi << 32) | lo) >> 11;
-  return ((double)v + 0.5) * (1.0 / 9007199254740992.0);
-}
-
-struct StretchArgs {
-  double* X; double* logL; int K;
-  const double* lo; const double* hi;
-  double a; uint64_t seed; int64_t step; int half;
-  double* Y;        // [K/2][17] proposals
-  double* zbuf;     // [K/2] z
-  double* lnu;      // [K/2] ln u'
-  int32_t* inbox;   // [K/2]
-  int32_t* partner; // [K/2]
-  const double* logLY;
-  int32_t* accepted;
-  double* log_buf;
-};
-
-__global__ void stretch_propose_kernel(StretchArgs s) {
-  const int i = blockIdx.x * blockDim.x + threadIdx.x;
-  const int H = s.K / 2;
-  if (i >= H) return;
-  const int k = s.half * H + i, ob = (1 - s.half) * H;
-  uint32_t c[4] = {(uint32_t)s.step, (uint32_t)((uint64_t)s.step >> 32), (uint32_t)(2 * i + s.half), 0u};
-  philox4x32(c, (uint32_t)s.seed, (uint32_t)(s.seed >> 32));
-  const double u1 = u53(c[0], c[1]), u2 = u53(c[2], c[3]);
-  uint32_t c2[4] = {(uint32_t)s.step, (uint32_t)((uint64_t)s.step >> 32), (uint32_t)(2 * i + s.half), 1u};
-  philox4x32(c2, (uint32_t)s.seed, (uint32_t)(s.seed >> 32));
-  const double u3 = u53(c2[0], c2[1]);
-  int j = ob + min((int)(u1 * H), H - 1);
-  const double sz = fma(s.a - 1.0, u2, 1.0);
-  const double z = sz * sz / s.a;
-  bool in = true;
-  for (int q = 0; q < EMRI_NPAR; ++q) {
-    const double xk = s.X[(size_t)k * EMRI_NPAR + q], xj = s.X[(size_t)j * EMRI_NPAR + q];
-    const bool fixed = !(s.lo[q] < s.hi[q]);
-    const double y = fixed ? xk : fma(z, xk - xj, xj);
-    s.Y[(size_t)i * EMRI_NPAR + q] = y;
-    in = in && (fixed || (y >= s.lo[q] && y <= s.hi[q]));
-  }
-  s.zbuf[i] = z; s.lnu[i] = log(u3); s.inbox[i] = in ? 1 : 0; s.partner[i] = j;
-}
-
-__global__ void stretch_accept_kernel(StretchArgs s) {
-  const int i = blockIdx.x * blockDim.x + threadIdx.x;
-  const int H = s.K / 2;
-  if (i >= H) return;
-  const int k = s.half * H + i;
-  int nfree = 0;
-  for (int q = 0; q < EMRI_NPAR; ++q) nfree += (s.lo[q] < s.hi[q]) ? 1 : 0;
-  const double lY = s.inbox[i] ? s.logLY[i] : -INFINITY;
-  const double lnq = (double)(nfree - 1) * log(s.zbuf[i]) + lY - s.logL[k];
-  const bool acc = isfinite(lY) && (s.lnu[i] < lnq);
-  if (s.log_buf) {
-    double* lb = s.log_buf + (size_t)i * (EMRI_NPAR + 4);
-    for (int q = 0; q < EMRI_NPAR; ++q) lb[q] = s.Y[(size_t)i * EMRI_NPAR + q];
-    lb[EMRI_NPAR] = s.zbuf[i]; lb[EMRI_NPAR + 1] = s.lnu[i]; lb[EMRI_NPAR + 2] = lY; lb[EMRI_NPAR + 3] = (double)s.partner[i];
-  }
-  if (acc) {
-    for (int q = 0; q < EMRI_NPAR; ++q) s.X[(size_t)k * EMRI_NPAR + q] = s.Y[(size_t)i * EMRI_NPAR + q];
-    s.logL[k] = lY;
-  }
-  if (s.accepted) s.accepted[k] = acc ? 1 : 0;
-}
-
-// ------------------------------------------------------------------ probes
-__global__ void __launch_bounds__(256) fp64_probe_kernel(double* out, int iters, double seed) {
-  double a0 = seed + threadIdx.x, a1 = a0 + 1, a2 = a0 + 2, a3 = a0 + 3, a4 = a0 + 4, a5 = a0 + 5, a6 = a0 + 6, a7 = a0 + 7;
-  const double m = 0.999999, c = 1e-9;
-  for (int i = 0; i < iters; ++i) {
-#pragma unroll
-    for (int r = 0; r < 8; ++r) {
-      a0 = fma(a0, m, c); a1 = fma(a1, m, c); a2 = fma(a2, m, c); a3 = fma(a3, m, c);
-      a4 = fma(a4, m, c); a5 = fma(a5, m, c); a6 = fma(a6, m, c); a7 = fma(a7, m, c);
-    }
-  }
-  double s = a0 + a1 + a2 + a3 + a4 + a5 + a6 + a7;
-  if (s == 123.456) out[0] = s;     // never true; keeps the chain alive
-}
-__global__ void __launch_bounds__(256) hbm_probe_kernel(const double2* in, int64_t n, double* out) {
-  double acc = 0.0;
-  for (int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; i < n; i += (int64_t)gridDim.x * blockDim.x) {
-    double2 v = __ldcs(in + i);
-    acc += v.x + v.y;
-  }
-  if (acc == 123.456) out[0] = acc;
-}
-
-}  // namespace
+#include "common.cuh"
+#include "orbit.cuh"
+#include "synth.cuh"
+#include "loglike.cuh"
+#include "stretch.cuh"
+#include "probe.cuh"
 
 // =================================================================== host side
 struct emri_plan {
@@ -793,6 +49,12 @@ struct emri_plan {
   double* d_ncoef = nullptr;
   int32_t* d_jpl = nullptr;
   int32_t* d_status = nullptr;
+  // multiple-shooting orbit (orbit.cuh): segment records, per-walker mode / tail start / post-plunge row
+  int orbit_mode = 1, seg_L = 0, seg_P = 0;
+  double* d_seg = nullptr;
+  double* d_plrow = nullptr;
+  int32_t* d_mode = nullptr;
+  int32_t* d_pclamp = nullptr;
   uint8_t* d_mterms = nullptr;
   // host-variant staging
   double* d_params = nullptr;
@@ -829,6 +91,20 @@ namespace {
     cufftResult r_ = (call);                            \
     if (r_ != CUFFT_SUCCESS) { p->last_err = (int)r_; return EMRI_ECUFFT; } \
   } while (0)
+
+// EMRI_DEBUG_SYNC=1 in the environment synchronises after every kernel of stage (a) and names the one that failed
+int debug_sync(emri_plan* p, cudaStream_t s, const char* what) {
+  static const bool on = std::getenv("EMRI_DEBUG_SYNC") != nullptr;
+  cudaError_t e = cudaGetLastError();
+  if (e == cudaSuccess && on) e = cudaStreamSynchronize(s);
+  if (e != cudaSuccess) {
+    p->last_err = (int)e;
+    if (on) std::fprintf(stderr, "[emri] %s failed: %s\n", what, cudaGetErrorString(e));
+    return EMRI_ECUDA;
+  }
+  return EMRI_OK;
+}
+#define DBG(what) do { int rc_ = debug_sync(p, s, what); if (rc_) return rc_; } while (0)
 
 template <class T> int dev_alloc(emri_plan* p, T** ptr, size_t count) {
   if (*ptr) { cudaFree(*ptr); *ptr = nullptr; }
@@ -879,6 +155,13 @@ int alloc_workspace(emri_plan* p) {
   p->Nc = (p->N + p->S - 1) / p->S;
   p->Nn = p->Nc + 3;
   if ((rc = dev_alloc(p, &p->d_nodes, (size_t)p->K_max * p->Nn * NODE_STRIDE))) return rc;
+  // segments of the parallel-in-time orbit: L = power of two nearest sqrt(n_steps / 2) (cost ~ P + 2 L steps)
+  const int64_t n_steps = p->Nc + 1;
+  int lg = (int)std::floor(0.5 * std::log2(0.5 * (double)n_steps) + 0.5);
+  if (lg < 2) lg = 2;
+  p->seg_L = 1 << lg;
+  p->seg_P = (int)((n_steps + p->seg_L - 1) / p->seg_L);
+  if ((rc = dev_alloc(p, &p->d_seg, (size_t)p->K_max * p->seg_P * SEG_STRIDE))) return rc;
   return EMRI_OK;
 }
 
@@ -936,7 +219,31 @@ int run_orbit(emri_plan* p, const double* params, int K, cudaStream_t s) {
   a.params = params; a.K = K; a.N = p->N; a.dt = p->dt; a.S = p->S; a.Nc = p->Nc; a.Nn = p->Nn; a.n_max = p->n_max;
   a.tH = kMpcMetre / (p->H0 * 1000.0); a.Om = p->Om;
   a.wc = p->d_wc; a.nodes = p->d_nodes; a.jpl = p->d_jpl; a.status = p->d_status; a.mterms = p->d_mterms;
-  orbit_kernel<<<(K + 31) / 32, 32, 0, s>>>(a);
+  if (p->orbit_mode == 0) {
+    // reference schedule: the whole recursion in one thread per walker
+    orbit_kernel<<<(K + 31) / 32, 32, 0, s>>>(a);
+    CK(cudaGetLastError());
+    return EMRI_OK;
+  }
+  ShootArgs sa;
+  sa.o = a; sa.L = p->seg_L; sa.P = p->seg_P; sa.n_steps = p->Nc + 1;
+  sa.seg = p->d_seg; sa.mode = p->d_mode; sa.pclamp = p->d_pclamp; sa.plrow = p->d_plrow;
+  sa.round = 0; sa.last_round = 0;
+  orbit_init_kernel<<<(K + 31) / 32, 32, 0, s>>>(sa);
+  DBG("orbit_init_kernel");
+  const int n_rounds = 3;
+  for (int r = 0; r < n_rounds; ++r) {
+    sa.round = r; sa.last_round = (r == n_rounds - 1);
+    const int64_t threads = (int64_t)K * sa.P * (r == 0 ? 3 : 1);
+    orbit_sweep_kernel<<<(unsigned)((threads + 63) / 64), 64, 0, s>>>(sa);
+    DBG("orbit_sweep_kernel");
+    orbit_correct_kernel<<<K, 32, (size_t)sa.P * 8 * sizeof(double), s>>>(sa);
+    DBG("orbit_correct_kernel");
+  }
+  orbit_tail_kernel<<<(K + 31) / 32, 32, 0, s>>>(sa);
+  DBG("orbit_tail_kernel");
+  const int64_t per_k = std::max<int64_t>(p->Nn, 64);
+  orbit_fixup_kernel<<<(unsigned)((per_k * K + 127) / 128), 128, 0, s>>>(sa);
   CK(cudaGetLastError());
   return EMRI_OK;
 }
@@ -1012,6 +319,9 @@ int emri_plan_create(emri_plan** out, int64_t N, double dt, int n_max, int K_max
   if ((rc = dev_alloc(p, &p->d_jpl, (size_t)K_max))) return fail(rc);
   if ((rc = dev_alloc(p, &p->d_status, (size_t)K_max))) return fail(rc);
   if ((rc = dev_alloc(p, &p->d_mterms, (size_t)K_max * (EMRI_NMAX_CAP + 1)))) return fail(rc);
+  if ((rc = dev_alloc(p, &p->d_mode, (size_t)K_max))) return fail(rc);
+  if ((rc = dev_alloc(p, &p->d_pclamp, (size_t)K_max))) return fail(rc);
+  if ((rc = dev_alloc(p, &p->d_plrow, (size_t)K_max * NODE_STRIDE))) return fail(rc);
   if ((rc = dev_alloc(p, &p->d_series, series.size()))) return fail(rc);
   if ((rc = dev_alloc(p, &p->d_ncoef, ncoef.size()))) return fail(rc);
   p->n_part = (int)((p->Nf + LL_TILE - 1) / LL_TILE) * LL_WARPS;
@@ -1055,7 +365,7 @@ int emri_plan_destroy(emri_plan* p) {
   for (auto e : p->ev) cudaEventDestroy(e);
   void* ptrs[] = {p->d_w, p->d_wc, p->d_nodes, p->d_hbuf, p->d_partial, p->d_series, p->d_ncoef, p->d_jpl, p->d_status,
                   p->d_mterms, p->d_params, p->d_data, p->d_logL, p->d_Y, p->d_z, p->d_lnu, p->d_logLY, p->d_inbox,
-                  p->d_partner, p->d_fftwork};
+                  p->d_partner, p->d_fftwork, p->d_seg, p->d_plrow, p->d_mode, p->d_pclamp};
   for (void* q : ptrs) if (q) cudaFree(q);
   delete p;
   return EMRI_OK;
@@ -1074,7 +384,21 @@ int emri_plan_set_coarse_stride(emri_plan* p, int S) {
   p->logS = 0;
   while ((1 << p->logS) < S) ++p->logS;
   if (p->d_nodes) p->bytes -= (int64_t)((size_t)p->K_max * p->Nn * NODE_STRIDE * sizeof(double));
+  if (p->d_seg) p->bytes -= (int64_t)((size_t)p->K_max * p->seg_P * SEG_STRIDE * sizeof(double));
   return alloc_workspace(p);
+}
+
+int emri_plan_set_orbit_schedule(emri_plan* p, int schedule) {
+  if (!p || (schedule != 0 && schedule != 1)) return EMRI_EINVAL;
+  p->orbit_mode = schedule;
+  return EMRI_OK;
+}
+
+int emri_plan_orbit_report(emri_plan* p, int K, int32_t* modes) {
+  if (!p || !modes || K < 1 || K > p->K_max) return EMRI_EINVAL;
+  CK(cudaDeviceSynchronize());
+  CK(cudaMemcpy(modes, p->d_mode, (size_t)K * sizeof(int32_t), cudaMemcpyDeviceToHost));
+  return EMRI_OK;
 }
 
 int emri_plan_set_chunk(emri_plan* p, int c) {
@@ -1322,3 +646,4 @@ int emri_probe_hbm_read(int64_t bytes, double* gbs, void* stream) {
 }
 
 }  // extern "C"
+
