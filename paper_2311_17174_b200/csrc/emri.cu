@@ -45,8 +45,8 @@ struct emri_plan {
   double* d_nodes = nullptr;
   double* d_hbuf = nullptr;
   double* d_partial = nullptr;
-  double2* d_series = nullptr;
-  double* d_ncoef = nullptr;
+  double4* d_base = nullptr;      // Taylor coefficients of the harmonic brackets in e^2 (synth.cuh)
+  double2* d_nodeaux = nullptr;
   int32_t* d_jpl = nullptr;
   int32_t* d_status = nullptr;
   // multiple-shooting orbit (orbit.cuh): segment records, per-walker mode / tail start / post-plunge row
@@ -55,7 +55,6 @@ struct emri_plan {
   double* d_plrow = nullptr;
   int32_t* d_mode = nullptr;
   int32_t* d_pclamp = nullptr;
-  uint8_t* d_mterms = nullptr;
   // host-variant staging
   double* d_params = nullptr;
   double* d_data = nullptr;
@@ -115,37 +114,36 @@ template <class T> int dev_alloc(emri_plan* p, T** ptr, size_t count) {
   return EMRI_OK;
 }
 
-// Bessel series and per-harmonic constants, built in long double
-void build_tables(int n_max, std::vector<double2>& series, std::vector<double>& ncoef) {
-  series.assign((size_t)(n_max + 1) * MCAP, make_double2(0.0, 0.0));
-  ncoef.assign((size_t)(n_max + 1) * NCOEF, 0.0);
+// Taylor coefficients in w = e^2 of the three harmonic brackets (synth.cuh), in long double.
+// With J_k(n e) = (n e/2)^k s_k(w), s_k(w) = sum_m sigma(k,m) w^m, sigma(k,m) = (-n^2/4)^m / (m! (m+k)!):
+//   n >= 2:  n [J_{n-2} - 2e J_{n-1} + (2/n) J_n + 2e J_{n+1} - J_{n+2}] = e^{n-2} PA_n(w)   etc.
+//   n == 1:  the same brackets with J_{-1} = -J_1 carry e^{+1}.
+void build_base_table(int n_max, std::vector<double4>& base) {
+  base.assign((size_t)(n_max + 1) * BASE_M, make_double4(0.0, 0.0, 0.0, 0.0));
+  std::vector<long double> fact(2 * BASE_M + EMRI_NMAX_CAP + 8);
+  fact[0] = 1.0L;
+  for (size_t i = 1; i < fact.size(); ++i) fact[i] = fact[i - 1] * (long double)i;
   for (int n = 1; n <= n_max; ++n) {
-    // scaled Bessel function Jhat_k(n e) = sum_m (-n^2/4)^m / (m! (k+1)_m) (e^2)^m, k = n+1 and n+2
-    long double y = -0.25L * n * n;
-    long double c1 = 1.0L, c2 = 1.0L;
-    for (int m = 0; m < MCAP; ++m) {
-      if (m > 0) {
-        c1 *= y / ((long double)m * (long double)(m + n + 1));
-        c2 *= y / ((long double)m * (long double)(m + n + 2));
+    const long double nn = n, y = -0.25L * nn * nn;
+    auto sigma = [&](int k, int m) -> long double {
+      if (m < 0) return 0.0L;
+      return powl(y, (long double)m) / (fact[m] * fact[m + k]);
+    };
+    for (int m = 0; m < BASE_M; ++m) {
+      long double pa, pb, pc;
+      if (n == 1) {
+        pa = 0.5L * sigma(1, m) - 2.0L * sigma(0, m) + 0.5L * sigma(2, m - 1) - 0.125L * sigma(3, m - 1);
+        pb = -1.5L * sigma(1, m) + 0.125L * sigma(3, m - 1);
+        pc = 0.5L * sigma(1, m);
+      } else {
+        const long double pref = powl(0.5L * nn, (long double)(n - 2));          // (n/2)^{n-2}
+        const long double n2 = nn * nn, n3 = n2 * nn, n4 = n2 * n2;
+        pa = nn * pref * (sigma(n - 2, m) - nn * sigma(n - 1, m - 1) + 0.5L * nn * sigma(n, m - 1) +
+                          0.25L * n3 * sigma(n + 1, m - 2) - 0.0625L * n4 * sigma(n + 2, m - 2));
+        pb = nn * pref * (sigma(n - 2, m) - 0.5L * n2 * sigma(n, m - 1) + 0.0625L * n4 * sigma(n + 2, m - 2));
+        pc = pref * 0.25L * n2 * sigma(n, m - 1);
       }
-      series[(size_t)n * MCAP + m] = make_double2((double)c1, (double)c2);
-    }
-    double* kc = &ncoef[(size_t)n * NCOEF];
-    long double nn = n;
-    kc[8] = (double)(nn * nn / (4.0L * (nn + 1) * (nn + 2)));        // J_n     from J_{n+1}, J_{n+2}
-    kc[9] = (double)(nn * nn / (4.0L * nn * (nn + 1)));              // J_{n-1} from J_n, J_{n+1}
-    if (n >= 2) {
-      long double r1 = nn / (2 * (nn - 1)), r2 = nn / (2 * nn), r3 = nn / (2 * (nn + 1)), r4 = nn / (2 * (nn + 2));
-      kc[0] = (double)nn;
-      kc[1] = (double)(-2 * nn * r1);
-      kc[2] = (double)(2 * r1 * r2);
-      kc[3] = (double)(2 * nn * r1 * r2 * r3);
-      kc[4] = (double)(-nn * r1 * r2 * r3 * r4);
-      kc[5] = (double)(-2 * nn * r1 * r2);
-      kc[6] = (double)(nn * r1 * r2 * r3 * r4);
-      kc[7] = (double)(r1 * r2);
-      kc[10] = (double)(nn * nn / (4.0L * (nn - 1) * nn));           // J_{n-2} from J_{n-1}, J_n
-      kc[11] = (double)(0.5L * powl((nn + 1) / nn, (long double)(n - 2)) * (nn + 1) / (nn - 1));   // t'_{n+1}/(e t'_n)
+      base[(size_t)n * BASE_M + m] = make_double4((double)pa, (double)pb, (double)pc, 0.0);
     }
   }
 }
@@ -155,6 +153,7 @@ int alloc_workspace(emri_plan* p) {
   p->Nc = (p->N + p->S - 1) / p->S;
   p->Nn = p->Nc + 3;
   if ((rc = dev_alloc(p, &p->d_nodes, (size_t)p->K_max * p->Nn * NODE_STRIDE))) return rc;
+  if ((rc = dev_alloc(p, &p->d_nodeaux, (size_t)p->K_max * p->Nn))) return rc;
   // segments of the parallel-in-time orbit: L = power of two nearest sqrt(n_steps / 2) (cost ~ P + 2 L steps)
   const int64_t n_steps = p->Nc + 1;
   int lg = (int)std::floor(0.5 * std::log2(0.5 * (double)n_steps) + 0.5);
@@ -218,10 +217,12 @@ int run_orbit(emri_plan* p, const double* params, int K, cudaStream_t s) {
   OrbitArgs a;
   a.params = params; a.K = K; a.N = p->N; a.dt = p->dt; a.S = p->S; a.Nc = p->Nc; a.Nn = p->Nn; a.n_max = p->n_max;
   a.tH = kMpcMetre / (p->H0 * 1000.0); a.Om = p->Om;
-  a.wc = p->d_wc; a.nodes = p->d_nodes; a.jpl = p->d_jpl; a.status = p->d_status; a.mterms = p->d_mterms;
+  a.wc = p->d_wc; a.nodes = p->d_nodes; a.jpl = p->d_jpl; a.status = p->d_status; a.nodeaux = p->d_nodeaux;
+  const unsigned aux_grid = (unsigned)(((int64_t)K * p->Nn + 127) / 128);
   if (p->orbit_mode == 0) {
     // reference schedule: the whole recursion in one thread per walker
     orbit_kernel<<<(K + 31) / 32, 32, 0, s>>>(a);
+    orbit_aux_kernel<<<aux_grid, 128, 0, s>>>(a);
     CK(cudaGetLastError());
     return EMRI_OK;
   }
@@ -242,20 +243,21 @@ int run_orbit(emri_plan* p, const double* params, int K, cudaStream_t s) {
   }
   orbit_tail_kernel<<<(K + 31) / 32, 32, 0, s>>>(sa);
   DBG("orbit_tail_kernel");
-  const int64_t per_k = std::max<int64_t>(p->Nn, 64);
-  orbit_fixup_kernel<<<(unsigned)((per_k * K + 127) / 128), 128, 0, s>>>(sa);
+  orbit_fixup_kernel<<<aux_grid, 128, 0, s>>>(sa);
+  orbit_aux_kernel<<<aux_grid, 128, 0, s>>>(a);
   CK(cudaGetLastError());
   return EMRI_OK;
 }
 
 int run_synth(emri_plan* p, int k0, int K, double* outI, double* outII, int64_t pitch, cudaStream_t s) {
   SynthArgs a;
-  a.wc = p->d_wc; a.nodes = p->d_nodes; a.jpl = p->d_jpl; a.status = p->d_status; a.mterms = p->d_mterms;
-  a.series = p->d_series; a.ncoef = p->d_ncoef;
+  a.wc = p->d_wc; a.nodes = p->d_nodes; a.nodeaux = p->d_nodeaux; a.jpl = p->d_jpl; a.status = p->d_status;
+  a.base = p->d_base; a.tol = 1e-16;
   a.k0 = k0; a.K = K; a.N = p->N; a.dt = p->dt; a.S = p->S; a.logS = p->logS; a.Nn = p->Nn; a.n_max = p->n_max;
   a.outI = outI; a.outII = outII; a.pitch = pitch;
   a.tiles_per_walker = (p->N + TILE - 1) / TILE;
-  int64_t total = (int64_t)K * a.tiles_per_walker;
+  a.units_per_walker = (a.tiles_per_walker + UNIT_TILES - 1) / UNIT_TILES;
+  int64_t total = (int64_t)K * a.units_per_walker;
   int grid = (int)std::min<int64_t>(total, p->synth_grid);
   synth_kernel<<<grid, SYNTH_THREADS, p->synth_smem, s>>>(a);
   CK(cudaGetLastError());
@@ -310,20 +312,17 @@ int emri_plan_create(emri_plan** out, int64_t N, double dt, int n_max, int K_max
   std::vector<double> w((size_t)p->Nf, 0.0);
   if (psd)
     for (int64_t m = 0; m < p->Nf; ++m) w[m] = (psd[m] > 0.0 && std::isfinite(psd[m])) ? 1.0 / psd[m] : 0.0;
-  std::vector<double2> series;
-  std::vector<double> ncoef;
-  build_tables(n_max, series, ncoef);
+  std::vector<double4> base;
+  build_base_table(n_max, base);
 
   if ((rc = dev_alloc(p, &p->d_w, (size_t)p->Nf))) return fail(rc);
   if ((rc = dev_alloc(p, &p->d_wc, (size_t)K_max * WC_STRIDE))) return fail(rc);
   if ((rc = dev_alloc(p, &p->d_jpl, (size_t)K_max))) return fail(rc);
   if ((rc = dev_alloc(p, &p->d_status, (size_t)K_max))) return fail(rc);
-  if ((rc = dev_alloc(p, &p->d_mterms, (size_t)K_max * (EMRI_NMAX_CAP + 1)))) return fail(rc);
   if ((rc = dev_alloc(p, &p->d_mode, (size_t)K_max))) return fail(rc);
   if ((rc = dev_alloc(p, &p->d_pclamp, (size_t)K_max))) return fail(rc);
   if ((rc = dev_alloc(p, &p->d_plrow, (size_t)K_max * NODE_STRIDE))) return fail(rc);
-  if ((rc = dev_alloc(p, &p->d_series, series.size()))) return fail(rc);
-  if ((rc = dev_alloc(p, &p->d_ncoef, ncoef.size()))) return fail(rc);
+  if ((rc = dev_alloc(p, &p->d_base, base.size()))) return fail(rc);
   p->n_part = (int)((p->Nf + LL_TILE - 1) / LL_TILE) * LL_WARPS;
   if ((rc = dev_alloc(p, &p->d_partial, (size_t)K_max * p->n_part))) return fail(rc);
   if ((rc = dev_alloc(p, &p->d_params, (size_t)K_max * EMRI_NPAR))) return fail(rc);
@@ -339,13 +338,12 @@ int emri_plan_create(emri_plan** out, int64_t N, double dt, int n_max, int K_max
   if ((rc = alloc_workspace(p))) return fail(rc);
   if ((rc = alloc_chunk(p))) return fail(rc);
   if (cudaMemcpy(p->d_w, w.data(), w.size() * sizeof(double), cudaMemcpyHostToDevice) != cudaSuccess ||
-      cudaMemcpy(p->d_series, series.data(), series.size() * sizeof(double2), cudaMemcpyHostToDevice) != cudaSuccess ||
-      cudaMemcpy(p->d_ncoef, ncoef.data(), ncoef.size() * sizeof(double), cudaMemcpyHostToDevice) != cudaSuccess)
+      cudaMemcpy(p->d_base, base.data(), base.size() * sizeof(double4), cudaMemcpyHostToDevice) != cudaSuccess)
     return fail(EMRI_ECUDA);
 
   // persistent grid for the synthesis kernel: resident CTAs per SM x SM count
-  p->synth_smem = (size_t)(n_max + 1) * MCAP * sizeof(double2) + (size_t)(n_max + 1) * NCOEF * sizeof(double) +
-                  WC_STRIDE * sizeof(double);
+  p->synth_smem = (size_t)(n_max + 1) * MLOC * sizeof(double4) + (size_t)6 * 2 * SYNTH_THREADS * sizeof(double) +
+                  (WC_STRIDE + 2 * UNIT_TILES + 4) * sizeof(double);
   if (cudaFuncSetAttribute(synth_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)p->synth_smem) != cudaSuccess)
     return fail(EMRI_ECUDA);
   int per_sm = 0;
@@ -363,8 +361,8 @@ int emri_plan_destroy(emri_plan* p) {
   cudaDeviceSynchronize();
   for (auto& kv : p->fft) cufftDestroy(kv.second);
   for (auto e : p->ev) cudaEventDestroy(e);
-  void* ptrs[] = {p->d_w, p->d_wc, p->d_nodes, p->d_hbuf, p->d_partial, p->d_series, p->d_ncoef, p->d_jpl, p->d_status,
-                  p->d_mterms, p->d_params, p->d_data, p->d_logL, p->d_Y, p->d_z, p->d_lnu, p->d_logLY, p->d_inbox,
+  void* ptrs[] = {p->d_w, p->d_wc, p->d_nodes, p->d_hbuf, p->d_partial, p->d_base, p->d_nodeaux, p->d_jpl, p->d_status,
+                  p->d_params, p->d_data, p->d_logL, p->d_Y, p->d_z, p->d_lnu, p->d_logLY, p->d_inbox,
                   p->d_partner, p->d_fftwork, p->d_seg, p->d_plrow, p->d_mode, p->d_pclamp};
   for (void* q : ptrs) if (q) cudaFree(q);
   delete p;
@@ -385,6 +383,7 @@ int emri_plan_set_coarse_stride(emri_plan* p, int S) {
   while ((1 << p->logS) < S) ++p->logS;
   if (p->d_nodes) p->bytes -= (int64_t)((size_t)p->K_max * p->Nn * NODE_STRIDE * sizeof(double));
   if (p->d_seg) p->bytes -= (int64_t)((size_t)p->K_max * p->seg_P * SEG_STRIDE * sizeof(double));
+  if (p->d_nodeaux) p->bytes -= (int64_t)((size_t)p->K_max * p->Nn * sizeof(double2));
   return alloc_workspace(p);
 }
 

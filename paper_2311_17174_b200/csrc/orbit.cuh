@@ -133,7 +133,7 @@ struct OrbitArgs {
   double* nodes;          // [K][Nn][NODE_STRIDE]
   int32_t* jpl;           // [K] first plunged node (index j), Nn if none
   int32_t* status;        // [K]
-  uint8_t* mterms;        // [K][EMRI_NMAX_CAP+1] Bessel series lengths per harmonic
+  double2* nodeaux;       // [K][Nn] {(2 pi M nu_j)^{2/3} mu/(Xi D), 1/nu_j} for the amplitude of stage (b)
 };
 
 DEVINL void store_node(double* row, const double y[5], const double k1[5], const double d[5]) {
@@ -289,18 +289,6 @@ __global__ void __launch_bounds__(32) orbit_kernel(OrbitArgs a) {
   wc[WC_EMAX] = emax;
   a.jpl[k] = jpl;
   a.status[k] = status;
-  // Bessel series lengths: smallest M with prod_{i<=M} y/(i(i+n+1)) < 2^-58, y = (n emax/2)^2
-  uint8_t* mt = a.mterms + (size_t)k * (EMRI_NMAX_CAP + 1);
-  for (int n = 1; n <= a.n_max; ++n) {
-    double yy = 0.25 * n * n * emax * emax, term = 1.0;
-    int M = 1;
-    while (M < MCAP) {
-      term *= yy / ((double)M * (double)(M + n + 1));
-      ++M;                      // M coefficients cover powers 0..M-1; `term` is the size of power M-1
-      if (term < 3.5e-18) break;
-    }
-    mt[n] = (uint8_t)M;
-  }
 }
 
 // ==================================================================== (a1) parallel-in-time evaluation
@@ -320,7 +308,7 @@ __global__ void __launch_bounds__(32) orbit_kernel(OrbitArgs a) {
 //      once more and whatever is still unverified is integrated sequentially by orbit_tail_kernel
 //      from the last verified boundary (so the result never depends on convergence);
 //   5. orbit_fixup_kernel    adds the per-segment angle offsets (prefix sum of the wrapped segment
-//                            totals), writes the post-plunge copies and the Bessel series lengths.
+//                            totals), writes the post-plunge copies.
 // nu and e are carried as Kahan pairs (value, compensation) exactly as in the sequential kernel, so
 // a segment boundary is matched in ~double-double precision.  (DESIGN.md section 6a.)
 constexpr int SEG_STRIDE = 32;
@@ -400,18 +388,6 @@ DEVINL bool state_ok(double p0, double nu, double p2, double e, double p4) {
 
 DEVINL void load_orbit_const(const double* __restrict__ wc, OrbitConst& oc) {
   oc.twoPiMs = wc[WC_TWOPIMS]; oc.Cnu = wc[WC_CNU]; oc.Ce = wc[WC_CE]; oc.a = wc[WC_A]; oc.sp = wc[WC_SP];
-}
-
-// Bessel series lengths of walker k: smallest M with prod_{i<=M} y/(i(i+n+1)) < 2^-58, y = (n emax/2)^2
-DEVINL uint8_t series_terms(int n, double emax) {
-  double yy = 0.25 * n * n * emax * emax, term = 1.0;
-  int M = 1;
-  while (M < MCAP) {
-    term *= yy / ((double)M * (double)(M + n + 1));
-    ++M;
-    if (term < 3.5e-18) break;
-  }
-  return (uint8_t)M;
 }
 
 // ---- 1. per walker: prologue, guard node, coarse sweep
@@ -703,18 +679,14 @@ __global__ void __launch_bounds__(32) orbit_tail_kernel(ShootArgs s) {
   a.wc[(size_t)k * WC_STRIDE + WC_EMAX] = emax;
 }
 
-// ---- 5. node-parallel: global angles, post-plunge copies, zero rows; Bessel series lengths
+// ---- 5. node-parallel: global angles, post-plunge copies, zero rows
 __global__ void __launch_bounds__(128) orbit_fixup_kernel(ShootArgs s) {
   const OrbitArgs& a = s.o;
-  const int64_t per_k = (a.Nn > 64) ? a.Nn : 64;
   const int64_t idx = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
-  if (idx >= per_k * a.K) return;
-  const int k = (int)(idx / per_k);
-  const int64_t m = idx - (int64_t)k * per_k;
+  if (idx >= a.Nn * a.K) return;
+  const int k = (int)(idx / a.Nn);
+  const int64_t m = idx - (int64_t)k * a.Nn;
   const int mode = s.mode[k];
-  if (m >= 1 && m <= a.n_max)
-    a.mterms[(size_t)k * (EMRI_NMAX_CAP + 1) + m] = series_terms((int)m, a.wc[(size_t)k * WC_STRIDE + WC_EMAX]);
-  if (m >= a.Nn) return;
   double2* row = reinterpret_cast<double2*>(a.nodes + ((size_t)k * a.Nn + m) * NODE_STRIDE);
   if (mode == OM_ZERO) {
 #pragma unroll
@@ -740,6 +712,21 @@ __global__ void __launch_bounds__(128) orbit_fixup_kernel(ShootArgs s) {
   v23.x = frac(v23.x + sg[SG_O1]);
   v4.x = frac(v4.x + sg[SG_O2]);
   row[0] = v01; row[1] = v23; row[2] = v4;
+}
+
+// ---- node-parallel (both schedules): per-node amplitude data for stage (b), {(2 pi M nu_j)^{2/3} mu/(Xi D), 1/nu_j}
+__global__ void __launch_bounds__(128) orbit_aux_kernel(OrbitArgs a) {
+  const int64_t idx = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+  if (idx >= a.Nn * a.K) return;
+  const int k = (int)(idx / a.Nn);
+  const double nu = a.nodes[(size_t)idx * NODE_STRIDE + 1];
+  const double* wc = a.wc + (size_t)k * WC_STRIDE;
+  double2 out = make_double2(0.0, 0.0);
+  if (nu > 0.0 && isfinite(nu)) {
+    const double cb = cbrt(wc[WC_TWOPIMS] * nu);
+    out = make_double2(cb * cb * wc[WC_AMP], 1.0 / nu);
+  }
+  a.nodeaux[idx] = out;
 }
 
 }  // namespace

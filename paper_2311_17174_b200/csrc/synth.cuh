@@ -1,19 +1,43 @@
-// synth.cuh -- stage (b): cubic-Hermite orbit, Peters-Mathews harmonic sum (Eq. 2), LISA response, propagation factors (Eqs. 4-6)
+// synth.cuh -- stage (b): cubic-Hermite orbit, Peters-Mathews harmonic sum (Eq. 2), LISA response
+// (PAPER.md:79, :118), propagation factors (Eqs. 4-6).
 // Part of the sm_100a implementation of include/emri.h; included by emri.cu (one translation unit).
+//
+// What is evaluated per (walker, sample) is S4 + S5 of DESIGN.md section 3.  How:
+//
+//  * Harmonic brackets as power series in w = e^2.  With J_k(ne) = (ne/2)^k s_k(w),
+//    s_k(w) = sum_m (-n^2 w/4)^m / (m! (m+k)!), the three brackets of BC Eqs. 7-9 are
+//        n [J_{n-2} - 2e J_{n-1} + (2/n) J_n + 2e J_{n+1} - J_{n+2}] = e^{n-2} PA_n(w)
+//        n [J_{n-2} - 2 J_n + J_{n+2}]                              = e^{n-2} PB_n(w)
+//        J_n                                                        = e^{n-2} PC_n(w)      (n >= 2; n = 1: e^{+1})
+//    with entire functions PA_n, PB_n, PC_n whose Taylor coefficients are tabulated on the host in long double
+//    (build_base_table in emri.cu).  The factor e^{n-2} rides on the rotation that advances cos/sin(n Phi), so one
+//    harmonic costs three Horner evaluations, three accumulations and one scaled rotation.  Well defined at e = 0.
+//  * Per unit (one walker, UNIT_TILES tiles of 256 samples) e^2 moves by ~1e-6, so the CTA first RE-EXPANDS the three
+//    series about the unit's mid-point w0 (Horner shift, orders 0..MLOC-1, in shared memory) and every sample then
+//    evaluates the short local series in x = w - w0.  The number of local orders kept per harmonic is the smallest that
+//    leaves a relative truncation < tol (1e-16); if order MLOC-1 is still significant the unit falls back to the
+//    base series (same loop, global table).  This is a rigorous re-summation, not an interpolation of amplitudes.
+//  * Everything of a sample that does not depend on n (Hermite, geometry, antenna patterns, phases, amplitude) is
+//    folded into six numbers a_I, b_I, c_I, a_II, b_II, c_II with h_alpha = a S_a + b S_b + c S_c, parked in shared
+//    memory during the harmonic loop to keep the loop at few registers.
 #pragma once
 #include "common.cuh"
 
 namespace {
 
-// ------------------------------------------------------------------ (b) synthesis
+constexpr int SYNTH_THREADS = 128;
+constexpr int TILE = 2 * SYNTH_THREADS;   // samples per tile (2 adjacent samples per thread)
+constexpr int UNIT_TILES = 4;             // tiles per unit (one re-expansion per unit)
+constexpr int MLOC = 9;                   // local expansion orders 0..8
+constexpr int BASE_M = 48;                // Taylor coefficients kept per harmonic in the base table
+
 struct SynthArgs {
   const double* wc;
   const double* nodes;
+  const double2* nodeaux;  // [K][Nn] {(2 pi M nu_j)^{2/3} mu/(Xi D), 1/nu_j}
   const int32_t* jpl;
   const int32_t* status;
-  const uint8_t* mterms;
-  const double2* series;   // [n_max+1][MCAP] {coef for order n+1, coef for order n+2} in powers of e^2
-  const double* ncoef;     // [n_max+1][NCOEF]
+  const double4* base;     // [n_max+1][BASE_M] Taylor coefficients {PA, PB, PC, 0} in w = e^2
   int k0, K;               // walkers k0 .. k0+K-1
   int64_t N;
   double dt;
@@ -23,49 +47,56 @@ struct SynthArgs {
   double* outI;            // row of walker k0+i at outI + i*pitch
   double* outII;
   int64_t pitch;
-  int64_t tiles_per_walker;
+  int64_t tiles_per_walker, units_per_walker;
+  double tol;              // relative truncation of the harmonic series
 };
 
-struct Sample {
-  double e2, e4, c1, s1;     // e^2, e^4, cos/sin of Phi_tot
-  double cn, sn;             // cos/sin(n Phi_tot)
-  double Sa, Sb, Sc;
+struct SampleOut {
+  double x, ec, es, C2, S2;     // w - w0;  e cos/sin(Phi_tot);  cos/sin(2 Phi_tot)
 };
 
-// cubic Hermite of the five orbital quantities at fraction s of interval j (node row jj = j+1)
-DEVINL void hermite5(const double* __restrict__ nodes, int64_t jj, double s, double Delta, double out[5]) {
-  const double2* r0 = reinterpret_cast<const double2*>(nodes + jj * NODE_STRIDE);
-  const double2* r1 = r0 + NODE_STRIDE / 2;
-  double2 v01 = __ldg(r0), v23 = __ldg(r0 + 1), v4m0 = __ldg(r0 + 2), m12 = __ldg(r0 + 3), m34 = __ldg(r0 + 4),
-          d01 = __ldg(r0 + 5), d23 = __ldg(r0 + 6), d4 = __ldg(r0 + 7);
-  double2 n4m0 = __ldg(r1 + 2), n12 = __ldg(r1 + 3), n34 = __ldg(r1 + 4);
-  const double s2 = s * s, s3 = s2 * s;
-  const double b = 3.0 * s2 - 2.0 * s3;
-  const double c0 = Delta * (s3 - 2.0 * s2 + s), c1 = Delta * (s3 - s2);
-  out[0] = v01.x + fma(b, d01.x, fma(c0, v4m0.y, c1 * n4m0.y));
-  out[1] = v01.y + fma(b, d01.y, fma(c0, m12.x, c1 * n12.x));
-  out[2] = v23.x + fma(b, d23.x, fma(c0, m12.y, c1 * n12.y));
-  out[3] = v23.y + fma(b, d23.y, fma(c0, m34.x, c1 * n34.x));
-  out[4] = v4m0.x + fma(b, d4.x, fma(c0, m34.y, c1 * n34.y));
-}
-
-struct Projection { double FIp, FIx, FIIp, FIIx, c2g, s2g, sq, A, Ln, e; };
-
-// everything of one sample that does not depend on the harmonic index
-DEVINL void sample_setup(const double* __restrict__ w, const double* __restrict__ nodes, int64_t i, int S, int logS,
-                         double dt, int32_t jpl, bool* live, Sample* sm, Projection* pr) {
+// Everything of sample i that does not depend on the harmonic index.  (cpb, spb) = cos/sin of the detector phase
+// phibar = 2 pi t_i / T_yr.  fin[0..5] (stride fs) receive a_I, b_I, c_I, a_II, b_II, c_II.
+DEVINL void sample_setup(const double* __restrict__ w, const double* __restrict__ nodes, const double2* __restrict__ aux,
+                         int64_t i, int S, int logS, double invS, double Delta, int32_t jpl, double cpb, double spb,
+                         double w0, SampleOut& o, double* __restrict__ fin, int fs) {
   // source-time split (reading D4)
   int64_t j = i >> logS;
-  double s = (double)(i & (S - 1)) * (1.0 / (double)S) - w[WC_SIGMA];
+  double s = (double)(i & (S - 1)) * invS - w[WC_SIGMA];
   if (s < 0.0) { s += 1.0; j -= 1; } else if (s >= 1.0) { s -= 1.0; j += 1; }
-  *live = (j + 1 < (int64_t)jpl);
-  double orb[5];
-  hermite5(nodes, j + 1, s, S * dt, orb);
-  const double Phic = orb[0], nu = orb[1], gamc = orb[2], e = orb[3], alpc = orb[4];
-  double sa, ca, s2gt, c2gt, spb, cpb;
+  const bool live = (j + 1 < (int64_t)jpl);
+  // cubic Hermite of (Phi_c, nu, gam_c, e, alp_c) on interval j (rows j+1, j+2)
+  const double2* r0 = reinterpret_cast<const double2*>(nodes + (j + 1) * NODE_STRIDE);
+  const double2* r1 = r0 + NODE_STRIDE / 2;
+  const double2 v01 = __ldg(r0), v23 = __ldg(r0 + 1), v4m0 = __ldg(r0 + 2), m12 = __ldg(r0 + 3), m34 = __ldg(r0 + 4),
+                d01 = __ldg(r0 + 5), d23 = __ldg(r0 + 6), d4 = __ldg(r0 + 7);
+  const double2 n4m0 = __ldg(r1 + 2), n12 = __ldg(r1 + 3), n34 = __ldg(r1 + 4);
+  const double2 ax = __ldg(aux + (j + 1));
+  const double s2 = s * s, s3 = s2 * s;
+  const double hb = fma(-2.0, s3, 3.0 * s2);
+  const double h0 = Delta * (s3 - 2.0 * s2 + s), h1 = Delta * (s3 - s2);
+  const double Phic = v01.x + fma(hb, d01.x, fma(h0, v4m0.y, h1 * n4m0.y));
+  const double dnu = fma(hb, d01.y, fma(h0, m12.x, h1 * n12.x));
+  const double nu = v01.y + dnu;
+  const double gamc = v23.x + fma(hb, d23.x, fma(h0, m12.y, h1 * n12.y));
+  const double e = v23.y + fma(hb, d23.y, fma(h0, m34.x, h1 * n34.x));
+  const double alpc = v4m0.x + fma(hb, d4.x, fma(h0, m34.y, h1 * n34.y));
+  // amplitude A = (2 pi M nu)^{2/3} mu / (Xi D)  (BC 10 with Eqs. 4-6 folded in): Taylor of (1+d)^{2/3} about the
+  // node value, d = (nu - nu_j)/nu_j; remainder 0.014 d^6 < 6e-17 for |d| <= 4e-3, else the cube root itself
+  double A;
+  {
+    const double d = dnu * ax.y;
+    if (fabs(d) <= 4e-3) {
+      const double p = fma(d, fma(d, fma(d, fma(d, 14.0 / 729.0, -7.0 / 243.0), 4.0 / 81.0), -1.0 / 9.0), 2.0 / 3.0);
+      A = fma(ax.x * d, p, ax.x);
+    } else {
+      const double cb = cbrt(w[WC_TWOPIMS] * nu);
+      A = cb * cb * w[WC_AMP];
+    }
+  }
+  double sa, ca, s2gt, c2gt;
   sincospi(2.0 * alpc, &sa, &ca);
   sincospi(4.0 * gamc, &s2gt, &c2gt);
-  sincospi(2.0 * frac(((double)i * dt) / kYearSec), &spb, &cpb);
   // orbital-plane normal and its projections (BC 19-21)
   const double Lx = fma(w[WC_A2X], sa, fma(w[WC_A1X], ca, w[WC_A0X]));
   const double Ly = fma(w[WC_A2Y], sa, fma(w[WC_A1Y], ca, w[WC_A0Y]));
@@ -75,7 +106,7 @@ DEVINL void sample_setup(const double* __restrict__ w, const double* __restrict_
   const double Ns = fma(w[WC_CL], Ln, -w[WC_SN]);
   const double Nc = fma(w[WC_B2], sa, w[WC_B1] * ca);
   const double den_b = fma(Nc, Nc, Ns * Ns);
-  // detector time quantities
+  // detector-time quantities (BC 17-18)
   const double cphS = w[WC_CPHS], sphS = w[WC_SPHS], cS = w[WC_CS], sS = w[WC_SS];
   const double cd = fma(cpb, cphS, spb * sphS), sd = fma(spb, cphS, -cpb * sphS);
   const double cthd = fma(-kHalfSqrt3 * sS, cd, 0.5 * cS);
@@ -88,9 +119,7 @@ DEVINL void sample_setup(const double* __restrict__ w, const double* __restrict_
   // one division for the three normalisations
   const double bp = den_b * den_p;
   const double inv = 1.0 / (bp * den_a);
-  const double ib = (den_b > 0.0) ? inv * (den_a * den_p) : 0.0;
-  const double ia = inv * bp;
-  const double ip = (den_p > 0.0) ? inv * (den_a * den_b) : 0.0;
+  const double ib = inv * (den_a * den_p), ia = inv * bp, ip = inv * (den_a * den_b);
   double c2b = fma(Nc, Nc, -Ns * Ns) * ib, s2b = 2.0 * Ns * Nc * ib;
   if (!(den_b > 0.0)) { c2b = 1.0; s2b = 0.0; }                     // reading R16: beta = 0
   const double c2a = fma(Qq, Qq, -Pq * Pq) * ia, s2a = 2.0 * Pq * Qq * ia;
@@ -100,139 +129,229 @@ DEVINL void sample_setup(const double* __restrict__ w, const double* __restrict_
   const double c2pb = fma(cpb, cpb, -spb * spb), s2pb = 2.0 * cpb * spb;
   const double c2p = fma(c2pb, c2a, -s2pb * s2a), s2p = fma(s2pb, c2a, c2pb * s2a);
   const double hh = 0.5 * fma(cthd, cthd, 1.0);
-  pr->FIp = fma(hh * c2p, c2s, -cthd * s2p * s2s);
-  pr->FIx = fma(hh * c2p, s2s, cthd * s2p * c2s);
-  pr->FIIp = fma(hh * s2p, c2s, cthd * c2p * s2s);
-  pr->FIIx = fma(hh * s2p, s2s, -cthd * c2p * c2s);
-  // amplitude A = (2 pi M nu)^{2/3} mu / (Xi D)   (BC 10 with Eqs. 4-6 folded in)
-  const double cb = cbrt(w[WC_TWOPIMS] * nu);
-  pr->A = cb * cb * w[WC_AMP];
-  pr->Ln = Ln;
-  pr->sq = sqrt(fma(-e, e, 1.0));
-  pr->c2g = c2g; pr->s2g = s2g; pr->e = e;
+  // antenna patterns (BC 15-16)
+  const double FIp = fma(hh * c2p, c2s, -cthd * s2p * s2s);
+  const double FIx = fma(hh * c2p, s2s, cthd * s2p * c2s);
+  const double FIIp = fma(hh * s2p, c2s, cthd * c2p * s2s);
+  const double FIIx = fma(hh * s2p, s2s, -cthd * c2p * c2s);
+  // h_alpha = (sqrt3/2)(F+ A+ + Fx Ax) with A+ = A{(1+Ln^2)(c2g Sa - s2g sq Sb) + 2(1-Ln^2) Sc},
+  // Ax = -2 A Ln (sq Sb c2g + Sa s2g)   (BC 7-9, 14 summed over n)  =>  h = a Sa + b Sb + c Sc
+  const double sq = sqrt(fma(-e, e, 1.0));
+  const double kA = live ? kHalfSqrt3 * A : 0.0;
+  const double Ln2 = Ln * Ln;
+  const double P1 = kA * (1.0 + Ln2), P2 = 2.0 * kA * Ln, P3 = 2.0 * kA * (1.0 - Ln2);
+  const double t1 = P1 * c2g, t2 = P2 * s2g, t3 = P1 * s2g, t4 = P2 * c2g;
+  fin[0 * fs] = fma(FIp, t1, -FIx * t2);
+  fin[1 * fs] = -sq * fma(FIp, t3, FIx * t4);
+  fin[2 * fs] = FIp * P3;
+  fin[3 * fs] = fma(FIIp, t1, -FIIx * t2);
+  fin[4 * fs] = -sq * fma(FIIp, t3, FIIx * t4);
+  fin[5 * fs] = FIIp * P3;
   // Doppler-shifted phase in cycles (BC 25)
   const double Phit = frac(fma(nu * w[WC_DOP], cd, Phic));
-  sincospi(2.0 * Phit, &sm->s1, &sm->c1);
-  sm->e2 = e * e;
-  sm->e4 = sm->e2 * sm->e2;
-  sm->cn = sm->c1; sm->sn = sm->s1;
-  sm->Sa = 0.0; sm->Sb = 0.0; sm->Sc = 0.0;
+  double s1, c1;
+  sincospi(2.0 * Phit, &s1, &c1);
+  o.x = fma(e, e, -w0);
+  o.ec = e * c1; o.es = e * s1;
+  o.C2 = fma(c1, c1, -s1 * s1); o.S2 = 2.0 * s1 * c1;
 }
 
-DEVINL void sample_finish(const Sample& sm, const Projection& pr, bool live, double* hI, double* hII) {
-  const double Ln2 = pr.Ln * pr.Ln;
-  const double sb = pr.sq * sm.Sb;
-  // A+ = A {(1+Ln^2)(c2g Sa - s2g sq Sb) + 2 (1-Ln^2) Sc},  Ax = -2 A Ln (sq Sb c2g + Sa s2g)   (BC 7-9 summed over n)
-  const double Ap = pr.A * fma(1.0 + Ln2, fma(pr.c2g, sm.Sa, -pr.s2g * sb), 2.0 * (1.0 - Ln2) * sm.Sc);
-  const double Ax = -2.0 * pr.A * pr.Ln * fma(sb, pr.c2g, sm.Sa * pr.s2g);
-  *hI = live ? kHalfSqrt3 * fma(pr.FIp, Ap, pr.FIx * Ax) : 0.0;
-  *hII = live ? kHalfSqrt3 * fma(pr.FIIp, Ap, pr.FIIx * Ax) : 0.0;
+DEVINL double4 ldg4(const double4* p) {
+  const double2* q = reinterpret_cast<const double2*>(p);
+  const double2 lo = __ldg(q), hi = __ldg(q + 1);
+  return make_double4(lo.x, lo.y, hi.x, hi.y);
+}
+
+// Horner evaluation of the three series of one harmonic for the thread's two samples (coefficients are warp-uniform)
+template <bool kLocal>
+DEVINL void series3(const double4* __restrict__ tab, int M, double xa, double xb, double& pa_a, double& pb_a, double& pc_a,
+                    double& pa_b, double& pb_b, double& pc_b) {
+  double4 c = kLocal ? tab[M - 1] : ldg4(tab + (M - 1));
+  pa_a = c.x; pb_a = c.y; pc_a = c.z;
+  pa_b = c.x; pb_b = c.y; pc_b = c.z;
+#pragma unroll 4
+  for (int m = M - 2; m >= 0; --m) {
+    c = kLocal ? tab[m] : ldg4(tab + m);
+    pa_a = fma(pa_a, xa, c.x); pb_a = fma(pb_a, xa, c.y); pc_a = fma(pc_a, xa, c.z);
+    pa_b = fma(pa_b, xb, c.x); pb_b = fma(pb_b, xb, c.y); pc_b = fma(pc_b, xb, c.z);
+  }
+}
+
+// harmonic sum n = 1..n_max for two samples; returns S_a, S_b, S_c of each
+template <bool kLocal>
+DEVINL void harmonic_sum(const double4* __restrict__ tab, int tab_stride, const int* __restrict__ Mn, int n_max,
+                         const SampleOut& A, const SampleOut& B, double out[6]) {
+  double pa_a, pb_a, pc_a, pa_b, pb_b, pc_b;
+  // n = 1: carrier e (cos, sin)(Phi)
+  series3<kLocal>(tab + tab_stride, Mn[1], A.x, B.x, pa_a, pb_a, pc_a, pa_b, pb_b, pc_b);
+  double SaA = pa_a * A.ec, SbA = pb_a * A.es, ScA = pc_a * A.ec;
+  double SaB = pa_b * B.ec, SbB = pb_b * B.es, ScB = pc_b * B.ec;
+  // n >= 2: carrier e^{n-2} (cos, sin)(n Phi), advanced by the scaled rotation (e cos Phi, e sin Phi)
+  double CA = A.C2, SA = A.S2, CB = B.C2, SB = B.S2;
+  for (int n = 2; n <= n_max; ++n) {
+    series3<kLocal>(tab + (size_t)n * tab_stride, Mn[n], A.x, B.x, pa_a, pb_a, pc_a, pa_b, pb_b, pc_b);
+    SaA = fma(pa_a, CA, SaA); SbA = fma(pb_a, SA, SbA); ScA = fma(pc_a, CA, ScA);
+    SaB = fma(pa_b, CB, SaB); SbB = fma(pb_b, SB, SbB); ScB = fma(pc_b, CB, ScB);
+    const double ta = CA, tb = CB;
+    CA = fma(CA, A.ec, -SA * A.es); SA = fma(SA, A.ec, ta * A.es);
+    CB = fma(CB, B.ec, -SB * B.es); SB = fma(SB, B.ec, tb * B.es);
+  }
+  out[0] = SaA; out[1] = SbA; out[2] = ScA; out[3] = SaB; out[4] = SbB; out[5] = ScB;
+}
+
+DEVINL double block_max(double v, double* s_red, int warp, int lane) {
+#pragma unroll
+  for (int off = 16; off > 0; off >>= 1) v = fmax(v, __shfl_xor_sync(0xffffffffu, v, off));
+  __syncthreads();
+  if (lane == 0) s_red[warp] = v;
+  __syncthreads();
+  return fmax(fmax(s_red[0], s_red[1]), fmax(s_red[2], s_red[3]));
 }
 
 __global__ void __launch_bounds__(SYNTH_THREADS, 4) synth_kernel(SynthArgs a) {
   extern __shared__ __align__(16) unsigned char smem_raw[];
-  double2* s_series = reinterpret_cast<double2*>(smem_raw);                         // [(n_max+1)*MCAP]
-  double* s_ncoef = reinterpret_cast<double*>(s_series + (size_t)(a.n_max + 1) * MCAP);   // [(n_max+1)*NCOEF]
-  double* s_wc = s_ncoef + (size_t)(a.n_max + 1) * NCOEF;                           // [WC_STRIDE]
-  __shared__ uint8_t s_mt[EMRI_NMAX_CAP + 1];
+  double4* s_tab = reinterpret_cast<double4*>(smem_raw);                               // [(n_max+1)][MLOC]
+  double* s_fin = reinterpret_cast<double*>(s_tab + (size_t)(a.n_max + 1) * MLOC);     // [6][2][SYNTH_THREADS]
+  double* s_wc = s_fin + 6 * 2 * SYNTH_THREADS;                                        // [WC_STRIDE]
+  double* s_rot = s_wc + WC_STRIDE;                                                    // [UNIT_TILES][2] + [4] scratch
+  __shared__ int s_M[EMRI_NMAX_CAP + 1];      // local orders kept per harmonic
+  __shared__ int s_Mb[EMRI_NMAX_CAP + 1];     // base-series terms per harmonic (fallback path)
+  __shared__ int s_fallback;
+  __shared__ double s_red[4];
 
-  for (int i = threadIdx.x; i < (a.n_max + 1) * MCAP; i += blockDim.x) s_series[i] = a.series[i];
-  for (int i = threadIdx.x; i < (a.n_max + 1) * NCOEF; i += blockDim.x) s_ncoef[i] = a.ncoef[i];
+  const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
+  const double Delta = a.S * a.dt, invS = 1.0 / (double)a.S;
+  const double inv_year = 1.0 / kYearSec;
+  // detector phase of the thread's first sample relative to the tile start, and of one sample step
+  double so, co, s1s, c1s;
+  sincospi(2.0 * ((double)(2 * tid) * a.dt * inv_year), &so, &co);
+  sincospi(2.0 * (a.dt * inv_year), &s1s, &c1s);
 
-  const int64_t total = (int64_t)a.K * a.tiles_per_walker;
+  const int64_t total = (int64_t)a.K * a.units_per_walker;
   int cur_k = -1;
-  for (int64_t t = blockIdx.x; t < total; t += gridDim.x) {
-    const int kl = (int)(t / a.tiles_per_walker);
-    const int64_t tile = t - (int64_t)kl * a.tiles_per_walker;
+  for (int64_t u = blockIdx.x; u < total; u += gridDim.x) {
+    const int kl = (int)(u / a.units_per_walker);
+    const int64_t ug = u - (int64_t)kl * a.units_per_walker;
     const int k = a.k0 + kl;
+    const int64_t tile0 = ug * UNIT_TILES;
+    const int64_t i_begin = tile0 * TILE;
+    const int64_t i_end = min(a.N, i_begin + (int64_t)UNIT_TILES * TILE);     // exclusive
+    const double* nodes = a.nodes + (size_t)k * a.Nn * NODE_STRIDE;
+    const double2* aux = a.nodeaux + (size_t)k * a.Nn;
+    __syncthreads();                      // the previous unit is done with the shared tables
     if (k != cur_k) {
-      __syncthreads();
-      if (threadIdx.x < WC_STRIDE) s_wc[threadIdx.x] = a.wc[(size_t)k * WC_STRIDE + threadIdx.x];
-      if (threadIdx.x <= EMRI_NMAX_CAP) s_mt[threadIdx.x] = a.mterms[(size_t)k * (EMRI_NMAX_CAP + 1) + threadIdx.x];
+      if (tid < WC_STRIDE) s_wc[tid] = a.wc[(size_t)k * WC_STRIDE + tid];
       cur_k = k;
-      __syncthreads();
     }
-    const int64_t i0 = tile * TILE + 2 * threadIdx.x;
-    if (i0 >= a.N) continue;
-    double* oI = a.outI + (size_t)kl * a.pitch + i0;
-    double* oII = a.outII + (size_t)kl * a.pitch + i0;
+    if (tid <= a.n_max) { s_M[tid] = 1; s_Mb[tid] = 1; }
+    if (tid == 0) s_fallback = 0;
     const int32_t st = a.status[k];
     if (st & (EMRI_ST_BADPARAM | EMRI_ST_DELAY | EMRI_ST_STATE)) {
-      *reinterpret_cast<double2*>(oI) = make_double2(0.0, 0.0);
-      *reinterpret_cast<double2*>(oII) = make_double2(0.0, 0.0);
+      for (int64_t i0 = i_begin + 2 * tid; i0 < i_end; i0 += TILE) {
+        *reinterpret_cast<double2*>(a.outI + (size_t)kl * a.pitch + i0) = make_double2(0.0, 0.0);
+        *reinterpret_cast<double2*>(a.outII + (size_t)kl * a.pitch + i0) = make_double2(0.0, 0.0);
+      }
       continue;
     }
-    const double* nodes = a.nodes + (size_t)k * a.Nn * NODE_STRIDE;
-    const int32_t jpl = a.jpl[k];
-    Sample A, B;
-    Projection pa, pb;
-    bool la, lb;
-    sample_setup(s_wc, nodes, i0, a.S, a.logS, a.dt, jpl, &la, &A, &pa);
-    sample_setup(s_wc, nodes, i0 + 1, a.S, a.logS, a.dt, jpl, &lb, &B, &pb);
-
-    // ---- harmonic n = 1 (brackets odd in e; J_{-1} = -J_1)
+    // ---- range of e over the unit from the node rows it touches (Hermite stays within pad of the nodes)
+    double w0, xmax, whi;
     {
-      const int M = s_mt[1];
-      const double2* tab = s_series + MCAP;
-      double2 c = tab[M - 1];
-      double j2a = c.x, j3a = c.y, j2b = c.x, j3b = c.y;     // scaled J_2, J_3
-      for (int m = M - 2; m >= 0; --m) {
-        c = tab[m];
-        j2a = fma(j2a, A.e2, c.x); j3a = fma(j3a, A.e2, c.y);
-        j2b = fma(j2b, B.e2, c.x); j3b = fma(j3b, B.e2, c.y);
+      int64_t rlo = (i_begin >> a.logS) - 1 + 1, rhi = ((i_end - 1) >> a.logS) + 2 + 1;       // rows = node index + 1
+      if (rlo < 0) rlo = 0;
+      if (rhi > a.Nn - 1) rhi = a.Nn - 1;
+      double emx = 0.0, emn_neg = -1.0, slp = 0.0, inc = 0.0;
+      for (int64_t r = rlo + tid; r <= rhi; r += SYNTH_THREADS) {
+        const double* row = nodes + r * NODE_STRIDE;
+        const double ev = __ldg(row + 3);
+        emx = fmax(emx, ev); emn_neg = fmax(emn_neg, -ev);
+        slp = fmax(slp, fabs(__ldg(row + 8))); inc = fmax(inc, fabs(__ldg(row + 13)));
       }
-      const double* kc = s_ncoef + NCOEF;
-#pragma unroll
-      for (int h = 0; h < 2; ++h) {
-        Sample& s = h ? B : A;
-        const double e = h ? pb.e : pa.e;
-        const double j2 = h ? j2b : j2a, j3 = h ? j3b : j3a;
-        const double j1 = fma(-s.e2 * kc[8], j3, j2);
-        const double j0 = fma(-s.e2 * kc[9], j2, j1);
-        const double ba = fma(s.e2, fma(-1.0 / 48.0, j3, 0.25 * j2), fma(0.5, j1, -2.0 * j0));
-        const double bb = fma(s.e2 * (1.0 / 48.0), j3, -1.5 * j1);
-        const double tc = e * s.cn, ts = e * s.sn;
-        s.Sa = ba * tc; s.Sb = bb * ts; s.Sc = 0.5 * j1 * tc;
-        const double cn = fma(s.cn, s.c1, -s.sn * s.s1), sn = fma(s.sn, s.c1, s.cn * s.s1);
-        s.cn = cn; s.sn = sn;
-      }
+      emx = block_max(emx, s_red, warp, lane);
+      emn_neg = block_max(emn_neg, s_red, warp, lane);
+      slp = block_max(slp, s_red, warp, lane);
+      inc = block_max(inc, s_red, warp, lane);
+      const double pad = 0.3 * fma(Delta, slp, inc) + 1e-15;
+      const double elo = fmax(-emn_neg - pad, 0.0), ehi = emx + pad;
+      whi = ehi * ehi;
+      w0 = 0.5 * fma(elo, elo, whi);
+      xmax = 0.5 * (whi - elo * elo) * (1.0 + 1e-9);
     }
-    // ---- harmonics n = 2 .. n_max
-    double ta = 1.0, tb = 1.0;     // t'_n = (n e/2)^{n-2}/(n-2)!
-    for (int n = 2; n <= a.n_max; ++n) {
-      const int M = s_mt[n];
-      const double2* tab = s_series + n * MCAP;
-      double2 c = tab[M - 1];
-      double p1a = c.x, p2a = c.y, p1b = c.x, p2b = c.y;     // scaled J_{n+1}, J_{n+2}
-      for (int m = M - 2; m >= 0; --m) {
-        c = tab[m];
-        p1a = fma(p1a, A.e2, c.x); p2a = fma(p2a, A.e2, c.y);
-        p1b = fma(p1b, B.e2, c.x); p2b = fma(p2b, B.e2, c.y);
+    // ---- re-expansion of the three series of every harmonic about w0 (thread = (harmonic, series))
+    for (int task = tid; task < 3 * a.n_max; task += SYNTH_THREADS) {
+      const int n = task / 3 + 1, si = task - 3 * (n - 1);
+      const double* bp = reinterpret_cast<const double*>(a.base + (size_t)n * BASE_M) + si;
+      // base terms that matter at w <= whi (terms rise, then fall: the running maximum is a safe scale)
+      int Mb = 1;
+      {
+        double pw = 1.0, mx = 0.0;
+        for (int m = 0; m < BASE_M; ++m) {
+          const double t = fabs(__ldg(bp + 4 * m)) * pw;
+          mx = fmax(mx, t);
+          if (t >= a.tol * mx && t > 0.0) Mb = m + 1;
+          pw *= whi;
+        }
       }
-      const double* kc = s_ncoef + n * NCOEF;
+      double d[MLOC];
 #pragma unroll
-      for (int h = 0; h < 2; ++h) {
-        Sample& s = h ? B : A;
-        const double p1 = h ? p1b : p1a, p2 = h ? p2b : p2a;
-        double& t = h ? tb : ta;
-        const double j0 = fma(-s.e2 * kc[8], p2, p1);        // scaled J_n
-        const double jm1 = fma(-s.e2 * kc[9], p1, j0);       // scaled J_{n-1}
-        const double jm2 = fma(-s.e2 * kc[10], j0, jm1);     // scaled J_{n-2}
-        const double ba = fma(s.e4, fma(kc[4], p2, kc[3] * p1), fma(s.e2, fma(kc[2], j0, kc[1] * jm1), kc[0] * jm2));
-        const double bb = fma(s.e4 * kc[6], p2, fma(s.e2 * kc[5], j0, kc[0] * jm2));
-        const double bc = s.e2 * kc[7] * j0;
-        const double tc = t * s.cn, ts = t * s.sn;
-        s.Sa = fma(ba, tc, s.Sa); s.Sb = fma(bb, ts, s.Sb); s.Sc = fma(bc, tc, s.Sc);
-        const double cn = fma(s.cn, s.c1, -s.sn * s.s1), sn = fma(s.sn, s.c1, s.cn * s.s1);
-        s.cn = cn; s.sn = sn;
-        t *= (h ? pb.e : pa.e) * kc[11];
+      for (int j = 0; j < MLOC; ++j) d[j] = 0.0;
+      for (int m = Mb - 1; m >= 0; --m) {
+        const double c = __ldg(bp + 4 * m);
+#pragma unroll
+        for (int j = MLOC - 1; j >= 1; --j) d[j] = fma(d[j], w0, d[j - 1]);
+        d[0] = fma(d[0], w0, c);
       }
+      int Ml = 1;
+      {
+        double pw = 1.0, mx = 0.0;
+#pragma unroll
+        for (int j = 0; j < MLOC; ++j) {
+          const double t = fabs(d[j]) * pw;
+          mx = fmax(mx, t);
+          if (t >= a.tol * mx && t > 0.0) Ml = j + 1;
+          pw *= xmax;
+        }
+      }
+      double* dst = reinterpret_cast<double*>(s_tab + (size_t)n * MLOC) + si;
+#pragma unroll
+      for (int j = 0; j < MLOC; ++j) dst[4 * j] = d[j];
+      atomicMax(&s_M[n], Ml);
+      atomicMax(&s_Mb[n], Mb);
+      if (Ml == MLOC) s_fallback = 1;          // order MLOC-1 still significant: the tail is not bounded
     }
-    double hIa, hIIa, hIb, hIIb;
-    sample_finish(A, pa, la, &hIa, &hIIa);
-    sample_finish(B, pb, lb, &hIb, &hIIb);
-    *reinterpret_cast<double2*>(oI) = make_double2(hIa, hIb);
-    *reinterpret_cast<double2*>(oII) = make_double2(hIIa, hIIb);
+    if (tid >= SYNTH_THREADS - UNIT_TILES) {
+      // detector phase at the start of each tile of the unit
+      const int t = tid - (SYNTH_THREADS - UNIT_TILES);
+      double sb, cb;
+      sincospi(2.0 * frac((double)(i_begin + (int64_t)t * TILE) * a.dt * inv_year), &sb, &cb);
+      s_rot[2 * t] = cb; s_rot[2 * t + 1] = sb;
+    }
+    __syncthreads();
+    const bool fallback = s_fallback != 0;
+    const double w0e = fallback ? 0.0 : w0;
+    const int32_t jpl = a.jpl[k];
+    for (int t = 0; t < UNIT_TILES; ++t) {
+      const int64_t i0 = i_begin + (int64_t)t * TILE + 2 * tid;
+      if (i0 >= i_end) break;
+      // detector phase: tile start (x) thread offset, then one sample step
+      const double cb = s_rot[2 * t], sb = s_rot[2 * t + 1];
+      const double cpa = fma(cb, co, -sb * so), spa = fma(sb, co, cb * so);
+      const double cpb2 = fma(cpa, c1s, -spa * s1s), spb2 = fma(spa, c1s, cpa * s1s);
+      SampleOut A, B;
+      double* fin = s_fin + tid;
+      sample_setup(s_wc, nodes, aux, i0, a.S, a.logS, invS, Delta, jpl, cpa, spa, w0e, A, fin, 2 * SYNTH_THREADS);
+      sample_setup(s_wc, nodes, aux, i0 + 1, a.S, a.logS, invS, Delta, jpl, cpb2, spb2, w0e, B, fin + SYNTH_THREADS,
+                   2 * SYNTH_THREADS);
+      double S[6];
+      if (!fallback) harmonic_sum<true>(s_tab, MLOC, s_M, a.n_max, A, B, S);
+      else harmonic_sum<false>(a.base, BASE_M, s_Mb, a.n_max, A, B, S);
+      const double hIa = fma(fin[0], S[0], fma(fin[2 * SYNTH_THREADS], S[1], fin[4 * SYNTH_THREADS] * S[2]));
+      const double hIIa = fma(fin[6 * SYNTH_THREADS], S[0], fma(fin[8 * SYNTH_THREADS], S[1], fin[10 * SYNTH_THREADS] * S[2]));
+      const double* fb = fin + SYNTH_THREADS;
+      const double hIb = fma(fb[0], S[3], fma(fb[2 * SYNTH_THREADS], S[4], fb[4 * SYNTH_THREADS] * S[5]));
+      const double hIIb = fma(fb[6 * SYNTH_THREADS], S[3], fma(fb[8 * SYNTH_THREADS], S[4], fb[10 * SYNTH_THREADS] * S[5]));
+      *reinterpret_cast<double2*>(a.outI + (size_t)kl * a.pitch + i0) = make_double2(hIa, hIb);
+      *reinterpret_cast<double2*>(a.outII + (size_t)kl * a.pitch + i0) = make_double2(hIIa, hIIb);
+    }
   }
 }
 
