@@ -22,10 +22,6 @@ constexpr double kHalfSqrt3 = 0.86602540378443864676;
 
 constexpr int NODE_STRIDE = 16;   // doubles per coarse node: 5 values, 5 slopes, 5 increments, 1 spare
 constexpr int WC_STRIDE = 48;     // doubles of per-walker constants
-constexpr int LL_THREADS = 256;
-constexpr int LL_BINS_PER_THREAD = 4;
-constexpr int LL_TILE = LL_THREADS * LL_BINS_PER_THREAD;
-constexpr int LL_WARPS = LL_THREADS / 32;
 
 // per-walker constant block
 enum {

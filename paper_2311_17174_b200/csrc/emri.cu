@@ -50,7 +50,7 @@ struct emri_plan {
   int32_t* d_jpl = nullptr;
   int32_t* d_status = nullptr;
   // multiple-shooting orbit (orbit.cuh): segment records, per-walker mode / tail start / post-plunge row
-  int orbit_mode = 1, seg_L = 0, seg_P = 0;
+  int orbit_mode = 1, seg_L = 0, seg_P = 0, unit_tiles_override = 0;
   double* d_seg = nullptr;
   double* d_plrow = nullptr;
   int32_t* d_mode = nullptr;
@@ -166,7 +166,7 @@ int alloc_workspace(emri_plan* p) {
 
 int alloc_chunk(emri_plan* p) {
   int rc;
-  if ((rc = dev_alloc(p, &p->d_hbuf, (size_t)2 * p->chunk * (p->N + 2)))) return rc;
+  if ((rc = dev_alloc(p, &p->d_hbuf, (size_t)2 * p->chunk * p->N))) return rc;      // z = h_I + i h_II, [chunk][N] complex
   for (auto& kv : p->fft) cufftDestroy(kv.second);
   p->fft.clear();
   return EMRI_OK;
@@ -179,10 +179,11 @@ int get_fft(emri_plan* p, int batch, cufftHandle* out) {
   CKF(cufftCreate(&h));
   CKF(cufftSetAutoAllocation(h, 0));
   long long n[1] = {(long long)p->N};
-  long long inembed[1] = {(long long)p->N + 2}, onembed[1] = {(long long)p->N / 2 + 1};
+  long long embed[1] = {(long long)p->N};
   size_t ws = 0;
-  cufftResult r = cufftMakePlanMany64(h, 1, n, inembed, 1, (long long)p->N + 2, onembed, 1, (long long)p->N / 2 + 1,
-                                      CUFFT_D2Z, (long long)batch, &ws);
+  // one complex transform per walker carries both real channels (loglike.cuh)
+  cufftResult r = cufftMakePlanMany64(h, 1, n, embed, 1, (long long)p->N, embed, 1, (long long)p->N, CUFFT_Z2Z,
+                                      (long long)batch, &ws);
   if (r != CUFFT_SUCCESS) { p->last_err = (int)r; cufftDestroy(h); return EMRI_ECUFFT; }
   if (ws > p->fftwork_bytes) {
     // grow the shared work area; every cached plan is re-pointed at it
@@ -249,14 +250,19 @@ int run_orbit(emri_plan* p, const double* params, int K, cudaStream_t s) {
   return EMRI_OK;
 }
 
-int run_synth(emri_plan* p, int k0, int K, double* outI, double* outII, int64_t pitch, cudaStream_t s) {
+int run_synth(emri_plan* p, int k0, int K, double* outI, double* outII, int64_t pitch, double* outZ, cudaStream_t s) {
   SynthArgs a;
   a.wc = p->d_wc; a.nodes = p->d_nodes; a.nodeaux = p->d_nodeaux; a.jpl = p->d_jpl; a.status = p->d_status;
   a.base = p->d_base; a.tol = 1e-16;
   a.k0 = k0; a.K = K; a.N = p->N; a.dt = p->dt; a.S = p->S; a.logS = p->logS; a.Nn = p->Nn; a.n_max = p->n_max;
-  a.outI = outI; a.outII = outII; a.pitch = pitch;
+  a.outI = outI; a.outII = outII; a.pitch = pitch; a.outZ = reinterpret_cast<double2*>(outZ);
   a.tiles_per_walker = (p->N + TILE - 1) / TILE;
-  a.units_per_walker = (a.tiles_per_walker + UNIT_TILES - 1) / UNIT_TILES;
+  // tiles per unit: as many as leave >= 8 units per resident CTA (one series re-expansion per unit)
+  int ut = UNIT_TILES_MAX;
+  while (ut > 1 && (int64_t)K * ((a.tiles_per_walker + ut - 1) / ut) < (int64_t)8 * p->synth_grid) ut >>= 1;
+  if (p->unit_tiles_override > 0) ut = p->unit_tiles_override;
+  a.unit_tiles = ut;
+  a.units_per_walker = (a.tiles_per_walker + ut - 1) / ut;
   int64_t total = (int64_t)K * a.units_per_walker;
   int grid = (int)std::min<int64_t>(total, p->synth_grid);
   synth_kernel<<<grid, SYNTH_THREADS, p->synth_smem, s>>>(a);
@@ -264,12 +270,21 @@ int run_synth(emri_plan* p, int k0, int K, double* outI, double* outII, int64_t 
   return EMRI_OK;
 }
 
-int run_like(emri_plan* p, int k0, int K, const double* H, const double* data_fft, cudaStream_t s) {
+int fft_chunk(emri_plan* p, int kc, double* z, cudaStream_t s) {
+  cufftHandle h;
+  int rc = get_fft(p, kc, &h);
+  if (rc) return rc;
+  CKF(cufftSetStream(h, s));
+  CKF(cufftExecZ2Z(h, reinterpret_cast<cufftDoubleComplex*>(z), reinterpret_cast<cufftDoubleComplex*>(z), CUFFT_FORWARD));
+  return EMRI_OK;
+}
+
+int run_like(emri_plan* p, int k0, int K, const double* Z, const double* data_fft, cudaStream_t s) {
   LikeArgs a;
-  a.H = reinterpret_cast<const double2*>(H);
+  a.Z = reinterpret_cast<const double2*>(Z);
   a.D = reinterpret_cast<const double2*>(data_fft);
-  a.w = p->d_w; a.partial = p->d_partial; a.k0 = k0; a.K = K; a.Nf = p->Nf; a.n_part = p->n_part;
-  int grid = (int)((p->Nf + LL_TILE - 1) / LL_TILE);
+  a.w = p->d_w; a.partial = p->d_partial; a.k0 = k0; a.K = K; a.N = p->N; a.Nf = p->Nf; a.n_part = p->n_part;
+  dim3 grid((unsigned)p->n_part, (unsigned)((K + LL_GROUP - 1) / LL_GROUP));
   loglike_kernel<<<grid, LL_THREADS, 0, s>>>(a);
   CK(cudaGetLastError());
   return EMRI_OK;
@@ -323,7 +338,7 @@ int emri_plan_create(emri_plan** out, int64_t N, double dt, int n_max, int K_max
   if ((rc = dev_alloc(p, &p->d_pclamp, (size_t)K_max))) return fail(rc);
   if ((rc = dev_alloc(p, &p->d_plrow, (size_t)K_max * NODE_STRIDE))) return fail(rc);
   if ((rc = dev_alloc(p, &p->d_base, base.size()))) return fail(rc);
-  p->n_part = (int)((p->Nf + LL_TILE - 1) / LL_TILE) * LL_WARPS;
+  p->n_part = (int)((p->Nf + LL_RANGE - 1) / LL_RANGE);
   if ((rc = dev_alloc(p, &p->d_partial, (size_t)K_max * p->n_part))) return fail(rc);
   if ((rc = dev_alloc(p, &p->d_params, (size_t)K_max * EMRI_NPAR))) return fail(rc);
   if ((rc = dev_alloc(p, &p->d_data, (size_t)4 * p->Nf))) return fail(rc);
@@ -343,7 +358,8 @@ int emri_plan_create(emri_plan** out, int64_t N, double dt, int n_max, int K_max
 
   // persistent grid for the synthesis kernel: resident CTAs per SM x SM count
   p->synth_smem = (size_t)(n_max + 1) * MLOC * sizeof(double4) + (size_t)6 * 2 * SYNTH_THREADS * sizeof(double) +
-                  (WC_STRIDE + 2 * UNIT_TILES + 4) * sizeof(double);
+                  (WC_STRIDE + 2 * UNIT_TILES_MAX) * sizeof(double);
+  if (const char* ev = std::getenv("EMRI_UNIT_TILES")) p->unit_tiles_override = std::max(1, std::min(UNIT_TILES_MAX, std::atoi(ev)));
   if (cudaFuncSetAttribute(synth_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)p->synth_smem) != cudaSuccess)
     return fail(EMRI_ECUDA);
   int per_sm = 0;
@@ -404,7 +420,7 @@ int emri_plan_set_chunk(emri_plan* p, int c) {
   if (!p || c < 1) return EMRI_EINVAL;
   if (c > p->K_max) c = p->K_max;
   CK(cudaDeviceSynchronize());
-  if (p->d_hbuf) p->bytes -= (int64_t)((size_t)2 * p->chunk * (p->N + 2) * sizeof(double));
+  if (p->d_hbuf) p->bytes -= (int64_t)((size_t)2 * p->chunk * p->N * sizeof(double));
   p->chunk = c;
   return alloc_chunk(p);
 }
@@ -433,7 +449,7 @@ int emri_waveform(emri_plan* p, const double* params, int K, double* h_I, double
   if (rc) return rc;
   mark(p, s);
   mark(p, s);
-  if ((rc = run_synth(p, 0, K, h_I, h_II, p->N, s))) return rc;
+  if ((rc = run_synth(p, 0, K, h_I, h_II, p->N, nullptr, s))) return rc;
   mark(p, s);
   mark(p, s);
   mark(p, s);
@@ -455,14 +471,16 @@ int emri_waveform_fft(emri_plan* p, const double* params, int K, double* spectra
   int nch = 0;
   for (int k0 = 0; k0 < K; k0 += p->chunk, ++nch) {
     const int kc = std::min(p->chunk, K - k0);
-    double* rows = spectra + (size_t)k0 * 2 * (p->N + 2);
     mark(p, s);
-    if ((rc = run_synth(p, k0, kc, rows, rows + (p->N + 2), 2 * (p->N + 2), s))) return rc;
+    if ((rc = run_synth(p, k0, kc, nullptr, nullptr, 0, p->d_hbuf, s))) return rc;
     mark(p, s);
-    cufftHandle h;
-    if ((rc = get_fft(p, 2 * kc, &h))) return rc;
-    CKF(cufftSetStream(h, s));
-    CKF(cufftExecD2Z(h, rows, reinterpret_cast<cufftDoubleComplex*>(rows)));
+    if ((rc = fft_chunk(p, kc, p->d_hbuf, s))) return rc;
+    {
+      const int64_t tot = (int64_t)kc * p->Nf;
+      unpack_spectrum_kernel<<<(unsigned)((tot + 255) / 256), 256, 0, s>>>(
+          reinterpret_cast<const double2*>(p->d_hbuf), reinterpret_cast<double2*>(spectra) + (size_t)k0 * 2 * p->Nf, kc, p->N, p->Nf);
+      CK(cudaGetLastError());
+    }
     mark(p, s);
     mark(p, s);
   }
@@ -477,13 +495,13 @@ int emri_waveform_fft(emri_plan* p, const double* params, int K, double* spectra
 int emri_data_fft(emri_plan* p, const double* d_I, const double* d_II, double* data_fft, void* stream) {
   if (!p || !d_I || !d_II || !data_fft) return EMRI_EINVAL;
   cudaStream_t s = (cudaStream_t)stream;
-  CK(cudaMemcpyAsync(data_fft, d_I, (size_t)p->N * sizeof(double), cudaMemcpyDeviceToDevice, s));
-  CK(cudaMemcpyAsync(data_fft + (p->N + 2), d_II, (size_t)p->N * sizeof(double), cudaMemcpyDeviceToDevice, s));
-  cufftHandle h;
-  int rc = get_fft(p, 2, &h);
+  pack_complex_kernel<<<(unsigned)((p->N + 255) / 256), 256, 0, s>>>(d_I, d_II, reinterpret_cast<double2*>(p->d_hbuf), p->N);
+  CK(cudaGetLastError());
+  int rc = fft_chunk(p, 1, p->d_hbuf, s);
   if (rc) return rc;
-  CKF(cufftSetStream(h, s));
-  CKF(cufftExecD2Z(h, data_fft, reinterpret_cast<cufftDoubleComplex*>(data_fft)));
+  unpack_spectrum_kernel<<<(unsigned)((p->Nf + 255) / 256), 256, 0, s>>>(reinterpret_cast<const double2*>(p->d_hbuf),
+                                                                         reinterpret_cast<double2*>(data_fft), 1, p->N, p->Nf);
+  CK(cudaGetLastError());
   return EMRI_OK;
 }
 
@@ -500,12 +518,9 @@ int emri_loglike(emri_plan* p, const double* params, int K, const double* data_f
   for (int k0 = 0; k0 < K; k0 += p->chunk, ++nch) {
     const int kc = std::min(p->chunk, K - k0);
     mark(p, s);
-    if ((rc = run_synth(p, k0, kc, p->d_hbuf, p->d_hbuf + (p->N + 2), 2 * (p->N + 2), s))) return rc;
+    if ((rc = run_synth(p, k0, kc, nullptr, nullptr, 0, p->d_hbuf, s))) return rc;
     mark(p, s);
-    cufftHandle h;
-    if ((rc = get_fft(p, 2 * kc, &h))) return rc;
-    CKF(cufftSetStream(h, s));
-    CKF(cufftExecD2Z(h, p->d_hbuf, reinterpret_cast<cufftDoubleComplex*>(p->d_hbuf)));
+    if ((rc = fft_chunk(p, kc, p->d_hbuf, s))) return rc;
     mark(p, s);
     if ((rc = run_like(p, k0, kc, p->d_hbuf, data_fft, s))) return rc;
     mark(p, s);

@@ -27,8 +27,11 @@ namespace {
 
 constexpr int SYNTH_THREADS = 128;
 constexpr int TILE = 2 * SYNTH_THREADS;   // samples per tile (2 adjacent samples per thread)
-constexpr int UNIT_TILES = 4;             // tiles per unit (one re-expansion per unit)
+constexpr int UNIT_TILES_MAX = 16;        // tiles per unit (one re-expansion per unit), chosen per launch
 constexpr int MLOC = 9;                   // local expansion orders 0..8
+#ifndef SYNTH_MINBLOCKS
+#define SYNTH_MINBLOCKS 4
+#endif
 constexpr int BASE_M = 48;                // Taylor coefficients kept per harmonic in the base table
 
 struct SynthArgs {
@@ -44,9 +47,11 @@ struct SynthArgs {
   int S, logS;
   int64_t Nn;
   int n_max;
-  double* outI;            // row of walker k0+i at outI + i*pitch
+  double* outI;            // separate channels: row of walker k0+i at outI + i*pitch (used when outZ == NULL)
   double* outII;
   int64_t pitch;
+  double2* outZ;           // interleaved z = h_I + i h_II, row of walker k0+i at outZ + i*N
+  int unit_tiles;
   int64_t tiles_per_walker, units_per_walker;
   double tol;              // relative truncation of the harmonic series
 };
@@ -162,62 +167,94 @@ DEVINL double4 ldg4(const double4* p) {
   return make_double4(lo.x, lo.y, hi.x, hi.y);
 }
 
-// Horner evaluation of the three series of one harmonic for the thread's two samples (coefficients are warp-uniform)
-template <bool kLocal>
-DEVINL void series3(const double4* __restrict__ tab, int M, double xa, double xb, double& pa_a, double& pb_a, double& pc_a,
-                    double& pa_b, double& pb_b, double& pc_b) {
-  double4 c = kLocal ? tab[M - 1] : ldg4(tab + (M - 1));
-  pa_a = c.x; pb_a = c.y; pc_a = c.z;
-  pa_b = c.x; pb_b = c.y; pc_b = c.z;
-#pragma unroll 4
+// Harmonic sum n = 1..n_max for the thread's two samples; returns S_a, S_b, S_c of each.  Coefficients are
+// warp-uniform.  Local version: M orders of the re-expanded series (compile-time M: fully unrolled Horner, the
+// coefficient loads of the next harmonic can be hoisted above the arithmetic of the current one).
+#define EMRI_ACCUM_FIRST()                                                                       \
+  double SaA = p[0] * A.ec, SbA = p[1] * A.es, ScA = p[2] * A.ec;                                \
+  double SaB = p[3] * B.ec, SbB = p[4] * B.es, ScB = p[5] * B.ec;                                \
+  double CA = A.C2, SA = A.S2, CB = B.C2, SB = B.S2;
+#define EMRI_ACCUM_NEXT()                                                                        \
+  SaA = fma(p[0], CA, SaA); SbA = fma(p[1], SA, SbA); ScA = fma(p[2], CA, ScA);                  \
+  SaB = fma(p[3], CB, SaB); SbB = fma(p[4], SB, SbB); ScB = fma(p[5], CB, ScB);                  \
+  {                                                                                              \
+    const double ta = CA, tb = CB;                                                               \
+    CA = fma(CA, A.ec, -SA * A.es); SA = fma(SA, A.ec, ta * A.es);                               \
+    CB = fma(CB, B.ec, -SB * B.es); SB = fma(SB, B.ec, tb * B.es);                               \
+  }
+
+template <int M>
+DEVINL void series_local(const double4* __restrict__ t, double xa, double xb, double p[6]) {
+  double4 c = t[M - 1];
+  p[0] = c.x; p[1] = c.y; p[2] = c.z; p[3] = c.x; p[4] = c.y; p[5] = c.z;
+#pragma unroll
   for (int m = M - 2; m >= 0; --m) {
-    c = kLocal ? tab[m] : ldg4(tab + m);
-    pa_a = fma(pa_a, xa, c.x); pb_a = fma(pb_a, xa, c.y); pc_a = fma(pc_a, xa, c.z);
-    pa_b = fma(pa_b, xb, c.x); pb_b = fma(pb_b, xb, c.y); pc_b = fma(pc_b, xb, c.z);
+    c = t[m];
+    p[0] = fma(p[0], xa, c.x); p[1] = fma(p[1], xa, c.y); p[2] = fma(p[2], xa, c.z);
+    p[3] = fma(p[3], xb, c.x); p[4] = fma(p[4], xb, c.y); p[5] = fma(p[5], xb, c.z);
   }
 }
 
-// harmonic sum n = 1..n_max for two samples; returns S_a, S_b, S_c of each
-template <bool kLocal>
-DEVINL void harmonic_sum(const double4* __restrict__ tab, int tab_stride, const int* __restrict__ Mn, int n_max,
-                         const SampleOut& A, const SampleOut& B, double out[6]) {
-  double pa_a, pb_a, pc_a, pa_b, pb_b, pc_b;
-  // n = 1: carrier e (cos, sin)(Phi)
-  series3<kLocal>(tab + tab_stride, Mn[1], A.x, B.x, pa_a, pb_a, pc_a, pa_b, pb_b, pc_b);
-  double SaA = pa_a * A.ec, SbA = pb_a * A.es, ScA = pc_a * A.ec;
-  double SaB = pa_b * B.ec, SbB = pb_b * B.es, ScB = pc_b * B.ec;
-  // n >= 2: carrier e^{n-2} (cos, sin)(n Phi), advanced by the scaled rotation (e cos Phi, e sin Phi)
-  double CA = A.C2, SA = A.S2, CB = B.C2, SB = B.S2;
+template <int M>
+DEVINL void harmonic_sum_local(const double4* __restrict__ tab, int n_max, const SampleOut& A, const SampleOut& B,
+                               double out[6]) {
+  double p[6];
+  // n = 1: carrier e (cos, sin)(Phi);  n >= 2: carrier e^{n-2} (cos, sin)(n Phi), advanced by the scaled rotation
+  series_local<M>(tab + MLOC, A.x, B.x, p);
+  EMRI_ACCUM_FIRST()
+#pragma unroll 2
   for (int n = 2; n <= n_max; ++n) {
-    series3<kLocal>(tab + (size_t)n * tab_stride, Mn[n], A.x, B.x, pa_a, pb_a, pc_a, pa_b, pb_b, pc_b);
-    SaA = fma(pa_a, CA, SaA); SbA = fma(pb_a, SA, SbA); ScA = fma(pc_a, CA, ScA);
-    SaB = fma(pa_b, CB, SaB); SbB = fma(pb_b, SB, SbB); ScB = fma(pc_b, CB, ScB);
-    const double ta = CA, tb = CB;
-    CA = fma(CA, A.ec, -SA * A.es); SA = fma(SA, A.ec, ta * A.es);
-    CB = fma(CB, B.ec, -SB * B.es); SB = fma(SB, B.ec, tb * B.es);
+    series_local<M>(tab + n * MLOC, A.x, B.x, p);
+    EMRI_ACCUM_NEXT()
   }
   out[0] = SaA; out[1] = SbA; out[2] = ScA; out[3] = SaB; out[4] = SbB; out[5] = ScB;
 }
 
-DEVINL double block_max(double v, double* s_red, int warp, int lane) {
-#pragma unroll
-  for (int off = 16; off > 0; off >>= 1) v = fmax(v, __shfl_xor_sync(0xffffffffu, v, off));
-  __syncthreads();
-  if (lane == 0) s_red[warp] = v;
-  __syncthreads();
-  return fmax(fmax(s_red[0], s_red[1]), fmax(s_red[2], s_red[3]));
+// Fallback version: the base series in w = e^2 straight from the global table, Mn[n] terms (rare, slow path)
+DEVINL void series_base(const double4* __restrict__ t, int M, double xa, double xb, double p[6]) {
+  double4 c = ldg4(t + (M - 1));
+  p[0] = c.x; p[1] = c.y; p[2] = c.z; p[3] = c.x; p[4] = c.y; p[5] = c.z;
+  for (int m = M - 2; m >= 0; --m) {
+    c = ldg4(t + m);
+    p[0] = fma(p[0], xa, c.x); p[1] = fma(p[1], xa, c.y); p[2] = fma(p[2], xa, c.z);
+    p[3] = fma(p[3], xb, c.x); p[4] = fma(p[4], xb, c.y); p[5] = fma(p[5], xb, c.z);
+  }
 }
 
-__global__ void __launch_bounds__(SYNTH_THREADS, 4) synth_kernel(SynthArgs a) {
+__device__ __noinline__ void harmonic_sum_base(const double4* __restrict__ base, const int* __restrict__ Mn, int n_max,
+                                               const SampleOut& A, const SampleOut& B, double out[6]) {
+  double p[6];
+  series_base(base + BASE_M, Mn[1], A.x, B.x, p);
+  EMRI_ACCUM_FIRST()
+  for (int n = 2; n <= n_max; ++n) {
+    series_base(base + (size_t)n * BASE_M, Mn[n], A.x, B.x, p);
+    EMRI_ACCUM_NEXT()
+  }
+  out[0] = SaA; out[1] = SbA; out[2] = ScA; out[3] = SaB; out[4] = SbB; out[5] = ScB;
+}
+
+// block-wide maximum of four values per thread (one barrier; the caller has synchronised since the last use of s_red)
+DEVINL void block_max4(double v[4], double (*s_red)[4], int warp, int lane) {
+#pragma unroll
+  for (int q = 0; q < 4; ++q) {
+#pragma unroll
+    for (int off = 16; off > 0; off >>= 1) v[q] = fmax(v[q], __shfl_xor_sync(0xffffffffu, v[q], off));
+    if (lane == 0) s_red[warp][q] = v[q];
+  }
+  __syncthreads();
+#pragma unroll
+  for (int q = 0; q < 4; ++q) v[q] = fmax(fmax(s_red[0][q], s_red[1][q]), fmax(s_red[2][q], s_red[3][q]));
+}
+
+__global__ void __launch_bounds__(SYNTH_THREADS, SYNTH_MINBLOCKS) synth_kernel(SynthArgs a) {
   extern __shared__ __align__(16) unsigned char smem_raw[];
   double4* s_tab = reinterpret_cast<double4*>(smem_raw);                               // [(n_max+1)][MLOC]
   double* s_fin = reinterpret_cast<double*>(s_tab + (size_t)(a.n_max + 1) * MLOC);     // [6][2][SYNTH_THREADS]
   double* s_wc = s_fin + 6 * 2 * SYNTH_THREADS;                                        // [WC_STRIDE]
-  double* s_rot = s_wc + WC_STRIDE;                                                    // [UNIT_TILES][2] + [4] scratch
-  __shared__ int s_M[EMRI_NMAX_CAP + 1];      // local orders kept per harmonic
+  double* s_rot = s_wc + WC_STRIDE;                                                    // [UNIT_TILES_MAX][2]
+  __shared__ int s_Mu;                        // local orders kept (maximum over the harmonics)
   __shared__ int s_Mb[EMRI_NMAX_CAP + 1];     // base-series terms per harmonic (fallback path)
-  __shared__ int s_fallback;
-  __shared__ double s_red[4];
+  __shared__ double s_red[4][4];
 
   const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
   const double Delta = a.S * a.dt, invS = 1.0 / (double)a.S;
@@ -233,9 +270,8 @@ __global__ void __launch_bounds__(SYNTH_THREADS, 4) synth_kernel(SynthArgs a) {
     const int kl = (int)(u / a.units_per_walker);
     const int64_t ug = u - (int64_t)kl * a.units_per_walker;
     const int k = a.k0 + kl;
-    const int64_t tile0 = ug * UNIT_TILES;
-    const int64_t i_begin = tile0 * TILE;
-    const int64_t i_end = min(a.N, i_begin + (int64_t)UNIT_TILES * TILE);     // exclusive
+    const int64_t i_begin = ug * a.unit_tiles * TILE;
+    const int64_t i_end = min(a.N, i_begin + (int64_t)a.unit_tiles * TILE);     // exclusive
     const double* nodes = a.nodes + (size_t)k * a.Nn * NODE_STRIDE;
     const double2* aux = a.nodeaux + (size_t)k * a.Nn;
     __syncthreads();                      // the previous unit is done with the shared tables
@@ -243,13 +279,18 @@ __global__ void __launch_bounds__(SYNTH_THREADS, 4) synth_kernel(SynthArgs a) {
       if (tid < WC_STRIDE) s_wc[tid] = a.wc[(size_t)k * WC_STRIDE + tid];
       cur_k = k;
     }
-    if (tid <= a.n_max) { s_M[tid] = 1; s_Mb[tid] = 1; }
-    if (tid == 0) s_fallback = 0;
+    if (tid <= a.n_max) s_Mb[tid] = 1;
+    if (tid == 0) s_Mu = 1;
     const int32_t st = a.status[k];
     if (st & (EMRI_ST_BADPARAM | EMRI_ST_DELAY | EMRI_ST_STATE)) {
       for (int64_t i0 = i_begin + 2 * tid; i0 < i_end; i0 += TILE) {
-        *reinterpret_cast<double2*>(a.outI + (size_t)kl * a.pitch + i0) = make_double2(0.0, 0.0);
-        *reinterpret_cast<double2*>(a.outII + (size_t)kl * a.pitch + i0) = make_double2(0.0, 0.0);
+        if (a.outZ) {
+          a.outZ[(size_t)kl * a.N + i0] = make_double2(0.0, 0.0);
+          a.outZ[(size_t)kl * a.N + i0 + 1] = make_double2(0.0, 0.0);
+        } else {
+          *reinterpret_cast<double2*>(a.outI + (size_t)kl * a.pitch + i0) = make_double2(0.0, 0.0);
+          *reinterpret_cast<double2*>(a.outII + (size_t)kl * a.pitch + i0) = make_double2(0.0, 0.0);
+        }
       }
       continue;
     }
@@ -259,19 +300,16 @@ __global__ void __launch_bounds__(SYNTH_THREADS, 4) synth_kernel(SynthArgs a) {
       int64_t rlo = (i_begin >> a.logS) - 1 + 1, rhi = ((i_end - 1) >> a.logS) + 2 + 1;       // rows = node index + 1
       if (rlo < 0) rlo = 0;
       if (rhi > a.Nn - 1) rhi = a.Nn - 1;
-      double emx = 0.0, emn_neg = -1.0, slp = 0.0, inc = 0.0;
+      double v[4] = {0.0, -1.0, 0.0, 0.0};       // max e, max -e, max |e'|, max |increment of e|
       for (int64_t r = rlo + tid; r <= rhi; r += SYNTH_THREADS) {
         const double* row = nodes + r * NODE_STRIDE;
         const double ev = __ldg(row + 3);
-        emx = fmax(emx, ev); emn_neg = fmax(emn_neg, -ev);
-        slp = fmax(slp, fabs(__ldg(row + 8))); inc = fmax(inc, fabs(__ldg(row + 13)));
+        v[0] = fmax(v[0], ev); v[1] = fmax(v[1], -ev);
+        v[2] = fmax(v[2], fabs(__ldg(row + 8))); v[3] = fmax(v[3], fabs(__ldg(row + 13)));
       }
-      emx = block_max(emx, s_red, warp, lane);
-      emn_neg = block_max(emn_neg, s_red, warp, lane);
-      slp = block_max(slp, s_red, warp, lane);
-      inc = block_max(inc, s_red, warp, lane);
-      const double pad = 0.3 * fma(Delta, slp, inc) + 1e-15;
-      const double elo = fmax(-emn_neg - pad, 0.0), ehi = emx + pad;
+      block_max4(v, s_red, warp, lane);
+      const double pad = 0.3 * fma(Delta, v[2], v[3]) + 1e-15;
+      const double elo = fmax(-v[1] - pad, 0.0), ehi = v[0] + pad;
       whi = ehi * ehi;
       w0 = 0.5 * fma(elo, elo, whi);
       xmax = 0.5 * (whi - elo * elo) * (1.0 + 1e-9);
@@ -284,10 +322,12 @@ __global__ void __launch_bounds__(SYNTH_THREADS, 4) synth_kernel(SynthArgs a) {
       int Mb = 1;
       {
         double pw = 1.0, mx = 0.0;
+        int below = 0;
         for (int m = 0; m < BASE_M; ++m) {
           const double t = fabs(__ldg(bp + 4 * m)) * pw;
           mx = fmax(mx, t);
-          if (t >= a.tol * mx && t > 0.0) Mb = m + 1;
+          if (t >= a.tol * mx && t > 0.0) { Mb = m + 1; below = 0; }
+          else if (t > 0.0 && ++below >= 3) break;      // past the peak the terms fall monotonically
           pw *= whi;
         }
       }
@@ -314,22 +354,22 @@ __global__ void __launch_bounds__(SYNTH_THREADS, 4) synth_kernel(SynthArgs a) {
       double* dst = reinterpret_cast<double*>(s_tab + (size_t)n * MLOC) + si;
 #pragma unroll
       for (int j = 0; j < MLOC; ++j) dst[4 * j] = d[j];
-      atomicMax(&s_M[n], Ml);
+      atomicMax(&s_Mu, Ml);                    // Ml == MLOC: order MLOC-1 still significant, the tail is not bounded
       atomicMax(&s_Mb[n], Mb);
-      if (Ml == MLOC) s_fallback = 1;          // order MLOC-1 still significant: the tail is not bounded
     }
-    if (tid >= SYNTH_THREADS - UNIT_TILES) {
+    if (tid >= SYNTH_THREADS - a.unit_tiles) {
       // detector phase at the start of each tile of the unit
-      const int t = tid - (SYNTH_THREADS - UNIT_TILES);
+      const int t = tid - (SYNTH_THREADS - a.unit_tiles);
       double sb, cb;
       sincospi(2.0 * frac((double)(i_begin + (int64_t)t * TILE) * a.dt * inv_year), &sb, &cb);
       s_rot[2 * t] = cb; s_rot[2 * t + 1] = sb;
     }
     __syncthreads();
-    const bool fallback = s_fallback != 0;
+    const int Mu = s_Mu;
+    const bool fallback = Mu >= MLOC;
     const double w0e = fallback ? 0.0 : w0;
     const int32_t jpl = a.jpl[k];
-    for (int t = 0; t < UNIT_TILES; ++t) {
+    for (int t = 0; t < a.unit_tiles; ++t) {
       const int64_t i0 = i_begin + (int64_t)t * TILE + 2 * tid;
       if (i0 >= i_end) break;
       // detector phase: tile start (x) thread offset, then one sample step
@@ -342,15 +382,29 @@ __global__ void __launch_bounds__(SYNTH_THREADS, 4) synth_kernel(SynthArgs a) {
       sample_setup(s_wc, nodes, aux, i0 + 1, a.S, a.logS, invS, Delta, jpl, cpb2, spb2, w0e, B, fin + SYNTH_THREADS,
                    2 * SYNTH_THREADS);
       double S[6];
-      if (!fallback) harmonic_sum<true>(s_tab, MLOC, s_M, a.n_max, A, B, S);
-      else harmonic_sum<false>(a.base, BASE_M, s_Mb, a.n_max, A, B, S);
+      switch (Mu) {
+        case 1: harmonic_sum_local<1>(s_tab, a.n_max, A, B, S); break;
+        case 2: harmonic_sum_local<2>(s_tab, a.n_max, A, B, S); break;
+        case 3: harmonic_sum_local<3>(s_tab, a.n_max, A, B, S); break;
+        case 4: harmonic_sum_local<4>(s_tab, a.n_max, A, B, S); break;
+        case 5: harmonic_sum_local<5>(s_tab, a.n_max, A, B, S); break;
+        case 6: harmonic_sum_local<6>(s_tab, a.n_max, A, B, S); break;
+        case 7: harmonic_sum_local<7>(s_tab, a.n_max, A, B, S); break;
+        case 8: harmonic_sum_local<8>(s_tab, a.n_max, A, B, S); break;
+        default: harmonic_sum_base(a.base, s_Mb, a.n_max, A, B, S); break;
+      }
       const double hIa = fma(fin[0], S[0], fma(fin[2 * SYNTH_THREADS], S[1], fin[4 * SYNTH_THREADS] * S[2]));
       const double hIIa = fma(fin[6 * SYNTH_THREADS], S[0], fma(fin[8 * SYNTH_THREADS], S[1], fin[10 * SYNTH_THREADS] * S[2]));
       const double* fb = fin + SYNTH_THREADS;
       const double hIb = fma(fb[0], S[3], fma(fb[2 * SYNTH_THREADS], S[4], fb[4 * SYNTH_THREADS] * S[5]));
       const double hIIb = fma(fb[6 * SYNTH_THREADS], S[3], fma(fb[8 * SYNTH_THREADS], S[4], fb[10 * SYNTH_THREADS] * S[5]));
-      *reinterpret_cast<double2*>(a.outI + (size_t)kl * a.pitch + i0) = make_double2(hIa, hIb);
-      *reinterpret_cast<double2*>(a.outII + (size_t)kl * a.pitch + i0) = make_double2(hIIa, hIIb);
+      if (a.outZ) {
+        a.outZ[(size_t)kl * a.N + i0] = make_double2(hIa, hIIa);
+        a.outZ[(size_t)kl * a.N + i0 + 1] = make_double2(hIb, hIIb);
+      } else {
+        *reinterpret_cast<double2*>(a.outI + (size_t)kl * a.pitch + i0) = make_double2(hIa, hIb);
+        *reinterpret_cast<double2*>(a.outII + (size_t)kl * a.pitch + i0) = make_double2(hIIa, hIIb);
+      }
     }
   }
 }
