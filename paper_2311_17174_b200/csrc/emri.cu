@@ -265,7 +265,7 @@ int run_synth(emri_plan* p, int k0, int K, double* outI, double* outII, int64_t 
   a.units_per_walker = (a.tiles_per_walker + ut - 1) / ut;
   int64_t total = (int64_t)K * a.units_per_walker;
   int grid = (int)std::min<int64_t>(total, p->synth_grid);
-  synth_kernel<<<grid, SYNTH_THREADS, p->synth_smem, s>>>(a);
+  synth_kernel<<<grid, SYNTH_BLOCK, p->synth_smem, s>>>(a);
   CK(cudaGetLastError());
   return EMRI_OK;
 }
@@ -357,13 +357,13 @@ int emri_plan_create(emri_plan** out, int64_t N, double dt, int n_max, int K_max
     return fail(EMRI_ECUDA);
 
   // persistent grid for the synthesis kernel: resident CTAs per SM x SM count
-  p->synth_smem = (size_t)(n_max + 1) * MLOC * sizeof(double4) + (size_t)6 * 2 * SYNTH_THREADS * sizeof(double) +
-                  (WC_STRIDE + 2 * UNIT_TILES_MAX) * sizeof(double);
+  p->synth_smem = (size_t)2 * (n_max + 1) * MLOC * sizeof(double4) + (size_t)SC_TAB * sizeof(double2) +
+                  (size_t)6 * 2 * SYNTH_THREADS * sizeof(double) + (size_t)2 * (WC_STRIDE + 2 * UNIT_TILES_MAX) * sizeof(double);
   if (const char* ev = std::getenv("EMRI_UNIT_TILES")) p->unit_tiles_override = std::max(1, std::min(UNIT_TILES_MAX, std::atoi(ev)));
   if (cudaFuncSetAttribute(synth_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)p->synth_smem) != cudaSuccess)
     return fail(EMRI_ECUDA);
   int per_sm = 0;
-  if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, synth_kernel, SYNTH_THREADS, p->synth_smem) != cudaSuccess ||
+  if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, synth_kernel, SYNTH_BLOCK, p->synth_smem) != cudaSuccess ||
       per_sm < 1)
     return fail(EMRI_ECUDA);
   p->synth_grid = per_sm * p->sm_count;

@@ -25,7 +25,8 @@
 
 namespace {
 
-constexpr int SYNTH_THREADS = 128;
+constexpr int SYNTH_THREADS = 128;        // consumer threads per CTA
+constexpr int SYNTH_BLOCK = SYNTH_THREADS + 32;   // + one producer warp
 constexpr int TILE = 2 * SYNTH_THREADS;   // samples per tile (2 adjacent samples per thread)
 constexpr int UNIT_TILES_MAX = 16;        // tiles per unit (one re-expansion per unit), chosen per launch
 constexpr int MLOC = 9;                   // local expansion orders 0..8
@@ -56,14 +57,41 @@ struct SynthArgs {
   double tol;              // relative truncation of the harmonic series
 };
 
+constexpr int SC_TAB = 1024;              // entries of the shared cos/sin table (one per 1/1024 cycle)
+
+// cos/sin(2 pi x) for x in cycles (|x| < 2^40): nearest table angle (round-to-nearest by the 1.5*2^52 trick, so the
+// remainder is exact) and a Taylor rotation by the remainder |z| <= pi/1024 (sin to z^5, cos to z^4: < 2e-18).
+DEVINL void sincos_cycles(const double2* __restrict__ tab, double x, double& sn, double& cs) {
+  const double magic = 6755399441055744.0;
+  const double t = fma(x, (double)SC_TAB, magic);
+  const int k = __double2loint(t) & (SC_TAB - 1);
+  const double r = fma(x, (double)SC_TAB, -(t - magic));
+  const double z = r * (kTwoPi / SC_TAB);
+  const double z2 = z * z;
+  const double sz = fma(z * z2, fma(z2, 1.0 / 120.0, -1.0 / 6.0), z);
+  const double cz = fma(z2, fma(z2, 1.0 / 24.0, -0.5), 1.0);
+  const double2 e = tab[k];
+  cs = fma(e.x, cz, -e.y * sz);
+  sn = fma(e.y, cz, e.x * sz);
+}
+
+// 1/x to ~1 ulp without the IEEE slow path: hardware seed (2^-23) and two Newton steps
+DEVINL double rcp_fast(double x) {
+  double r;
+  asm("rcp.approx.ftz.f64 %0, %1;" : "=d"(r) : "d"(x));
+  r = fma(r, fma(-x, r, 1.0), r);
+  r = fma(r, fma(-x, r, 1.0), r);
+  return r;
+}
+
 struct SampleOut {
   double x, ec, es, C2, S2;     // w - w0;  e cos/sin(Phi_tot);  cos/sin(2 Phi_tot)
 };
 
 // Everything of sample i that does not depend on the harmonic index.  (cpb, spb) = cos/sin of the detector phase
 // phibar = 2 pi t_i / T_yr.  fin[0..5] (stride fs) receive a_I, b_I, c_I, a_II, b_II, c_II.
-DEVINL void sample_setup(const double* __restrict__ w, const double* __restrict__ nodes, const double2* __restrict__ aux,
-                         int64_t i, int S, int logS, double invS, double Delta, int32_t jpl, double cpb, double spb,
+DEVINL void sample_setup(const double* __restrict__ w, const double2* __restrict__ sct, const double* __restrict__ nodes,
+                         const double2* __restrict__ aux, int64_t i, int S, int logS, double invS, double Delta, int32_t jpl, double cpb, double spb,
                          double w0, SampleOut& o, double* __restrict__ fin, int fs) {
   // source-time split (reading D4)
   int64_t j = i >> logS;
@@ -100,8 +128,8 @@ DEVINL void sample_setup(const double* __restrict__ w, const double* __restrict_
     }
   }
   double sa, ca, s2gt, c2gt;
-  sincospi(2.0 * alpc, &sa, &ca);
-  sincospi(4.0 * gamc, &s2gt, &c2gt);
+  sincos_cycles(sct, alpc, sa, ca);
+  sincos_cycles(sct, 2.0 * gamc, s2gt, c2gt);
   // orbital-plane normal and its projections (BC 19-21)
   const double Lx = fma(w[WC_A2X], sa, fma(w[WC_A1X], ca, w[WC_A0X]));
   const double Ly = fma(w[WC_A2Y], sa, fma(w[WC_A1Y], ca, w[WC_A0Y]));
@@ -123,7 +151,7 @@ DEVINL void sample_setup(const double* __restrict__ w, const double* __restrict_
   const double den_p = fma(Npsi, Npsi, Dpsi * Dpsi);
   // one division for the three normalisations
   const double bp = den_b * den_p;
-  const double inv = 1.0 / (bp * den_a);
+  const double inv = rcp_fast(bp * den_a);
   const double ib = inv * (den_a * den_p), ia = inv * bp, ip = inv * (den_a * den_b);
   double c2b = fma(Nc, Nc, -Ns * Ns) * ib, s2b = 2.0 * Ns * Nc * ib;
   if (!(den_b > 0.0)) { c2b = 1.0; s2b = 0.0; }                     // reading R16: beta = 0
@@ -153,9 +181,8 @@ DEVINL void sample_setup(const double* __restrict__ w, const double* __restrict_
   fin[4 * fs] = -sq * fma(FIIp, t3, FIIx * t4);
   fin[5 * fs] = FIIp * P3;
   // Doppler-shifted phase in cycles (BC 25)
-  const double Phit = frac(fma(nu * w[WC_DOP], cd, Phic));
   double s1, c1;
-  sincospi(2.0 * Phit, &s1, &c1);
+  sincos_cycles(sct, fma(nu * w[WC_DOP], cd, Phic), s1, c1);
   o.x = fma(e, e, -w0);
   o.ec = e * c1; o.es = e * s1;
   o.C2 = fma(c1, c1, -s1 * s1); o.S2 = 2.0 * s1 * c1;
@@ -233,180 +260,217 @@ __device__ __noinline__ void harmonic_sum_base(const double4* __restrict__ base,
   out[0] = SaA; out[1] = SbA; out[2] = ScA; out[3] = SaB; out[4] = SbB; out[5] = ScB;
 }
 
-// block-wide maximum of four values per thread (one barrier; the caller has synchronised since the last use of s_red)
-DEVINL void block_max4(double v[4], double (*s_red)[4], int warp, int lane) {
+// ---- per-unit tables, prepared by the producer warp one unit ahead of the consumers (double-buffered)
+struct UnitMeta {
+  double w0e;         // expansion point subtracted from e^2 (0 on the fallback path)
+  int Mu;             // local orders kept (maximum over the harmonics); >= MLOC: fallback to the base series
+  int skip;           // walker has a fatal status: the unit is zero-filled
+  int32_t jpl;
+  int pad;
+};
+
+DEVINL double warp_max(double v) {
 #pragma unroll
-  for (int q = 0; q < 4; ++q) {
-#pragma unroll
-    for (int off = 16; off > 0; off >>= 1) v[q] = fmax(v[q], __shfl_xor_sync(0xffffffffu, v[q], off));
-    if (lane == 0) s_red[warp][q] = v[q];
-  }
-  __syncthreads();
-#pragma unroll
-  for (int q = 0; q < 4; ++q) v[q] = fmax(fmax(s_red[0][q], s_red[1][q]), fmax(s_red[2][q], s_red[3][q]));
+  for (int off = 16; off > 0; off >>= 1) v = fmax(v, __shfl_xor_sync(0xffffffffu, v, off));
+  return v;
 }
 
-__global__ void __launch_bounds__(SYNTH_THREADS, SYNTH_MINBLOCKS) synth_kernel(SynthArgs a) {
+// Executed by ONE warp: everything of unit (k, i_begin..i_end) that is shared by its samples.
+DEVINL void prepare_unit(const SynthArgs& a, int lane, int k, int64_t i_begin, int64_t i_end, double Delta, double inv_year,
+                         double4* __restrict__ tab, double* __restrict__ s_wc, double* __restrict__ s_rot,
+                         int* __restrict__ s_Mb, UnitMeta* __restrict__ meta) {
+  for (int q = lane; q < WC_STRIDE; q += 32) s_wc[q] = a.wc[(size_t)k * WC_STRIDE + q];
+  for (int q = lane; q <= a.n_max; q += 32) s_Mb[q] = 1;
+  const int32_t st = a.status[k];
+  const bool skip = (st & (EMRI_ST_BADPARAM | EMRI_ST_DELAY | EMRI_ST_STATE)) != 0;
+  if (lane == 0) { meta->skip = skip ? 1 : 0; meta->jpl = a.jpl[k]; }
+  if (skip) return;
+  const double* nodes = a.nodes + (size_t)k * a.Nn * NODE_STRIDE;
+  // range of e over the unit from the node rows it touches (the Hermite cubic stays within pad of the nodes)
+  int64_t rlo = (i_begin >> a.logS), rhi = ((i_end - 1) >> a.logS) + 3;       // rows = node index + 1
+  if (rlo < 0) rlo = 0;
+  if (rhi > a.Nn - 1) rhi = a.Nn - 1;
+  double v0 = 0.0, v1 = -1.0, v2 = 0.0, v3 = 0.0;       // max e, max -e, max |e'|, max |increment of e|
+  for (int64_t r = rlo + lane; r <= rhi; r += 32) {
+    const double* row = nodes + r * NODE_STRIDE;
+    const double ev = __ldg(row + 3);
+    v0 = fmax(v0, ev); v1 = fmax(v1, -ev);
+    v2 = fmax(v2, fabs(__ldg(row + 8))); v3 = fmax(v3, fabs(__ldg(row + 13)));
+  }
+  v0 = warp_max(v0); v1 = warp_max(v1); v2 = warp_max(v2); v3 = warp_max(v3);
+  const double pad = 0.3 * fma(Delta, v2, v3) + 1e-15;
+  const double elo = fmax(-v1 - pad, 0.0), ehi = v0 + pad;
+  const double whi = ehi * ehi;
+  const double w0 = 0.5 * fma(elo, elo, whi);
+  const double xmax = 0.5 * (whi - elo * elo) * (1.0 + 1e-9);
+  __syncwarp();
+  // re-expansion of the three series of every harmonic about w0 (task = (harmonic, series))
+  int Mu = 1;
+  for (int task = lane; task < 3 * a.n_max; task += 32) {
+    const int n = task / 3 + 1, si = task - 3 * (n - 1);
+    const double* bp = reinterpret_cast<const double*>(a.base + (size_t)n * BASE_M) + si;
+    // base terms that matter at w <= whi (terms rise, then fall: the running maximum is a safe scale)
+    int Mb = 1;
+    {
+      double pw = 1.0, mx = 0.0;
+      int below = 0;
+      for (int m = 0; m < BASE_M; ++m) {
+        const double t = fabs(__ldg(bp + 4 * m)) * pw;
+        mx = fmax(mx, t);
+        if (t >= a.tol * mx && t > 0.0) { Mb = m + 1; below = 0; }
+        else if (t > 0.0 && ++below >= 3) break;      // past the peak the terms fall monotonically
+        pw *= whi;
+      }
+    }
+    double d[MLOC];
+#pragma unroll
+    for (int j = 0; j < MLOC; ++j) d[j] = 0.0;
+    for (int m = Mb - 1; m >= 0; --m) {
+      const double c = __ldg(bp + 4 * m);
+#pragma unroll
+      for (int j = MLOC - 1; j >= 1; --j) d[j] = fma(d[j], w0, d[j - 1]);
+      d[0] = fma(d[0], w0, c);
+    }
+    int Ml = 1;
+    {
+      double pw = 1.0, mx = 0.0;
+#pragma unroll
+      for (int j = 0; j < MLOC; ++j) {
+        const double t = fabs(d[j]) * pw;
+        mx = fmax(mx, t);
+        if (t >= a.tol * mx && t > 0.0) Ml = j + 1;
+        pw *= xmax;
+      }
+    }
+    double* dst = reinterpret_cast<double*>(tab + (size_t)n * MLOC) + si;
+#pragma unroll
+    for (int j = 0; j < MLOC; ++j) dst[4 * j] = d[j];
+    Mu = max(Mu, Ml);                          // Ml == MLOC: order MLOC-1 still significant, the tail is not bounded
+    atomicMax(&s_Mb[n], Mb);
+  }
+#pragma unroll
+  for (int off = 16; off > 0; off >>= 1) Mu = max(Mu, __shfl_xor_sync(0xffffffffu, Mu, off));
+  if (lane == 0) { meta->Mu = Mu; meta->w0e = (Mu >= MLOC) ? 0.0 : w0; }
+  // detector phase at the start of each tile of the unit
+  if (lane < a.unit_tiles) {
+    double sb, cb;
+    sincospi(2.0 * frac((double)(i_begin + (int64_t)lane * TILE) * a.dt * inv_year), &sb, &cb);
+    s_rot[2 * lane] = cb; s_rot[2 * lane + 1] = sb;
+  }
+}
+
+// Consumers (warps 0..3): 2 adjacent samples per thread per tile.  Producer (warp 4): tables of the NEXT unit.
+__global__ void __launch_bounds__(SYNTH_BLOCK, SYNTH_MINBLOCKS) synth_kernel(SynthArgs a) {
   extern __shared__ __align__(16) unsigned char smem_raw[];
-  double4* s_tab = reinterpret_cast<double4*>(smem_raw);                               // [(n_max+1)][MLOC]
-  double* s_fin = reinterpret_cast<double*>(s_tab + (size_t)(a.n_max + 1) * MLOC);     // [6][2][SYNTH_THREADS]
-  double* s_wc = s_fin + 6 * 2 * SYNTH_THREADS;                                        // [WC_STRIDE]
-  double* s_rot = s_wc + WC_STRIDE;                                                    // [UNIT_TILES_MAX][2]
-  __shared__ int s_Mu;                        // local orders kept (maximum over the harmonics)
-  __shared__ int s_Mb[EMRI_NMAX_CAP + 1];     // base-series terms per harmonic (fallback path)
-  __shared__ double s_red[4][4];
+  const size_t tab_elems = (size_t)(a.n_max + 1) * MLOC;
+  double4* s_tab = reinterpret_cast<double4*>(smem_raw);                               // [2][(n_max+1)][MLOC]
+  double2* s_sct = reinterpret_cast<double2*>(s_tab + 2 * tab_elems);                  // [SC_TAB] {cos, sin}
+  double* s_fin = reinterpret_cast<double*>(s_sct + SC_TAB);                           // [6][2][SYNTH_THREADS]
+  double* s_wc = s_fin + 6 * 2 * SYNTH_THREADS;                                        // [2][WC_STRIDE]
+  double* s_rot = s_wc + 2 * WC_STRIDE;                                                // [2][2 UNIT_TILES_MAX]
+  __shared__ int s_Mb[2][EMRI_NMAX_CAP + 1];  // base-series terms per harmonic (fallback path)
+  __shared__ UnitMeta s_meta[2];
 
   const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
+  const bool producer = warp == SYNTH_THREADS / 32;
   const double Delta = a.S * a.dt, invS = 1.0 / (double)a.S;
   const double inv_year = 1.0 / kYearSec;
+  for (int q = tid; q < SC_TAB; q += SYNTH_BLOCK) {
+    double sv, cv;
+    sincospi(2.0 * (double)q / (double)SC_TAB, &sv, &cv);
+    s_sct[q] = make_double2(cv, sv);
+  }
   // detector phase of the thread's first sample relative to the tile start, and of one sample step
   double so, co, s1s, c1s;
   sincospi(2.0 * ((double)(2 * tid) * a.dt * inv_year), &so, &co);
   sincospi(2.0 * (a.dt * inv_year), &s1s, &c1s);
 
   const int64_t total = (int64_t)a.K * a.units_per_walker;
-  int cur_k = -1;
-  for (int64_t u = blockIdx.x; u < total; u += gridDim.x) {
-    const int kl = (int)(u / a.units_per_walker);
+  const int64_t unit_len = (int64_t)a.unit_tiles * TILE;
+  auto unit_of = [&](int64_t u, int& kl, int64_t& ib, int64_t& ie) {
+    kl = (int)(u / a.units_per_walker);
     const int64_t ug = u - (int64_t)kl * a.units_per_walker;
-    const int k = a.k0 + kl;
-    const int64_t i_begin = ug * a.unit_tiles * TILE;
-    const int64_t i_end = min(a.N, i_begin + (int64_t)a.unit_tiles * TILE);     // exclusive
-    const double* nodes = a.nodes + (size_t)k * a.Nn * NODE_STRIDE;
-    const double2* aux = a.nodeaux + (size_t)k * a.Nn;
-    __syncthreads();                      // the previous unit is done with the shared tables
-    if (k != cur_k) {
-      if (tid < WC_STRIDE) s_wc[tid] = a.wc[(size_t)k * WC_STRIDE + tid];
-      cur_k = k;
-    }
-    if (tid <= a.n_max) s_Mb[tid] = 1;
-    if (tid == 0) s_Mu = 1;
-    const int32_t st = a.status[k];
-    if (st & (EMRI_ST_BADPARAM | EMRI_ST_DELAY | EMRI_ST_STATE)) {
-      for (int64_t i0 = i_begin + 2 * tid; i0 < i_end; i0 += TILE) {
-        if (a.outZ) {
-          a.outZ[(size_t)kl * a.N + i0] = make_double2(0.0, 0.0);
-          a.outZ[(size_t)kl * a.N + i0 + 1] = make_double2(0.0, 0.0);
-        } else {
-          *reinterpret_cast<double2*>(a.outI + (size_t)kl * a.pitch + i0) = make_double2(0.0, 0.0);
-          *reinterpret_cast<double2*>(a.outII + (size_t)kl * a.pitch + i0) = make_double2(0.0, 0.0);
+    ib = ug * unit_len;
+    ie = min(a.N, ib + unit_len);
+  };
+  if (producer && (int64_t)blockIdx.x < total) {
+    int kl; int64_t ib, ie;
+    unit_of(blockIdx.x, kl, ib, ie);
+    prepare_unit(a, lane, a.k0 + kl, ib, ie, Delta, inv_year, s_tab, s_wc, s_rot, s_Mb[0], &s_meta[0]);
+  }
+  __syncthreads();
+  int buf = 0;
+  for (int64_t u = blockIdx.x; u < total; u += gridDim.x, buf ^= 1) {
+    if (producer) {
+      const int64_t un = u + gridDim.x;
+      if (un < total) {
+        int kl; int64_t ib, ie;
+        unit_of(un, kl, ib, ie);
+        const int nb = buf ^ 1;
+        prepare_unit(a, lane, a.k0 + kl, ib, ie, Delta, inv_year, s_tab + nb * tab_elems, s_wc + nb * WC_STRIDE,
+                     s_rot + nb * 2 * UNIT_TILES_MAX, s_Mb[nb], &s_meta[nb]);
+      }
+    } else {
+      int kl; int64_t i_begin, i_end;
+      unit_of(u, kl, i_begin, i_end);
+      const int k = a.k0 + kl;
+      const UnitMeta mt = s_meta[buf];
+      if (mt.skip) {
+        for (int64_t i0 = i_begin + 2 * tid; i0 < i_end; i0 += TILE) {
+          if (a.outZ) {
+            a.outZ[(size_t)kl * a.N + i0] = make_double2(0.0, 0.0);
+            a.outZ[(size_t)kl * a.N + i0 + 1] = make_double2(0.0, 0.0);
+          } else {
+            *reinterpret_cast<double2*>(a.outI + (size_t)kl * a.pitch + i0) = make_double2(0.0, 0.0);
+            *reinterpret_cast<double2*>(a.outII + (size_t)kl * a.pitch + i0) = make_double2(0.0, 0.0);
+          }
         }
-      }
-      continue;
-    }
-    // ---- range of e over the unit from the node rows it touches (Hermite stays within pad of the nodes)
-    double w0, xmax, whi;
-    {
-      int64_t rlo = (i_begin >> a.logS) - 1 + 1, rhi = ((i_end - 1) >> a.logS) + 2 + 1;       // rows = node index + 1
-      if (rlo < 0) rlo = 0;
-      if (rhi > a.Nn - 1) rhi = a.Nn - 1;
-      double v[4] = {0.0, -1.0, 0.0, 0.0};       // max e, max -e, max |e'|, max |increment of e|
-      for (int64_t r = rlo + tid; r <= rhi; r += SYNTH_THREADS) {
-        const double* row = nodes + r * NODE_STRIDE;
-        const double ev = __ldg(row + 3);
-        v[0] = fmax(v[0], ev); v[1] = fmax(v[1], -ev);
-        v[2] = fmax(v[2], fabs(__ldg(row + 8))); v[3] = fmax(v[3], fabs(__ldg(row + 13)));
-      }
-      block_max4(v, s_red, warp, lane);
-      const double pad = 0.3 * fma(Delta, v[2], v[3]) + 1e-15;
-      const double elo = fmax(-v[1] - pad, 0.0), ehi = v[0] + pad;
-      whi = ehi * ehi;
-      w0 = 0.5 * fma(elo, elo, whi);
-      xmax = 0.5 * (whi - elo * elo) * (1.0 + 1e-9);
-    }
-    // ---- re-expansion of the three series of every harmonic about w0 (thread = (harmonic, series))
-    for (int task = tid; task < 3 * a.n_max; task += SYNTH_THREADS) {
-      const int n = task / 3 + 1, si = task - 3 * (n - 1);
-      const double* bp = reinterpret_cast<const double*>(a.base + (size_t)n * BASE_M) + si;
-      // base terms that matter at w <= whi (terms rise, then fall: the running maximum is a safe scale)
-      int Mb = 1;
-      {
-        double pw = 1.0, mx = 0.0;
-        int below = 0;
-        for (int m = 0; m < BASE_M; ++m) {
-          const double t = fabs(__ldg(bp + 4 * m)) * pw;
-          mx = fmax(mx, t);
-          if (t >= a.tol * mx && t > 0.0) { Mb = m + 1; below = 0; }
-          else if (t > 0.0 && ++below >= 3) break;      // past the peak the terms fall monotonically
-          pw *= whi;
-        }
-      }
-      double d[MLOC];
-#pragma unroll
-      for (int j = 0; j < MLOC; ++j) d[j] = 0.0;
-      for (int m = Mb - 1; m >= 0; --m) {
-        const double c = __ldg(bp + 4 * m);
-#pragma unroll
-        for (int j = MLOC - 1; j >= 1; --j) d[j] = fma(d[j], w0, d[j - 1]);
-        d[0] = fma(d[0], w0, c);
-      }
-      int Ml = 1;
-      {
-        double pw = 1.0, mx = 0.0;
-#pragma unroll
-        for (int j = 0; j < MLOC; ++j) {
-          const double t = fabs(d[j]) * pw;
-          mx = fmax(mx, t);
-          if (t >= a.tol * mx && t > 0.0) Ml = j + 1;
-          pw *= xmax;
-        }
-      }
-      double* dst = reinterpret_cast<double*>(s_tab + (size_t)n * MLOC) + si;
-#pragma unroll
-      for (int j = 0; j < MLOC; ++j) dst[4 * j] = d[j];
-      atomicMax(&s_Mu, Ml);                    // Ml == MLOC: order MLOC-1 still significant, the tail is not bounded
-      atomicMax(&s_Mb[n], Mb);
-    }
-    if (tid >= SYNTH_THREADS - a.unit_tiles) {
-      // detector phase at the start of each tile of the unit
-      const int t = tid - (SYNTH_THREADS - a.unit_tiles);
-      double sb, cb;
-      sincospi(2.0 * frac((double)(i_begin + (int64_t)t * TILE) * a.dt * inv_year), &sb, &cb);
-      s_rot[2 * t] = cb; s_rot[2 * t + 1] = sb;
-    }
-    __syncthreads();
-    const int Mu = s_Mu;
-    const bool fallback = Mu >= MLOC;
-    const double w0e = fallback ? 0.0 : w0;
-    const int32_t jpl = a.jpl[k];
-    for (int t = 0; t < a.unit_tiles; ++t) {
-      const int64_t i0 = i_begin + (int64_t)t * TILE + 2 * tid;
-      if (i0 >= i_end) break;
-      // detector phase: tile start (x) thread offset, then one sample step
-      const double cb = s_rot[2 * t], sb = s_rot[2 * t + 1];
-      const double cpa = fma(cb, co, -sb * so), spa = fma(sb, co, cb * so);
-      const double cpb2 = fma(cpa, c1s, -spa * s1s), spb2 = fma(spa, c1s, cpa * s1s);
-      SampleOut A, B;
-      double* fin = s_fin + tid;
-      sample_setup(s_wc, nodes, aux, i0, a.S, a.logS, invS, Delta, jpl, cpa, spa, w0e, A, fin, 2 * SYNTH_THREADS);
-      sample_setup(s_wc, nodes, aux, i0 + 1, a.S, a.logS, invS, Delta, jpl, cpb2, spb2, w0e, B, fin + SYNTH_THREADS,
-                   2 * SYNTH_THREADS);
-      double S[6];
-      switch (Mu) {
-        case 1: harmonic_sum_local<1>(s_tab, a.n_max, A, B, S); break;
-        case 2: harmonic_sum_local<2>(s_tab, a.n_max, A, B, S); break;
-        case 3: harmonic_sum_local<3>(s_tab, a.n_max, A, B, S); break;
-        case 4: harmonic_sum_local<4>(s_tab, a.n_max, A, B, S); break;
-        case 5: harmonic_sum_local<5>(s_tab, a.n_max, A, B, S); break;
-        case 6: harmonic_sum_local<6>(s_tab, a.n_max, A, B, S); break;
-        case 7: harmonic_sum_local<7>(s_tab, a.n_max, A, B, S); break;
-        case 8: harmonic_sum_local<8>(s_tab, a.n_max, A, B, S); break;
-        default: harmonic_sum_base(a.base, s_Mb, a.n_max, A, B, S); break;
-      }
-      const double hIa = fma(fin[0], S[0], fma(fin[2 * SYNTH_THREADS], S[1], fin[4 * SYNTH_THREADS] * S[2]));
-      const double hIIa = fma(fin[6 * SYNTH_THREADS], S[0], fma(fin[8 * SYNTH_THREADS], S[1], fin[10 * SYNTH_THREADS] * S[2]));
-      const double* fb = fin + SYNTH_THREADS;
-      const double hIb = fma(fb[0], S[3], fma(fb[2 * SYNTH_THREADS], S[4], fb[4 * SYNTH_THREADS] * S[5]));
-      const double hIIb = fma(fb[6 * SYNTH_THREADS], S[3], fma(fb[8 * SYNTH_THREADS], S[4], fb[10 * SYNTH_THREADS] * S[5]));
-      if (a.outZ) {
-        a.outZ[(size_t)kl * a.N + i0] = make_double2(hIa, hIIa);
-        a.outZ[(size_t)kl * a.N + i0 + 1] = make_double2(hIb, hIIb);
       } else {
-        *reinterpret_cast<double2*>(a.outI + (size_t)kl * a.pitch + i0) = make_double2(hIa, hIb);
-        *reinterpret_cast<double2*>(a.outII + (size_t)kl * a.pitch + i0) = make_double2(hIIa, hIIb);
+        const double* nodes = a.nodes + (size_t)k * a.Nn * NODE_STRIDE;
+        const double2* aux = a.nodeaux + (size_t)k * a.Nn;
+        const double4* tab = s_tab + buf * tab_elems;
+        const double* wc = s_wc + buf * WC_STRIDE;
+        const double* rot = s_rot + buf * 2 * UNIT_TILES_MAX;
+        for (int t = 0; t < a.unit_tiles; ++t) {
+          const int64_t i0 = i_begin + (int64_t)t * TILE + 2 * tid;
+          if (i0 >= i_end) break;
+          // detector phase: tile start (x) thread offset, then one sample step
+          const double cb = rot[2 * t], sb = rot[2 * t + 1];
+          const double cpa = fma(cb, co, -sb * so), spa = fma(sb, co, cb * so);
+          const double cpb2 = fma(cpa, c1s, -spa * s1s), spb2 = fma(spa, c1s, cpa * s1s);
+          SampleOut A, B;
+          double* fin = s_fin + tid;
+          sample_setup(wc, s_sct, nodes, aux, i0, a.S, a.logS, invS, Delta, mt.jpl, cpa, spa, mt.w0e, A, fin, 2 * SYNTH_THREADS);
+          sample_setup(wc, s_sct, nodes, aux, i0 + 1, a.S, a.logS, invS, Delta, mt.jpl, cpb2, spb2, mt.w0e, B,
+                       fin + SYNTH_THREADS, 2 * SYNTH_THREADS);
+          double S[6];
+          switch (mt.Mu) {
+            case 1: harmonic_sum_local<1>(tab, a.n_max, A, B, S); break;
+            case 2: harmonic_sum_local<2>(tab, a.n_max, A, B, S); break;
+            case 3: harmonic_sum_local<3>(tab, a.n_max, A, B, S); break;
+            case 4: harmonic_sum_local<4>(tab, a.n_max, A, B, S); break;
+            case 5: harmonic_sum_local<5>(tab, a.n_max, A, B, S); break;
+            case 6: harmonic_sum_local<6>(tab, a.n_max, A, B, S); break;
+            case 7: harmonic_sum_local<7>(tab, a.n_max, A, B, S); break;
+            case 8: harmonic_sum_local<8>(tab, a.n_max, A, B, S); break;
+            default: harmonic_sum_base(a.base, s_Mb[buf], a.n_max, A, B, S); break;
+          }
+          const double hIa = fma(fin[0], S[0], fma(fin[2 * SYNTH_THREADS], S[1], fin[4 * SYNTH_THREADS] * S[2]));
+          const double hIIa = fma(fin[6 * SYNTH_THREADS], S[0], fma(fin[8 * SYNTH_THREADS], S[1], fin[10 * SYNTH_THREADS] * S[2]));
+          const double* fb = fin + SYNTH_THREADS;
+          const double hIb = fma(fb[0], S[3], fma(fb[2 * SYNTH_THREADS], S[4], fb[4 * SYNTH_THREADS] * S[5]));
+          const double hIIb = fma(fb[6 * SYNTH_THREADS], S[3], fma(fb[8 * SYNTH_THREADS], S[4], fb[10 * SYNTH_THREADS] * S[5]));
+          if (a.outZ) {
+            a.outZ[(size_t)kl * a.N + i0] = make_double2(hIa, hIIa);
+            a.outZ[(size_t)kl * a.N + i0 + 1] = make_double2(hIb, hIIb);
+          } else {
+            *reinterpret_cast<double2*>(a.outI + (size_t)kl * a.pitch + i0) = make_double2(hIa, hIb);
+            *reinterpret_cast<double2*>(a.outII + (size_t)kl * a.pitch + i0) = make_double2(hIIa, hIIb);
+          }
+        }
       }
     }
+    __syncthreads();      // unit u consumed and the tables of unit u + gridDim.x complete
   }
 }
-
 }  // namespace
