@@ -1,0 +1,144 @@
+"""BASELINE.json configs at FULL size, in the launch configuration bench.py times (whole ensemble in one
+emri_loglike call), compared with the oracle on a seeded subset of walkers and on sampled outputs;
+plus the edge cases of the boundary (non-power-of-two N, one walker, the n_max cap, masked bins)."""
+import numpy as np
+import pytest
+
+from paper_2311_17174_b200 import workloads as W
+
+torch = pytest.importorskip("torch")
+pytestmark = pytest.mark.gpu
+H_TOL = 1e-9
+
+
+@pytest.fixture(scope="module")
+def emri():
+    if not torch.cuda.is_available():
+        pytest.skip("no CUDA device")
+    from paper_2311_17174_b200 import emri as m
+    m.load()
+    return m
+
+
+def dev(a):
+    return torch.from_numpy(np.ascontiguousarray(a)).cuda()
+
+
+def logl_ok(got, ref):
+    return np.all(np.abs(got - ref) <= 1e-9 * np.abs(ref) + 1e-6)
+
+
+@pytest.mark.parametrize("ci,n_sub", [(0, 8), (1, 4), (2, 4), (3, 4)])
+def test_full_size_loglike_on_walker_subset(emri, oracle, ci, n_sub):
+    cfg = W.CONFIGS[ci]
+    P = W.draw_params(cfg)
+    psd = W.lisa_psd_barack_cutler(cfg.N, cfg.dt)
+    sub = W.parity_walker_subset(P, n=n_sub)
+    hI, hII, st0 = oracle.waveform(P[0], cfg.N, cfg.dt, cfg.n_max)
+    D = np.stack([oracle.rfft(hI), oracle.rfft(hII)])
+    if cfg.noise_seed:
+        D = D + W.noise_fft(cfg.N, cfg.dt, psd, cfg.noise_seed)
+    ref, st_ref = oracle.loglike_batch(P[sub], cfg.N, cfg.dt, cfg.n_max, D, psd)
+    plan = emri.Plan(cfg.N, cfg.dt, cfg.n_max, cfg.K, psd)
+    st = torch.zeros(cfg.K, dtype=torch.int32, device="cuda")
+    got = plan.loglike(dev(P), dev(D), status=st)
+    torch.cuda.synchronize()
+    got, st = got.cpu().numpy(), st.cpu().numpy()
+    print(f"cfg{ci} K={cfg.K} N={cfg.N} n_max={cfg.n_max}: walkers {sub} logL ref {ref} |diff| {np.abs(got[sub] - ref)}")
+    assert not st.any() and not st_ref.any()
+    assert np.all(np.isfinite(got)) and logl_ok(got[sub], ref)
+    if not cfg.noise_seed:
+        assert abs(got[0]) <= 1e-6          # noise-less data = walker 0's own waveform
+    modes = plan.orbit_report(cfg.K)
+    assert np.all(modes == 1)              # every walker's parallel-in-time orbit verified
+    plan.close()
+
+
+@pytest.mark.parametrize("ci", [1, 2])
+def test_full_size_waveform_sampled(emri, oracle, ci):
+    cfg = W.CONFIGS[ci]
+    P = W.draw_params(cfg)
+    sub = W.parity_walker_subset(P, n=6)
+    plan = emri.Plan(cfg.N, cfg.dt, cfg.n_max, len(sub))
+    hI, hII = plan.waveform(dev(P[sub]))
+    torch.cuda.synchronize()
+    hI, hII = hI.cpu().numpy(), hII.cpu().numpy()
+    rng = np.random.default_rng(100 + ci)
+    idx = np.unique(np.concatenate([np.arange(0, 520), np.arange(cfg.N - 520, cfg.N), rng.integers(0, cfg.N, 3000)]))
+    for r, k in enumerate(sub):
+        a, b, st = oracle.waveform(P[k], cfg.N, cfg.dt, cfg.n_max, idx=idx)
+        eI = np.max(np.abs(hI[r, idx] - a)) / np.max(np.abs(hI[r]))
+        eII = np.max(np.abs(hII[r, idx] - b)) / np.max(np.abs(hII[r]))
+        assert st == 0 and eI <= H_TOL and eII <= H_TOL, (k, eI, eII)
+    plan.close()
+
+
+def test_non_power_of_two_length_and_single_walker(emri, oracle):
+    """N = 1000 (cuFFT takes any even N); the oracle's transform here is its naive O(N^2) DFT"""
+    cfg = W.scaled(W.CONFIGS[1], K=3, N=1000)
+    P = W.draw_params(cfg)
+    psd = W.lisa_psd_barack_cutler(cfg.N, cfg.dt)
+    h_ref, _ = oracle.waveform_batch(P, cfg.N, cfg.dt, cfg.n_max)
+    D = np.stack([oracle.dft_naive(h_ref[0, 0]), oracle.dft_naive(h_ref[0, 1])]) + W.noise_fft(cfg.N, cfg.dt, psd, 7)
+    ref = np.array([oracle.loglike(np.stack([oracle.dft_naive(h_ref[k, 0]), oracle.dft_naive(h_ref[k, 1])]), D, psd,
+                                   cfg.N, cfg.dt) for k in range(cfg.K)])
+    plan = emri.Plan(cfg.N, cfg.dt, cfg.n_max, cfg.K, psd)
+    got = plan.loglike(dev(P), dev(D))
+    one = plan.loglike(dev(P[1:2]), dev(D))
+    sp = plan.waveform_fft(dev(P[:1]))
+    torch.cuda.synchronize()
+    assert logl_ok(got.cpu().numpy(), ref)
+    assert one.cpu().numpy()[0] == got.cpu().numpy()[1]                 # K = 1 gives the same bits
+    H0 = oracle.dft_naive(h_ref[0, 0])
+    assert np.max(np.abs(sp.cpu().numpy()[0, 0] - H0)) <= 1e-9 * np.max(np.abs(H0))
+    plan.close()
+
+
+def test_harmonic_cap_and_eccentric_walkers(emri, oracle):
+    """n_max = 48 (EMRI_NMAX_CAP) with e0 up to 0.5: long base series, high local orders"""
+    cfg = W.scaled(W.CONFIGS[3], K=6, N=1 << 12, n_max=48)
+    P = W.draw_params(cfg)
+    P[:, W.P_E0] = np.linspace(0.0, 0.5, cfg.K)
+    for k in range(cfg.K):
+        P[k, W.P_NU0] = W.nu0_for_plunge_after(P[k, W.P_M], P[k, W.P_MU], P[k, W.P_E0], 4.0 * cfg.T_obs)
+    plan = emri.Plan(cfg.N, cfg.dt, cfg.n_max, cfg.K)
+    hI, hII = plan.waveform(dev(P))
+    torch.cuda.synchronize()
+    h_ref, st = oracle.waveform_batch(P, cfg.N, cfg.dt, cfg.n_max)
+    assert not st.any()
+    for ch, got in ((0, hI.cpu().numpy()), (1, hII.cpu().numpy())):
+        err = np.max(np.abs(got - h_ref[:, ch]), axis=1) / np.max(np.abs(h_ref[:, ch]), axis=1)
+        print("n_max=48 err", err)
+        assert np.all(err <= H_TOL)
+    plan.close()
+
+
+def test_circular_orbit_has_only_the_quadrupole(emri, oracle):
+    """e = 0 exactly (reading R18): e' = 0 keeps it there and only n = 2 survives: n_max = 2 and 30 agree"""
+    cfg = W.scaled(W.CONFIGS[1], K=2, N=1 << 12)
+    P = W.draw_params(cfg)
+    P[:, W.P_E0] = 0.0
+    out = []
+    for n_max in (2, 30):
+        plan = emri.Plan(cfg.N, cfg.dt, n_max, cfg.K)
+        hI, hII = plan.waveform(dev(P))
+        torch.cuda.synchronize()
+        out.append((hI.cpu().numpy(), hII.cpu().numpy()))
+        plan.close()
+    assert np.array_equal(out[0][0], out[1][0]) and np.array_equal(out[0][1], out[1][1])
+    h_ref, _ = oracle.waveform_batch(P, cfg.N, cfg.dt, 30)
+    assert np.max(np.abs(out[1][0] - h_ref[:, 0])) <= H_TOL * np.max(np.abs(h_ref[:, 0]))
+
+
+def test_fully_masked_psd_gives_zero_and_invalid_walker_minus_inf(emri):
+    cfg = W.scaled(W.CONFIGS[0], K=3, N=1 << 10)
+    P = W.draw_params(cfg)
+    P[2, W.P_DL] = -1.0
+    psd = np.full(cfg.N // 2 + 1, np.inf)
+    plan = emri.Plan(cfg.N, cfg.dt, cfg.n_max, cfg.K, psd)
+    D = torch.ones((2, cfg.N // 2 + 1), dtype=torch.complex128, device="cuda")
+    st = torch.zeros(cfg.K, dtype=torch.int32, device="cuda")
+    got = plan.loglike(dev(P), D, status=st).cpu().numpy()
+    assert got[0] == 0.0 and got[1] == 0.0 and got[2] == -np.inf
+    assert list(st.cpu().numpy()) == [0, 0, 1]
+    plan.close()

@@ -1,0 +1,130 @@
+"""Config 4 (ensemble MCMC on the device) against the oracle -- protocol of SURVEY 8(d)-4 at a reduced size.
+Chains are chaotic under 1e-9 differences of logL, so the comparison is teacher-forced on the GPU's logged
+state: (A) partner, z, ln u', proposals recomputed by the oracle's own generator; (B) logL of the proposals by
+the oracle; (C) every accept flag consistent with the logged numbers (decisions inside the tolerance band are
+counted as ambiguous); (D) an independent oracle chain agrees with the GPU chain up to the first ambiguous
+decision."""
+import numpy as np
+import pytest
+
+from oracle import stretch
+from paper_2311_17174_b200 import workloads as W
+
+torch = pytest.importorskip("torch")
+pytestmark = pytest.mark.gpu
+
+A_STRETCH, SEED = 2.0, 20231117
+
+
+@pytest.fixture(scope="module")
+def emri():
+    if not torch.cuda.is_available():
+        pytest.skip("no CUDA device")
+    from paper_2311_17174_b200 import emri as m
+    m.load()
+    return m
+
+
+def dev(a):
+    return torch.from_numpy(np.ascontiguousarray(a)).cuda()
+
+
+def setup(oracle, K, N, n_max):
+    cfg = W.scaled(W.CONFIGS[4], K=K, N=N, n_max=n_max)
+    X0 = W.draw_params(cfg)
+    lo, hi = W.prior_box(cfg)
+    psd = W.lisa_psd_barack_cutler(N, cfg.dt)
+    hI, hII, st = oracle.waveform(X0[0], N, cfg.dt, n_max)
+    assert st == 0
+    D = np.stack([oracle.rfft(hI), oracle.rfft(hII)]) + W.noise_fft(N, cfg.dt, psd, cfg.noise_seed)
+    return cfg, X0, lo, hi, psd, D
+
+
+def test_stretch_steps_teacher_forced(emri, oracle):
+    K, N, n_max, steps = 16, 1 << 12, 5, 12
+    cfg, X0, lo, hi, psd, D = setup(oracle, K, N, n_max)
+    H = K // 2
+    plan = emri.Plan(N, cfg.dt, n_max, K, psd)
+    X, D_d, lo_d, hi_d = dev(X0), dev(D), dev(lo), dev(hi)
+    logL = plan.loglike(X, D_d)
+    torch.cuda.synchronize()
+    ref0, _ = oracle.loglike_batch(X0, N, cfg.dt, n_max, D, psd)
+    assert np.all(np.abs(logL.cpu().numpy() - ref0) <= 1e-9 * np.abs(ref0) + 1e-6)
+    acc_d = torch.zeros(K, dtype=torch.int32, device="cuda")
+    log_d = torch.zeros((H, 21), dtype=torch.float64, device="cuda")
+    n_free = int(np.sum(lo < hi))
+    # independent oracle chain (D), advanced with its own logL
+    Xo, Lo = X0.copy(), ref0.copy()
+    diverged, ambiguous, accepted = False, 0, 0
+
+    def oracle_logl(Y):
+        return oracle.loglike_batch(Y, N, cfg.dt, n_max, D, psd)[0]
+
+    for step in range(steps):
+        for half in (0, 1):
+            Xb, Lb = X.cpu().numpy().copy(), logL.cpu().numpy().copy()      # GPU state before the half step
+            plan.stretch_step(X, logL, D_d, lo_d, hi_d, A_STRETCH, SEED, step, half, accepted=acc_d, log_buf=log_d)
+            torch.cuda.synchronize()
+            lg, acc = log_d.cpu().numpy(), acc_d.cpu().numpy()[half * H:half * H + H].astype(bool)
+            # (A) generator and proposal arithmetic, teacher-forced on the GPU's state
+            prop = stretch.propose(Xb, lo, hi, A_STRETCH, SEED, step, half)
+            assert np.array_equal(lg[:, 20].astype(np.int64), prop["partner"])
+            np.testing.assert_allclose(lg[:, 17], prop["z"], rtol=1e-15)
+            np.testing.assert_allclose(lg[:, 18], prop["lnu"], rtol=1e-14, atol=1e-15)
+            # Y = X_j + z (X_k - X_j): one rounding of each operation, relative to the operands (the difference cancels)
+            act0 = slice(half * H, half * H + H)
+            scale = np.abs(Xb[act0]) + np.abs(Xb[prop["partner"]])
+            assert np.all(np.abs(lg[:, :17] - prop["Y"]) <= 1e-15 * scale)
+            # (B) logL of the proposals
+            lY_ref = np.where(prop["inbox"], oracle_logl(prop["Y"]), -np.inf)
+            fin = np.isfinite(lY_ref)
+            assert np.array_equal(np.isfinite(lg[:, 19]), fin)
+            tol = 1e-9 * np.abs(lY_ref[fin]) + 1e-6
+            assert np.all(np.abs(lg[fin, 19] - lY_ref[fin]) <= tol)
+            # (C) accept flags against the logged numbers; margin inside the band = ambiguous
+            act = slice(half * H, half * H + H)
+            lnq = (n_free - 1) * np.log(lg[:, 17]) + lg[:, 19] - Lb[act]
+            margin = lnq - lg[:, 18]
+            band = 2e-9 * (np.abs(lg[:, 19]) + np.abs(Lb[act])) + 2e-6
+            clear = fin & (np.abs(margin) > band)
+            assert np.array_equal(acc[clear], margin[clear] > 0)
+            assert not acc[~fin].any()
+            ambiguous += int(np.sum(fin & ~clear))
+            accepted += int(acc.sum())
+            # accepted walkers moved to the proposal, the others stayed; logL follows
+            Xa, La = X.cpu().numpy(), logL.cpu().numpy()
+            assert np.array_equal(Xa[act][acc], lg[acc, :17]) and np.array_equal(Xa[act][~acc], Xb[act][~acc])
+            assert np.array_equal(La[act][acc], lg[acc, 19]) and np.array_equal(La[act][~acc], Lb[act][~acc])
+            # (D) independent chain
+            if not diverged:
+                acc_o, prop_o, lY_o = stretch.half_step(Xo, Lo, lo, hi, A_STRETCH, SEED, step, half, oracle_logl)
+                lnq_o = (n_free - 1) * np.log(prop_o["z"]) + np.where(prop_o["inbox"], lY_o, -np.inf) - Lb[act]
+                if np.any(np.abs(lnq_o - prop_o["lnu"]) <= 2e-9 * (np.abs(lY_o) + np.abs(Lb[act])) + 2e-6):
+                    diverged = True          # an ambiguous decision: the chains may legitimately part here
+                else:
+                    assert np.array_equal(acc_o, acc)
+                    np.testing.assert_allclose(Xo, Xa, rtol=1e-13, atol=0)
+                    assert np.all(np.abs(Lo - La) <= 1e-9 * np.abs(Lo) + 1e-6)
+    print(f"accepted {accepted} of {2 * steps * H}, ambiguous {ambiguous}, independent chain diverged: {diverged}")
+    assert accepted > 0 and ambiguous <= 2
+    plan.close()
+
+
+def test_out_of_box_proposals_are_rejected_without_changing_the_walker(emri, oracle):
+    K, N, n_max = 8, 1 << 10, 5
+    cfg, X0, lo, hi, psd, D = setup(oracle, K, N, n_max)
+    lo2, hi2 = lo.copy(), hi.copy()
+    hi2[W.P_DL] = X0[:, W.P_DL].min() * (1 - 1e-12)      # every D_L proposal above this is outside
+    lo2[W.P_DL] = 0.0
+    plan = emri.Plan(N, cfg.dt, n_max, K, psd)
+    X, D_d = dev(X0), dev(D)
+    logL = plan.loglike(X, D_d)
+    acc = torch.zeros(K, dtype=torch.int32, device="cuda")
+    before = X.clone()
+    plan.stretch_step(X, logL, D_d, dev(lo2), dev(hi2), A_STRETCH, SEED, 0, 0, accepted=acc)
+    torch.cuda.synchronize()
+    prop = stretch.propose(X0, lo2, hi2, A_STRETCH, SEED, 0, 0)
+    a = acc.cpu().numpy()[:K // 2].astype(bool)
+    assert not a[~prop["inbox"]].any() and (~prop["inbox"]).any()
+    assert torch.equal(X[:K // 2][~torch.from_numpy(a).cuda()], before[:K // 2][~torch.from_numpy(a).cuda()])
+    plan.close()
