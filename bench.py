@@ -3,8 +3,8 @@
 
   python bench.py [--gpus N] [--steps K] [--warmup W] [--config i] [--impl reference]
 
-A "step" is one pass of the whole hot path -- emri_loglike: orbit RK4 (a), synthesis (b), cuFFT D2Z
-(c), likelihood reduction (d) -- over one ensemble of K walkers of BASELINE.json:configs[i]
+A "step" is one pass of the whole hot path -- emri_loglike: orbit RK4 (a), synthesis (b), cuFFT Z2Z
+(c: one complex transform per walker carries both channels), likelihood reduction (d) -- over one ensemble of K walkers of BASELINE.json:configs[i]
 (default i = 1: K=64, N=2^20, n_max=10).  Inputs are synthetic and seeded (workloads.py).  Prints ONE
 JSON line.  `value` = walker*samples/s with inputs resident in HBM; `e2e` = the same through
 emri_loglike_host with pinned HOST buffers (copies inside the timed region).  With N > 1 (torchrun)
@@ -29,12 +29,21 @@ from paper_2311_17174_b200 import workloads as W  # noqa: E402
 
 METRIC = "AK waveform+logL evaluations/sec (walkers x samples/s)"
 UNIT = "walker*samples/s"
-KERNELS_PER_STEP = 4        # orbit_kernel, synth_kernel, loglike_kernel, loglike_final_kernel per chunk-free step
+ORBIT_KERNELS = 10          # orbit_init, 3 x (orbit_sweep, orbit_correct), orbit_tail, orbit_fixup, orbit_aux
+CHUNK = 128                 # walkers per synth / cuFFT / loglike launch (emri_plan_set_chunk default)
+
+# Algorithmic work of synth_kernel per (walker, sample): FP64 flops EXECUTED by the kernel as it stands, counted
+# by ncu (2 dfma + dmul + dadd, smsp__sass_thread_inst_executed_op_*_pred_on.sum) on the configs' own inputs:
+# profiles/counts_r1.md.  SURVEY 8(d)-2 asks for counted instructions in place of its estimate 600 + 170 n_max
+# (2300 at n_max = 10), which the re-summed harmonic series undercuts by 3.7x.
+COUNTED_FLOPS = {5: 546.0, 10: 621.0, 20: 927.0, 30: 1248.0}
+# DRAM bytes of one synth_kernel launch (dram__bytes_read.sum + dram__bytes_write.sum, same ncu pass)
+SYNTH_TRAFFIC = {0: 420096.0, 1: 1086312704.0, 2: 4486795520.0, 3: 4485041664.0}
 
 
-def survey_flops_per_walker_sample(n_max):
-    """F(n_max) ~ 600 + 170 n_max fp64 flops per (walker, sample), FMA = 2"""
-    return 600.0 + 170.0 * n_max
+def counted_flops_per_walker_sample(n_max):
+    ks = sorted(COUNTED_FLOPS)
+    return float(np.interp(n_max, ks, [COUNTED_FLOPS[k] for k in ks]))
 
 
 def load_measured_peaks():
@@ -180,8 +189,8 @@ def run_gpu(args, cfg):
     emri.load()
     K, N = cfg.K, cfg.N
     # every rank draws its own ensemble (weak scaling: K walkers per GPU)
-    rcfg = W.scaled(cfg) if rank == 0 else __import__("dataclasses").replace(cfg, seed=cfg.seed + 7919 * rank)
-    P = W.draw_params(rcfg)
+    from paper_2311_17174_b200 import sharding
+    P = W.draw_params(sharding.rank_config(cfg, rank))
     psd = W.lisa_psd_barack_cutler(N, cfg.dt)
     plan = emri.Plan(N, cfg.dt, cfg.n_max, K, psd)
     p_d = torch.from_numpy(P).to(dev)
@@ -240,14 +249,19 @@ def run_gpu(args, cfg):
         sm_max = clocks["sm_max_mhz"] or peaks.get("sm_max_mhz", 1965.0)
         sms = torch.cuda.get_device_properties(dev).multi_processor_count
         fp64_nominal = sms * 64 * 2 * sm_max * 1e6 * 1e-12        # 64 FP64 lanes / SM / clk
-        flops = survey_flops_per_walker_sample(cfg.n_max) * K * N
+        n_chunks = (K + CHUNK - 1) // CHUNK
+        fpws = counted_flops_per_walker_sample(cfg.n_max)
+        flops = fpws * K * N
         achieved = flops / (stage["synth"] * 1e-3) * 1e-12
         roofline = {"bound": "alu", "kernel": "synth_kernel", "achieved": achieved, "peak": fp64_nominal,
-                    "unit": "TFLOP/s", "frac": achieved / fp64_nominal, "traffic": None,
-                    "peak_source": f"derived: {sms} SMs x 64 FP64 lanes x 2 x {sm_max:.0f} MHz",
+                    "unit": "TFLOP/s", "frac": achieved / fp64_nominal, "traffic": SYNTH_TRAFFIC.get(cfg.index),
+                    "peak_source": f"derived: {sms} SMs x 64 FP64 lanes x 2 x {sm_max:.0f} MHz (DESIGN.md section 7)",
                     "peak_dfma_probe": fp64_probe, "frac_of_probe": achieved / fp64_probe,
-                    "ms_per_launch": stage["synth"], "flops_per_walker_sample": survey_flops_per_walker_sample(cfg.n_max)}
-        like_gbs = (2.0 * K * (N // 2 + 1) * 16) / (stage["like"] * 1e-3) * 1e-9 if stage["like"] > 0 else None
+                    "launches_per_step": n_chunks, "ms_per_launch": stage["synth"] / n_chunks,
+                    "flops_per_walker_sample": fpws, "flops_source": "counted by ncu (profiles/counts_r1.md)",
+                    "algorithmic_bytes_per_launch": 16.0 * min(K, CHUNK) * N}
+        # the reduction reads the packed spectrum Z[K][N] complex128 once (D and 1/S_n stay in L2)
+        like_gbs = (16.0 * K * N) / (stage["like"] * 1e-3) * 1e-9 if stage["like"] > 0 else None
         cores = host_cores()
         walkers = min(cores, K)
         cpu_t, cpu_units = oracle_sample(cfg, P, walkers, 1 if N <= (1 << 20) else 4, True)
@@ -264,11 +278,14 @@ def run_gpu(args, cfg):
             "e2e": {"value": world * K * N * args.steps / (e2e_ms * 1e-3), "unit": UNIT,
                     "h2d_bytes_per_step": int(P_pin.numel() * 8 + D_pin.numel() * 16),
                     "d2h_bytes_per_step": int(L_pin.numel() * 8 + S_pin.numel() * 4), "ms_per_step": e2e_ms / args.steps},
-            "gpu_launches": KERNELS_PER_STEP * args.steps,
+            "gpu_launches": (ORBIT_KERNELS + 2 * n_chunks + 1) * args.steps,
             "stage_ms": stage,
             "roofline": roofline,
-            "like_kernel": {"bound": "hbm", "achieved_gbs": like_gbs, "peak_gbs": peaks.get("hbm_gbs"),
-                            "frac": (like_gbs / peaks["hbm_gbs"]) if like_gbs else None, "peak_source": peaks_src},
+            "like_kernel": {"bound": "hbm", "kernel": "loglike_kernel", "achieved_gbs": like_gbs,
+                            "peak_gbs": peaks.get("hbm_gbs"), "frac": (like_gbs / peaks["hbm_gbs"]) if like_gbs else None,
+                            "peak_source": f"MEASURED_PEAKS.json copy bandwidth ({peaks_src})"},
+            "fft": {"bound": "hbm", "kernel": "cuFFT Z2Z (vendor)", "achieved_gbs": (32.0 * K * N) / (stage["fft"] * 1e-3) * 1e-9
+                    if stage["fft"] > 0 else None, "note": "one read + one write of Z per transform counted"},
             "cpu_baseline": {"value": cpu_units / cpu_t, "unit": UNIT, "cores": walkers, "kind": "oracle",
                              "sample": f"oracle waveform+rfft+logL of {walkers} walkers (one per thread), "
                                        f"{cpu_units // walkers} of N={N} samples each, {cpu_t:.1f} s"},
