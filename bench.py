@@ -202,8 +202,25 @@ def run_gpu(args, cfg):
     logL = torch.empty(K, dtype=torch.float64, device=dev)
     status = torch.zeros(K, dtype=torch.int32, device=dev)
 
-    for _ in range(max(args.warmup, 3)):
+    mcmc = cfg.index == 4
+    if mcmc:
+        # configs[4]: a step is one full stretch-move update (both half-ensembles), proposals / accept on the device
+        lo_d, hi_d = (torch.from_numpy(v).to(dev) for v in W.prior_box(cfg))
+        acc = torch.zeros(K, dtype=torch.int32, device=dev)
         plan.loglike(p_d, D, logL, status)
+        X = p_d.clone()
+        counter = [0]
+
+        def one_step():
+            for half in (0, 1):
+                plan.stretch_step(X, logL, D, lo_d, hi_d, 2.0, 20231117, counter[0], half, accepted=acc)
+            counter[0] += 1
+    else:
+        def one_step():
+            plan.loglike(p_d, D, logL, status)
+
+    for _ in range(max(args.warmup, 3)):
+        one_step()
     barrier()
     sampler = ClockSampler(torch.cuda.current_device() if "CUDA_VISIBLE_DEVICES" not in os.environ else local)
     sampler.start()
@@ -211,11 +228,13 @@ def run_gpu(args, cfg):
     barrier()
     e0.record()
     for _ in range(args.steps):
-        plan.loglike(p_d, D, logL, status)
+        one_step()
     e1.record()
     barrier()
     ms = max_over_ranks(e0.elapsed_time(e1))
     n_bad = int((status != 0).sum().item())
+    if mcmc:        # the chain has moved X and logL; the e2e check below is against the initial ensemble
+        logL = plan.loglike(p_d, D, status=status)
     logL_host = logL.cpu().numpy()
 
     # ---- end to end: pinned host buffers in, logL out, through emri_loglike_host
@@ -258,7 +277,7 @@ def run_gpu(args, cfg):
                     "peak_source": f"derived: {sms} SMs x 64 FP64 lanes x 2 x {sm_max:.0f} MHz (DESIGN.md section 7)",
                     "peak_dfma_probe": fp64_probe, "frac_of_probe": achieved / fp64_probe,
                     "launches_per_step": n_chunks, "ms_per_launch": stage["synth"] / n_chunks,
-                    "flops_per_walker_sample": fpws, "flops_source": "counted by ncu (profiles/counts_r1.md)",
+                    "flops_per_walker_sample": fpws, "flops_source": "counted by ncu (profiles/counts_r1.md)" + (", figure of configs[2] at the same n_max" if mcmc else ""),
                     "algorithmic_bytes_per_launch": 16.0 * min(K, CHUNK) * N}
         # the reduction reads the packed spectrum Z[K][N] complex128 once (D and 1/S_n stay in L2)
         like_gbs = (16.0 * K * N) / (stage["like"] * 1e-3) * 1e-9 if stage["like"] > 0 else None
@@ -302,7 +321,7 @@ def main():
     ap.add_argument("--gpus", type=int, default=1)
     ap.add_argument("--steps", type=int, default=10)
     ap.add_argument("--warmup", type=int, default=3)
-    ap.add_argument("--config", type=int, default=1, help="index into BASELINE.json:configs (0-3)")
+    ap.add_argument("--config", type=int, default=1, help="index into BASELINE.json:configs (0-4; 4 = stretch-move steps)")
     ap.add_argument("--impl", default="b200", choices=["b200", "reference"])
     args = ap.parse_args()
     cfg = W.CONFIGS[args.config]
