@@ -42,7 +42,7 @@ DEVINL void cosmo_integrals(double z, double Om, double* I1, double* I2) {
 DEVINL double z_of_dL(double D, double tH, double Om) {
   double lo = 0.0, hi = 20.0;
   double z = fmin(D / tH, 1.0);
-  for (int it = 0; it < 60; ++it) {
+  for (int it = 0; it < 24; ++it) {
     double I1, I2;
     cosmo_integrals(z, Om, &I1, &I2);
     double f = (1.0 + z) * tH * I1 - D;
@@ -50,7 +50,7 @@ DEVINL double z_of_dL(double D, double tH, double Om) {
     double fp = tH * (I1 + (1.0 + z) / Ez(z, Om));
     double zn = z - f / fp;
     if (!(zn > lo && zn < hi)) zn = 0.5 * (lo + hi);
-    if (fabs(zn - z) <= 4e-16 * fmax(zn, 1e-300)) { z = zn; break; }
+    if (fabs(zn - z) <= 2e-15 * fmax(zn, 1e-300)) { z = zn; break; }      // Newton: the step before was ~1e-8
     z = zn;
   }
   return z;
