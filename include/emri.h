@@ -139,6 +139,17 @@ int emri_data_fft(emri_plan* p, const double* d_I, const double* d_II, double* d
 int emri_loglike(emri_plan* p, const double* params, int K, const double* data_fft, double* logL,
                  int32_t* status, void* cuda_stream);
 
+/* emri_loglike with the frequency-dependent propagation of Eq. 7 (alpha_M = F(z,f), alpha_T = G(z,f),
+ * "a power series expansion sum_n a_n(z) (f/f_*)^n ... such frequency-dependent terms need to act upon a tabulated
+ * waveform in frequency space"; get_damping(), get_modified_speed()).  Every walker's spectrum is
+ * multiplied per bin, inside the reduction kernel, by
+ *     G_k(f) = exp(-Dm_k(f)) exp(-2 pi i f tau_k(f)),   Dm_k = sum_{n=1..3} a_{k,n} (f/f_*)^n,  tau_k = sum_{n=1..3} b_{k,n} (f/f_*)^n [s]
+ * (the integrated friction and delay series of Eqs. 4-5; the n = 0 terms are Xi(z) and Delta T of the parameter row)
+ * and logL[k] = -(2 dt/N) sum |D - G_k H_k|^2 / S_n.   fcoef: DEV [K][6] rows {a1,a2,a3,b1,b2,b3}; f_star > 0 [Hz].
+ * All-zero rows reproduce emri_loglike bit for bit up to the factor G = 1 (exp(0), cos(0)). */
+int emri_loglike_fdep(emri_plan* p, const double* params, int K, const double* fcoef, double f_star,
+                      const double* data_fft, double* logL, int32_t* status, void* cuda_stream);
+
 /* Same as emri_loglike with HOST buffers: copies params (and data_fft, unless it is NULL, in which
  * case the data uploaded by the previous non-NULL call is reused) to the device, runs the path,
  * copies logL and status back and synchronises the stream.  This is the end-to-end entry point

@@ -635,6 +635,37 @@ double emri_o_loglike(const double* H, const double* D, const double* psd, int64
 }
 
 // <a|b> = 4 Re sum_chan sum_m conj(a~) b~ / S_n df with a~ = dt A[m]: = (4 dt / N) Re sum conj(A) B / S
+// Frequency-dependent propagation (Eq. 7: alpha_M = F(z,f), alpha_T = G(z,f), "an example includes a
+// power series expansion sum_n a_n(z) (f/f_*)^n ... such frequency-dependent terms need to act upon a tabulated
+// waveform in frequency space"; get_damping(), get_modified_speed() at PAPER.md:143).  Reading D11 of DESIGN.md: by
+// Eq. 4-5 a frequency-dependent friction multiplies the spectrum by exp(-Dm(f)) and a frequency-dependent speed
+// delays it by tau(f), i.e. multiplies it by exp(-2 pi i f tau(f)) (k -> 2 pi f), with the integrated power series
+//   Dm(f) = sum_{n=1..3} a_n (f/f_*)^n,      tau(f) = sum_{n=1..3} b_n (f/f_*)^n  [s],     fcoef = {a1,a2,a3,b1,b2,b3}.
+// The n = 0 terms are the frequency-independent Xi(z) and Delta T already inside the waveform.
+//   logL = -(2 dt/N) sum_ch sum_m |D[m] - G[m] H[m]|^2 / S_n(f_m),   G[m] = exp(-Dm(f_m)) exp(-2 pi i f_m tau(f_m)).
+double emri_o_loglike_fdep(const double* H, const double* D, const double* psd, int64_t N, double dt, const double* fcoef,
+                           double fstar) {
+  const int64_t Nf = N / 2 + 1;
+  const long double twopi = 6.283185307179586476925286766559L;
+  long double acc = 0;
+  for (int ch = 0; ch < 2; ++ch)
+    for (int64_t m = 0; m < Nf; ++m) {
+      double s = psd[m];
+      if (!(s > 0) || !std::isfinite(s)) continue;
+      const long double f = (long double)m / ((long double)N * (long double)dt);
+      const long double x = f / (long double)fstar;
+      const long double Dm = fcoef[0] * x + fcoef[1] * x * x + fcoef[2] * x * x * x;
+      const long double tau = fcoef[3] * x + fcoef[4] * x * x + fcoef[5] * x * x * x;
+      const long double g = expl(-Dm), ph = -twopi * f * tau;
+      const long double gr = g * cosl(ph), gi = g * sinl(ph);
+      const long double hr = H[2 * (ch * Nf + m)], hi = H[2 * (ch * Nf + m) + 1];
+      const long double dr = (long double)D[2 * (ch * Nf + m)] - (gr * hr - gi * hi);
+      const long double di = (long double)D[2 * (ch * Nf + m) + 1] - (gr * hi + gi * hr);
+      acc += (dr * dr + di * di) / (long double)s;
+    }
+  return (double)(-(2.0L * (long double)dt / (long double)N) * acc);
+}
+
 double emri_o_inner(const double* A, const double* B, const double* psd, int64_t N, double dt) {
   const int64_t Nf = N / 2 + 1;
   long double acc = 0;

@@ -61,6 +61,8 @@ class Oracle:
         L.emri_o_dft_naive.argtypes = [_dp, C.c_int64, _dp]
         L.emri_o_loglike.restype = C.c_double
         L.emri_o_loglike.argtypes = [_dp, _dp, _dp, C.c_int64, C.c_double]
+        L.emri_o_loglike_fdep.restype = C.c_double
+        L.emri_o_loglike_fdep.argtypes = [_dp, _dp, _dp, C.c_int64, C.c_double, _dp, C.c_double]
         L.emri_o_inner.restype = C.c_double
         L.emri_o_inner.argtypes = [_dp, _dp, _dp, C.c_int64, C.c_double]
         L.emri_o_loglike_batch.restype = C.c_int
@@ -189,6 +191,13 @@ class Oracle:
         Dc = np.ascontiguousarray(D, dtype=np.complex128)
         s = _f64(psd)
         return self.lib.emri_o_loglike(_d(Hc.view(np.float64)), _d(Dc.view(np.float64)), _d(s), N, dt)
+
+    def loglike_fdep(self, H, D, psd, N, dt, fcoef, fstar=1e-3):
+        """Eq. 8 with the frequency-dependent propagation factor of Eq. 7 applied to H (reading D11)"""
+        Hc = np.ascontiguousarray(H, dtype=np.complex128)
+        Dc = np.ascontiguousarray(D, dtype=np.complex128)
+        s, fc = _f64(psd), _f64(fcoef)
+        return self.lib.emri_o_loglike_fdep(_d(Hc.view(np.float64)), _d(Dc.view(np.float64)), _d(s), N, dt, _d(fc), fstar)
 
     def inner(self, A, B, psd, N, dt):
         Ac = np.ascontiguousarray(A, dtype=np.complex128)

@@ -279,13 +279,18 @@ int fft_chunk(emri_plan* p, int kc, double* z, cudaStream_t s) {
   return EMRI_OK;
 }
 
-int run_like(emri_plan* p, int k0, int K, const double* Z, const double* data_fft, cudaStream_t s) {
+int run_like(emri_plan* p, int k0, int K, const double* Z, const double* data_fft, const double* fcoef, double fstar,
+             cudaStream_t s) {
   LikeArgs a;
   a.Z = reinterpret_cast<const double2*>(Z);
   a.D = reinterpret_cast<const double2*>(data_fft);
   a.w = p->d_w; a.partial = p->d_partial; a.k0 = k0; a.K = K; a.N = p->N; a.Nf = p->Nf; a.n_part = p->n_part;
+  a.fcoef = fcoef;
+  a.f_per_bin = 1.0 / ((double)p->N * p->dt);
+  a.x_per_bin = fcoef ? a.f_per_bin / fstar : 0.0;
   dim3 grid((unsigned)p->n_part, (unsigned)((K + LL_GROUP - 1) / LL_GROUP));
-  loglike_kernel<<<grid, LL_THREADS, 0, s>>>(a);
+  if (fcoef) loglike_kernel<true><<<grid, LL_THREADS, 0, s>>>(a);
+  else loglike_kernel<false><<<grid, LL_THREADS, 0, s>>>(a);
   CK(cudaGetLastError());
   return EMRI_OK;
 }
@@ -505,8 +510,8 @@ int emri_data_fft(emri_plan* p, const double* d_I, const double* d_II, double* d
   return EMRI_OK;
 }
 
-int emri_loglike(emri_plan* p, const double* params, int K, const double* data_fft, double* logL, int32_t* status,
-                 void* stream) {
+static int loglike_impl(emri_plan* p, const double* params, int K, const double* fcoef, double fstar, const double* data_fft,
+                        double* logL, int32_t* status, void* stream) {
   if (!valid_call(p, params, K) || !data_fft || !logL) return EMRI_EINVAL;
   cudaStream_t s = (cudaStream_t)stream;
   p->ev_used = 0; p->had_like = true;
@@ -522,7 +527,7 @@ int emri_loglike(emri_plan* p, const double* params, int K, const double* data_f
     mark(p, s);
     if ((rc = fft_chunk(p, kc, p->d_hbuf, s))) return rc;
     mark(p, s);
-    if ((rc = run_like(p, k0, kc, p->d_hbuf, data_fft, s))) return rc;
+    if ((rc = run_like(p, k0, kc, p->d_hbuf, data_fft, fcoef, fstar, s))) return rc;
     mark(p, s);
   }
   p->n_chunks_last = nch;
@@ -530,6 +535,17 @@ int emri_loglike(emri_plan* p, const double* params, int K, const double* data_f
   loglike_final_kernel<<<(K + 3) / 4, 128, 0, s>>>(p->d_partial, p->n_part, K, scale, p->d_status, logL, status);
   CK(cudaGetLastError());
   return EMRI_OK;
+}
+
+int emri_loglike(emri_plan* p, const double* params, int K, const double* data_fft, double* logL, int32_t* status,
+                 void* stream) {
+  return loglike_impl(p, params, K, nullptr, 1.0, data_fft, logL, status, stream);
+}
+
+int emri_loglike_fdep(emri_plan* p, const double* params, int K, const double* fcoef, double f_star, const double* data_fft,
+                      double* logL, int32_t* status, void* stream) {
+  if (!fcoef || !(f_star > 0.0) || !std::isfinite(f_star)) return EMRI_EINVAL;
+  return loglike_impl(p, params, K, fcoef, f_star, data_fft, logL, status, stream);
 }
 
 int emri_loglike_host(emri_plan* p, const double* params, int K, const double* data_fft, double* logL, int32_t* status,

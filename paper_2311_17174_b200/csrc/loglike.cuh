@@ -30,11 +30,28 @@ struct LikeArgs {
   int k0, K;
   int64_t N, Nf;
   int n_part;              // partial sums per walker = number of bin ranges
+  const double* fcoef;     // [K_total][6] {a1,a2,a3,b1,b2,b3} of Eq. 7's power series (kFdep only), row k0 + walker
+  double x_per_bin;        // (1/(N dt)) / f_*
+  double f_per_bin;        // 1/(N dt)
 };
 
 // grid (bin ranges, walker groups).  Each thread owns bins m = range_begin + tid + 256 j and LL_GROUP walkers:
 // the 2 LL_GROUP loads of Z are issued together (memory-level parallelism), D and w come from L2.
+//
+// kFdep: frequency-dependent propagation (Eq. 7; reading D11): every walker's spectrum is multiplied
+// per bin by G = exp(-Dm(f)) exp(-2 pi i f tau(f)), Dm = sum a_n x^n, tau = sum b_n x^n, x = f/f_*, n = 1..3, before
+// the residual is taken -- "such frequency-dependent terms need to act upon a tabulated waveform in frequency space".
+template <bool kFdep>
 __global__ void __launch_bounds__(LL_THREADS) loglike_kernel(LikeArgs a) {
+  __shared__ double s_fc[LL_GROUP][6];
+  if (kFdep) {
+    if (threadIdx.x < LL_GROUP * 6) {
+      const int g = threadIdx.x / 6, c = threadIdx.x - 6 * g;
+      const int kk = min((int)blockIdx.y * LL_GROUP + g, a.K - 1);
+      s_fc[g][c] = a.fcoef[(size_t)(a.k0 + kk) * 6 + c];
+    }
+    __syncthreads();
+  }
   const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
   const int kg0 = blockIdx.y * LL_GROUP;
   const int64_t m_begin = (int64_t)blockIdx.x * LL_RANGE;
@@ -58,6 +75,17 @@ __global__ void __launch_bounds__(LL_THREADS) loglike_kernel(LikeArgs a) {
     for (int g = 0; g < LL_GROUP; ++g) {
       double2 HI, HII;
       split_channels(zm[g], zn[g], HI, HII);
+      if (kFdep) {
+        const double x = (double)m * a.x_per_bin, f = (double)m * a.f_per_bin;
+        const double Dm = x * fma(x, fma(x, s_fc[g][2], s_fc[g][1]), s_fc[g][0]);
+        const double tau = x * fma(x, fma(x, s_fc[g][5], s_fc[g][4]), s_fc[g][3]);
+        const double amp = exp(-Dm);
+        double sn, cs;
+        sincospi(-2.0 * (f * tau), &sn, &cs);
+        const double gr = amp * cs, gi = amp * sn;
+        HI = make_double2(fma(gr, HI.x, -gi * HI.y), fma(gr, HI.y, gi * HI.x));
+        HII = make_double2(fma(gr, HII.x, -gi * HII.y), fma(gr, HII.y, gi * HII.x));
+      }
       const double ar = dI.x - HI.x, ai = dI.y - HI.y, br = dII.x - HII.x, bi = dII.y - HII.y;
       const double pw = fma(ar, ar, ai * ai) + fma(br, br, bi * bi);
       acc[g] = fma(wt, pw, acc[g]);

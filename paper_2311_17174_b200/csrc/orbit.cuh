@@ -40,17 +40,20 @@ DEVINL void cosmo_integrals(double z, double Om, double* I1, double* I2) {
 }
 // solve (1+z) tH I1(z) = D for z in [0, 20]: safeguarded Newton
 DEVINL double z_of_dL(double D, double tH, double Om) {
+  // f(z) = d_L(z) - D is increasing and convex, so Newton converges monotonically from above after the first step
+  // (quadratically: ~6 steps).  The convergence test comes BEFORE the bracket safeguard: a converged step lands on
+  // the bracket's edge, and bisecting there would throw the iterate away.
   double lo = 0.0, hi = 20.0;
   double z = fmin(D / tH, 1.0);
-  for (int it = 0; it < 24; ++it) {
+  for (int it = 0; it < 60; ++it) {
     double I1, I2;
     cosmo_integrals(z, Om, &I1, &I2);
-    double f = (1.0 + z) * tH * I1 - D;
-    if (f > 0.0) hi = z; else lo = z;
-    double fp = tH * (I1 + (1.0 + z) / Ez(z, Om));
+    const double f = (1.0 + z) * tH * I1 - D;
+    const double fp = tH * (I1 + (1.0 + z) / Ez(z, Om));
     double zn = z - f / fp;
-    if (!(zn > lo && zn < hi)) zn = 0.5 * (lo + hi);
-    if (fabs(zn - z) <= 2e-15 * fmax(zn, 1e-300)) { z = zn; break; }      // Newton: the step before was ~1e-8
+    if (fabs(zn - z) <= 2e-15 * fmax(fabs(zn), 1e-300)) { z = zn; break; }
+    if (f > 0.0) hi = z; else lo = z;
+    if (!(zn >= lo && zn <= hi)) zn = 0.5 * (lo + hi);
     z = zn;
   }
   return z;

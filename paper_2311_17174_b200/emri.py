@@ -18,7 +18,7 @@ _lib = None
 EXPORTS = (
     "emri_strerror", "emri_plan_create", "emri_plan_destroy", "emri_plan_set_cosmology",
     "emri_plan_set_coarse_stride", "emri_plan_set_orbit_schedule", "emri_plan_orbit_report", "emri_plan_set_chunk", "emri_orbit", "emri_plan_num_nodes", "emri_waveform",
-    "emri_waveform_fft", "emri_data_fft", "emri_loglike", "emri_loglike_host", "emri_plan_enable_timings",
+    "emri_waveform_fft", "emri_data_fft", "emri_loglike", "emri_loglike_fdep", "emri_loglike_host", "emri_plan_enable_timings",
     "emri_plan_get_timings", "emri_plan_last_cuda_error", "emri_plan_workspace_bytes", "emri_stretch_step",
     "emri_probe_fp64_peak", "emri_probe_hbm_read",
 )
@@ -55,6 +55,7 @@ def load():
     L.emri_data_fft.argtypes = [vp, vp, vp, vp, vp]
     L.emri_loglike.argtypes = [vp, vp, i32, vp, vp, vp, vp]
     L.emri_loglike_host.argtypes = [vp, vp, i32, vp, vp, vp, vp]
+    L.emri_loglike_fdep.argtypes = [vp, vp, i32, vp, dbl, vp, vp, vp, vp]
     L.emri_plan_enable_timings.argtypes = [vp, i32]
     L.emri_plan_get_timings.argtypes = [vp, C.POINTER(dbl)]
     L.emri_plan_last_cuda_error.argtypes = [vp]
@@ -222,6 +223,18 @@ class Plan:
         self._check(self._L.emri_loglike(self._h, _ptr(params, torch.float64, (K, NPAR)), K,
                                          _ptr(data_fft, torch.complex128, (2, self.Nf)),
                                          _ptr(logL, torch.float64, (K,)), _ptr(status, torch.int32, (K,)), _stream()))
+        return logL
+
+    def loglike_fdep(self, params, fcoef, f_star, data_fft, logL=None, status=None):
+        """Eq. 8 with the frequency-dependent propagation factor of Eq. 7; fcoef: CUDA [K][6]"""
+        import torch
+        K = params.shape[0]
+        if logL is None:
+            logL = torch.empty((K,), dtype=torch.float64, device=params.device)
+        self._check(self._L.emri_loglike_fdep(self._h, _ptr(params, torch.float64, (K, NPAR)), K,
+                                              _ptr(fcoef, torch.float64, (K, 6)), float(f_star),
+                                              _ptr(data_fft, torch.complex128, (2, self.Nf)),
+                                              _ptr(logL, torch.float64, (K,)), _ptr(status, torch.int32, (K,)), _stream()))
         return logL
 
     def loglike_host(self, params, data_fft=None, logL=None, status=None):

@@ -178,3 +178,38 @@ def test_loglike_is_zero_for_own_noiseless_injection(emri):
     logL = logL.cpu().numpy()
     assert abs(logL[0]) <= 1e-12 and np.all(logL[1:] < -1e-3)
     plan.close()
+
+
+# ------------------------------------------------------------------ next row f-1: frequency-dependent propagation (Eq. 7)
+@pytest.mark.parametrize("ci,K,N", [(2, 11, 1 << 13), (1, 5, 1 << 12)])
+def test_loglike_fdep_matches_oracle(emri, oracle, ci, K, N):
+    cfg = small_cfg(ci, K=K, N=N)
+    P = W.draw_params(cfg)
+    psd = W.lisa_psd_barack_cutler(N, cfg.dt)
+    rng = np.random.default_rng(77)
+    fstar = 0.03                                           # ~ Nyquist (1/30 Hz): x = f/f* <= 1.1
+    # friction series of order 0.1, delays of a few sample spacings at f ~ f*
+    fc = np.column_stack([rng.uniform(-0.3, 0.3, K), rng.uniform(-0.1, 0.1, K), rng.uniform(-0.03, 0.03, K),
+                          rng.uniform(-40, 40, K), rng.uniform(-10, 10, K), rng.uniform(-3, 3, K)])
+    fc[1] = 0.0                                            # one walker without the frequency dependence
+    hI, hII, _ = oracle.waveform(P[0], N, cfg.dt, cfg.n_max)
+    D = np.stack([oracle.rfft(hI), oracle.rfft(hII)]) + W.noise_fft(N, cfg.dt, psd, 31)
+    plain, st_ref, sp = oracle.loglike_batch(P, N, cfg.dt, cfg.n_max, D, psd, spectra=True)
+    ref = np.array([oracle.loglike_fdep(sp[k], D, psd, N, cfg.dt, fc[k], fstar) for k in range(K)])
+    plan = emri.Plan(N, cfg.dt, cfg.n_max, K, psd)
+    st = torch.zeros(K, dtype=torch.int32, device="cuda")
+    got = plan.loglike_fdep(dev(P), dev(fc), fstar, dev(D), status=st)
+    base = plan.loglike(dev(P), dev(D))
+    torch.cuda.synchronize()
+    got, base = got.cpu().numpy(), base.cpu().numpy()
+    print(f"fdep cfg{ci}: ref {ref[:3]} plain {plain[:3]} max abs diff {np.max(np.abs(got - ref)):.3e} "
+          f"max diff/tolerance {np.max(np.abs(got - ref) / (1e-9 * np.abs(ref) + 1e-6)):.2e}")
+    assert np.array_equal(st.cpu().numpy(), st_ref)
+    assert np.all(np.abs(got - ref) <= 1e-9 * np.abs(ref) + 1e-6)
+    assert got[1] == base[1]                               # G = 1 exactly when the series vanish
+    assert np.all(np.abs(got[[0, 2]] - base[[0, 2]]) > 1e-2)    # and it does act otherwise (logL is noise-dominated)
+    plan.set_chunk(4)                                      # chunking picks the right coefficient rows
+    got2 = plan.loglike_fdep(dev(P), dev(fc), fstar, dev(D))
+    torch.cuda.synchronize()
+    assert np.array_equal(got2.cpu().numpy(), got)
+    plan.close()

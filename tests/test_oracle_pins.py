@@ -764,3 +764,73 @@ def test_psd_models_are_positive_and_masked_at_ends():
         # LISA bucket near a few mHz
         f = W.freqs(1 << 12, 15.0)
         assert 1e-3 < f[np.argmin(s[1:-1]) + 1] < 2e-2
+
+
+# ----------------------------------------------------------------------------- frequency-dependent propagation (Eq. 7)
+def _fdep_case(seed=3, N=256, dt=15.0):
+    rng = np.random.default_rng(seed)
+    Nf = N // 2 + 1
+    H = rng.normal(size=(2, Nf)) + 1j * rng.normal(size=(2, Nf))
+    D = rng.normal(size=(2, Nf)) + 1j * rng.normal(size=(2, Nf))
+    psd = rng.uniform(0.5, 2.0, Nf)
+    psd[0] = psd[-1] = np.inf
+    return H, D, psd, N, dt
+
+
+def test_fdep_reduces_to_eq8_when_the_series_vanish(oracle):
+    H, D, psd, N, dt = _fdep_case()
+    assert oracle.loglike_fdep(H, D, psd, N, dt, np.zeros(6)) == oracle.loglike(H, D, psd, N, dt)
+
+
+def test_fdep_factor_restated_with_numpy(oracle):
+    """G = exp(-Dm(f)) exp(-2 pi i f tau(f)) applied to H, then Eq. 8"""
+    H, D, psd, N, dt = _fdep_case(4)
+    fc, fstar = np.array([0.3, -0.2, 0.05, 40.0, -15.0, 6.0]), 2e-3
+    f = np.arange(N // 2 + 1) / (N * dt)
+    x = f / fstar
+    G = np.exp(-(fc[0] * x + fc[1] * x ** 2 + fc[2] * x ** 3)) * np.exp(-2j * np.pi * f * (fc[3] * x + fc[4] * x ** 2 + fc[5] * x ** 3))
+    ok = np.isfinite(psd)
+    want = -(2 * dt / N) * np.sum(np.abs(D - G * H)[:, ok] ** 2 / psd[ok])
+    assert abs(oracle.loglike_fdep(H, D, psd, N, dt, fc, fstar) - want) <= 1e-12 * abs(want)
+    # it equals the plain likelihood of the pre-multiplied spectrum
+    assert abs(oracle.loglike(G * H, D, psd, N, dt) - want) <= 1e-12 * abs(want)
+
+
+def test_fdep_pure_delay_leaves_signal_power_unchanged_and_damping_scales_it(oracle):
+    H, D, psd, N, dt = _fdep_case(5)
+    Z = np.zeros_like(D)
+    base = oracle.loglike(H, Z, psd, N, dt)
+    # a speed-only modification is a pure phase: <h|h> is invariant
+    assert abs(oracle.loglike_fdep(H, Z, psd, N, dt, [0, 0, 0, 30.0, 5.0, -2.0]) - base) <= 1e-13 * abs(base)
+    # a single unmasked bin: friction a1 scales the power by exp(-2 a1 f/f*)
+    m0, fstar = 37, 1e-3
+    psd1 = np.full_like(psd, np.inf)
+    psd1[m0] = 1.3
+    f0 = m0 / (N * dt)
+    b1 = oracle.loglike(H, Z, psd1, N, dt)
+    got = oracle.loglike_fdep(H, Z, psd1, N, dt, [0.7, 0, 0, 0, 0, 0], fstar)
+    assert abs(got - b1 * np.exp(-2 * 0.7 * f0 / fstar)) <= 1e-13 * abs(b1)
+    # data that carries exactly the delayed, damped signal gives logL = 0
+    fc = np.array([0.1, 0.0, 0.0, 12.0, 0.0, 0.0])
+    f = np.arange(N // 2 + 1) / (N * dt)
+    G = np.exp(-fc[0] * f / fstar) * np.exp(-2j * np.pi * f * fc[3] * f / fstar)
+    assert abs(oracle.loglike_fdep(H, G * H, psd, N, dt, fc, fstar)) <= 1e-25
+
+
+def test_fdep_linear_in_f_delay_is_a_quadratic_phase_ie_a_dispersion(oracle):
+    """tau(f) = b1 f/f*: the phase -2 pi b1 f^2/f* has group delay d(phase)/d(2 pi f) = -2 b1 f/f*, twice tau:
+    checked through the factor the oracle applies, extracted with a one-bin probe"""
+    N, dt, fstar, b1 = 128, 10.0, 5e-3, 3.0
+    Nf = N // 2 + 1
+    psd = np.ones(Nf)
+    for m0 in (5, 20, 41):
+        H = np.zeros((2, Nf), dtype=complex)
+        H[0, m0] = 1.0
+        f0 = m0 / (N * dt)
+        # logL(D = c) = -(2dt/N) |c - G|^2 is maximal (zero) at c = G: scan the phase of c
+        ph = -2 * np.pi * f0 * b1 * f0 / fstar
+        Dm = np.zeros_like(H)
+        Dm[0, m0] = np.exp(1j * ph)
+        assert abs(oracle.loglike_fdep(H, Dm, psd, N, dt, [0, 0, 0, b1, 0, 0], fstar)) <= 1e-28
+        Dm[0, m0] = np.exp(1j * (ph + 0.01))
+        assert oracle.loglike_fdep(H, Dm, psd, N, dt, [0, 0, 0, b1, 0, 0], fstar) < -1e-6
