@@ -142,3 +142,48 @@ def test_fully_masked_psd_gives_zero_and_invalid_walker_minus_inf(emri):
     assert got[0] == 0.0 and got[1] == 0.0 and got[2] == -np.inf
     assert list(st.cpu().numpy()) == [0, 0, 1]
     plan.close()
+
+
+def test_status_bits_delay_and_cosmology_setting(emri, oracle):
+    """bit 4: |Delta T| beyond the one-interval guard (reading R20) => zero rows, logL = -inf, as the oracle;
+    emri_plan_set_cosmology reaches the amplitude through z(D_L) and Xi(z)"""
+    cfg = W.scaled(W.CONFIGS[2], K=4, N=1 << 12)
+    P = W.draw_params(cfg)
+    P[1, W.P_DELT] = 1e-12            # |Delta T| ~ 1e5 s > Delta = 3840 s
+    P[2, W.P_DELT] = -3e-14           # ~ 3e3 s: inside the guard
+    psd = W.lisa_psd_barack_cutler(cfg.N, cfg.dt)
+    h_ref, st_ref = oracle.waveform_batch(P, cfg.N, cfg.dt, cfg.n_max)
+    assert list(st_ref) == [0, 4, 0, 0]
+    plan = emri.Plan(cfg.N, cfg.dt, cfg.n_max, cfg.K, psd)
+    st = torch.zeros(cfg.K, dtype=torch.int32, device="cuda")
+    hI, hII = plan.waveform(dev(P), status=st)
+    D = plan.data_fft(hI[0].contiguous(), hII[0].contiguous())
+    logL = plan.loglike(dev(P), D)
+    torch.cuda.synchronize()
+    assert list(st.cpu().numpy()) == [0, 4, 0, 0]
+    hI = hI.cpu().numpy()
+    assert not hI[1].any() and logL.cpu().numpy()[1] == -np.inf
+    for k in (0, 2, 3):
+        assert np.max(np.abs(hI[k] - h_ref[k, 0])) <= H_TOL * np.max(np.abs(h_ref[k, 0]))
+    # another cosmology: both sides move together
+    plan.set_cosmology(73.0, 0.27)
+    hI2, _ = plan.waveform(dev(P))
+    torch.cuda.synchronize()
+    h2, _ = oracle.waveform_batch(P, cfg.N, cfg.dt, cfg.n_max, H0=73.0, Om=0.27)
+    hI2 = hI2.cpu().numpy()
+    assert np.max(np.abs(hI2[0] - h2[0, 0])) <= H_TOL * np.max(np.abs(h2[0, 0]))
+    assert np.max(np.abs(hI2[0] - hI[0])) > 1e-4 * np.max(np.abs(hI[0]))       # Xi(z) differs (Xi0 != 1 in this config)
+    plan.close()
+
+
+def test_argument_errors_on_the_device(emri):
+    cfg = W.scaled(W.CONFIGS[0], K=2, N=1 << 10)
+    plan = emri.Plan(cfg.N, cfg.dt, cfg.n_max, cfg.K)
+    P3 = dev(W.draw_params(cfg, K=3))
+    with pytest.raises(emri.EmriError, match="invalid argument"):
+        plan.waveform(P3)                                   # K > K_max
+    with pytest.raises(emri.EmriError, match="invalid argument"):
+        plan.set_coarse_stride(100)                         # not a power of two
+    with pytest.raises(emri.EmriError, match="invalid argument"):
+        plan.set_cosmology(-1.0, 0.3)
+    plan.close()
