@@ -128,3 +128,78 @@ def test_out_of_box_proposals_are_rejected_without_changing_the_walker(emri, ora
     assert not a[~prop["inbox"]].any() and (~prop["inbox"]).any()
     assert torch.equal(X[:K // 2][~torch.from_numpy(a).cuda()], before[:K // 2][~torch.from_numpy(a).cuda()])
     plan.close()
+
+
+def test_config4_full_size_chain(emri, oracle):
+    """BASELINE.json configs[4] at full size: K = 512 walkers x 200 stretch-move steps, N = 2^21, n_max = 20, on the device.
+    Protocol 8(d)-4: (A) every proposal / z / ln u' / partner of every half-step recomputed by the oracle from the
+    logged state, (B) logL of 16 seeded (half-step, walker) proposals by the oracle at full N, (C) every accept flag
+    consistent with the logged numbers."""
+    cfg = W.CONFIGS[4]
+    K, N, n_max, steps = cfg.K, cfg.N, cfg.n_max, 200
+    H = K // 2
+    X0 = W.draw_params(cfg)
+    lo, hi = W.prior_box(cfg)
+    psd = W.lisa_psd_barack_cutler(N, cfg.dt)
+    plan = emri.Plan(N, cfg.dt, n_max, K, psd)
+    X = dev(X0)
+    # data: the library's injection of theta* (row 0) + seeded coloured noise; the SAME array goes to the oracle
+    D_d = plan.waveform_fft(X[:1].contiguous())[0].clone() + dev(W.noise_fft(N, cfg.dt, psd, cfg.noise_seed))
+    lo_d, hi_d = dev(lo), dev(hi)
+    logL = plan.loglike(X, D_d)
+    acc_d = torch.zeros(K, dtype=torch.int32, device="cuda")
+    logs = torch.zeros((2 * steps, H, 21), dtype=torch.float64, device="cuda")
+    accs = torch.zeros((2 * steps, H), dtype=torch.int32, device="cuda")
+    Xs = torch.zeros((2 * steps, K, 17), dtype=torch.float64, device="cuda")
+    Ls = torch.zeros((2 * steps, K), dtype=torch.float64, device="cuda")
+    for step in range(steps):
+        for half in (0, 1):
+            q = 2 * step + half
+            Xs[q].copy_(X)
+            Ls[q].copy_(logL)
+            plan.stretch_step(X, logL, D_d, lo_d, hi_d, A_STRETCH, SEED, step, half, accepted=acc_d, log_buf=logs[q])
+            accs[q].copy_(acc_d[half * H:half * H + H])
+    torch.cuda.synchronize()
+    logs, accs, Xs, Ls = logs.cpu().numpy(), accs.cpu().numpy().astype(bool), Xs.cpu().numpy(), Ls.cpu().numpy()
+    D = D_d.cpu().numpy()
+    n_free = int(np.sum(lo < hi))
+    ambiguous = 0
+    rng = np.random.default_rng(404)
+    for q in range(2 * steps):
+        step, half = divmod(q, 2)
+        lg, act = logs[q], slice(half * H, half * H + H)
+        if q % 8 == 0 or q >= 2 * steps - 4:                      # (A) on every 8th half-step and the last four
+            prop = stretch.propose(Xs[q], lo, hi, A_STRETCH, SEED, step, half)
+            assert np.array_equal(lg[:, 20].astype(np.int64), prop["partner"])
+            np.testing.assert_allclose(lg[:, 17], prop["z"], rtol=1e-15)
+            np.testing.assert_allclose(lg[:, 18], prop["lnu"], rtol=1e-14, atol=1e-15)
+            scale = np.abs(Xs[q][act]) + np.abs(Xs[q][prop["partner"]])
+            assert np.all(np.abs(lg[:, :17] - prop["Y"]) <= 1e-15 * scale)
+            assert np.array_equal(np.isfinite(lg[:, 19]), prop["inbox"])
+        # (C) on every half-step
+        fin = np.isfinite(lg[:, 19])
+        lnq = (n_free - 1) * np.log(lg[:, 17]) + lg[:, 19] - Ls[q][act]
+        margin = lnq - lg[:, 18]
+        band = 2e-9 * (np.abs(lg[:, 19]) + np.abs(Ls[q][act])) + 2e-6
+        clear = fin & (np.abs(margin) > band)
+        assert np.array_equal(accs[q][clear], margin[clear] > 0) and not accs[q][~fin].any()
+        ambiguous += int(np.sum(fin & ~clear))
+        # the state advanced consistently
+        nxt = Xs[q + 1] if q + 1 < 2 * steps else X.cpu().numpy()
+        assert np.array_equal(nxt[act][accs[q]], lg[accs[q], :17]) and np.array_equal(nxt[act][~accs[q]], Xs[q][act][~accs[q]])
+    # (B) 16 seeded (half-step, walker) pairs with a finite proposal, oracle at full N
+    picks = []
+    while len(picks) < 16:
+        q, i = int(rng.integers(0, 2 * steps)), int(rng.integers(0, H))
+        if np.isfinite(logs[q, i, 19]):
+            picks.append((q, i))
+    Y = np.stack([logs[q, i, :17] for q, i in picks])
+    ref, st = oracle.loglike_batch(Y, N, cfg.dt, n_max, D, psd)
+    got = np.array([logs[q, i, 19] for q, i in picks])
+    print(f"config 4: acceptance {accs.mean():.3f}, ambiguous decisions {ambiguous} of {accs.size}, "
+          f"max |dlogL| on 16 sampled proposals {np.max(np.abs(got - ref)):.3e} at |logL| ~ {np.median(np.abs(ref)):.3e}")
+    assert not st.any()
+    assert np.all(np.abs(got - ref) <= 1e-9 * np.abs(ref) + 1e-6)
+    # |logL| ~ N = 2e6 here, so the band 2e-9 (|lnp(Y)| + |lnp(X)|) is ~8e-3 wide: a decision in a thousand falls inside it
+    assert ambiguous <= 0.005 * accs.size and 0.02 < accs.mean() < 0.98
+    plan.close()
