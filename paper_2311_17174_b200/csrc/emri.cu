@@ -67,6 +67,10 @@ struct emri_plan {
   std::map<int, cufftHandle> fft;
   void* d_fftwork = nullptr;
   size_t fftwork_bytes = 0;
+  // copy stream of emri_loglike_host: the data spectrum is uploaded while stages (a)-(c) run
+  cudaStream_t s_copy = nullptr;
+  cudaEvent_t ev_call = nullptr, ev_data = nullptr;
+  cudaEvent_t wait_before_like = nullptr;     // set for the duration of one loglike_impl call
   // timings
   bool timing = false;
   std::vector<cudaEvent_t> ev;
@@ -372,6 +376,10 @@ int emri_plan_create(emri_plan** out, int64_t N, double dt, int n_max, int K_max
       per_sm < 1)
     return fail(EMRI_ECUDA);
   p->synth_grid = per_sm * p->sm_count;
+  if (cudaStreamCreateWithFlags(&p->s_copy, cudaStreamNonBlocking) != cudaSuccess ||
+      cudaEventCreateWithFlags(&p->ev_call, cudaEventDisableTiming) != cudaSuccess ||
+      cudaEventCreateWithFlags(&p->ev_data, cudaEventDisableTiming) != cudaSuccess)
+    return fail(EMRI_ECUDA);
   if (cudaDeviceSynchronize() != cudaSuccess) return fail(EMRI_ECUDA);
   *out = p;
   return EMRI_OK;
@@ -382,6 +390,9 @@ int emri_plan_destroy(emri_plan* p) {
   cudaDeviceSynchronize();
   for (auto& kv : p->fft) cufftDestroy(kv.second);
   for (auto e : p->ev) cudaEventDestroy(e);
+  if (p->ev_call) cudaEventDestroy(p->ev_call);
+  if (p->ev_data) cudaEventDestroy(p->ev_data);
+  if (p->s_copy) cudaStreamDestroy(p->s_copy);
   void* ptrs[] = {p->d_w, p->d_wc, p->d_nodes, p->d_hbuf, p->d_partial, p->d_base, p->d_nodeaux, p->d_jpl, p->d_status,
                   p->d_params, p->d_data, p->d_logL, p->d_Y, p->d_z, p->d_lnu, p->d_logLY, p->d_inbox,
                   p->d_partner, p->d_fftwork, p->d_seg, p->d_plrow, p->d_mode, p->d_pclamp};
@@ -527,6 +538,7 @@ static int loglike_impl(emri_plan* p, const double* params, int K, const double*
     mark(p, s);
     if ((rc = fft_chunk(p, kc, p->d_hbuf, s))) return rc;
     mark(p, s);
+    if (p->wait_before_like) { CK(cudaStreamWaitEvent(s, p->wait_before_like, 0)); p->wait_before_like = nullptr; }
     if ((rc = run_like(p, k0, kc, p->d_hbuf, data_fft, fcoef, fstar, s))) return rc;
     mark(p, s);
   }
@@ -555,10 +567,17 @@ int emri_loglike_host(emri_plan* p, const double* params, int K, const double* d
   cudaStream_t s = (cudaStream_t)stream;
   CK(cudaMemcpyAsync(p->d_params, params, (size_t)K * EMRI_NPAR * sizeof(double), cudaMemcpyHostToDevice, s));
   if (data_fft) {
-    CK(cudaMemcpyAsync(p->d_data, data_fft, (size_t)4 * p->Nf * sizeof(double), cudaMemcpyHostToDevice, s));
+    // upload on the copy stream, ordered after everything already enqueued on s (an earlier reader of d_data);
+    // the reduction kernel, the only reader, waits for it -- the orbit, synthesis and transform do not
+    CK(cudaEventRecord(p->ev_call, s));
+    CK(cudaStreamWaitEvent(p->s_copy, p->ev_call, 0));
+    CK(cudaMemcpyAsync(p->d_data, data_fft, (size_t)4 * p->Nf * sizeof(double), cudaMemcpyHostToDevice, p->s_copy));
+    CK(cudaEventRecord(p->ev_data, p->s_copy));
+    p->wait_before_like = p->ev_data;
     p->data_loaded = true;
   }
   int rc = emri_loglike(p, p->d_params, K, p->d_data, p->d_logL, nullptr, stream);
+  p->wait_before_like = nullptr;
   if (rc) return rc;
   CK(cudaMemcpyAsync(logL, p->d_logL, (size_t)K * sizeof(double), cudaMemcpyDeviceToHost, s));
   if (status) CK(cudaMemcpyAsync(status, p->d_status, (size_t)K * sizeof(int32_t), cudaMemcpyDeviceToHost, s));
