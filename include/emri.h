@@ -94,6 +94,14 @@ int emri_plan_set_coarse_stride(emri_plan* p, int S);
  * the schedule and used by the tests).  Both evaluate the same scheme (S3). */
 int emri_plan_set_orbit_schedule(emri_plan* p, int schedule);
 
+/* Where the orbital state of the parameter row is given.  0 (default): at the first sample, t = 0, integrated forward.
+ * 1: the paper's own convention ("initial conditions at the LSO ... integrated backwards"): the row's
+ * e0, Phi0, gam0, alp0 are the values AT PLUNGE, placed at the last coarse node t = ceil(N/S) S dt (the end of the window),
+ * nu there is nu_LSO(e0) = ((1-e0^2)/(6+2 e0))^{3/2} / (2 pi M) (column nu0 is ignored but must be positive), and the
+ * same fixed-step RK4 runs backwards.  Nothing plunges inside the window; if e leaves [0,1) on the way back the
+ * walker gets EMRI_ST_STATE (zero rows, logL = -inf).  Applies to every later call of the plan. */
+int emri_plan_set_anchor(emri_plan* p, int at_lso);
+
 /* Diagnostics of the last parallel-in-time orbit evaluation: modes[k] (HOST int32 [K]) is 1 if
  * walker k's segments were all verified after a Newton round, 2 if a sequential tail was needed
  * from the first unverified boundary, 3 if its node rows are zero (invalid parameters, plunge at

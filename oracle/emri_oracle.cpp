@@ -226,7 +226,79 @@ void rk4_increment(const Walker& w, const real y[5], real h, int pn_mask, real d
   for (int q = 0; q < 5; ++q) d[q] = (h / 6) * (k1[q] + 2 * k2[q] + 2 * k3[q] + k4[q]);
 }
 
+// The paper's own initial-condition convention ("initial conditions at the LSO ... integrated
+// backwards", nu_LSO = c^3/(2 pi G M) ((1-e^2)/(6+2e))^{3/2}; reading D12 of DESIGN.md): the parameter row's
+// (e, Phi, gamma~, alpha) are the values AT PLUNGE, placed at the last coarse node t_A = Nc*Delta (the end of the window),
+// nu there is nu_LSO(e_LSO) (column nu0 is ignored), and the same fixed-step RK4 runs backwards, node Nc -> node -1.
+// The interval increments are stored in forward time (inc[j] = y_{j+1} - y_j); one forward step gives the guard node
+// Nc+1.  Nothing plunges inside the window by construction; a bad state (e leaving [0,1)) sets ST_STATE.
+int g_anchor_end = 0;
+
+Orbit integrate_orbit_from_lso(const Walker& w, int64_t N, real dt, int S, int pn_mask) {
+  Orbit o;
+  o.G = 1;
+  o.Nc = (N + S - 1) / S;
+  o.Nn = o.Nc + 1 + 2 * o.G;
+  o.Delta = S * dt;
+  o.jpl = o.Nn;
+  o.status = w.status;
+  for (int q = 0; q < 5; ++q) {
+    o.val[q].assign(o.Nn, 0);
+    o.slope[q].assign(o.Nn, 0);
+    o.inc[q].assign(o.Nn, 0);
+  }
+  if (w.status & ST_BADPARAM) return o;
+  const int G = o.G;
+  real y[5], d[5], k1[5];
+  for (int q = 0; q < 5; ++q) y[q] = w.p0[q];
+  y[1] = nu_lso(w.Ms, y[3]);
+  auto fail = [&]() {
+    for (int q = 0; q < 5; ++q) {
+      std::fill(o.val[q].begin(), o.val[q].end(), (real)0);
+      std::fill(o.slope[q].begin(), o.slope[q].end(), (real)0);
+      std::fill(o.inc[q].begin(), o.inc[q].end(), (real)0);
+    }
+    o.status |= ST_STATE;
+    return o;
+  };
+  // forward guard step: node Nc+1 = anchor advanced by +Delta
+  {
+    rk4_increment(w, y, o.Delta, pn_mask, d, k1);
+    real yp[5];
+    for (int q = 0; q < 5; ++q) yp[q] = y[q] + d[q];
+    yp[0] = frac(yp[0]); yp[2] = frac(yp[2]); yp[4] = frac(yp[4]);
+    if (!state_ok(yp)) return fail();
+    real kp[5];
+    rhs(w, yp, pn_mask, kp);
+    const int64_t jj = o.Nc + 1 + G;
+    for (int q = 0; q < 5; ++q) { o.val[q][jj] = yp[q]; o.slope[q][jj] = kp[q]; o.inc[q][jj] = 0; }
+    for (int q = 0; q < 5; ++q) o.inc[q][o.Nc + G] = d[q];
+  }
+  // backward sweep; nu and e carry a Kahan compensation term
+  real comp_nu = 0, comp_e = 0;
+  for (int64_t j = o.Nc; j >= -G; --j) {
+    const int64_t jj = j + G;
+    if (j == -G) {                 // last node: one extra slope evaluation
+      rhs(w, y, pn_mask, k1);
+      for (int q = 0; q < 5; ++q) { o.val[q][jj] = y[q]; o.slope[q][jj] = k1[q]; }
+      break;
+    }
+    rk4_increment(w, y, -o.Delta, pn_mask, d, k1);
+    for (int q = 0; q < 5; ++q) { o.val[q][jj] = y[q]; o.slope[q][jj] = k1[q]; o.inc[q][jj - 1] = -d[q]; }
+    real yn[5];
+    yn[0] = frac(y[0] + d[0]);
+    yn[2] = frac(y[2] + d[2]);
+    yn[4] = frac(y[4] + d[4]);
+    { real a = d[1] - comp_nu, t = y[1] + a; comp_nu = (t - y[1]) - a; yn[1] = t; }
+    { real a = d[3] - comp_e, t = y[3] + a; comp_e = (t - y[3]) - a; yn[3] = t; }
+    if (!state_ok(yn)) return fail();
+    for (int q = 0; q < 5; ++q) y[q] = yn[q];
+  }
+  return o;
+}
+
 Orbit integrate_orbit(const Walker& w, int64_t N, real dt, int S, int pn_mask) {
+  if (g_anchor_end) return integrate_orbit_from_lso(w, N, dt, S, pn_mask);
   Orbit o;
   o.G = 1;
   o.Nc = (N + S - 1) / S;
@@ -475,6 +547,9 @@ void fft_c(std::vector<real>& re, std::vector<real>& im) {
 
 // =================================================================== C ABI (double I/O)
 extern "C" {
+
+// 0 (default): the parameter row is the state at the first sample; 1: at plunge, at the last coarse node (reading D12)
+void emri_o_set_anchor(int at_lso) { g_anchor_end = at_lso ? 1 : 0; }
 
 int emri_o_real_bits(void) { return (int)std::numeric_limits<real>::digits; }
 

@@ -69,6 +69,10 @@ class Oracle:
         L.emri_o_loglike_batch.argtypes = [_dp, C.c_int, C.c_int64, C.c_double, C.c_int, C.c_int, C.c_double,
                                            C.c_double, _dp, _dp, _dp, _i32p, _dp]
 
+    def set_anchor(self, at_lso):
+        """False (default): the parameter row is the state at t = 0; True: at plunge, at the last coarse node (D12)"""
+        self.lib.emri_o_set_anchor(1 if at_lso else 0)
+
     # ---- scalars
     def real_bits(self):
         return self.lib.emri_o_real_bits()

@@ -50,7 +50,7 @@ struct emri_plan {
   int32_t* d_jpl = nullptr;
   int32_t* d_status = nullptr;
   // multiple-shooting orbit (orbit.cuh): segment records, per-walker mode / tail start / post-plunge row
-  int orbit_mode = 1, seg_L = 0, seg_P = 0, unit_tiles_override = 0;
+  int orbit_mode = 1, anchor_end = 0, seg_L = 0, seg_P = 0, unit_tiles_override = 0;
   double* d_seg = nullptr;
   double* d_plrow = nullptr;
   int32_t* d_mode = nullptr;
@@ -221,7 +221,7 @@ void mark(emri_plan* p, cudaStream_t s) {
 int run_orbit(emri_plan* p, const double* params, int K, cudaStream_t s) {
   OrbitArgs a;
   a.params = params; a.K = K; a.N = p->N; a.dt = p->dt; a.S = p->S; a.Nc = p->Nc; a.Nn = p->Nn; a.n_max = p->n_max;
-  a.tH = kMpcMetre / (p->H0 * 1000.0); a.Om = p->Om;
+  a.tH = kMpcMetre / (p->H0 * 1000.0); a.Om = p->Om; a.anchor_end = p->anchor_end;
   a.wc = p->d_wc; a.nodes = p->d_nodes; a.jpl = p->d_jpl; a.status = p->d_status; a.nodeaux = p->d_nodeaux;
   const unsigned aux_grid = (unsigned)(((int64_t)K * p->Nn + 127) / 128);
   if (p->orbit_mode == 0) {
@@ -422,6 +422,12 @@ int emri_plan_set_coarse_stride(emri_plan* p, int S) {
 int emri_plan_set_orbit_schedule(emri_plan* p, int schedule) {
   if (!p || (schedule != 0 && schedule != 1)) return EMRI_EINVAL;
   p->orbit_mode = schedule;
+  return EMRI_OK;
+}
+
+int emri_plan_set_anchor(emri_plan* p, int at_lso) {
+  if (!p || (at_lso != 0 && at_lso != 1)) return EMRI_EINVAL;
+  p->anchor_end = at_lso;
   return EMRI_OK;
 }
 

@@ -132,6 +132,7 @@ struct OrbitArgs {
   int64_t Nc, Nn;
   int n_max;
   double tH, Om;          // Hubble time [s], Omega_m
+  int anchor_end;         // 0: the parameter row is the state at t = 0; 1: at plunge, at the last coarse node (reading D12)
   double* wc;             // [K][WC_STRIDE]
   double* nodes;          // [K][Nn][NODE_STRIDE]
   int32_t* jpl;           // [K] first plunged node (index j), Nn if none
@@ -149,6 +150,46 @@ DEVINL void store_node(double* row, const double y[5], const double k1[5], const
   r[5] = make_double2(d[0], d[1]);
   r[6] = make_double2(d[2], d[3]);
   r[7] = make_double2(d[4], 0.0);
+}
+
+// Recursion node r (0 = where the parameters are given) -> node row.  Forward: node j = r, row r + 1.  Anchored at the
+// LSO: node j = Nc - r, row Nc + 1 - r, and the step is -Delta.  A row holds the value and slope at its node and the
+// increment over the interval [j, j+1] in FORWARD time: forward, that is the step leaving the node (one row write);
+// backward, it is minus the step that ARRIVED at the node, so value + slope and the increment are written separately.
+DEVINL int64_t row_of(const OrbitArgs& a, int64_t r) { return a.anchor_end ? a.Nc + 1 - r : r + 1; }
+DEVINL void store_value_slope(double* row, const double y[5], const double k1[5]) {
+  double2* q = reinterpret_cast<double2*>(row);
+  q[0] = make_double2(y[0], y[1]);
+  q[1] = make_double2(y[2], y[3]);
+  q[2] = make_double2(y[4], k1[0]);
+  q[3] = make_double2(k1[1], k1[2]);
+  q[4] = make_double2(k1[3], k1[4]);
+}
+DEVINL void store_increment(double* row, const double d[5], double sign) {
+  double2* q = reinterpret_cast<double2*>(row);
+  q[5] = make_double2(sign * d[0], sign * d[1]);
+  q[6] = make_double2(sign * d[2], sign * d[3]);
+  q[7] = make_double2(sign * d[4], 0.0);
+}
+// node rows of recursion step r -> r + 1 with increment d taken from state y (slope k1)
+DEVINL void store_step(const OrbitArgs& a, double* nodes, int64_t r, const double y[5], const double k1[5], const double d[5]) {
+  if (!a.anchor_end) {
+    store_node(nodes + row_of(a, r) * NODE_STRIDE, y, k1, d);
+  } else {
+    store_value_slope(nodes + row_of(a, r) * NODE_STRIDE, y, k1);
+    store_increment(nodes + row_of(a, r + 1) * NODE_STRIDE, d, -1.0);
+  }
+}
+// the last recursion node: value and slope; forward it has no interval after it
+DEVINL void store_last(const OrbitArgs& a, double* nodes, int64_t r, const double y[5], const double k1[5]) {
+  const double zero5[5] = {0, 0, 0, 0, 0};
+  if (!a.anchor_end) store_node(nodes + row_of(a, r) * NODE_STRIDE, y, k1, zero5);
+  else store_value_slope(nodes + row_of(a, r) * NODE_STRIDE, y, k1);
+}
+// nu_LSO(e) = ((1-e^2)/(6+2e))^{3/2} / (2 pi M)
+DEVINL double nu_lso(double twoPiMs, double e) {
+  const double t = (1.0 - e * e) / (6.0 + 2.0 * e);
+  return t * sqrt(t) / twoPiMs;
 }
 
 // (a0) validity, per-walker scalars and the constant block of walker k.
@@ -228,46 +269,50 @@ __global__ void __launch_bounds__(32) orbit_kernel(OrbitArgs a) {
   OrbitConst oc;
   const bool ok = walker_prologue(a, p, wc, oc, status);
 
-  // ---- (a1) RK4 on the coarse grid
+  // ---- (a1) RK4 on the coarse grid, in the direction of the recursion (forward from t = 0, or backward from the LSO)
   double y[5] = {frac(p[P_PHI0] / kTwoPi), p[P_NU0], frac(p[P_GAM0] / kTwoPi), p[P_E0], frac(p[P_ALP0] / kTwoPi)};
+  if (a.anchor_end) y[1] = nu_lso(oc.twoPiMs, y[3]);
+  const double h = (a.anchor_end ? -1.0 : 1.0) * Delta;
   double emax = ok ? y[3] : 0.0;
   const double zero5[5] = {0, 0, 0, 0, 0};
   bool run = ok;
-  if (run && plunged(oc, y[1], y[3])) { status |= EMRI_ST_PLUNGE; jpl = 0; run = false; }
-  if (!run) {
-    for (int64_t m = 0; m < a.Nn; ++m) store_node(nodes + m * NODE_STRIDE, zero5, zero5, zero5);
-  } else {
+  if (run && !a.anchor_end && plunged(oc, y[1], y[3])) { status |= EMRI_ST_PLUNGE; jpl = 0; run = false; }
+  if (run) {
     RkOut r;
-    // backward guard step: node -1
-    rk4_increment(oc, y, -Delta, r);
+    // guard step against the direction of the recursion
+    rk4_increment(oc, y, -h, r);
     double ym[5] = {frac(y[0] + r.d[0]), y[1] + r.d[1], frac(y[2] + r.d[2]), y[3] + r.d[3], frac(y[4] + r.d[4])};
     bool okm = isfinite(ym[0]) && isfinite(ym[1]) && isfinite(ym[2]) && isfinite(ym[3]) && isfinite(ym[4]) &&
                ym[3] >= 0.0 && ym[3] < 1.0 && ym[1] > 0.0;
     if (!okm) {
       status |= EMRI_ST_STATE;
-      for (int64_t m = 0; m < a.Nn; ++m) store_node(nodes + m * NODE_STRIDE, zero5, zero5, zero5);
+      run = false;
     } else {
       double km[5], dm[5];
       km[0] = ym[1];
       rhs(oc, ym[1], ym[3], &km[1], &km[2], &km[3], &km[4]);
+      if (!a.anchor_end) {
 #pragma unroll
-      for (int q = 0; q < 5; ++q) dm[q] = -r.d[q];
-      store_node(nodes, ym, km, dm);
+        for (int q = 0; q < 5; ++q) dm[q] = -r.d[q];
+        store_node(nodes, ym, km, dm);
+      } else {
+        store_node(nodes + (a.Nc + 2) * NODE_STRIDE, ym, km, zero5);
+        store_increment(nodes + (a.Nc + 1) * NODE_STRIDE, r.d, 1.0);
+      }
       emax = fmax(emax, ym[3]);
-      // forward sweep; nu and e are Kahan-compensated (reading D3)
+      // sweep; nu and e are Kahan-compensated (reading D3)
       double comp_nu = 0.0, comp_e = 0.0;
-      const int64_t last = a.Nc + 1;          // node index j of the last node (G = 1)
+      const int64_t last = a.Nc + 1;          // recursion index of the last node (G = 1)
       for (int64_t j = 0; j <= last; ++j) {
-        double* row = nodes + (j + 1) * NODE_STRIDE;
         if (j == last) {
           double k1[5];
           k1[0] = y[1];
           rhs(oc, y[1], y[3], &k1[1], &k1[2], &k1[3], &k1[4]);
-          store_node(row, y, k1, zero5);
+          store_last(a, nodes, j, y, k1);
           break;
         }
-        rk4_increment(oc, y, Delta, r);
-        store_node(row, y, r.k1, r.d);
+        rk4_increment(oc, y, h, r);
+        store_step(a, nodes, j, y, r.k1, r.d);
         double yn[5];
         yn[0] = frac(y[0] + r.d[0]);
         yn[2] = frac(y[2] + r.d[2]);
@@ -276,9 +321,10 @@ __global__ void __launch_bounds__(32) orbit_kernel(OrbitArgs a) {
         { double t = r.d[3] - comp_e, s = y[3] + t; comp_e = (s - y[3]) - t; yn[3] = s; }
         bool okn = isfinite(yn[0]) && isfinite(yn[1]) && isfinite(yn[2]) && isfinite(yn[3]) && isfinite(yn[4]) &&
                    yn[3] >= 0.0 && yn[3] < 1.0 && yn[1] > 0.0;
-        bool pl = okn && plunged(oc, yn[1], yn[3]);
+        bool pl = okn && !a.anchor_end && plunged(oc, yn[1], yn[3]);
         if (!okn || pl) {
           status |= okn ? EMRI_ST_PLUNGE : EMRI_ST_STATE;
+          if (a.anchor_end) { run = false; break; }      // anchored at the LSO a bad state invalidates the walker
           jpl = (int32_t)(j + 1);
           // nodes from j_pl on are copies of node j_pl - 1 with zero increments
           for (int64_t m = j + 1; m <= last; ++m) store_node(nodes + (m + 1) * NODE_STRIDE, y, r.k1, zero5);
@@ -288,6 +334,9 @@ __global__ void __launch_bounds__(32) orbit_kernel(OrbitArgs a) {
         for (int q = 0; q < 5; ++q) y[q] = yn[q];
       }
     }
+  }
+  if (!run) {
+    for (int64_t m = 0; m < a.Nn; ++m) store_node(nodes + m * NODE_STRIDE, zero5, zero5, zero5);
   }
   wc[WC_EMAX] = emax;
   a.jpl[k] = jpl;
@@ -407,15 +456,17 @@ __global__ void __launch_bounds__(32) orbit_init_kernel(ShootArgs s) {
   OrbitConst oc;
   const bool ok = walker_prologue(a, p, wc, oc, status);
   double y[5] = {frac(p[P_PHI0] / kTwoPi), p[P_NU0], frac(p[P_GAM0] / kTwoPi), p[P_E0], frac(p[P_ALP0] / kTwoPi)};
+  if (a.anchor_end) y[1] = nu_lso(oc.twoPiMs, y[3]);
+  const double dir = a.anchor_end ? -1.0 : 1.0;
   int mode = OM_ACTIVE;
   int32_t jpl = (int32_t)a.Nn;
   double emax = ok ? y[3] : 0.0;
   if (!ok) mode = OM_ZERO;
-  else if (plunged(oc, y[1], y[3])) { status |= EMRI_ST_PLUNGE; jpl = 0; mode = OM_ZERO; }
+  else if (!a.anchor_end && plunged(oc, y[1], y[3])) { status |= EMRI_ST_PLUNGE; jpl = 0; mode = OM_ZERO; }
   if (mode == OM_ACTIVE) {
-    // backward guard step: node -1 (row 0), global angles
+    // guard step against the direction of the recursion: node -1 (row 0) forward, node Nc+1 (row Nc+2) at the LSO
     RkOut r;
-    rk4_increment(oc, y, -Delta, r);
+    rk4_increment(oc, y, -dir * Delta, r);
     double ym[5] = {frac(y[0] + r.d[0]), y[1] + r.d[1], frac(y[2] + r.d[2]), y[3] + r.d[3], frac(y[4] + r.d[4])};
     if (!state_ok(ym[0], ym[1], ym[2], ym[3], ym[4])) {
       status |= EMRI_ST_STATE;
@@ -424,15 +475,21 @@ __global__ void __launch_bounds__(32) orbit_init_kernel(ShootArgs s) {
       double km[5], dm[5];
       km[0] = ym[1];
       rhs(oc, ym[1], ym[3], &km[1], &km[2], &km[3], &km[4]);
+      if (!a.anchor_end) {
 #pragma unroll
-      for (int q = 0; q < 5; ++q) dm[q] = -r.d[q];
-      store_node(nodes, ym, km, dm);
+        for (int q = 0; q < 5; ++q) dm[q] = -r.d[q];
+        store_node(nodes, ym, km, dm);
+      } else {
+        const double zero5[5] = {0, 0, 0, 0, 0};
+        store_node(nodes + (a.Nc + 2) * NODE_STRIDE, ym, km, zero5);
+        store_increment(nodes + (a.Nc + 1) * NODE_STRIDE, r.d, 1.0);      // interval [Nc, Nc+1]
+      }
       emax = fmax(emax, ym[3]);
     }
   }
   if (mode == OM_ACTIVE) {
     // coarse sweep: one RK4 step of L*Delta per segment
-    const double H = (double)s.L * Delta;
+    const double H = dir * (double)s.L * Delta;
     double nu = y[1], e = y[3];
     for (int pp = 0; pp < s.P; ++pp) {
       double* sg = seg + (size_t)pp * SEG_STRIDE;
@@ -465,7 +522,7 @@ __global__ void __launch_bounds__(64) orbit_sweep_kernel(ShootArgs s) {
   double* sg = s.seg + ((size_t)k * s.P + pp) * SEG_STRIDE;
   OrbitConst oc;
   load_orbit_const(a.wc + (size_t)k * WC_STRIDE, oc);
-  const double Delta = a.S * a.dt;
+  const double Delta = (a.anchor_end ? -1.0 : 1.0) * (a.S * a.dt);      // signed step of the recursion
   const int64_t j0 = (int64_t)pp * s.L;
   const int nst = (int)((s.n_steps - j0 < (int64_t)s.L) ? (s.n_steps - j0) : (int64_t)s.L);
   double nu = sg[SG_NU], cnu = sg[SG_CNU], e = sg[SG_E], ce = sg[SG_CE];
@@ -490,7 +547,6 @@ __global__ void __launch_bounds__(64) orbit_sweep_kernel(ShootArgs s) {
     const double* p = a.params + (size_t)k * EMRI_NPAR;
     ang0 = frac(p[P_PHI0] / kTwoPi); ang1 = frac(p[P_GAM0] / kTwoPi); ang2 = frac(p[P_ALP0] / kTwoPi);
   }
-  const double zero5[5] = {0, 0, 0, 0, 0};
   double emax = e;
   int64_t stop = 0;
   int kind = 0;
@@ -499,13 +555,13 @@ __global__ void __launch_bounds__(64) orbit_sweep_kernel(ShootArgs s) {
     const int64_t j = j0 + i;
     const double y[5] = {ang0, nu, ang1, e, ang2};
     rk4_increment(oc, y, Delta, r);
-    store_node(nodes + (j + 1) * NODE_STRIDE, y, r.k1, r.d);
+    store_step(a, nodes, j, y, r.k1, r.d);
     const double n0 = frac(ang0 + r.d[0]), n2 = frac(ang1 + r.d[2]), n4 = frac(ang2 + r.d[4]);
     double nn = nu, nc = cnu, en = e, ec = ce;
     kahan_add(nn, nc, r.d[1]);
     kahan_add(en, ec, r.d[3]);
     const bool okn = state_ok(n0, nn, n2, en, n4);
-    if (!okn || plunged(oc, nn, en)) { stop = j + 1; kind = okn ? EMRI_ST_PLUNGE : EMRI_ST_STATE; break; }
+    if (!okn || (!a.anchor_end && plunged(oc, nn, en))) { stop = j + 1; kind = okn ? EMRI_ST_PLUNGE : EMRI_ST_STATE; break; }
     ang0 = n0; ang1 = n2; ang2 = n4; nu = nn; cnu = nc; e = en; ce = ec;
     emax = fmax(emax, e);
   }
@@ -515,7 +571,7 @@ __global__ void __launch_bounds__(64) orbit_sweep_kernel(ShootArgs s) {
     double k1[5];
     k1[0] = nu;
     rhs(oc, nu, e, &k1[1], &k1[2], &k1[3], &k1[4]);
-    store_node(nodes + (s.n_steps + 1) * NODE_STRIDE, y, k1, zero5);
+    store_last(a, nodes, s.n_steps, y, k1);
   }
   sg[SG_ENU] = nu; sg[SG_ECNU] = cnu; sg[SG_EE] = e; sg[SG_ECE] = ce;
   sg[SG_T0] = ang0; sg[SG_T1] = ang1; sg[SG_T2] = ang2;
@@ -617,6 +673,12 @@ __global__ void __launch_bounds__(32) orbit_correct_kernel(ShootArgs s) {
       s.mode[k] = OM_TAIL;
     } else {
       s.pclamp[k] = P - 1;
+      if (stop_seg >= 0 && a.anchor_end) {
+        // anchored at the LSO nothing plunges; a bad state (e leaving [0,1)) invalidates the walker
+        a.status[k] |= EMRI_ST_STATE;
+        s.mode[k] = OM_ZERO;
+        return;
+      }
       if (stop_seg >= 0) {
         const double* sg = seg + (size_t)stop_seg * SEG_STRIDE;
         const int64_t jst = (int64_t)sg[SG_STOP];
@@ -645,11 +707,10 @@ __global__ void __launch_bounds__(32) orbit_tail_kernel(ShootArgs s) {
   double* nodes = a.nodes + (size_t)k * a.Nn * NODE_STRIDE;
   OrbitConst oc;
   load_orbit_const(a.wc + (size_t)k * WC_STRIDE, oc);
-  const double Delta = a.S * a.dt;
+  const double Delta = (a.anchor_end ? -1.0 : 1.0) * (a.S * a.dt);      // signed step of the recursion
   double nu = sg[SG_NU], cnu = sg[SG_CNU], e = sg[SG_E], ce = sg[SG_CE];
   double ang0 = 0.0, ang1 = 0.0, ang2 = 0.0;       // local to the tail; orbit_fixup_kernel adds the offset
   double emax = fmax(a.wc[(size_t)k * WC_STRIDE + WC_EMAX], e);
-  const double zero5[5] = {0, 0, 0, 0, 0};
   RkOut r;
   for (int64_t j = (int64_t)pb * s.L; j <= s.n_steps; ++j) {
     const double y[5] = {ang0, nu, ang1, e, ang2};
@@ -657,19 +718,20 @@ __global__ void __launch_bounds__(32) orbit_tail_kernel(ShootArgs s) {
       double k1[5];
       k1[0] = nu;
       rhs(oc, nu, e, &k1[1], &k1[2], &k1[3], &k1[4]);
-      store_node(nodes + (j + 1) * NODE_STRIDE, y, k1, zero5);
+      store_last(a, nodes, j, y, k1);
       break;
     }
     rk4_increment(oc, y, Delta, r);
-    store_node(nodes + (j + 1) * NODE_STRIDE, y, r.k1, r.d);
+    store_step(a, nodes, j, y, r.k1, r.d);
     const double n0 = frac(ang0 + r.d[0]), n2 = frac(ang1 + r.d[2]), n4 = frac(ang2 + r.d[4]);
     double nn = nu, nc = cnu, en = e, ec = ce;
     kahan_add(nn, nc, r.d[1]);
     kahan_add(en, ec, r.d[3]);
     const bool okn = state_ok(n0, nn, n2, en, n4);
-    if (!okn || plunged(oc, nn, en)) {
-      a.jpl[k] = (int32_t)(j + 1);
+    if (!okn || (!a.anchor_end && plunged(oc, nn, en))) {
       a.status[k] |= okn ? EMRI_ST_PLUNGE : EMRI_ST_STATE;
+      if (a.anchor_end) { s.mode[k] = OM_ZERO; break; }       // anchored at the LSO a bad state invalidates the walker
+      a.jpl[k] = (int32_t)(j + 1);
       double* dst = s.plrow + (size_t)k * NODE_STRIDE;
       dst[0] = frac(ang0 + sg[SG_O0]); dst[1] = nu; dst[2] = frac(ang1 + sg[SG_O1]); dst[3] = e; dst[4] = frac(ang2 + sg[SG_O2]);
       for (int q = 0; q < 5; ++q) { dst[5 + q] = r.k1[q]; dst[10 + q] = 0.0; }
@@ -696,16 +758,18 @@ __global__ void __launch_bounds__(128) orbit_fixup_kernel(ShootArgs s) {
     for (int q = 0; q < NODE_STRIDE / 2; ++q) row[q] = make_double2(0.0, 0.0);
     return;
   }
-  const int64_t j = m - 1;
-  if (j < 0) return;
+  // recursion index of this row's node: forward r = j = m - 1 (row 0 is the guard node, global angles already);
+  // anchored at the LSO r = Nc - j = Nc + 1 - m (row Nc + 2 is the guard node)
+  const int64_t r = a.anchor_end ? a.Nc + 1 - m : m - 1;
+  if (r < 0) return;
   const int32_t jpl = a.jpl[k];
-  if (j >= (int64_t)jpl) {
+  if (!a.anchor_end && r >= (int64_t)jpl) {
     const double2* src = reinterpret_cast<const double2*>(s.plrow + (size_t)k * NODE_STRIDE);
 #pragma unroll
     for (int q = 0; q < NODE_STRIDE / 2; ++q) row[q] = src[q];
     return;
   }
-  int64_t p = j / s.L;
+  int64_t p = r / s.L;
   const int pc = s.pclamp[k];
   if (p > pc) p = pc;
   if (p == 0) return;

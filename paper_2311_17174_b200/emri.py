@@ -17,7 +17,7 @@ _lib = None
 
 EXPORTS = (
     "emri_strerror", "emri_plan_create", "emri_plan_destroy", "emri_plan_set_cosmology",
-    "emri_plan_set_coarse_stride", "emri_plan_set_orbit_schedule", "emri_plan_orbit_report", "emri_plan_set_chunk", "emri_orbit", "emri_plan_num_nodes", "emri_waveform",
+    "emri_plan_set_coarse_stride", "emri_plan_set_orbit_schedule", "emri_plan_set_anchor", "emri_plan_orbit_report", "emri_plan_set_chunk", "emri_orbit", "emri_plan_num_nodes", "emri_waveform",
     "emri_waveform_fft", "emri_data_fft", "emri_loglike", "emri_loglike_fdep", "emri_loglike_host", "emri_plan_enable_timings",
     "emri_plan_get_timings", "emri_plan_last_cuda_error", "emri_plan_workspace_bytes", "emri_stretch_step",
     "emri_probe_fp64_peak", "emri_probe_hbm_read",
@@ -47,6 +47,7 @@ def load():
     L.emri_plan_set_chunk.argtypes = [vp, i32]
     L.emri_plan_set_orbit_schedule.argtypes = [vp, i32]
     L.emri_plan_orbit_report.argtypes = [vp, i32, vp]
+    L.emri_plan_set_anchor.argtypes = [vp, i32]
     L.emri_orbit.argtypes = [vp, vp, i32, vp, vp, vp]
     L.emri_plan_num_nodes.restype = i64
     L.emri_plan_num_nodes.argtypes = [vp]
@@ -149,6 +150,10 @@ class Plan:
     def set_orbit_schedule(self, schedule):
         """1 = parallel in time (default), 0 = sequential recursion (same scheme)"""
         self._check(self._L.emri_plan_set_orbit_schedule(self._h, int(schedule)))
+
+    def set_anchor(self, at_lso):
+        """False: the parameter row is the state at t = 0 (default); True: at plunge, at the end of the window"""
+        self._check(self._L.emri_plan_set_anchor(self._h, 1 if at_lso else 0))
 
     def orbit_report(self, K):
         """modes of the last parallel-in-time orbit: 1 verified, 2 sequential tail, 3 zero rows"""

@@ -119,3 +119,87 @@ def test_invalid_and_immediately_plunged_walkers(emri):
         nodes, st, modes = run_orbit(emri, P, cfg.N, cfg.dt, cfg.n_max, schedule)
         assert list(st) == [0, 1, 2, 1]
         assert not nodes[1:].any() and nodes[0].any()
+
+
+# ------------------------------------------------------------------ next row f-3: the paper's IC convention (anchored at the LSO)
+def lso_params(cfg, K, e_hi=0.5):
+    P = W.draw_params(cfg, K=K)
+    P[:, W.P_E0] = np.linspace(0.0, e_hi, K)          # e at plunge, including the circular case
+    return P
+
+
+@pytest.mark.parametrize("ci,N,S", [(1, 1 << 18, 256), (3, 1 << 16, 64), (2, 1 << 20, 256)])
+def test_lso_anchored_orbit_matches_oracle_and_sequential(emri, oracle, ci, N, S):
+    cfg = W.scaled(W.CONFIGS[ci], K=10, N=N)
+    P = lso_params(cfg, cfg.K)
+    out = {}
+    for schedule in (1, 0):
+        plan = emri.Plan(N, cfg.dt, cfg.n_max, cfg.K)
+        if S != 256:
+            plan.set_coarse_stride(S)
+        plan.set_orbit_schedule(schedule)
+        plan.set_anchor(True)
+        st = torch.zeros(cfg.K, dtype=torch.int32, device="cuda")
+        nodes = plan.orbit(dev(P), status=st)
+        torch.cuda.synchronize()
+        out[schedule] = (nodes.cpu().numpy(), st.cpu().numpy(), plan.orbit_report(cfg.K) if schedule else None)
+        plan.close()
+    n1, s1, modes = out[1]
+    n0, s0, _ = out[0]
+    print("status", s1, "modes", modes)
+    assert np.array_equal(s0, s1)
+    oracle.set_anchor(True)
+    try:
+        for k in range(cfg.K):
+            ref = oracle.orbit(P[k], N, cfg.dt, S)
+            assert s1[k] == ref["status"]
+            if ref["status"]:
+                assert not n1[k].any() and not n0[k].any()
+                continue
+            val, slope, inc = n1[k, :, 0:5].T, n1[k, :, 5:10].T, n1[k, :, 10:15].T
+            for q in (0, 2, 4):
+                assert np.max(np.abs(circ_diff(val[q], ref["val"][q]))) < 2e-11
+                assert np.max(np.abs(circ_diff(val[q], n0[k, :, q]))) < 2e-12
+                np.testing.assert_allclose(inc[q], ref["inc"][q], rtol=1e-13, atol=1e-15)
+            for q in (1, 3):
+                np.testing.assert_allclose(val[q], ref["val"][q], rtol=2e-14, atol=1e-300)
+                np.testing.assert_allclose(val[q], n0[k, :, q], rtol=4e-16, atol=1e-300)
+                np.testing.assert_allclose(inc[q], ref["inc"][q], rtol=1e-11, atol=1e-25)
+            np.testing.assert_allclose(slope, ref["slope"], rtol=1e-12, atol=1e-30)
+    finally:
+        oracle.set_anchor(False)
+    assert (s1 == 0).sum() >= 5
+
+
+def test_lso_anchored_waveform_and_loglike_match_oracle(emri, oracle):
+    cfg = W.scaled(W.CONFIGS[2], K=6, N=1 << 13)
+    P = lso_params(cfg, cfg.K, e_hi=0.4)
+    psd = W.lisa_psd_barack_cutler(cfg.N, cfg.dt)
+    oracle.set_anchor(True)
+    try:
+        h_ref, st_ref = oracle.waveform_batch(P, cfg.N, cfg.dt, cfg.n_max)
+        D = np.stack([oracle.rfft(h_ref[1, 0]), oracle.rfft(h_ref[1, 1])]) + W.noise_fft(cfg.N, cfg.dt, psd, 9)
+        L_ref, _ = oracle.loglike_batch(P, cfg.N, cfg.dt, cfg.n_max, D, psd)
+    finally:
+        oracle.set_anchor(False)
+    plan = emri.Plan(cfg.N, cfg.dt, cfg.n_max, cfg.K, psd)
+    plan.set_anchor(True)
+    st = torch.zeros(cfg.K, dtype=torch.int32, device="cuda")
+    hI, hII = plan.waveform(dev(P), status=st)
+    logL = plan.loglike(dev(P), dev(D))
+    torch.cuda.synchronize()
+    assert np.array_equal(st.cpu().numpy(), st_ref) and not st_ref.any()
+    for ch, got in ((0, hI.cpu().numpy()), (1, hII.cpu().numpy())):
+        err = np.max(np.abs(got - h_ref[:, ch]), axis=1) / np.max(np.abs(h_ref[:, ch]), axis=1)
+        print("LSO-anchored waveform err", err)
+        assert np.all(err <= 1e-9)
+        assert np.all(got[:, -1] != 0.0)                      # live up to the last sample: the window ends at plunge
+    got = logL.cpu().numpy()
+    assert np.all(np.abs(got - L_ref) <= 1e-9 * np.abs(L_ref) + 1e-6)
+    # back to the default convention on the same plan
+    plan.set_anchor(False)
+    h2, _ = plan.waveform(dev(P))
+    torch.cuda.synchronize()
+    ref2, _ = oracle.waveform_batch(P[:1], cfg.N, cfg.dt, cfg.n_max)
+    assert np.max(np.abs(h2.cpu().numpy()[0] - ref2[0, 0])) <= 1e-9 * np.max(np.abs(ref2[0, 0]))
+    plan.close()

@@ -834,3 +834,83 @@ def test_fdep_linear_in_f_delay_is_a_quadratic_phase_ie_a_dispersion(oracle):
         assert abs(oracle.loglike_fdep(H, Dm, psd, N, dt, [0, 0, 0, b1, 0, 0], fstar)) <= 1e-28
         Dm[0, m0] = np.exp(1j * (ph + 0.01))
         assert oracle.loglike_fdep(H, Dm, psd, N, dt, [0, 0, 0, b1, 0, 0], fstar) < -1e-6
+
+
+# ----------------------------------------------------------------------------- the paper's IC convention: anchored at the LSO
+@pytest.fixture()
+def lso(oracle):
+    oracle.set_anchor(True)
+    yield oracle
+    oracle.set_anchor(False)
+
+
+def _lso_params(e_lso=0.3):
+    p = W.draw_params(W.CONFIGS[1], K=1)[0].copy()
+    p[W.P_E0] = e_lso
+    return p
+
+
+def test_lso_anchor_sits_on_the_plunge_frequency(lso):
+    """nu_LSO = c^3/(2 pi G M) ((1-e^2)/(6+2e))^{3/2} at the last coarse node, integrated backwards"""
+    p = _lso_params(0.3)
+    N, dt, S = 1 << 16, 15.0, 256
+    orb = lso.orbit(p, N, dt, S)
+    assert orb["status"] == 0 and orb["jpl"] == orb["Nn"]
+    x = ((1 - 0.09) / 6.6) ** 1.5 / (2 * np.pi * p[W.P_M] * 4.925490947e-6)
+    assert orb["val"][1][-2] == pytest.approx(x, rel=1e-15)
+    assert orb["val"][3][-2] == 0.3
+    # going back in time the orbit is wider and more eccentric, monotonically
+    assert np.all(np.diff(orb["val"][1]) > 0) and np.all(np.diff(orb["val"][3]) < 0)
+    for q, col in ((0, W.P_PHI0), (2, W.P_GAM0), (4, W.P_ALP0)):
+        assert abs(circ_diff(orb["val"][q][-2], (p[col] / (2 * np.pi)) % 1.0)) < 1e-15
+
+
+def test_lso_increments_and_slopes_are_consistent(lso):
+    p = _lso_params(0.2)
+    orb = lso.orbit(p, 1 << 16, 15.0, 256)
+    v, inc, sl = orb["val"], orb["inc"], orb["slope"]
+    for q in (0, 2, 4):
+        assert np.max(np.abs(circ_diff(v[q][:-1] + inc[q][:-1], v[q][1:]))) < 1e-14
+    for q in (1, 3):
+        np.testing.assert_allclose(v[q][:-1] + inc[q][:-1], v[q][1:], rtol=1e-15)
+    for jj in (0, 1, 17, orb["Nn"] - 2, orb["Nn"] - 1):
+        np.testing.assert_array_equal(sl[:, jj], lso.rhs(p, v[:, jj]))
+
+
+def test_lso_backward_orbit_against_dop853_and_forward_rerun(lso):
+    p = _lso_params(0.3)
+    N, dt, S = 1 << 18, 15.0, 256
+    orb = lso.orbit(p, N, dt, S)
+    assert orb["status"] == 0
+    yA = [orb["val"][q][-2] for q in range(5)]
+    T = (orb["Nn"] - 3) * S * dt                     # from node Nc back to node 0
+    sol = scipy.integrate.solve_ivp(lambda t, y: lso.rhs(p, y), (0.0, -T), yA, method="DOP853", rtol=1e-13,
+                                    atol=[1e-9, 1e-19, 1e-9, 1e-16, 1e-9])
+    y0 = sol.y[:, -1]
+    assert orb["val"][1][1] == pytest.approx(y0[1], rel=5e-11)
+    assert orb["val"][3][1] == pytest.approx(y0[3], rel=5e-10)
+    for q in (0, 2, 4):
+        assert abs(circ_diff(orb["val"][q][1], y0[q] % 1.0)) < 5e-7       # the last hours before plunge are stiff for RK4
+    # the forward scheme started from node 0 of the backward orbit returns to the anchor (both are O(Delta^4) accurate)
+    lso.set_anchor(False)
+    q0 = p.copy()
+    q0[W.P_NU0], q0[W.P_E0] = orb["val"][1][1], orb["val"][3][1]
+    q0[W.P_PHI0], q0[W.P_GAM0], q0[W.P_ALP0] = (2 * np.pi * orb["val"][k][1] for k in (0, 2, 4))
+    fwd = lso.orbit(q0, N - S, dt, S)                # stops short of the LSO node, so nothing plunges
+    assert fwd["status"] == 0
+    assert fwd["val"][1][-3] == pytest.approx(orb["val"][1][-4], rel=1e-8)
+    assert fwd["val"][3][-3] == pytest.approx(orb["val"][3][-4], rel=1e-8)
+
+
+def test_lso_waveform_ends_at_plunge_and_is_finite(lso):
+    p = _lso_params(0.3)
+    N, dt = 1 << 14, 15.0
+    hI, hII, st = lso.waveform(p, N, dt, 10)
+    assert st == 0 and np.all(np.isfinite(hI)) and np.abs(hI[-200:]).max() > 0
+    # the window ends AT plunge: every sample is live (no truncation flag), unlike a forward orbit that crosses the LSO
+    assert hI[-1] != 0.0 and hII[-1] != 0.0
+    lso.set_anchor(False)
+    q = p.copy()
+    q[W.P_NU0] = 0.999 * lso.nu_lso(p[W.P_M], p[W.P_E0])
+    _, _, st_fwd = lso.waveform(q, N, dt, 10)
+    assert st_fwd == 2
