@@ -17,6 +17,8 @@
  *    cudaMemcpyAsync on the same stream and DO synchronise the stream before returning.
  *  - One plan must not be used from two streams concurrently (the workspace is shared).
  *  - All functions return EMRI_OK (0) or a negative error code; they never throw or exit.
+ *  - EMRI_DEBUG_SYNC=1 in the environment makes stage (a) synchronise after each of its kernels and name on stderr
+ *    the one that failed (debugging aid; off by default).
  *
  * Parameter row, P = EMRI_NPAR = 17 doubles per walker, row-major params[K][17]
  * (first three are M, mu, S/M^2 as PAPER.md:149 prescribes):
@@ -108,7 +110,7 @@ int emri_plan_set_anchor(emri_plan* p, int at_lso);
  * t = 0, bad guard step).  Synchronises the device. */
 int emri_plan_orbit_report(emri_plan* p, int K, int32_t* modes);
 
-/* Number of walkers processed per internal chunk (bounds the workspace: 2*chunk*(N+2) doubles
+/* Number of walkers processed per internal chunk (bounds the workspace: chunk*N complex128 for z = h_I + i h_II
  * plus the cuFFT work area).  Default min(K_max, 128).  Reallocates; synchronises. */
 int emri_plan_set_chunk(emri_plan* p, int walkers_per_chunk);
 

@@ -1,13 +1,14 @@
 // emri.cu -- sm_100a implementation of include/emri.h (the hot path of EMRI_MC, arXiv 2311.17174).
 //
-// Stages:
-//   (a) orbit_kernel      one thread per walker: per-walker scalars (Eq. 6) and the
-//                         fixed-step RK4 integration of Eq. 1 on the coarse grid
-//   (b) synth_kernel      persistent CTAs over (walker, 256-sample tile): cubic-Hermite orbit,
-//                         Peters-Mathews harmonic sum n = 1..n_max (Eq. 2), LISA response
-//                         (PAPER.md:79, :118), propagation factors (Eqs. 4-6)
-//   (c) cufftExecD2Z      batched in-place real-to-complex transform, the one vendor call
-//   (d) loglike_kernel    streaming reduction of Eq. 8 + fixed-order final sum
+// Host side of the library: plan, workspace, stage sequencing, cuFFT.  Stages:
+//   (a) orbit.cuh    per-walker scalars (Eq. 6) and the fixed-step RK4 integration of Eq. 1
+//                     on the coarse grid, evaluated parallel in time (multiple shooting)
+//   (b) synth.cuh    persistent CTAs over (walker, unit of 256-sample tiles): cubic-Hermite orbit, Peters-Mathews
+//                    harmonic sum n = 1..n_max (Eq. 2), LISA response,
+//                    propagation factors (Eqs. 4-6); writes z = h_I + i h_II
+//   (c) cufftExecZ2Z one in-place complex transform per walker carries both channels, the one vendor call
+//   (d) loglike.cuh  streaming reduction of Eq. 8 on the packed spectrum (+ Eq. 7's factor) and the
+//                    fixed-order final sum
 // Nothing here is shared with oracle/ (which is test infrastructure).  FP64 throughout.
 #include <cuda_runtime.h>
 #include <cufft.h>
