@@ -36,9 +36,9 @@ CHUNK = 128                 # walkers per synth / cuFFT / loglike launch (emri_p
 # by ncu (2 dfma + dmul + dadd, smsp__sass_thread_inst_executed_op_*_pred_on.sum) on the configs' own inputs:
 # profiles/counts_r1.md.  SURVEY 8(d)-2 asks for counted instructions in place of its estimate 600 + 170 n_max
 # (2300 at n_max = 10), which the re-summed harmonic series undercuts by 3.7x.
-COUNTED_FLOPS = {5: 546.0, 10: 621.0, 20: 927.0, 30: 1248.0}
+COUNTED_FLOPS = {5: 546.0, 10: 619.0, 20: 921.0, 30: 1213.0}
 # DRAM bytes of one synth_kernel launch (dram__bytes_read.sum + dram__bytes_write.sum, same ncu pass)
-SYNTH_TRAFFIC = {0: 420096.0, 1: 1086312704.0, 2: 4486795520.0, 3: 4485041664.0}
+SYNTH_TRAFFIC = {0: 415488.0, 1: 1073785088.0, 2: 4438271488.0, 3: 4444701696.0}
 
 
 def counted_flops_per_walker_sample(n_max):
