@@ -265,6 +265,7 @@ def run_gpu(args, cfg):
     if rank == 0:
         peaks, peaks_src = load_measured_peaks()
         fp64_probe = emri.probe_fp64_peak()
+        fp64_probe3 = emri.probe_fp64_peak3()
         sm_max = clocks["sm_max_mhz"] or peaks.get("sm_max_mhz", 1965.0)
         sms = torch.cuda.get_device_properties(dev).multi_processor_count
         fp64_nominal = sms * 64 * 2 * sm_max * 1e6 * 1e-12        # 64 FP64 lanes / SM / clk
@@ -276,6 +277,7 @@ def run_gpu(args, cfg):
                     "unit": "TFLOP/s", "frac": achieved / fp64_nominal, "traffic": SYNTH_TRAFFIC.get(cfg.index),
                     "peak_source": f"derived: {sms} SMs x 64 FP64 lanes x 2 x {sm_max:.0f} MHz (DESIGN.md section 7)",
                     "peak_dfma_probe": fp64_probe, "frac_of_probe": achieved / fp64_probe,
+                    "peak_dfma_probe_3_register_operands": fp64_probe3,
                     "launches_per_step": n_chunks, "ms_per_launch": stage["synth"] / n_chunks,
                     "flops_per_walker_sample": fpws, "flops_source": "counted by ncu (profiles/counts_r1.md)" + (", figure of configs[2] at the same n_max" if mcmc else ""),
                     "algorithmic_bytes_per_launch": 16.0 * min(K, CHUNK) * N}

@@ -200,6 +200,9 @@ int emri_stretch_step(emri_plan* p, double* X, double* logL, int K, const double
  * emri_probe_fp64_peak: runs a dependent-chain-free DFMA kernel and returns TFLOP/s (FMA = 2).
  * emri_probe_hbm_read: streams `bytes` of device memory once and returns GB/s. */
 int emri_probe_fp64_peak(double* tflops, void* cuda_stream);
+/* The same with three fresh vector-register operands per DFMA (no constant, uniform-register or reused operand):
+ * what register-bound FP64 code can reach (on B200 2/3 of the figure above). */
+int emri_probe_fp64_peak3(double* tflops, void* cuda_stream);
 int emri_probe_hbm_read(int64_t bytes, double* gbs, void* cuda_stream);
 
 #ifdef __cplusplus

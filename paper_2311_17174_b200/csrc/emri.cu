@@ -670,6 +670,36 @@ int emri_probe_fp64_peak(double* tflops, void* stream) {
   return EMRI_OK;
 }
 
+int emri_probe_fp64_peak3(double* tflops, void* stream) {
+  if (!tflops) return EMRI_EINVAL;
+  cudaStream_t s = (cudaStream_t)stream;
+  int dev = 0, sms = 0;
+  if (cudaGetDevice(&dev) != cudaSuccess || cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev) != cudaSuccess)
+    return EMRI_ECUDA;
+  double* d = nullptr;
+  if (cudaMalloc(&d, 512 * sizeof(double)) != cudaSuccess) return EMRI_ENOMEM;
+  cudaMemsetAsync(d, 0, 512 * sizeof(double), s);
+  const int iters = 4096, blocks = sms * 8;
+  cudaEvent_t e0, e1;
+  cudaEventCreate(&e0); cudaEventCreate(&e1);
+  fp64_probe3_kernel<<<blocks, 256, 0, s>>>(d + 300, 64, d);      // warm-up
+  double best = 0.0;
+  for (int rep = 0; rep < 3; ++rep) {
+    cudaEventRecord(e0, s);
+    fp64_probe3_kernel<<<blocks, 256, 0, s>>>(d + 300, iters, d);
+    cudaEventRecord(e1, s);
+    if (cudaEventSynchronize(e1) != cudaSuccess) { cudaFree(d); return EMRI_ECUDA; }
+    float ms = 0.f;
+    cudaEventElapsedTime(&ms, e0, e1);
+    const double fl = 2.0 * 6.0 * (double)iters * 256.0 * (double)blocks;
+    best = std::max(best, fl / (ms * 1e-3) * 1e-12);
+  }
+  cudaEventDestroy(e0); cudaEventDestroy(e1);
+  cudaFree(d);
+  *tflops = best;
+  return EMRI_OK;
+}
+
 int emri_probe_hbm_read(int64_t bytes, double* gbs, void* stream) {
   if (!gbs || bytes < (1 << 20)) return EMRI_EINVAL;
   cudaStream_t s = (cudaStream_t)stream;

@@ -20,7 +20,7 @@ EXPORTS = (
     "emri_plan_set_coarse_stride", "emri_plan_set_orbit_schedule", "emri_plan_set_anchor", "emri_plan_orbit_report", "emri_plan_set_chunk", "emri_orbit", "emri_plan_num_nodes", "emri_waveform",
     "emri_waveform_fft", "emri_data_fft", "emri_loglike", "emri_loglike_fdep", "emri_loglike_host", "emri_plan_enable_timings",
     "emri_plan_get_timings", "emri_plan_last_cuda_error", "emri_plan_workspace_bytes", "emri_stretch_step",
-    "emri_probe_fp64_peak", "emri_probe_hbm_read",
+    "emri_probe_fp64_peak", "emri_probe_fp64_peak3", "emri_probe_hbm_read",
 )
 
 
@@ -64,6 +64,7 @@ def load():
     L.emri_plan_workspace_bytes.argtypes = [vp]
     L.emri_stretch_step.argtypes = [vp, vp, vp, i32, vp, vp, vp, dbl, u64, i64, i32, vp, vp, vp]
     L.emri_probe_fp64_peak.argtypes = [C.POINTER(dbl), vp]
+    L.emri_probe_fp64_peak3.argtypes = [C.POINTER(dbl), vp]
     L.emri_probe_hbm_read.argtypes = [i64, C.POINTER(dbl), vp]
     for name in EXPORTS:
         if name not in ("emri_strerror", "emri_plan_num_nodes", "emri_plan_workspace_bytes"):
@@ -95,6 +96,15 @@ def probe_fp64_peak():
     """TFLOP/s of a chain-free DFMA kernel on the current device (roofline denominator of stage b)."""
     v = C.c_double()
     rc = load().emri_probe_fp64_peak(C.byref(v), _stream())
+    if rc:
+        raise EmriError(f"fp64 probe failed ({rc})")
+    return v.value
+
+
+def probe_fp64_peak3():
+    """TFLOP/s of DFMAs with three fresh vector-register operands (register-file-bound FP64 rate)."""
+    v = C.c_double()
+    rc = load().emri_probe_fp64_peak3(C.byref(v), _stream())
     if rc:
         raise EmriError(f"fp64 probe failed ({rc})")
     return v.value
