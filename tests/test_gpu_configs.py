@@ -187,3 +187,27 @@ def test_argument_errors_on_the_device(emri):
     with pytest.raises(emri.EmriError, match="invalid argument"):
         plan.set_cosmology(-1.0, 0.3)
     plan.close()
+
+
+@pytest.mark.parametrize("N,S", [(4, 256), (16, 2), (258, 256), (514, 64), (2050, 256)])
+def test_tiny_and_ragged_lengths(emri, oracle, N, S):
+    """the smallest plans: one coarse interval, one shooting segment, a single ragged tile; stride 2 with 4 samples per
+    tile row; waveform parity and both orbit schedules"""
+    cfg = W.scaled(W.CONFIGS[1], K=3, N=N)
+    P = W.draw_params(W.scaled(W.CONFIGS[1], K=3, N=1 << 16))      # nu0 placed for an 11-day window: nothing plunges here
+    out = []
+    for schedule in (1, 0):
+        plan = emri.Plan(N, cfg.dt, cfg.n_max, cfg.K)
+        plan.set_coarse_stride(S)
+        plan.set_orbit_schedule(schedule)
+        st = torch.zeros(cfg.K, dtype=torch.int32, device="cuda")
+        hI, hII = plan.waveform(dev(P), status=st)
+        torch.cuda.synchronize()
+        out.append((hI.cpu().numpy(), hII.cpu().numpy(), st.cpu().numpy()))
+        plan.close()
+    h_ref, st_ref = oracle.waveform_batch(P, N, cfg.dt, cfg.n_max, S=S)
+    for hI, hII, st in out:
+        assert np.array_equal(st, st_ref) and not st.any()
+        assert np.max(np.abs(hI - h_ref[:, 0])) <= H_TOL * np.max(np.abs(h_ref[:, 0]))
+        assert np.max(np.abs(hII - h_ref[:, 1])) <= H_TOL * np.max(np.abs(h_ref[:, 1]))
+    assert np.max(np.abs(out[0][0] - out[1][0])) <= 1e-12 * np.max(np.abs(out[1][0]))
