@@ -227,3 +227,15 @@ def parity_walker_subset(params, n=16, seed=12345):
             break
         pick.append(int(k))
     return np.array(sorted(set(pick)))[:n]
+
+
+def paper_fig1_params(path):
+    """params[9][17] of the paper's Figure 1 grid (tests/golden/paper_fig1_parameters.txt), for a
+    plan anchored at the LSO: e0 = e_LSO, Phi0 = gamma0 = alpha0 = 0 at plunge; nu0 is ignored in that mode; GR."""
+    rows = np.loadtxt(path)
+    P = np.zeros((rows.shape[0], NPAR))
+    P[:, P_M], P[:, P_MU], P[:, P_A], P[:, P_E0] = rows[:, 0], rows[:, 1], rows[:, 2], rows[:, 3]
+    P[:, P_THS], P[:, P_PHS], P[:, P_THK], P[:, P_PHK], P[:, P_LAM], P[:, P_DL] = (rows[:, c] for c in range(4, 10))
+    P[:, P_NU0] = 1e-3
+    P[:, P_XI0] = 1.0
+    return P

@@ -203,3 +203,37 @@ def test_lso_anchored_waveform_and_loglike_match_oracle(emri, oracle):
     ref2, _ = oracle.waveform_batch(P[:1], cfg.N, cfg.dt, cfg.n_max)
     assert np.max(np.abs(h2.cpu().numpy()[0] - ref2[0, 0])) <= 1e-9 * np.max(np.abs(ref2[0, 0]))
     plan.close()
+
+
+def test_paper_fig1_grid_matches_oracle(emri, oracle):
+    """the paper's own illustration (Figure 1): M = 1e6, mu = 10, spins 0 / 0.4 / 0.8, e_LSO = 0 / 0.3 / 0.6,
+    the last hour before the LSO, and the same nine systems over the last year (N = 2^21, sampled)"""
+    import os
+    P = W.paper_fig1_params(os.path.join(os.path.dirname(os.path.abspath(__file__)), "golden", "paper_fig1_parameters.txt"))
+    oracle.set_anchor(True)
+    try:
+        for N, n_max, idx in ((256, 20, None), (1 << 21, 30, "sampled")):
+            dt = 15.0
+            plan = emri.Plan(N, dt, n_max, 9)
+            plan.set_anchor(True)
+            st = torch.zeros(9, dtype=torch.int32, device="cuda")
+            hI, hII = plan.waveform(dev(P), status=st)
+            torch.cuda.synchronize()
+            hI, hII, st = hI.cpu().numpy(), hII.cpu().numpy(), st.cpu().numpy()
+            if idx is not None:
+                rng = np.random.default_rng(1)
+                idx = np.unique(np.concatenate([np.arange(0, 300), np.arange(N - 600, N), rng.integers(0, N, 1200)]))
+            for k in range(9):
+                a, b, s_ref = oracle.waveform(P[k], N, dt, n_max, idx=idx)
+                assert st[k] == s_ref
+                if s_ref:
+                    assert not hI[k].any()          # e grew past 1 on the way back: invalid on both sides
+                    continue
+                sel = slice(None) if idx is None else idx
+                eI = np.max(np.abs(hI[k][sel] - a)) / np.max(np.abs(hI[k]))
+                eII = np.max(np.abs(hII[k][sel] - b)) / np.max(np.abs(hII[k]))
+                assert eI <= 1e-9 and eII <= 1e-9, (N, k, eI, eII)
+            print(f"Fig. 1 grid, N = {N}: status {st}, modes {plan.orbit_report(9)}")
+            plan.close()
+    finally:
+        oracle.set_anchor(False)

@@ -5,6 +5,7 @@ something other than itself: a library routine of different construction (scipy/
 closed form, an identity, a limit, a convergence order, or brute force on a tiny input.
 """
 import math
+import os
 
 import mpmath
 import numpy as np
@@ -914,3 +915,36 @@ def test_lso_waveform_ends_at_plunge_and_is_finite(lso):
     q[W.P_NU0] = 0.999 * lso.nu_lso(p[W.P_M], p[W.P_E0])
     _, _, st_fwd = lso.waveform(q, N, dt, 10)
     assert st_fwd == 2
+
+
+# ----------------------------------------------------------------------------- the paper's Figure 1 set-up (inputs only)
+FIG1 = os.path.join(os.path.dirname(os.path.abspath(__file__)), "golden", "paper_fig1_parameters.txt")
+
+
+def test_paper_fig1_grid_last_hour_before_plunge(lso):
+    """nine waveforms over the last hour before the LSO.  What the text fixes: the orbit ends on nu_LSO
+    (PAPER.md:120), the waveforms are finite and live to the last sample, and for e_LSO = 0 the signal is the n = 2
+    quadrupole at 2 nu_LSO = 2 / (2 pi M 6^{3/2}) = 4.397 mHz for M = 1e6 Msun."""
+    P = W.paper_fig1_params(FIG1)
+    assert P.shape == (9, 17)
+    dt, N, S = 15.0, 256, 256                        # 64 min: one coarse interval ending at plunge
+    for p in P:
+        hI, hII, st = lso.waveform(p, N, dt, 20, S=S)
+        assert st == 0 and np.all(np.isfinite(hI)) and np.all(np.isfinite(hII))
+        assert hI[-1] != 0.0 and 1e-24 < np.max(np.abs(hI)) < 1e-20           # strain of a 10 Msun body at 1 Gpc
+        orb = lso.orbit(p, N, dt, S)
+        assert orb["val"][1][-2] == pytest.approx(lso.nu_lso(p[W.P_M], p[W.P_E0]), rel=1e-15)
+    # circular cases: only n = 2 survives, h ~ cos(2 Phi + 2 gamma): the GW frequency is twice the AZIMUTHAL frequency
+    # nu + gamma~'/2pi (in the AK model nu is the radial frequency; at the LSO the periapsis advance gamma~' is as large as
+    # nu itself), here from the rates at the two nodes bracketing the hour; count the zero crossings
+    f_orb = 1.0 / (2 * np.pi * 1e6 * 4.925490947e-6 * 6 ** 1.5)
+    assert f_orb == pytest.approx(2.1985e-3, rel=1e-3)             # nu_LSO(e = 0), PAPER.md:120
+    for p in P[[0, 3, 6]]:
+        hI, _, _ = lso.waveform(p, N, dt, 20, S=S)
+        orb = lso.orbit(p, N, dt, S)
+        assert orb["val"][1][-2] == pytest.approx(f_orb, rel=1e-12)
+        f_az = 0.5 * ((orb["slope"][0][1] + orb["slope"][2][1]) + (orb["slope"][0][-2] + orb["slope"][2][-2]))
+        assert 1.5 * f_orb < f_az < 2.5 * f_orb
+        crossings = np.sum(np.signbit(hI[1:]) != np.signbit(hI[:-1]))
+        # (with spin the precession of the orbital plane, alpha' ~ 0.1 nu at a = 0.8, shifts the observed phase by a few per cent)
+        assert crossings == pytest.approx(2 * (2 * f_az) * N * dt, rel=0.10)
