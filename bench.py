@@ -114,6 +114,7 @@ def oracle_sample(cfg, P, walkers, stride, with_likelihood):
     from concurrent.futures import ThreadPoolExecutor
     from oracle.oracle import Oracle
     orc = Oracle()
+    orc.set_anchor(cfg.index == 5)
     idx = None if stride == 1 else np.arange(0, cfg.N, stride, dtype=np.int64)
     n = cfg.N if idx is None else idx.size
     psd = W.lisa_psd_barack_cutler(cfg.N, cfg.dt) if with_likelihood else None
@@ -193,6 +194,8 @@ def run_gpu(args, cfg):
     P = W.draw_params(sharding.rank_config(cfg, rank))
     psd = W.lisa_psd_barack_cutler(N, cfg.dt)
     plan = emri.Plan(N, cfg.dt, cfg.n_max, K, psd)
+    if cfg.index == 5:
+        plan.set_anchor(True)            # the paper's convention: initial conditions at the LSO, integrated backwards
     p_d = torch.from_numpy(P).to(dev)
     # data = the library's own injection of walker 0 (+ seeded coloured noise when the config says so)
     spec = plan.waveform_fft(p_d[:1].contiguous())
@@ -202,7 +205,7 @@ def run_gpu(args, cfg):
     logL = torch.empty(K, dtype=torch.float64, device=dev)
     status = torch.zeros(K, dtype=torch.int32, device=dev)
 
-    mcmc = cfg.index == 4
+    mcmc = cfg.index in (4, 5)
     if mcmc:
         # configs[4]: a step is one full stretch-move update (both half-ensembles), proposals / accept on the device
         lo_d, hi_d = (torch.from_numpy(v).to(dev) for v in W.prior_box(cfg))
@@ -326,7 +329,8 @@ def main():
     ap.add_argument("--gpus", type=int, default=1)
     ap.add_argument("--steps", type=int, default=10)
     ap.add_argument("--warmup", type=int, default=3)
-    ap.add_argument("--config", type=int, default=1, help="index into BASELINE.json:configs (0-4; 4 = stretch-move steps)")
+    ap.add_argument("--config", type=int, default=1,
+                    help="index into BASELINE.json:configs (0-4; 4 = stretch-move steps); 5 = the paper's own run shape")
     ap.add_argument("--impl", default="b200", choices=["b200", "reference"])
     args = ap.parse_args()
     cfg = W.CONFIGS[args.config]

@@ -56,7 +56,13 @@ CONFIGS = (
            "logL only"),
     Config(4, 512, 1 << 21, 15.0, 20, 4, (5.5, 6.5), (0.5, 1.5), (0.0, 0.95), (0.0, 0.3), (0.5, 3.0), False, 1004,
            "ensemble MCMC, 200 stretch-move steps"),
+    # not in BASELINE.json: the shape of the paper's own run: 8 walkers, 4 free parameters
+    # (M, mu, S/M^2, Xi0), one year at 0.1 Hz (dt = 10 s; N = 3 * 2^20 = 364.1 d), noise-less data, orbit anchored at the
+    # LSO with e_LSO = 0.3 and the angles of PAPER.md:147; n_max is not stated in the paper (20 here), nor n of Eq. 6 (2)
+    Config(5, 8, 3 << 20, 10.0, 20, 5, (6.0, 6.0), (1.0, 1.0), (0.1, 0.1), (0.3, 0.3), (1.0, 1.0), False, 0,
+           "the paper's run shape: 8 walkers, 4 free parameters, 1 yr at 0.1 Hz, anchored at the LSO"),
 )
+PAPER_RUN_FREE = (P_M, P_MU, P_A, P_XI0)
 
 
 def scaled(cfg, K=None, N=None, n_max=None):
@@ -124,6 +130,8 @@ def draw_params(cfg, K=None):
     K = cfg.K if K is None else K
     if cfg.index == 4:
         return _draw_mcmc_ensemble(rng, cfg, K)
+    if cfg.index == 5:
+        return _draw_paper_run(rng, K)
     return np.stack([_draw_row(rng, cfg) for _ in range(K)])
 
 
@@ -142,9 +150,32 @@ def _draw_mcmc_ensemble(rng, cfg, K):
     return P
 
 
+def _draw_paper_run(rng, K):
+    """the paper's fiducial system at the LSO and K walkers in a small ball in its 4 free parameters"""
+    star = np.zeros(NPAR)
+    star[P_M], star[P_MU], star[P_A], star[P_E0], star[P_NU0] = 1e6, 10.0, 0.1, 0.3, 1e-3
+    star[P_LAM], star[P_THS], star[P_PHS], star[P_THK], star[P_PHK] = np.pi / 6, np.pi / 4, 0.0, np.pi / 8, 0.0
+    star[P_DL], star[P_XI0], star[P_NXI] = 1.0, 1.0, 2.0
+    P = np.tile(star, (K, 1))
+    g = rng.standard_normal((K, NPAR))
+    g[0] = 0.0
+    P[:, P_M] *= 1.0 + 1e-7 * g[:, P_M]
+    P[:, P_MU] *= 1.0 + 1e-7 * g[:, P_MU]
+    P[:, P_A] += 1e-7 * g[:, P_A]
+    P[:, P_XI0] += 1e-2 * g[:, P_XI0]
+    return P
+
+
 def prior_box(cfg):
-    """Uniform box prior of config 4: lo[17], hi[17] (the config-1 ranges + propagation ranges)."""
+    """Uniform box prior of config 4: lo[17], hi[17] (the config-1 ranges + propagation ranges); config 5: only the paper's
+    four free parameters have a range, every other column is held fixed (lo = hi)."""
     lo, hi = np.zeros(NPAR), np.zeros(NPAR)
+    if cfg.index == 5:
+        lo[P_M], hi[P_M] = 1e5, 1e7
+        lo[P_MU], hi[P_MU] = 1.0, 100.0
+        lo[P_A], hi[P_A] = 0.0, 0.95
+        lo[P_XI0], hi[P_XI0] = 0.5, 1.5
+        return lo, hi
     lo[P_M], hi[P_M] = 10.0 ** cfg.log10_M[0], 10.0 ** cfg.log10_M[1]
     lo[P_MU], hi[P_MU] = 10.0 ** cfg.log10_mu[0], 10.0 ** cfg.log10_mu[1]
     lo[P_A], hi[P_A] = 0.0, 0.95
