@@ -244,7 +244,7 @@ int run_orbit(emri_plan* p, const double* params, int K, cudaStream_t s) {
     const int64_t threads = (int64_t)K * sa.P * (r == 0 ? 3 : 1);
     orbit_sweep_kernel<<<(unsigned)((threads + 63) / 64), 64, 0, s>>>(sa);
     DBG("orbit_sweep_kernel");
-    orbit_correct_kernel<<<K, 32, (size_t)sa.P * 8 * sizeof(double), s>>>(sa);
+    orbit_correct_kernel<<<K, 32, (size_t)sa.P * 12 * sizeof(double), s>>>(sa);
     DBG("orbit_correct_kernel");
   }
   orbit_tail_kernel<<<(K + 31) / 32, 32, 0, s>>>(sa);

@@ -580,7 +580,8 @@ __global__ void __launch_bounds__(64) orbit_sweep_kernel(ShootArgs s) {
 
 // ---- 3. per walker (one warp): defects, verification, Newton correction or finalisation
 __global__ void __launch_bounds__(32) orbit_correct_kernel(ShootArgs s) {
-  extern __shared__ double sm_c[];          // [P][8]: D_nu, D_e, J00, J01, J10, J11, stop, finite
+  extern __shared__ double sm_c[];          // [P][CS]: D_nu, D_e, J00, J01, J10, J11, stop, finite, tol_nu, tol_e, d_nu, d_e
+  constexpr int CS = 12;
   const OrbitArgs& a = s.o;
   const int k = blockIdx.x, lane = threadIdx.x;
   if (s.mode[k] != OM_ACTIVE) return;
@@ -589,7 +590,7 @@ __global__ void __launch_bounds__(32) orbit_correct_kernel(ShootArgs s) {
   // boundary b = p+1 between segment p and p+1: defect of segment p's end against segment p+1's start
   for (int p = lane; p < P; p += 32) {
     double* sg = seg + (size_t)p * SEG_STRIDE;
-    double* o = sm_c + (size_t)p * 8;
+    double* o = sm_c + (size_t)p * CS;
     if (s.round == 0) {
       const double dn1 = (sg[SG_P1NU] - sg[SG_ENU]) - (sg[SG_P1CNU] - sg[SG_ECNU]);
       const double de1 = (sg[SG_P1E] - sg[SG_EE]) - (sg[SG_P1CE] - sg[SG_ECE]);
@@ -607,7 +608,8 @@ __global__ void __launch_bounds__(32) orbit_correct_kernel(ShootArgs s) {
       De = (sg[SG_EE] - nx[SG_E]) - (sg[SG_ECE] - nx[SG_CE]);
     }
     o[0] = Dn; o[1] = De;
-    sg[SG_O0] = 0.0; sg[SG_O1] = 0.0;      // correction of this segment's start (set by the scan below)
+    o[8] = 4e-17 * fabs(sg[SG_ENU]); o[9] = 4e-17 * fabs(sg[SG_EE]);      // verification tolerance of boundary p+1
+    o[10] = 0.0; o[11] = 0.0;              // correction of THIS segment's start (set by the scan below)
     o[7] = (isfinite(Dn) && isfinite(De) && isfinite(o[2]) && isfinite(o[3]) && isfinite(o[4]) && isfinite(o[5])) ? 1.0 : 0.0;
   }
   __syncwarp();
@@ -617,20 +619,16 @@ __global__ void __launch_bounds__(32) orbit_correct_kernel(ShootArgs s) {
     int first_bad = -1, stop_seg = -1;
     double dn = 0.0, de = 0.0;
     for (int p = 0; p < P; ++p) {
-      const double* o = sm_c + (size_t)p * 8;
+      double* o = sm_c + (size_t)p * CS;
       if (o[6] != 0.0) { if (first_bad < 0) stop_seg = p; break; }
       if (p + 1 == P) break;
-      const double* sg = seg + (size_t)p * SEG_STRIDE;
-      const double tn = 4e-17 * fabs(sg[SG_ENU]), te = 4e-17 * fabs(sg[SG_EE]);
-      const bool small = (o[7] != 0.0) && fabs(o[0]) <= tn && fabs(o[1]) <= te;
+      const bool small = (o[7] != 0.0) && fabs(o[0]) <= o[8] && fabs(o[1]) <= o[9];
       if (!small && first_bad < 0) first_bad = p + 1;
       if (o[7] != 0.0) {
         const double nn = o[0] + fma(o[2], dn, o[3] * de), ne = o[1] + fma(o[4], dn, o[5] * de);
         dn = nn; de = ne;
       } else { dn = 0.0; de = 0.0; }
-      // SG_O0 / SG_O1 of segment p+1 hold its correction until the walker is finalised
-      seg[(size_t)(p + 1) * SEG_STRIDE + SG_O0] = dn;
-      seg[(size_t)(p + 1) * SEG_STRIDE + SG_O1] = de;
+      o[CS + 10] = dn; o[CS + 11] = de;      // correction of segment p+1's start (the scan touches shared memory only)
     }
     sh_first_bad = first_bad; sh_stop_seg = stop_seg;
     sh_converged = (first_bad < 0) ? 1 : 0;
@@ -641,7 +639,7 @@ __global__ void __launch_bounds__(32) orbit_correct_kernel(ShootArgs s) {
     // Newton (chord) update of the segment starts, in compensated form
     for (int p = 1 + lane; p < P; p += 32) {
       double* sg = seg + (size_t)p * SEG_STRIDE;
-      const double dn = sg[SG_O0], de = sg[SG_O1];
+      const double dn = sm_c[(size_t)p * CS + 10], de = sm_c[(size_t)p * CS + 11];
       if (isfinite(dn) && isfinite(de)) {
         const double yn = sg[SG_NU] + dn; sg[SG_CNU] += (yn - sg[SG_NU]) - dn; sg[SG_NU] = yn;
         const double ye = sg[SG_E] + de; sg[SG_CE] += (ye - sg[SG_E]) - de; sg[SG_E] = ye;
