@@ -210,6 +210,12 @@ DEVINL double4 ldg4(const double4* p) {
     CB = fma(CB, B.ec, -SB * B.es); SB = fma(SB, B.ec, tb * B.es);                               \
   }
 
+// The six Horner chains of one harmonic (2 samples x 3 series) are issued in an order in which every consecutive
+// pair of DFMAs shares one operand in the same slot -- A_a, B_a (coefficient a), B_b (x_B), A_b (coefficient b), A_c (x_A),
+// B_c (coefficient c) -- so that the operand-reuse cache feeds it and each DFMA reads two fresh registers, not three.
+// Measured on B200 (section 7 of DESIGN.md): 28.9 TFLOP/s for this pattern against 20.9 in the compiler's own order.
+// `asm volatile` pins the order.
+#define EMRI_FMA(d, a, b, c) asm volatile("fma.rn.f64 %0, %1, %2, %3;" : "=d"(d) : "d"(a), "d"(b), "d"(c))
 template <int M>
 DEVINL void series_local(const double4* __restrict__ t, double xa, double xb, double p[6]) {
   double4 c = t[M - 1];
@@ -217,8 +223,9 @@ DEVINL void series_local(const double4* __restrict__ t, double xa, double xb, do
 #pragma unroll
   for (int m = M - 2; m >= 0; --m) {
     c = t[m];
-    p[0] = fma(p[0], xa, c.x); p[1] = fma(p[1], xa, c.y); p[2] = fma(p[2], xa, c.z);
-    p[3] = fma(p[3], xb, c.x); p[4] = fma(p[4], xb, c.y); p[5] = fma(p[5], xb, c.z);
+    EMRI_FMA(p[0], p[0], xa, c.x); EMRI_FMA(p[3], p[3], xb, c.x);
+    EMRI_FMA(p[4], p[4], xb, c.y); EMRI_FMA(p[1], p[1], xa, c.y);
+    EMRI_FMA(p[2], p[2], xa, c.z); EMRI_FMA(p[5], p[5], xb, c.z);
   }
 }
 
