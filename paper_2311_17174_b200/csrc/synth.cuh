@@ -197,17 +197,22 @@ DEVINL double4 ldg4(const double4* p) {
 // Harmonic sum n = 1..n_max for the thread's two samples; returns S_a, S_b, S_c of each.  Coefficients are
 // warp-uniform.  Local version: M orders of the re-expanded series (compile-time M: fully unrolled Horner, the
 // coefficient loads of the next harmonic can be hoisted above the arithmetic of the current one).
+#define EMRI_FMA(d, a, b, c) asm volatile("fma.rn.f64 %0, %1, %2, %3;" : "=d"(d) : "d"(a), "d"(b), "d"(c))
+#define EMRI_MUL(d, a, b) asm volatile("mul.rn.f64 %0, %1, %2;" : "=d"(d) : "d"(a), "d"(b))
 #define EMRI_ACCUM_FIRST()                                                                       \
   double SaA = p[0] * A.ec, SbA = p[1] * A.es, ScA = p[2] * A.ec;                                \
   double SaB = p[3] * B.ec, SbB = p[4] * B.es, ScB = p[5] * B.ec;                                \
   double CA = A.C2, SA = A.S2, CB = B.C2, SB = B.S2;
 #define EMRI_ACCUM_NEXT()                                                                        \
-  SaA = fma(p[0], CA, SaA); SbA = fma(p[1], SA, SbA); ScA = fma(p[2], CA, ScA);                  \
-  SaB = fma(p[3], CB, SaB); SbB = fma(p[4], SB, SbB); ScB = fma(p[5], CB, ScB);                  \
   {                                                                                              \
-    const double ta = CA, tb = CB;                                                               \
-    CA = fma(CA, A.ec, -SA * A.es); SA = fma(SA, A.ec, ta * A.es);                               \
-    CB = fma(CB, B.ec, -SB * B.es); SB = fma(SB, B.ec, tb * B.es);                               \
+    /* issue order chosen so that consecutive instructions share an operand slot (see series_local) */ \
+    double ta, ua, tb, ub;                                                                       \
+    EMRI_FMA(SaA, p[0], CA, SaA); EMRI_FMA(ScA, p[2], CA, ScA); EMRI_FMA(SbA, p[1], SA, SbA);    \
+    EMRI_MUL(ta, SA, A.es); EMRI_MUL(ua, CA, A.es);                                              \
+    EMRI_FMA(CA, CA, A.ec, -ta); EMRI_FMA(SA, SA, A.ec, ua);                                     \
+    EMRI_FMA(SaB, p[3], CB, SaB); EMRI_FMA(ScB, p[5], CB, ScB); EMRI_FMA(SbB, p[4], SB, SbB);    \
+    EMRI_MUL(tb, SB, B.es); EMRI_MUL(ub, CB, B.es);                                              \
+    EMRI_FMA(CB, CB, B.ec, -tb); EMRI_FMA(SB, SB, B.ec, ub);                                     \
   }
 
 // The six Horner chains of one harmonic (2 samples x 3 series) are issued in an order in which every consecutive
@@ -215,7 +220,6 @@ DEVINL double4 ldg4(const double4* p) {
 // B_c (coefficient c) -- so that the operand-reuse cache feeds it and each DFMA reads two fresh registers, not three.
 // Measured on B200 (section 7 of DESIGN.md): 28.9 TFLOP/s for this pattern against 20.9 in the compiler's own order.
 // `asm volatile` pins the order.
-#define EMRI_FMA(d, a, b, c) asm volatile("fma.rn.f64 %0, %1, %2, %3;" : "=d"(d) : "d"(a), "d"(b), "d"(c))
 template <int M>
 DEVINL void series_local(const double4* __restrict__ t, double xa, double xb, double p[6]) {
   double4 c = t[M - 1];
