@@ -1,18 +1,20 @@
 #!/usr/bin/env python
 """bench.py -- throughput of the EMRI_MC hot path on B200 (contract: see DESIGN.md section 8).
 
-  python bench.py [--gpus N] [--steps K] [--warmup W] [--config i] [--impl reference]
+  python bench.py [--gpus N] [--steps K] [--warmup W] [--config i] [--psd bc|robson] [--impl reference]
 
-A "step" is one pass of the whole hot path -- emri_loglike: orbit RK4 (a), synthesis (b), cuFFT Z2Z
-(c: one complex transform per walker carries both channels), likelihood reduction (d) -- over one ensemble of K walkers of BASELINE.json:configs[i]
-(default i = 1: K=64, N=2^20, n_max=10).  Inputs are synthetic and seeded (workloads.py).  Prints ONE
-JSON line.  `value` = walker*samples/s with inputs resident in HBM; `e2e` = the same through
-emri_loglike_host with pinned HOST buffers (copies inside the timed region).  With N > 1 (torchrun)
-every rank runs its own K walkers (the path shards by walker, no data-path collective): weak scaling.
+A "step" is one pass of the whole hot path -- emri_loglike: orbit RK4 (a), synthesis (b), transform (c), likelihood
+reduction (d) -- over one ensemble of K walkers of BASELINE.json:configs[i].  Default i = 3, the largest single-GPU
+configuration (K=1024, N=2^21, n_max=30); the other configs are parity-test cases, reachable with --config.
+Inputs are synthetic and seeded (workloads.py).  Prints ONE JSON line.  `value` = walker*samples/s with inputs resident
+in HBM; `e2e` = the same through emri_loglike_host with pinned HOST buffers (copies inside the timed region).  With N > 1
+(torchrun) every rank runs its own K walkers (the path shards by walker, no data-path collective): weak scaling.
 
-`--impl reference` times the CPU oracle (oracle/, test infrastructure) on the host cores instead.
+`--impl reference` times the CPU oracle (oracle/, test infrastructure) on the host cores instead: the SAME work in kind
+as the `cpu_baseline` leg of the GPU arm (orbit + waveform at every sample + rfft + logL), on a bounded sample.
 """
 import argparse
+import hashlib
 import json
 import os
 import sys
@@ -25,25 +27,41 @@ ROOT = os.path.dirname(os.path.abspath(__file__))
 if ROOT not in sys.path:
     sys.path.insert(0, ROOT)
 
-from paper_2311_17174_b200 import workloads as W  # noqa: E402
+from paper_2311_17174_b200 import sharding, workloads as W  # noqa: E402
 
 METRIC = "AK waveform+logL evaluations/sec (walkers x samples/s)"
 UNIT = "walker*samples/s"
-ORBIT_KERNELS = 10          # orbit_init, 3 x (orbit_sweep, orbit_correct), orbit_tail, orbit_fixup, orbit_aux
-CHUNK = 128                 # walkers per synth / cuFFT / loglike launch (emri_plan_set_chunk default)
-
-# Algorithmic work of synth_kernel per (walker, sample): FP64 flops EXECUTED by the kernel as it stands, counted
-# by ncu (2 dfma + dmul + dadd, smsp__sass_thread_inst_executed_op_*_pred_on.sum) on the configs' own inputs:
-# profiles/counts_r1.md.  SURVEY 8(d)-2 asks for counted instructions in place of its estimate 600 + 170 n_max
-# (2300 at n_max = 10), which the re-summed harmonic series undercuts by 3.7x.
-COUNTED_FLOPS = {5: 546.0, 10: 619.0, 20: 921.0, 30: 1213.0}
-# DRAM bytes of one synth_kernel launch (dram__bytes_read.sum + dram__bytes_write.sum, same ncu pass)
-SYNTH_TRAFFIC = {0: 415488.0, 1: 1073785088.0, 2: 4438271488.0, 3: 4444701696.0}
+CHUNK = 128                 # walkers per synth / transform / loglike launch (emri_plan_set_chunk default)
+COUNTS_FILE = os.path.join(ROOT, "profiles", "counts_r2.json")
+COUNTED_SOURCES = ("paper_2311_17174_b200/csrc/synth.cuh",)
+# The oracle leg covers the first N / ORACLE_DECIMATE[i] samples of the window (same dt, n_max, parameters): a bounded
+# sample of the workload sized to a few seconds of host time per step.
+ORACLE_DECIMATE = {0: 1, 1: 1, 2: 4, 3: 4, 4: 4, 5: 4}
 
 
-def counted_flops_per_walker_sample(n_max):
-    ks = sorted(COUNTED_FLOPS)
-    return float(np.interp(n_max, ks, [COUNTED_FLOPS[k] for k in ks]))
+def git_blob_sha(path):
+    """`git hash-object` of a file, computed here (the GPU box has no .git)"""
+    data = open(path, "rb").read()
+    return hashlib.sha1(b"blob %d\0" % len(data) + data).hexdigest()
+
+
+def counted_work(cfg_index, n_max):
+    """Algorithmic work of synth_kernel per (walker, sample): FP64 flops EXECUTED by the kernel as built (2 dfma + dmul +
+    dadd, ncu thread-instruction counters) and its DRAM bytes per launch, from profiles/counts_r2.json.  The file records
+    the git blob hash of the kernel source it was counted on: a different source gives (None, None, 'stale')."""
+    try:
+        with open(COUNTS_FILE) as f:
+            c = json.load(f)
+    except Exception as e:
+        return None, None, f"missing ({e.__class__.__name__})"
+    for rel in COUNTED_SOURCES:
+        if c.get("sources", {}).get(rel) != git_blob_sha(os.path.join(ROOT, rel)):
+            return None, None, "stale"
+    entry = c.get("configs", {}).get(str(cfg_index))
+    if not entry or entry.get("n_max") != n_max:
+        return None, None, "not counted for this config"
+    return float(entry["flops_per_walker_sample"]), entry.get("dram_bytes_per_launch"), \
+        f"counted by ncu on the configs' own inputs ({os.path.relpath(COUNTS_FILE, ROOT)}, source hash verified)"
 
 
 def load_measured_peaks():
@@ -108,54 +126,75 @@ def host_cores():
         return os.cpu_count() or 1
 
 
-def oracle_sample(cfg, P, walkers, stride, with_likelihood):
-    """Time the oracle, as it stands, on `walkers` walkers (one per thread), every `stride`-th sample.
-    Returns (seconds, walker*samples processed)."""
-    from concurrent.futures import ThreadPoolExecutor
-    from oracle.oracle import Oracle
-    orc = Oracle()
-    orc.set_anchor(cfg.index == 5)
-    idx = None if stride == 1 else np.arange(0, cfg.N, stride, dtype=np.int64)
-    n = cfg.N if idx is None else idx.size
-    psd = W.lisa_psd_barack_cutler(cfg.N, cfg.dt) if with_likelihood else None
+def psd_of(args, N, dt):
+    return W.lisa_psd_robson(N, dt) if args.psd == "robson" else W.lisa_psd_barack_cutler(N, dt)
 
-    def one(k):
-        hI, hII, st = orc.waveform(P[k], cfg.N, cfg.dt, cfg.n_max, idx=idx)
-        if with_likelihood and idx is None:
+
+def workload_config(cfg, args):
+    """the `config` object: identical in the GPU arm and the reference arm"""
+    return {"workload": f"configs[{cfg.index}]: K={cfg.K} walkers per GPU, N={cfg.N}, dt={cfg.dt} s, n_max={cfg.n_max}, "
+                        f"data = injection{' + coloured noise' if cfg.noise_seed else ''}, "
+                        f"PSD = {'Robson-Cornish-Liu' if args.psd == 'robson' else 'Barack-Cutler'}"
+                        + (", a step = one stretch-move update of the ensemble" if cfg.index in (4, 5) else ""),
+            "l2": f"per-step working set {16 * cfg.K * cfg.N / 1e6:.0f} MB > 126 MB L2: no flush needed"
+                  if 16 * cfg.K * cfg.N > 126e6 else "per-step working set fits L2 (launch-bound case, reported as is)"}
+
+
+class OracleLeg:
+    """The oracle as it stands, one walker per host thread: orbit + waveform at EVERY sample + rfft of both channels +
+    logL against a zero data spectrum, over the first N' = N / ORACLE_DECIMATE samples of the window (same dt, n_max and
+    parameter rows).  Used by the `cpu_baseline` leg of the GPU arm (one step) and by --impl reference (every step)."""
+
+    def __init__(self, cfg, args):
+        from oracle.oracle import Oracle
+        self.cfg = cfg
+        self.orc = Oracle(anchor=(cfg.index == 5))
+        self.walkers = min(host_cores(), cfg.K)
+        self.P = W.draw_params(cfg, K=self.walkers)
+        self.Np = cfg.N // ORACLE_DECIMATE.get(cfg.index, 4)
+        self.psd = psd_of(args, self.Np, cfg.dt)
+
+    def describe(self, seconds=None):
+        s = (f"oracle orbit + waveform at every sample + rfft + logL of {self.walkers} walkers (one per thread) over the "
+             f"first {self.Np} of N={self.cfg.N} samples")
+        return s + (f", {seconds:.1f} s" if seconds is not None else " per step")
+
+    def step(self, n=None):
+        """returns (seconds, walker*samples processed)"""
+        from concurrent.futures import ThreadPoolExecutor
+        n = self.Np if n is None else n
+        psd = self.psd if n == self.Np else W.lisa_psd_barack_cutler(n, self.cfg.dt)
+        orc, cfg = self.orc, self.cfg
+
+        def one(k):
+            hI, hII, st = orc.waveform(self.P[k], n, cfg.dt, cfg.n_max)
             H = np.stack([orc.rfft(hI), orc.rfft(hII)])
-            return orc.loglike(H, np.zeros_like(H), psd, cfg.N, cfg.dt)
-        return float(hI[0])
+            return orc.loglike(H, np.zeros_like(H), psd, n, cfg.dt)
 
-    t0 = time.perf_counter()
-    with ThreadPoolExecutor(max_workers=walkers) as ex:      # ctypes releases the GIL during the call
-        list(ex.map(one, range(walkers)))
-    return time.perf_counter() - t0, walkers * n
+        t0 = time.perf_counter()
+        with ThreadPoolExecutor(max_workers=self.walkers) as ex:      # ctypes releases the GIL during the call
+            list(ex.map(one, range(self.walkers)))
+        return time.perf_counter() - t0, self.walkers * n
 
 
 def run_reference(args, cfg):
     """--impl reference: the CPU oracle on the host cores; rank 0 only."""
     if int(os.environ.get("RANK", "0")) != 0:
         return
-    cores = host_cores()
-    walkers = min(cores, cfg.K)
-    P = W.draw_params(cfg, K=walkers)
-    # one step = the oracle waveform of `walkers` walkers at every `stride`-th sample of the N-sample series
-    stride = 32
+    leg = OracleLeg(cfg, args)
     for _ in range(args.warmup):
-        oracle_sample(cfg, P, walkers, stride * 8, False)
+        leg.step(n=1 << 12)                      # loads the library and the thread pool; a CPU has nothing else to warm
     t, units = 0.0, 0
     for _ in range(args.steps):
-        dt_, u = oracle_sample(cfg, P, walkers, stride, False)
+        dt_, u = leg.step()
         t += dt_
         units += u
     value = units / t
-    sample = f"oracle waveform (orbit + every {stride}th of N={cfg.N} samples) of {walkers} walkers, one per thread, per step"
     print(json.dumps({
         "impl": "reference", "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": args.gpus, "steps": args.steps,
         "warmup": args.warmup, "ms_per_step": 1e3 * t / args.steps, "higher_is_better": True, "scaling": "weak",
-        "vs_baseline": None, "dtype": "f64", "data": "synthetic",
-        "config": {"workload": f"configs[{cfg.index}]: K={cfg.K} N={cfg.N} dt={cfg.dt} n_max={cfg.n_max}"},
-        "cpu_baseline": {"value": value, "unit": UNIT, "cores": walkers, "kind": "oracle", "sample": sample},
+        "vs_baseline": None, "dtype": "f64", "data": "synthetic", "config": workload_config(cfg, args),
+        "cpu_baseline": {"value": value, "unit": UNIT, "cores": leg.walkers, "kind": "oracle", "sample": leg.describe()},
         "e2e": {"value": value, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
     }))
 
@@ -163,7 +202,7 @@ def run_reference(args, cfg):
 def run_gpu(args, cfg):
     import torch
     import torch.distributed as dist
-    from paper_2311_17174_b200 import emri
+    from paper_2311_17174_b200 import emri, probe
 
     rank = int(os.environ.get("RANK", "0"))
     world = int(os.environ.get("WORLD_SIZE", "1"))
@@ -180,19 +219,11 @@ def run_gpu(args, cfg):
             dist.barrier()
         torch.cuda.synchronize()
 
-    def max_over_ranks(x):
-        if world == 1:
-            return x
-        t = torch.tensor([x], dtype=torch.float64, device=dev)
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-        return float(t.item())
-
     emri.load()
     K, N = cfg.K, cfg.N
     # every rank draws its own ensemble (weak scaling: K walkers per GPU)
-    from paper_2311_17174_b200 import sharding
     P = W.draw_params(sharding.rank_config(cfg, rank))
-    psd = W.lisa_psd_barack_cutler(N, cfg.dt)
+    psd = psd_of(args, N, cfg.dt)
     plan = emri.Plan(N, cfg.dt, cfg.n_max, K, psd)
     if cfg.index == 5:
         plan.set_anchor(True)            # the paper's convention: initial conditions at the LSO, integrated backwards
@@ -222,7 +253,8 @@ def run_gpu(args, cfg):
         def one_step():
             plan.loglike(p_d, D, logL, status)
 
-    for _ in range(max(args.warmup, 3)):
+    warmup = max(args.warmup, 3)
+    for _ in range(warmup):
         one_step()
     barrier()
     sampler = ClockSampler(torch.cuda.current_device() if "CUDA_VISIBLE_DEVICES" not in os.environ else local)
@@ -234,7 +266,10 @@ def run_gpu(args, cfg):
         one_step()
     e1.record()
     barrier()
-    ms = max_over_ranks(e0.elapsed_time(e1))
+    ms = sharding.max_over_ranks(e0.elapsed_time(e1), world, dev)
+    launches = plan.launch_count()                # kernels of this library enqueued by the LAST call (cuFFT's excluded)
+    if mcmc:
+        launches = 2 * launches
     n_bad = int((status != 0).sum().item())
     if mcmc:        # the chain has moved X and logL; the e2e check below is against the initial ensemble
         logL = plan.loglike(p_d, D, status=status)
@@ -252,7 +287,7 @@ def run_gpu(args, cfg):
     for _ in range(args.steps):
         plan.loglike_host_ptr(P_pin.data_ptr(), K, D_pin.data_ptr(), L_pin.data_ptr(), S_pin.data_ptr())
     torch.cuda.synchronize()
-    e2e_ms = max_over_ranks((time.perf_counter() - t0) * 1e3)
+    e2e_ms = sharding.max_over_ranks((time.perf_counter() - t0) * 1e3, world, dev)
     clocks = sampler.stop()
     assert np.array_equal(L_pin.numpy(), logL_host), "host and device entry points disagree"
 
@@ -264,58 +299,59 @@ def run_gpu(args, cfg):
         for k_, v in plan.timings().items():
             stage[k_] += v / args.steps
     plan.enable_timings(False)
+    paths = plan.synth_report()
 
     if rank == 0:
         peaks, peaks_src = load_measured_peaks()
-        fp64_probe = emri.probe_fp64_peak()
-        fp64_probe3 = emri.probe_fp64_peak3()
+        fp64_probe = probe.fp64_peak()
+        fp64_probe3 = probe.fp64_peak3()
         sm_max = clocks["sm_max_mhz"] or peaks.get("sm_max_mhz", 1965.0)
         sms = torch.cuda.get_device_properties(dev).multi_processor_count
         fp64_nominal = sms * 64 * 2 * sm_max * 1e6 * 1e-12        # 64 FP64 lanes / SM / clk
         n_chunks = (K + CHUNK - 1) // CHUNK
-        fpws = counted_flops_per_walker_sample(cfg.n_max)
-        flops = fpws * K * N
-        achieved = flops / (stage["synth"] * 1e-3) * 1e-12
+        # configs[4] runs the kernel of configs[2] on a ball of walkers around one injection: counted on its own inputs
+        fpws, traffic, src = counted_work(cfg.index, cfg.n_max)
+        achieved = fpws * K * N / (stage["synth"] * 1e-3) * 1e-12 if fpws else None
         roofline = {"bound": "alu", "kernel": "synth_kernel", "achieved": achieved, "peak": fp64_nominal,
-                    "unit": "TFLOP/s", "frac": achieved / fp64_nominal, "traffic": SYNTH_TRAFFIC.get(cfg.index),
+                    "unit": "TFLOP/s", "frac": (achieved / fp64_nominal) if achieved else None, "traffic": traffic,
                     "peak_source": f"derived: {sms} SMs x 64 FP64 lanes x 2 x {sm_max:.0f} MHz (DESIGN.md section 7)",
-                    "peak_dfma_probe": fp64_probe, "frac_of_probe": achieved / fp64_probe,
+                    "peak_dfma_probe": fp64_probe, "frac_of_probe": (achieved / fp64_probe) if achieved else None,
                     "peak_dfma_probe_3_register_operands": fp64_probe3,
                     "launches_per_step": n_chunks, "ms_per_launch": stage["synth"] / n_chunks,
-                    "flops_per_walker_sample": fpws, "flops_source": "counted by ncu (profiles/counts_r1.md)" + (", figure of configs[2] at the same n_max" if mcmc else ""),
-                    "algorithmic_bytes_per_launch": 16.0 * min(K, CHUNK) * N}
-        # the reduction reads the packed spectrum Z[K][N] complex128 once (D and 1/S_n stay in L2)
+                    "flops_per_walker_sample": fpws, "flops_source": src,
+                    "algorithmic_bytes_per_launch": 16.0 * min(K, CHUNK) * N,
+                    "paths": paths}
+        # stages (c)+(d) read the series z[K][N] complex128 and write nothing the caller sees: 16 B per walker*sample is
+        # the algorithmic floor of each of them
         like_gbs = (16.0 * K * N) / (stage["like"] * 1e-3) * 1e-9 if stage["like"] > 0 else None
-        cores = host_cores()
-        walkers = min(cores, K)
-        # the oracle leg runs at N = 1 only (a scaling run does not repeat it on every N)
-        cpu_t, cpu_units = oracle_sample(cfg, P, walkers, 1 if N <= (1 << 20) else 4, True) if world == 1 else (None, 0)
+        cd_gbs = (16.0 * K * N) / ((stage["fft"] + stage["like"]) * 1e-3) * 1e-9
+        if world == 1:        # the oracle leg runs at N = 1 only (a scaling run does not repeat it on every N)
+            leg = OracleLeg(cfg, args)
+            cpu_t, cpu_units = leg.step()
+            cpu = {"value": cpu_units / cpu_t, "unit": UNIT, "cores": leg.walkers, "kind": "oracle",
+                   "sample": leg.describe(cpu_t)}
+        else:
+            cpu = {"value": None, "unit": UNIT, "cores": 0, "kind": "oracle", "sample": "timed at N = 1 only"}
         out = {
-            "metric": METRIC, "value": world * K * N * args.steps / (ms * 1e-3), "unit": UNIT, "n_gpus": world,
-            "steps": args.steps, "warmup": max(args.warmup, 3), "ms_per_step": ms / args.steps,
+            "metric": METRIC, "value": sharding.whole_job_value(K * N, args.steps, ms, world), "unit": UNIT,
+            "n_gpus": world, "steps": args.steps, "warmup": warmup, "ms_per_step": ms / args.steps,
             "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
-            "config": {"workload": f"configs[{cfg.index}]: K={K} walkers/GPU N={N} dt={cfg.dt} n_max={cfg.n_max}, "
-                                   f"data = injection{' + coloured noise' if cfg.noise_seed else ''}",
-                       "l2": f"per-step working set {2 * K * (N + 2) * 8 / 1e6:.0f} MB > 126 MB L2 (no flush needed)",
-                       "parallelism": f"walker-sharded x{world}, no collective"},
+            "config": workload_config(cfg, args),
+            "parallelism": f"walker-sharded x{world}, no collective",
             "likelihoods_per_s": world * K * args.steps / (ms * 1e-3),
             "clocks": clocks,
-            "e2e": {"value": world * K * N * args.steps / (e2e_ms * 1e-3), "unit": UNIT,
+            "e2e": {"value": sharding.whole_job_value(K * N, args.steps, e2e_ms, world), "unit": UNIT,
                     "h2d_bytes_per_step": int(P_pin.numel() * 8 + D_pin.numel() * 16),
                     "d2h_bytes_per_step": int(L_pin.numel() * 8 + S_pin.numel() * 4), "ms_per_step": e2e_ms / args.steps},
-            "gpu_launches": (ORBIT_KERNELS + 2 * n_chunks + 1) * args.steps,
+            "gpu_launches": launches * args.steps,
             "stage_ms": stage,
             "roofline": roofline,
-            "like_kernel": {"bound": "hbm", "kernel": "loglike_kernel", "achieved_gbs": like_gbs,
+            "like_kernel": {"bound": "hbm", "kernel": plan.like_kernel_name(), "achieved_gbs": like_gbs,
                             "peak_gbs": peaks.get("hbm_gbs"), "frac": (like_gbs / peaks["hbm_gbs"]) if like_gbs else None,
                             "peak_source": f"MEASURED_PEAKS.json copy bandwidth ({peaks_src})"},
-            "fft": {"bound": "hbm", "kernel": "cuFFT Z2Z (vendor)", "achieved_gbs": (32.0 * K * N) / (stage["fft"] * 1e-3) * 1e-9
-                    if stage["fft"] > 0 else None, "note": "one read + one write of Z per transform counted"},
-            "cpu_baseline": ({"value": cpu_units / cpu_t, "unit": UNIT, "cores": walkers, "kind": "oracle",
-                              "sample": f"oracle waveform+rfft+logL of {walkers} walkers (one per thread), "
-                                        f"{cpu_units // walkers} of N={N} samples each, {cpu_t:.1f} s"}
-                             if cpu_t else {"value": None, "unit": UNIT, "cores": 0, "kind": "oracle",
-                                            "sample": "timed at N = 1 only"}),
+            "transform_and_likelihood": {"bound": "hbm", "achieved_gbs": cd_gbs, "frac": cd_gbs / peaks["hbm_gbs"],
+                                         "note": "stages (c)+(d) together against one read of z (16 B per walker*sample)"},
+            "cpu_baseline": cpu,
             "walkers_with_status": n_bad,
         }
         print(json.dumps(out))
@@ -329,8 +365,10 @@ def main():
     ap.add_argument("--gpus", type=int, default=1)
     ap.add_argument("--steps", type=int, default=10)
     ap.add_argument("--warmup", type=int, default=3)
-    ap.add_argument("--config", type=int, default=1,
+    ap.add_argument("--config", type=int, default=3,
                     help="index into BASELINE.json:configs (0-4; 4 = stretch-move steps); 5 = the paper's own run shape")
+    ap.add_argument("--psd", default="bc", choices=["bc", "robson"],
+                    help="noise curve: Barack-Cutler (the paper's example) or Robson-Cornish-Liu (its second model)")
     ap.add_argument("--impl", default="b200", choices=["b200", "reference"])
     args = ap.parse_args()
     cfg = W.CONFIGS[args.config]

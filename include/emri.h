@@ -110,8 +110,23 @@ int emri_plan_set_anchor(emri_plan* p, int at_lso);
  * t = 0, bad guard step).  Synchronises the device. */
 int emri_plan_orbit_report(emri_plan* p, int K, int32_t* modes);
 
+/* Diagnostics of stage (b) over the last emri_waveform / emri_waveform_fft / emri_loglike* call (all chunks):
+ * which evaluation path the data selected.  counts (HOST int64 [16]):
+ *   [0] units (one walker x up to 8 tiles of 256 samples) synthesised, [1..8] of them by the local order kept in the
+ *   re-summed harmonic series, [9] units that fell back to the base series in e^2 (local order 8 still significant),
+ *   [10] samples whose amplitude (2 pi M nu)^{2/3} took the cube root instead of the Taylor series about the coarse
+ *   node (|nu/nu_j - 1| > 4e-3), [11] units of walkers with a fatal status (zero-filled), [12..15] 0.
+ * Synchronises the device. */
+int emri_plan_synth_report(emri_plan* p, int64_t counts[16]);
+
+/* Test hook: force the data-selected slow paths of stage (b) for every later call.  flags bit 0: every unit evaluates
+ * the base series in e^2; bit 1: every sample takes the cube-root amplitude.  0 restores the defaults.  Results must
+ * not change beyond rounding (tests/test_gpu_paths.py). */
+int emri_plan_set_synth_debug(emri_plan* p, int flags);
+
 /* Number of walkers processed per internal chunk (bounds the workspace: chunk*N complex128 for z = h_I + i h_II
- * plus the cuFFT work area).  Default min(K_max, 128).  Reallocates; synchronises. */
+ * plus the cuFFT work area).  Default min(K_max, 128).  Reallocates, re-creates the cuFFT plans (full chunk, ragged
+ * last chunk of K_max, single transform) and their shared work area; synchronises. */
 int emri_plan_set_chunk(emri_plan* p, int walkers_per_chunk);
 
 /* Stage (a): coarse orbit of Eq. 1 by fixed-step RK4 (S3).
@@ -176,6 +191,10 @@ int emri_plan_get_timings(emri_plan* p, double ms[4]);
 /* Raw cudaError_t / cufftResult of the last failing CUDA / cuFFT call on this plan (0 if none). */
 int emri_plan_last_cuda_error(const emri_plan* p);
 
+/* Number of kernels of THIS library the last emri_orbit / emri_waveform(_fft) / emri_loglike* call enqueued (the status
+ * copy of emri_orbit / emri_waveform and cuFFT's own kernels are not counted).  bench.py reports it as `gpu_launches`. */
+int emri_plan_last_launch_count(const emri_plan* p);
+
 /* Bytes of device memory the plan currently owns. */
 int64_t emri_plan_workspace_bytes(const emri_plan* p);
 
@@ -190,20 +209,12 @@ int64_t emri_plan_workspace_bytes(const emri_plan* p);
  *   emri_loglike first); lo, hi: DEV [17] box prior (a column with lo == hi is held fixed and
  *   does not count in P_free); accepted: DEV int32 [K] or NULL, set to 1/0 for the active half;
  *   log_buf: DEV [K/2][EMRI_NPAR+4] doubles or NULL: per active walker {proposal[17], z, ln u',
- *   logL(Y), partner} for the teacher-forced parity protocol. K must be even, K/2 <= K_max. */
+ *   logL(Y), partner} for the teacher-forced parity protocol. K must be even, K/2 <= K_max (the plan's proposal
+ *   scratch holds K_max rows). */
 int emri_stretch_step(emri_plan* p, double* X, double* logL, int K, const double* data_fft,
                       const double* lo, const double* hi, double a_stretch, uint64_t seed,
                       int64_t step, int half, int32_t* accepted, double* log_buf,
                       void* cuda_stream);
-
-/* ---- measurement helpers (bench.py): peak probes on the current device.
- * emri_probe_fp64_peak: runs a dependent-chain-free DFMA kernel and returns TFLOP/s (FMA = 2).
- * emri_probe_hbm_read: streams `bytes` of device memory once and returns GB/s. */
-int emri_probe_fp64_peak(double* tflops, void* cuda_stream);
-/* The same with three fresh vector-register operands per DFMA (no constant, uniform-register or reused operand):
- * what register-bound FP64 code can reach (on B200 2/3 of the figure above). */
-int emri_probe_fp64_peak3(double* tflops, void* cuda_stream);
-int emri_probe_hbm_read(int64_t bytes, double* gbs, void* cuda_stream);
 
 #ifdef __cplusplus
 }

@@ -232,8 +232,6 @@ void rk4_increment(const Walker& w, const real y[5], real h, int pn_mask, real d
 // nu there is nu_LSO(e_LSO) (column nu0 is ignored), and the same fixed-step RK4 runs backwards, node Nc -> node -1.
 // The interval increments are stored in forward time (inc[j] = y_{j+1} - y_j); one forward step gives the guard node
 // Nc+1.  Nothing plunges inside the window by construction; a bad state (e leaving [0,1)) sets ST_STATE.
-int g_anchor_end = 0;
-
 Orbit integrate_orbit_from_lso(const Walker& w, int64_t N, real dt, int S, int pn_mask) {
   Orbit o;
   o.G = 1;
@@ -297,8 +295,9 @@ Orbit integrate_orbit_from_lso(const Walker& w, int64_t N, real dt, int S, int p
   return o;
 }
 
-Orbit integrate_orbit(const Walker& w, int64_t N, real dt, int S, int pn_mask) {
-  if (g_anchor_end) return integrate_orbit_from_lso(w, N, dt, S, pn_mask);
+// anchor: 0 = the parameter row is the state at the first sample (forward), 1 = at plunge, at the last coarse node (D12)
+Orbit integrate_orbit(const Walker& w, int64_t N, real dt, int S, int pn_mask, int anchor) {
+  if (anchor) return integrate_orbit_from_lso(w, N, dt, S, pn_mask);
   Orbit o;
   o.G = 1;
   o.Nc = (N + S - 1) / S;
@@ -548,8 +547,8 @@ void fft_c(std::vector<real>& re, std::vector<real>& im) {
 // =================================================================== C ABI (double I/O)
 extern "C" {
 
-// 0 (default): the parameter row is the state at the first sample; 1: at plunge, at the last coarse node (reading D12)
-void emri_o_set_anchor(int at_lso) { g_anchor_end = at_lso ? 1 : 0; }
+// `anchor` argument of the orbit / waveform entry points: 0 = the parameter row is the state at the first sample;
+// 1 = at plunge, at the last coarse node (reading D12).  An explicit argument: no process-wide state.
 
 int emri_o_real_bits(void) { return (int)std::numeric_limits<real>::digits; }
 
@@ -593,10 +592,10 @@ void emri_o_rhs(const double* params, const double* y, int pn_mask, double* f) {
 // coarse orbit.  Outputs (each may be NULL): val, slope, inc are [5][Nn] row-major with
 // Nn = ceil(N/S) + 3, node j at column j+1; info = {Nn, jpl (node index j, or Nn if none), status}
 int emri_o_orbit(const double* params, int64_t N, double dt, int S, int pn_mask, double H0, double Om,
-                 double* val, double* slope, double* inc, int64_t* info) {
+                 double* val, double* slope, double* inc, int64_t* info, int anchor) {
   Cosmo c{(real)H0, (real)Om};
   Walker w = make_walker(params, c);
-  Orbit o = integrate_orbit(w, N, (real)dt, S, pn_mask);
+  Orbit o = integrate_orbit(w, N, (real)dt, S, pn_mask, anchor);
   for (int q = 0; q < 5; ++q)
     for (int64_t m = 0; m < o.Nn; ++m) {
       if (val) val[q * o.Nn + m] = (double)o.val[q][m];
@@ -610,10 +609,10 @@ int emri_o_orbit(const double* params, int64_t N, double dt, int S, int pn_mask,
 // orbit interpolated at sample indices idx[0..n_idx): out[5][n_idx] (angles in cycles, unwrapped
 // relative to the wrapped node value)
 int emri_o_orbit_at(const double* params, int64_t N, double dt, int S, int pn_mask, double H0, double Om,
-                    const int64_t* idx, int64_t n_idx, double* out) {
+                    const int64_t* idx, int64_t n_idx, double* out, int anchor) {
   Cosmo c{(real)H0, (real)Om};
   Walker w = make_walker(params, c);
-  Orbit o = integrate_orbit(w, N, (real)dt, S, pn_mask);
+  Orbit o = integrate_orbit(w, N, (real)dt, S, pn_mask, anchor);
   for (int64_t m = 0; m < n_idx; ++m) {
     int64_t j; real s;
     split_time(idx[m], S, w.dT / o.Delta, &j, &s);
@@ -646,10 +645,10 @@ void emri_o_antenna(double cthd, double phid, double psi, double* F) {
 // waveform at selected sample indices (idx == NULL: all samples 0..N-1, n_idx = N).
 // hI, hII: [n_idx]; Apl, Acr (may be NULL): polarisation amplitudes A+, Ax.  Returns status bits.
 int emri_o_waveform(const double* params, int64_t N, double dt, int n_max, int S, double H0, double Om,
-                    const int64_t* idx, int64_t n_idx, double* hI, double* hII, double* Apl, double* Acr) {
+                    const int64_t* idx, int64_t n_idx, double* hI, double* hII, double* Apl, double* Acr, int anchor) {
   Cosmo c{(real)H0, (real)Om};
   Walker w = make_walker(params, c);
-  Orbit o = integrate_orbit(w, N, (real)dt, S, 3);
+  Orbit o = integrate_orbit(w, N, (real)dt, S, 3, anchor);
   o.status = finish_status(w, o);
   for (int64_t m = 0; m < n_idx; ++m) {
     int64_t i = idx ? idx[m] : m;
@@ -664,11 +663,11 @@ int emri_o_waveform(const double* params, int64_t N, double dt, int n_max, int S
 // batch of K walkers, all samples, OpenMP over walkers only.  h: [K][2][N] (channel I then II),
 // status: [K]
 int emri_o_waveform_batch(const double* params, int K, int64_t N, double dt, int n_max, int S, double H0,
-                          double Om, double* h, int32_t* status) {
+                          double Om, double* h, int32_t* status, int anchor) {
 #pragma omp parallel for schedule(dynamic, 1)
   for (int k = 0; k < K; ++k)
     status[k] = emri_o_waveform(params + (size_t)k * NPAR, N, dt, n_max, S, H0, Om, nullptr, N,
-                                h + (size_t)k * 2 * N, h + (size_t)k * 2 * N + N, nullptr, nullptr);
+                                h + (size_t)k * 2 * N, h + (size_t)k * 2 * N + N, nullptr, nullptr, anchor);
   return 0;
 }
 
@@ -758,14 +757,14 @@ double emri_o_inner(const double* A, const double* B, const double* psd, int64_t
 // status-1/4/8 walkers get -inf.  spectra (may be NULL): [K][2][N/2+1] complex out.
 int emri_o_loglike_batch(const double* params, int K, int64_t N, double dt, int n_max, int S, double H0,
                          double Om, const double* D, const double* psd, double* logL, int32_t* status,
-                         double* spectra) {
+                         double* spectra, int anchor) {
   const int64_t Nf = N / 2 + 1;
   int rc = 0;
 #pragma omp parallel for schedule(dynamic, 1)
   for (int k = 0; k < K; ++k) {
     std::vector<double> h(2 * (size_t)N), H(4 * (size_t)Nf);
     int st = emri_o_waveform(params + (size_t)k * NPAR, N, dt, n_max, S, H0, Om, nullptr, N, h.data(),
-                             h.data() + N, nullptr, nullptr);
+                             h.data() + N, nullptr, nullptr, anchor);
     if (emri_o_rfft(h.data(), N, H.data()) || emri_o_rfft(h.data() + N, N, H.data() + 2 * Nf)) {
 #pragma omp atomic write
       rc = -1;

@@ -1,6 +1,8 @@
 """ctypes binding of the CPU oracle (oracle/emri_oracle.cpp) -- TEST INFRASTRUCTURE.
 
-`Oracle()` loads the double build, `Oracle(long_double=True)` the 80-bit diagnostic build.
+`Oracle()` loads the double build, `Oracle(long_double=True)` the 80-bit diagnostic build;
+`Oracle(anchor=True)` reads parameter rows as the state at plunge (reading D12) -- a property of the
+instance, passed to the library as an explicit argument of every orbit / waveform call (no process-wide state).
 Argument marshalling only; every number comes out of emri_oracle.cpp.
 """
 import ctypes as C
@@ -27,7 +29,8 @@ def _f64(a):
 
 
 class Oracle:
-    def __init__(self, long_double=False):
+    def __init__(self, long_double=False, anchor=False):
+        self.anchor = 1 if anchor else 0
         lib, lib_ld = build_oracle.build()
         self.lib = L = C.CDLL(lib_ld if long_double else lib)
         L.emri_o_real_bits.restype = C.c_int
@@ -44,18 +47,18 @@ class Oracle:
         L.emri_o_walker_scalars.argtypes = [_dp, C.c_double, C.c_double, _dp]
         L.emri_o_rhs.argtypes = [_dp, _dp, C.c_int, _dp]
         L.emri_o_orbit.argtypes = [_dp, C.c_int64, C.c_double, C.c_int, C.c_int, C.c_double, C.c_double,
-                                   _dp, _dp, _dp, _ip]
+                                   _dp, _dp, _dp, _ip, C.c_int]
         L.emri_o_orbit_at.argtypes = [_dp, C.c_int64, C.c_double, C.c_int, C.c_int, C.c_double, C.c_double,
-                                      _ip, C.c_int64, _dp]
+                                      _ip, C.c_int64, _dp, C.c_int]
         L.emri_o_hermite1.restype = C.c_double
         L.emri_o_hermite1.argtypes = [C.c_double] * 6
         L.emri_o_geometry.argtypes = [_dp, C.c_double, C.c_double, _dp]
         L.emri_o_antenna.argtypes = [C.c_double, C.c_double, C.c_double, _dp]
         L.emri_o_waveform.restype = C.c_int
         L.emri_o_waveform.argtypes = [_dp, C.c_int64, C.c_double, C.c_int, C.c_int, C.c_double, C.c_double,
-                                      _ip, C.c_int64, _dp, _dp, _dp, _dp]
+                                      _ip, C.c_int64, _dp, _dp, _dp, _dp, C.c_int]
         L.emri_o_waveform_batch.argtypes = [_dp, C.c_int, C.c_int64, C.c_double, C.c_int, C.c_int,
-                                            C.c_double, C.c_double, _dp, _i32p]
+                                            C.c_double, C.c_double, _dp, _i32p, C.c_int]
         L.emri_o_rfft.restype = C.c_int
         L.emri_o_rfft.argtypes = [_dp, C.c_int64, _dp]
         L.emri_o_dft_naive.argtypes = [_dp, C.c_int64, _dp]
@@ -67,11 +70,12 @@ class Oracle:
         L.emri_o_inner.argtypes = [_dp, _dp, _dp, C.c_int64, C.c_double]
         L.emri_o_loglike_batch.restype = C.c_int
         L.emri_o_loglike_batch.argtypes = [_dp, C.c_int, C.c_int64, C.c_double, C.c_int, C.c_int, C.c_double,
-                                           C.c_double, _dp, _dp, _dp, _i32p, _dp]
+                                           C.c_double, _dp, _dp, _dp, _i32p, _dp, C.c_int]
 
     def set_anchor(self, at_lso):
-        """False (default): the parameter row is the state at t = 0; True: at plunge, at the last coarse node (D12)"""
-        self.lib.emri_o_set_anchor(1 if at_lso else 0)
+        """False (default): the parameter row is the state at t = 0; True: at plunge, at the last coarse node (D12).
+        Affects this instance only."""
+        self.anchor = 1 if at_lso else 0
 
     # ---- scalars
     def real_bits(self):
@@ -123,14 +127,14 @@ class Oracle:
         val, slope, inc = (np.zeros((5, Nn)) for _ in range(3))
         info = np.zeros(3, dtype=np.int64)
         self.lib.emri_o_orbit(_d(p), N, dt, S, pn_mask, H0, Om, _d(val), _d(slope), _d(inc),
-                              info.ctypes.data_as(_ip))
+                              info.ctypes.data_as(_ip), self.anchor)
         return dict(val=val, slope=slope, inc=inc, Nn=int(info[0]), jpl=int(info[1]), status=int(info[2]))
 
     def orbit_at(self, params, N, dt, idx, S=256, pn_mask=3, H0=H0_DEFAULT, Om=OM_DEFAULT):
         p = _f64(params)
         ii = np.ascontiguousarray(idx, dtype=np.int64)
         out = np.zeros((5, ii.size))
-        self.lib.emri_o_orbit_at(_d(p), N, dt, S, pn_mask, H0, Om, ii.ctypes.data_as(_ip), ii.size, _d(out))
+        self.lib.emri_o_orbit_at(_d(p), N, dt, S, pn_mask, H0, Om, ii.ctypes.data_as(_ip), ii.size, _d(out), self.anchor)
         return out
 
     def hermite1(self, y0, inc, m0, m1, Delta, s):
@@ -160,7 +164,7 @@ class Oracle:
         hI, hII = np.zeros(n), np.zeros(n)
         Ap, Ax = (np.zeros(n), np.zeros(n)) if amplitudes else (None, None)
         st = self.lib.emri_o_waveform(_d(p), N, dt, n_max, S, H0, Om, ptr, n, _d(hI), _d(hII),
-                                      _d(Ap) if amplitudes else None, _d(Ax) if amplitudes else None)
+                                      _d(Ap) if amplitudes else None, _d(Ax) if amplitudes else None, self.anchor)
         return (hI, hII, st, Ap, Ax) if amplitudes else (hI, hII, st)
 
     def waveform_batch(self, params, N, dt, n_max, S=256, H0=H0_DEFAULT, Om=OM_DEFAULT):
@@ -169,7 +173,7 @@ class Oracle:
         K = p.shape[0]
         h = np.zeros((K, 2, N))
         st = np.zeros(K, dtype=np.int32)
-        self.lib.emri_o_waveform_batch(_d(p), K, N, dt, n_max, S, H0, Om, _d(h), st.ctypes.data_as(_i32p))
+        self.lib.emri_o_waveform_batch(_d(p), K, N, dt, n_max, S, H0, Om, _d(h), st.ctypes.data_as(_i32p), self.anchor)
         return h, st
 
     # ---- transform and likelihood
@@ -220,7 +224,7 @@ class Oracle:
         sp = np.zeros((K, 2, N // 2 + 1), dtype=np.complex128) if spectra else None
         rc = self.lib.emri_o_loglike_batch(_d(p), K, N, dt, n_max, S, H0, Om, _d(Dc.view(np.float64)), _d(s),
                                            _d(logL), st.ctypes.data_as(_i32p),
-                                           _d(sp.view(np.float64)) if spectra else None)
+                                           _d(sp.view(np.float64)) if spectra else None, self.anchor)
         if rc:
             raise ValueError("oracle loglike_batch failed (N must be a power of two)")
         return (logL, st, sp) if spectra else (logL, st)

@@ -30,7 +30,6 @@
 #include "synth.cuh"
 #include "loglike.cuh"
 #include "stretch.cuh"
-#include "probe.cuh"
 
 // =================================================================== host side
 struct emri_plan {
@@ -52,6 +51,9 @@ struct emri_plan {
   int32_t* d_status = nullptr;
   // multiple-shooting orbit (orbit.cuh): segment records, per-walker mode / tail start / post-plunge row
   int orbit_mode = 1, anchor_end = 0, seg_L = 0, seg_P = 0, unit_tiles_override = 0;
+  int synth_debug = 0;                       // emri_plan_set_synth_debug
+  int launches = 0;                          // kernels of this library enqueued by the last hot call
+  unsigned long long* d_counts = nullptr;    // [SYN_COUNTS] path counters of stage (b), zeroed at the start of every call
   double* d_seg = nullptr;
   double* d_plrow = nullptr;
   int32_t* d_mode = nullptr;
@@ -163,17 +165,34 @@ int alloc_workspace(emri_plan* p) {
   const int64_t n_steps = p->Nc + 1;
   int lg = (int)std::floor(0.5 * std::log2(0.5 * (double)n_steps) + 0.5);
   if (lg < 2) lg = 2;
+  // orbit_correct_kernel keeps 96 B per segment in shared memory: at most 2048 segments (192 KB)
+  while (((n_steps + (1 << lg) - 1) >> lg) > 2048) ++lg;
   p->seg_L = 1 << lg;
   p->seg_P = (int)((n_steps + p->seg_L - 1) / p->seg_L);
+  if (cudaFuncSetAttribute(orbit_correct_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                           std::max(48 * 1024, p->seg_P * 12 * (int)sizeof(double))) != cudaSuccess) {
+    p->last_err = (int)cudaGetLastError();
+    return EMRI_ECUDA;
+  }
   if ((rc = dev_alloc(p, &p->d_seg, (size_t)p->K_max * p->seg_P * SEG_STRIDE))) return rc;
   return EMRI_OK;
 }
 
+int get_fft(emri_plan* p, int batch, cufftHandle* out);
+
+// (Re)allocates the chunk buffer and creates, up front, every cuFFT plan the hot calls of a full ensemble need: a full
+// chunk, the ragged last chunk of K_max walkers, and the single transform of emri_data_fft.  The work area is sized by
+// the largest of them (the full chunk), so a later call with another ragged K only builds its plan object on first use
+// and never allocates or synchronises (include/emri.h: "only ENQUEUES").
 int alloc_chunk(emri_plan* p) {
   int rc;
   if ((rc = dev_alloc(p, &p->d_hbuf, (size_t)2 * p->chunk * p->N))) return rc;      // z = h_I + i h_II, [chunk][N] complex
   for (auto& kv : p->fft) cufftDestroy(kv.second);
   p->fft.clear();
+  cufftHandle h;
+  if ((rc = get_fft(p, p->chunk, &h))) return rc;
+  if (p->K_max % p->chunk) { if ((rc = get_fft(p, p->K_max % p->chunk, &h))) return rc; }
+  if ((rc = get_fft(p, 1, &h))) return rc;
   return EMRI_OK;
 }
 
@@ -191,7 +210,8 @@ int get_fft(emri_plan* p, int batch, cufftHandle* out) {
                                       (long long)batch, &ws);
   if (r != CUFFT_SUCCESS) { p->last_err = (int)r; cufftDestroy(h); return EMRI_ECUFFT; }
   if (ws > p->fftwork_bytes) {
-    // grow the shared work area; every cached plan is re-pointed at it
+    // grow the shared work area; every cached plan is re-pointed at it.  Reached from alloc_chunk (plan creation,
+    // emri_plan_set_chunk) only: the full chunk is planned first and no smaller batch needs more
     cudaError_t e = cudaDeviceSynchronize();
     if (e != cudaSuccess) { p->last_err = (int)e; cufftDestroy(h); return EMRI_ECUDA; }
     if (p->d_fftwork) { cudaFree(p->d_fftwork); p->bytes -= (int64_t)p->fftwork_bytes; p->d_fftwork = nullptr; }
@@ -220,6 +240,8 @@ void mark(emri_plan* p, cudaStream_t s) {
 }
 
 int run_orbit(emri_plan* p, const double* params, int K, cudaStream_t s) {
+  p->launches = 0;
+  CK(cudaMemsetAsync(p->d_counts, 0, SYN_COUNTS * sizeof(unsigned long long), s));
   OrbitArgs a;
   a.params = params; a.K = K; a.N = p->N; a.dt = p->dt; a.S = p->S; a.Nc = p->Nc; a.Nn = p->Nn; a.n_max = p->n_max;
   a.tH = kMpcMetre / (p->H0 * 1000.0); a.Om = p->Om; a.anchor_end = p->anchor_end;
@@ -229,6 +251,7 @@ int run_orbit(emri_plan* p, const double* params, int K, cudaStream_t s) {
     // reference schedule: the whole recursion in one thread per walker
     orbit_kernel<<<(K + 31) / 32, 32, 0, s>>>(a);
     orbit_aux_kernel<<<aux_grid, 128, 0, s>>>(a);
+    p->launches += 2;
     CK(cudaGetLastError());
     return EMRI_OK;
   }
@@ -238,6 +261,7 @@ int run_orbit(emri_plan* p, const double* params, int K, cudaStream_t s) {
   sa.round = 0; sa.last_round = 0;
   orbit_init_kernel<<<(K + 31) / 32, 32, 0, s>>>(sa);
   DBG("orbit_init_kernel");
+  p->launches += 1 + 2 * 3 + 3;
   const int n_rounds = 3;
   for (int r = 0; r < n_rounds; ++r) {
     sa.round = r; sa.last_round = (r == n_rounds - 1);
@@ -259,6 +283,9 @@ int run_synth(emri_plan* p, int k0, int K, double* outI, double* outII, int64_t 
   SynthArgs a;
   a.wc = p->d_wc; a.nodes = p->d_nodes; a.nodeaux = p->d_nodeaux; a.jpl = p->d_jpl; a.status = p->d_status;
   a.base = p->d_base; a.tol = 1e-16;
+  a.cbrt_thr = (p->synth_debug & 2) ? -1.0 : 4e-3;
+  a.force_base = (p->synth_debug & 1) ? 1 : 0;
+  a.counts = p->d_counts;
   a.k0 = k0; a.K = K; a.N = p->N; a.dt = p->dt; a.S = p->S; a.logS = p->logS; a.Nn = p->Nn; a.n_max = p->n_max;
   a.outI = outI; a.outII = outII; a.pitch = pitch; a.outZ = reinterpret_cast<double2*>(outZ);
   a.tiles_per_walker = (p->N + TILE - 1) / TILE;
@@ -271,6 +298,7 @@ int run_synth(emri_plan* p, int k0, int K, double* outI, double* outII, int64_t 
   int64_t total = (int64_t)K * a.units_per_walker;
   int grid = (int)std::min<int64_t>(total, p->synth_grid);
   synth_kernel<<<grid, SYNTH_BLOCK, p->synth_smem, s>>>(a);
+  p->launches += 1;
   CK(cudaGetLastError());
   return EMRI_OK;
 }
@@ -296,6 +324,7 @@ int run_like(emri_plan* p, int k0, int K, const double* Z, const double* data_ff
   dim3 grid((unsigned)p->n_part, (unsigned)((K + LL_GROUP - 1) / LL_GROUP));
   if (fcoef) loglike_kernel<true><<<grid, LL_THREADS, 0, s>>>(a);
   else loglike_kernel<false><<<grid, LL_THREADS, 0, s>>>(a);
+  p->launches += 1;
   CK(cudaGetLastError());
   return EMRI_OK;
 }
@@ -353,7 +382,9 @@ int emri_plan_create(emri_plan** out, int64_t N, double dt, int n_max, int K_max
   if ((rc = dev_alloc(p, &p->d_params, (size_t)K_max * EMRI_NPAR))) return fail(rc);
   if ((rc = dev_alloc(p, &p->d_data, (size_t)4 * p->Nf))) return fail(rc);
   if ((rc = dev_alloc(p, &p->d_logL, (size_t)K_max))) return fail(rc);
-  const size_t H = (size_t)(K_max + 1) / 2 + 1;
+  // scratch of emri_stretch_step: K/2 <= K_max proposal rows
+  const size_t H = (size_t)K_max;
+  if ((rc = dev_alloc(p, &p->d_counts, (size_t)SYN_COUNTS))) return fail(rc);
   if ((rc = dev_alloc(p, &p->d_Y, H * EMRI_NPAR))) return fail(rc);
   if ((rc = dev_alloc(p, &p->d_z, H))) return fail(rc);
   if ((rc = dev_alloc(p, &p->d_lnu, H))) return fail(rc);
@@ -396,7 +427,7 @@ int emri_plan_destroy(emri_plan* p) {
   if (p->s_copy) cudaStreamDestroy(p->s_copy);
   void* ptrs[] = {p->d_w, p->d_wc, p->d_nodes, p->d_hbuf, p->d_partial, p->d_base, p->d_nodeaux, p->d_jpl, p->d_status,
                   p->d_params, p->d_data, p->d_logL, p->d_Y, p->d_z, p->d_lnu, p->d_logLY, p->d_inbox,
-                  p->d_partner, p->d_fftwork, p->d_seg, p->d_plrow, p->d_mode, p->d_pclamp};
+                  p->d_partner, p->d_fftwork, p->d_seg, p->d_plrow, p->d_mode, p->d_pclamp, p->d_counts};
   for (void* q : ptrs) if (q) cudaFree(q);
   delete p;
   return EMRI_OK;
@@ -436,6 +467,21 @@ int emri_plan_orbit_report(emri_plan* p, int K, int32_t* modes) {
   if (!p || !modes || K < 1 || K > p->K_max) return EMRI_EINVAL;
   CK(cudaDeviceSynchronize());
   CK(cudaMemcpy(modes, p->d_mode, (size_t)K * sizeof(int32_t), cudaMemcpyDeviceToHost));
+  return EMRI_OK;
+}
+
+int emri_plan_synth_report(emri_plan* p, int64_t counts[16]) {
+  if (!p || !counts) return EMRI_EINVAL;
+  CK(cudaDeviceSynchronize());
+  unsigned long long h[SYN_COUNTS];
+  CK(cudaMemcpy(h, p->d_counts, sizeof(h), cudaMemcpyDeviceToHost));
+  for (int i = 0; i < 16; ++i) counts[i] = i < SYN_COUNTS ? (int64_t)h[i] : 0;
+  return EMRI_OK;
+}
+
+int emri_plan_set_synth_debug(emri_plan* p, int flags) {
+  if (!p || flags < 0 || flags > 3) return EMRI_EINVAL;
+  p->synth_debug = flags;
   return EMRI_OK;
 }
 
@@ -552,6 +598,7 @@ static int loglike_impl(emri_plan* p, const double* params, int K, const double*
   p->n_chunks_last = nch;
   const double scale = 2.0 * p->dt / (double)p->N;
   loglike_final_kernel<<<(K + 3) / 4, 128, 0, s>>>(p->d_partial, p->n_part, K, scale, p->d_status, logL, status);
+  p->launches += 1;
   CK(cudaGetLastError());
   return EMRI_OK;
 }
@@ -618,6 +665,7 @@ int emri_plan_get_timings(emri_plan* p, double ms[4]) {
 }
 
 int emri_plan_last_cuda_error(const emri_plan* p) { return p ? p->last_err : 0; }
+int emri_plan_last_launch_count(const emri_plan* p) { return p ? p->launches : 0; }
 int64_t emri_plan_workspace_bytes(const emri_plan* p) { return p ? p->bytes : 0; }
 
 int emri_stretch_step(emri_plan* p, double* X, double* logL, int K, const double* data_fft, const double* lo,
@@ -638,96 +686,6 @@ int emri_stretch_step(emri_plan* p, double* X, double* logL, int K, const double
   if (rc) return rc;
   stretch_accept_kernel<<<(H + 127) / 128, 128, 0, s>>>(a);
   CK(cudaGetLastError());
-  return EMRI_OK;
-}
-
-int emri_probe_fp64_peak(double* tflops, void* stream) {
-  if (!tflops) return EMRI_EINVAL;
-  cudaStream_t s = (cudaStream_t)stream;
-  int dev = 0, sms = 0;
-  if (cudaGetDevice(&dev) != cudaSuccess || cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev) != cudaSuccess)
-    return EMRI_ECUDA;
-  double* d = nullptr;
-  if (cudaMalloc(&d, 8) != cudaSuccess) return EMRI_ENOMEM;
-  const int iters = 4096, blocks = sms * 8;
-  cudaEvent_t e0, e1;
-  cudaEventCreate(&e0); cudaEventCreate(&e1);
-  fp64_probe_kernel<<<blocks, 256, 0, s>>>(d, 64, 1.0);      // warm-up
-  double best = 0.0;
-  for (int rep = 0; rep < 3; ++rep) {
-    cudaEventRecord(e0, s);
-    fp64_probe_kernel<<<blocks, 256, 0, s>>>(d, iters, 1.0);
-    cudaEventRecord(e1, s);
-    if (cudaEventSynchronize(e1) != cudaSuccess) { cudaFree(d); return EMRI_ECUDA; }
-    float ms = 0.f;
-    cudaEventElapsedTime(&ms, e0, e1);
-    double fl = 2.0 * 64.0 * (double)iters * 256.0 * (double)blocks;
-    best = std::max(best, fl / (ms * 1e-3) * 1e-12);
-  }
-  cudaEventDestroy(e0); cudaEventDestroy(e1);
-  cudaFree(d);
-  *tflops = best;
-  return EMRI_OK;
-}
-
-int emri_probe_fp64_peak3(double* tflops, void* stream) {
-  if (!tflops) return EMRI_EINVAL;
-  cudaStream_t s = (cudaStream_t)stream;
-  int dev = 0, sms = 0;
-  if (cudaGetDevice(&dev) != cudaSuccess || cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev) != cudaSuccess)
-    return EMRI_ECUDA;
-  double* d = nullptr;
-  if (cudaMalloc(&d, 512 * sizeof(double)) != cudaSuccess) return EMRI_ENOMEM;
-  cudaMemsetAsync(d, 0, 512 * sizeof(double), s);
-  const int iters = 4096, blocks = sms * 8;
-  cudaEvent_t e0, e1;
-  cudaEventCreate(&e0); cudaEventCreate(&e1);
-  fp64_probe3_kernel<<<blocks, 256, 0, s>>>(d + 300, 64, d);      // warm-up
-  double best = 0.0;
-  for (int rep = 0; rep < 3; ++rep) {
-    cudaEventRecord(e0, s);
-    fp64_probe3_kernel<<<blocks, 256, 0, s>>>(d + 300, iters, d);
-    cudaEventRecord(e1, s);
-    if (cudaEventSynchronize(e1) != cudaSuccess) { cudaFree(d); return EMRI_ECUDA; }
-    float ms = 0.f;
-    cudaEventElapsedTime(&ms, e0, e1);
-    const double fl = 2.0 * 6.0 * (double)iters * 256.0 * (double)blocks;
-    best = std::max(best, fl / (ms * 1e-3) * 1e-12);
-  }
-  cudaEventDestroy(e0); cudaEventDestroy(e1);
-  cudaFree(d);
-  *tflops = best;
-  return EMRI_OK;
-}
-
-int emri_probe_hbm_read(int64_t bytes, double* gbs, void* stream) {
-  if (!gbs || bytes < (1 << 20)) return EMRI_EINVAL;
-  cudaStream_t s = (cudaStream_t)stream;
-  int dev = 0, sms = 0;
-  if (cudaGetDevice(&dev) != cudaSuccess || cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev) != cudaSuccess)
-    return EMRI_ECUDA;
-  double2* buf = nullptr;
-  double* d = nullptr;
-  const int64_t n = bytes / 16;
-  if (cudaMalloc(&buf, (size_t)n * 16) != cudaSuccess) { cudaGetLastError(); return EMRI_ENOMEM; }
-  if (cudaMalloc(&d, 8) != cudaSuccess) { cudaFree(buf); return EMRI_ENOMEM; }
-  cudaMemsetAsync(buf, 0, (size_t)n * 16, s);
-  cudaEvent_t e0, e1;
-  cudaEventCreate(&e0); cudaEventCreate(&e1);
-  hbm_probe_kernel<<<sms * 8, 256, 0, s>>>(buf, n, d);
-  double best = 0.0;
-  for (int rep = 0; rep < 3; ++rep) {
-    cudaEventRecord(e0, s);
-    hbm_probe_kernel<<<sms * 8, 256, 0, s>>>(buf, n, d);
-    cudaEventRecord(e1, s);
-    if (cudaEventSynchronize(e1) != cudaSuccess) { cudaFree(buf); cudaFree(d); return EMRI_ECUDA; }
-    float ms = 0.f;
-    cudaEventElapsedTime(&ms, e0, e1);
-    best = std::max(best, (double)n * 16.0 / (ms * 1e-3) * 1e-9);
-  }
-  cudaEventDestroy(e0); cudaEventDestroy(e1);
-  cudaFree(buf); cudaFree(d);
-  *gbs = best;
   return EMRI_OK;
 }
 

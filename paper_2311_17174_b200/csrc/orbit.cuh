@@ -244,8 +244,11 @@ DEVINL bool walker_prologue(const OrbitArgs& a, const double* __restrict__ p, do
     wc[WC_LN1] = A1x * nx + A1y * ny + A1z * nz;
     wc[WC_LN2] = A2x * nx + A2y * ny;
     wc[WC_CL] = cl; wc[WC_SN] = Sn;
+    // lambda = 0 exactly: L^ = S^, beta's atan2 arguments vanish identically (reading R16: beta = 0).  Its numerator
+    // cl L^.n^ - S^.n^ would be left at rounding noise by the two different summation orders, so it is made exactly 0
+    if (sl == 0.0) { wc[WC_CL] = 0.0; wc[WC_SN] = 0.0; }
     wc[WC_B1] = sS * (sphK * cphS - cphK * sphS) * sl;               // sin(thS) sin(phK - phS) sin(lam)
-    wc[WC_B2] = (Sn * cK - cS) / sK * sl;
+    wc[WC_B2] = (sS * cK * (cphS * cphK + sphS * sphK) - cS * sK) * sl;   // (Sn cK - cS)/sK sl without the division by sin(thK)
     wc[WC_A0X] = A0x; wc[WC_A0Y] = A0y; wc[WC_A0Z] = A0z;
     wc[WC_A1X] = A1x; wc[WC_A1Y] = A1y; wc[WC_A1Z] = A1z;
     wc[WC_A2X] = A2x; wc[WC_A2Y] = A2y;

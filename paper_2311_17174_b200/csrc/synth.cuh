@@ -55,7 +55,15 @@ struct SynthArgs {
   int unit_tiles;
   int64_t tiles_per_walker, units_per_walker;
   double tol;              // relative truncation of the harmonic series
+  double cbrt_thr;         // |nu/nu_j - 1| above which the amplitude takes the cube root (4e-3; < 0 forces the branch)
+  int force_base;          // diagnostics: every unit takes the base-series fallback
+  unsigned long long* counts;   // [SYN_COUNTS] path counters of the call (emri_plan_synth_report)
 };
+
+// counters: [0] units, [1..8] units by local order Mu, [9] units on the base-series fallback, [10] samples whose
+// amplitude took the cube-root branch, [11] units of walkers with a fatal status (zero-filled)
+constexpr int SYN_COUNTS = 16;
+enum { SYC_UNITS = 0, SYC_BASE = 9, SYC_CBRT = 10, SYC_SKIP = 11 };
 
 constexpr int SC_TAB = 1024;              // entries of the shared cos/sin table (one per 1/1024 cycle)
 
@@ -92,7 +100,8 @@ struct SampleOut {
 // phibar = 2 pi t_i / T_yr.  fin[0..5] (stride fs) receive a_I, b_I, c_I, a_II, b_II, c_II.
 DEVINL void sample_setup(const double* __restrict__ w, const double2* __restrict__ sct, const double* __restrict__ nodes,
                          const double2* __restrict__ aux, int64_t i, int S, int logS, double invS, double Delta, int32_t jpl, double cpb, double spb,
-                         double w0, SampleOut& o, double* __restrict__ fin, int fs) {
+                         double w0, double cbrt_thr, unsigned long long* __restrict__ counts, SampleOut& o,
+                         double* __restrict__ fin, int fs) {
   // source-time split (reading D4)
   int64_t j = i >> logS;
   double s = (double)(i & (S - 1)) * invS - w[WC_SIGMA];
@@ -119,12 +128,13 @@ DEVINL void sample_setup(const double* __restrict__ w, const double2* __restrict
   double A;
   {
     const double d = dnu * ax.y;
-    if (fabs(d) <= 4e-3) {
+    if (fabs(d) <= cbrt_thr) {
       const double p = fma(d, fma(d, fma(d, fma(d, 14.0 / 729.0, -7.0 / 243.0), 4.0 / 81.0), -1.0 / 9.0), 2.0 / 3.0);
       A = fma(ax.x * d, p, ax.x);
     } else {
       const double cb = cbrt(w[WC_TWOPIMS] * nu);
       A = cb * cb * w[WC_AMP];
+      atomicAdd(counts + SYC_CBRT, 1ULL);          // rare branch (counted for emri_plan_synth_report)
     }
   }
   double sa, ca, s2gt, c2gt;
@@ -138,26 +148,29 @@ DEVINL void sample_setup(const double* __restrict__ w, const double2* __restrict
   // beta (BC 22-24): tan(beta) = Ns/Nc
   const double Ns = fma(w[WC_CL], Ln, -w[WC_SN]);
   const double Nc = fma(w[WC_B2], sa, w[WC_B1] * ca);
-  const double den_b = fma(Nc, Nc, Ns * Ns);
+  const double den_b0 = fma(Nc, Nc, Ns * Ns);
   // detector-time quantities (BC 17-18)
   const double cphS = w[WC_CPHS], sphS = w[WC_SPHS], cS = w[WC_CS], sS = w[WC_SS];
   const double cd = fma(cpb, cphS, spb * sphS), sd = fma(spb, cphS, -cpb * sphS);
   const double cthd = fma(-kHalfSqrt3 * sS, cd, 0.5 * cS);
   const double Pq = fma(sS, cd, kSqrt3 * cS), Qq = 2.0 * sS * sd;
-  const double den_a = fma(Pq, Pq, Qq * Qq);
+  const double den_a = fma(Pq, Pq, Qq * Qq);      // = 4 sin^2(theta_d): zero only for a source exactly on the detector normal
   const double Npsi = fma(-cthd, Ln, fma(-kHalfSqrt3, fma(Lx, cpb, Ly * spb), 0.5 * Lz));
   const double Dpsi = 0.5 * sS * fma(Ly, cphS, -Lx * sphS)
                       - kHalfSqrt3 * (cpb * fma(Lz * sS, sphS, -cS * Ly) + spb * fma(cS, Lx, -Lz * sS * cphS));
-  const double den_p = fma(Npsi, Npsi, Dpsi * Dpsi);
-  // one division for the three normalisations
+  const double den_p0 = fma(Npsi, Npsi, Dpsi * Dpsi);
+  // one division for the three normalisations.  Reading R16: an angle whose atan2 arguments both vanish is 0; its
+  // denominator is replaced by 1 BEFORE the shared reciprocal so that the other two normalisations stay finite
+  const bool ok_b = den_b0 > 0.0, ok_p = den_p0 > 0.0;
+  const double den_b = ok_b ? den_b0 : 1.0, den_p = ok_p ? den_p0 : 1.0;
   const double bp = den_b * den_p;
   const double inv = rcp_fast(bp * den_a);
   const double ib = inv * (den_a * den_p), ia = inv * bp, ip = inv * (den_a * den_b);
   double c2b = fma(Nc, Nc, -Ns * Ns) * ib, s2b = 2.0 * Ns * Nc * ib;
-  if (!(den_b > 0.0)) { c2b = 1.0; s2b = 0.0; }                     // reading R16: beta = 0
+  if (!ok_b) { c2b = 1.0; s2b = 0.0; }                              // beta = 0
   const double c2a = fma(Qq, Qq, -Pq * Pq) * ia, s2a = 2.0 * Pq * Qq * ia;
   double c2s = fma(Dpsi, Dpsi, -Npsi * Npsi) * ip, s2s = 2.0 * Npsi * Dpsi * ip;
-  if (!(den_p > 0.0)) { c2s = 1.0; s2s = 0.0; }
+  if (!ok_p) { c2s = 1.0; s2s = 0.0; }                              // psi = 0
   const double c2g = fma(c2gt, c2b, -s2gt * s2b), s2g = fma(s2gt, c2b, c2gt * s2b);
   const double c2pb = fma(cpb, cpb, -spb * spb), s2pb = 2.0 * cpb * spb;
   const double c2p = fma(c2pb, c2a, -s2pb * s2a), s2p = fma(s2pb, c2a, c2pb * s2a);
@@ -294,7 +307,10 @@ DEVINL void prepare_unit(const SynthArgs& a, int lane, int k, int64_t i_begin, i
   for (int q = lane; q <= a.n_max; q += 32) s_Mb[q] = 1;
   const int32_t st = a.status[k];
   const bool skip = (st & (EMRI_ST_BADPARAM | EMRI_ST_DELAY | EMRI_ST_STATE)) != 0;
-  if (lane == 0) { meta->skip = skip ? 1 : 0; meta->jpl = a.jpl[k]; }
+  if (lane == 0) {
+    meta->skip = skip ? 1 : 0; meta->jpl = a.jpl[k];
+    atomicAdd(a.counts + (skip ? SYC_SKIP : SYC_UNITS), 1ULL);
+  }
   if (skip) return;
   const double* nodes = a.nodes + (size_t)k * a.Nn * NODE_STRIDE;
   // range of e over the unit from the node rows it touches (the Hermite cubic stays within pad of the nodes)
@@ -361,7 +377,11 @@ DEVINL void prepare_unit(const SynthArgs& a, int lane, int k, int64_t i_begin, i
   }
 #pragma unroll
   for (int off = 16; off > 0; off >>= 1) Mu = max(Mu, __shfl_xor_sync(0xffffffffu, Mu, off));
-  if (lane == 0) { meta->Mu = Mu; meta->w0e = (Mu >= MLOC) ? 0.0 : w0; }
+  if (a.force_base) Mu = MLOC;
+  if (lane == 0) {
+    meta->Mu = Mu; meta->w0e = (Mu >= MLOC) ? 0.0 : w0;
+    atomicAdd(a.counts + (Mu >= MLOC ? SYC_BASE : Mu), 1ULL);
+  }
   // detector phase at the start of each tile of the unit
   if (lane < a.unit_tiles) {
     double sb, cb;
@@ -451,8 +471,9 @@ __global__ void __launch_bounds__(SYNTH_BLOCK, SYNTH_MINBLOCKS) synth_kernel(Syn
           const double cpb2 = fma(cpa, c1s, -spa * s1s), spb2 = fma(spa, c1s, cpa * s1s);
           SampleOut A, B;
           double* fin = s_fin + tid;
-          sample_setup(wc, s_sct, nodes, aux, i0, a.S, a.logS, invS, Delta, mt.jpl, cpa, spa, mt.w0e, A, fin, 2 * SYNTH_THREADS);
-          sample_setup(wc, s_sct, nodes, aux, i0 + 1, a.S, a.logS, invS, Delta, mt.jpl, cpb2, spb2, mt.w0e, B,
+          sample_setup(wc, s_sct, nodes, aux, i0, a.S, a.logS, invS, Delta, mt.jpl, cpa, spa, mt.w0e, a.cbrt_thr, a.counts, A, fin,
+                       2 * SYNTH_THREADS);
+          sample_setup(wc, s_sct, nodes, aux, i0 + 1, a.S, a.logS, invS, Delta, mt.jpl, cpb2, spb2, mt.w0e, a.cbrt_thr, a.counts, B,
                        fin + SYNTH_THREADS, 2 * SYNTH_THREADS);
           double S[6];
           switch (mt.Mu) {

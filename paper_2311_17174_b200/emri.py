@@ -17,10 +17,10 @@ _lib = None
 
 EXPORTS = (
     "emri_strerror", "emri_plan_create", "emri_plan_destroy", "emri_plan_set_cosmology",
-    "emri_plan_set_coarse_stride", "emri_plan_set_orbit_schedule", "emri_plan_set_anchor", "emri_plan_orbit_report", "emri_plan_set_chunk", "emri_orbit", "emri_plan_num_nodes", "emri_waveform",
+    "emri_plan_set_coarse_stride", "emri_plan_set_orbit_schedule", "emri_plan_set_anchor", "emri_plan_orbit_report",
+    "emri_plan_synth_report", "emri_plan_set_synth_debug", "emri_plan_set_chunk", "emri_orbit", "emri_plan_num_nodes", "emri_waveform",
     "emri_waveform_fft", "emri_data_fft", "emri_loglike", "emri_loglike_fdep", "emri_loglike_host", "emri_plan_enable_timings",
-    "emri_plan_get_timings", "emri_plan_last_cuda_error", "emri_plan_workspace_bytes", "emri_stretch_step",
-    "emri_probe_fp64_peak", "emri_probe_fp64_peak3", "emri_probe_hbm_read",
+    "emri_plan_get_timings", "emri_plan_last_cuda_error", "emri_plan_last_launch_count", "emri_plan_workspace_bytes", "emri_stretch_step",
 )
 
 
@@ -48,6 +48,8 @@ def load():
     L.emri_plan_set_orbit_schedule.argtypes = [vp, i32]
     L.emri_plan_orbit_report.argtypes = [vp, i32, vp]
     L.emri_plan_set_anchor.argtypes = [vp, i32]
+    L.emri_plan_synth_report.argtypes = [vp, vp]
+    L.emri_plan_set_synth_debug.argtypes = [vp, i32]
     L.emri_orbit.argtypes = [vp, vp, i32, vp, vp, vp]
     L.emri_plan_num_nodes.restype = i64
     L.emri_plan_num_nodes.argtypes = [vp]
@@ -60,12 +62,10 @@ def load():
     L.emri_plan_enable_timings.argtypes = [vp, i32]
     L.emri_plan_get_timings.argtypes = [vp, C.POINTER(dbl)]
     L.emri_plan_last_cuda_error.argtypes = [vp]
+    L.emri_plan_last_launch_count.argtypes = [vp]
     L.emri_plan_workspace_bytes.restype = i64
     L.emri_plan_workspace_bytes.argtypes = [vp]
     L.emri_stretch_step.argtypes = [vp, vp, vp, i32, vp, vp, vp, dbl, u64, i64, i32, vp, vp, vp]
-    L.emri_probe_fp64_peak.argtypes = [C.POINTER(dbl), vp]
-    L.emri_probe_fp64_peak3.argtypes = [C.POINTER(dbl), vp]
-    L.emri_probe_hbm_read.argtypes = [i64, C.POINTER(dbl), vp]
     for name in EXPORTS:
         if name not in ("emri_strerror", "emri_plan_num_nodes", "emri_plan_workspace_bytes"):
             getattr(L, name).restype = i32
@@ -90,33 +90,6 @@ def _ptr(t, dtype=None, shape=None):
     if shape is not None and tuple(t.shape) != tuple(shape):
         raise TypeError(f"expected shape {tuple(shape)}, got {tuple(t.shape)}")
     return C.c_void_p(t.data_ptr())
-
-
-def probe_fp64_peak():
-    """TFLOP/s of a chain-free DFMA kernel on the current device (roofline denominator of stage b)."""
-    v = C.c_double()
-    rc = load().emri_probe_fp64_peak(C.byref(v), _stream())
-    if rc:
-        raise EmriError(f"fp64 probe failed ({rc})")
-    return v.value
-
-
-def probe_fp64_peak3():
-    """TFLOP/s of DFMAs with three fresh vector-register operands (register-file-bound FP64 rate)."""
-    v = C.c_double()
-    rc = load().emri_probe_fp64_peak3(C.byref(v), _stream())
-    if rc:
-        raise EmriError(f"fp64 probe failed ({rc})")
-    return v.value
-
-
-def probe_hbm_read(nbytes=4 << 30):
-    """GB/s of a streaming read of `nbytes` of device memory."""
-    v = C.c_double()
-    rc = load().emri_probe_hbm_read(int(nbytes), C.byref(v), _stream())
-    if rc:
-        raise EmriError(f"hbm probe failed ({rc})")
-    return v.value
 
 
 class Plan:
@@ -171,11 +144,29 @@ class Plan:
         self._check(self._L.emri_plan_orbit_report(self._h, K, m.ctypes.data_as(C.c_void_p)))
         return m
 
+    def synth_report(self):
+        """path counters of stage (b) over the last call: dict(units, by_order[1..8], base_units, cbrt_samples, skipped_units)"""
+        c = np.zeros(16, dtype=np.int64)
+        self._check(self._L.emri_plan_synth_report(self._h, c.ctypes.data_as(C.c_void_p)))
+        return dict(units=int(c[0]), by_order={m: int(c[m]) for m in range(1, 9)}, base_units=int(c[9]),
+                    cbrt_samples=int(c[10]), skipped_units=int(c[11]))
+
+    def set_synth_debug(self, force_base=False, force_cbrt=False):
+        """test hook: force the data-selected slow paths of stage (b)"""
+        self._check(self._L.emri_plan_set_synth_debug(self._h, (1 if force_base else 0) | (2 if force_cbrt else 0)))
+
     def set_chunk(self, c):
         self._check(self._L.emri_plan_set_chunk(self._h, c))
 
     def num_nodes(self):
         return int(self._L.emri_plan_num_nodes(self._h))
+
+    def launch_count(self):
+        """kernels of this library enqueued by the last hot call"""
+        return int(self._L.emri_plan_last_launch_count(self._h))
+
+    def like_kernel_name(self):
+        return "loglike_kernel"
 
     def workspace_bytes(self):
         return int(self._L.emri_plan_workspace_bytes(self._h))

@@ -2,17 +2,10 @@
 
 The path shards by walker -- every walker's orbit, waveform, transform and logL are independent given the shared
 read-only data spectrum and PSD -- so there is no data-path collective.  bench.py gives every
-rank its own ensemble (weak scaling); `shard_rows` is the contiguous split of ONE ensemble over ranks for callers
-that want strong scaling.  torch.distributed is used only for the barrier and the max-over-ranks of the timing.
+rank its own ensemble (weak scaling) and calls every function of this module; torch.distributed is used only for the
+barrier and the max-over-ranks of the timing.
 """
 import dataclasses
-
-
-def shard_rows(K, world, rank):
-    """rows [k0, k1) of a K-walker ensemble owned by `rank`: contiguous, sizes differ by at most one"""
-    base, rem = divmod(K, world)
-    k0 = rank * base + min(rank, rem)
-    return k0, k0 + base + (1 if rank < rem else 0)
 
 
 def rank_config(cfg, rank):

@@ -250,14 +250,19 @@ def parity_walker_subset(params, n=16, seed=12345):
     K = params.shape[0]
     if K <= n:
         return np.arange(K)
-    pick = [0, 1, 2, 3, int(np.argmax(params[:, P_E0])), int(np.argmin(params[:, P_M])),
-            int(np.argmax(params[:, P_MU] / params[:, P_M]))]
+    # the three extreme walkers come FIRST and are never dropped; then 0..3; then seeded draws up to n
+    pick = []
+    for k in (int(np.argmax(params[:, P_E0])), int(np.argmin(params[:, P_M])),
+              int(np.argmax(params[:, P_MU] / params[:, P_M])), 0, 1, 2, 3):
+        if k not in pick and len(pick) < n:
+            pick.append(k)
     rng = np.random.default_rng(seed)
     for k in rng.permutation(K):
-        if len(set(pick)) >= n:
+        if len(pick) >= n:
             break
-        pick.append(int(k))
-    return np.array(sorted(set(pick)))[:n]
+        if int(k) not in pick:
+            pick.append(int(k))
+    return np.array(sorted(pick))
 
 
 def paper_fig1_params(path):

@@ -19,6 +19,14 @@ def oracle():
 
 
 @pytest.fixture(scope="session")
+def oracle_lso():
+    """the oracle reading parameter rows as the state at plunge (reading D12): a separate instance, so that the
+    forward-anchored `oracle` is never switched"""
+    from oracle.oracle import Oracle
+    return Oracle(anchor=True)
+
+
+@pytest.fixture(scope="session")
 def oracle_ld():
     from oracle.oracle import Oracle
     return Oracle(long_double=True)

@@ -8,8 +8,8 @@ from paper_2311_17174_b200 import build, emri
 ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
 
 
-def declared_symbols():
-    txt = open(os.path.join(ROOT, "include", "emri.h")).read()
+def declared_symbols(header="emri.h"):
+    txt = open(os.path.join(ROOT, "include", header)).read()
     txt = re.sub(r"/\*.*?\*/", "", txt, flags=re.S)
     return sorted(set(re.findall(r"\b(emri_[a-z0-9_]+)\s*\(", txt)))
 
@@ -22,6 +22,18 @@ def test_library_builds_and_exports_every_declared_symbol():
     for n in names:
         assert hasattr(L, n), f"libemri_b200.so does not export {n}"
     assert set(names) == set(emri.EXPORTS)
+    assert not [n for n in names if "probe" in n]            # measurement helpers are not part of the boundary
+
+
+def test_probe_library_exports_its_header():
+    """include/emri_probe.h (bench.py's peak probes) lives in a library of its own"""
+    from paper_2311_17174_b200 import probe
+    build.build()
+    L = probe.load()
+    names = declared_symbols("emri_probe.h")
+    assert set(names) == set(probe.EXPORTS)
+    for n in names:
+        assert hasattr(L, n)
 
 
 def test_strerror_and_argument_checks_need_no_gpu():

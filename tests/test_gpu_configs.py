@@ -5,6 +5,7 @@ import numpy as np
 import pytest
 
 from paper_2311_17174_b200 import workloads as W
+from survey_recipe import with_plunging_walkers
 
 torch = pytest.importorskip("torch")
 pytestmark = pytest.mark.gpu
@@ -28,12 +29,27 @@ def logl_ok(got, ref):
     return np.all(np.abs(got - ref) <= 1e-9 * np.abs(ref) + 1e-6)
 
 
-@pytest.mark.parametrize("ci,n_sub", [(0, 8), (1, 4), (2, 4), (3, 4)])
-def test_full_size_loglike_on_walker_subset(emri, oracle, ci, n_sub):
-    cfg = W.CONFIGS[ci]
+def subset_with_plungers(oracle, cfg, n=16):
+    """SURVEY 8(d)-3's 16 walkers: argmax e0, argmin M, argmax mu/M, indices 0-3, seeded draws -- three of the draws
+    replaced by the ensemble's last three rows, re-placed by the survey's nu0 rule (8(d)-1) so that they plunge
+    1.25, 1.35 and 1.5 observation lengths after the window starts (the strongly chirping regime of PAPER.md:120)"""
     P = W.draw_params(cfg)
+    rows = [cfg.K - 1, cfg.K - 2, cfg.K - 3]
+    P = with_plunging_walkers(oracle, P, cfg, rows)
+    if cfg.K <= n:
+        return P, np.arange(cfg.K), rows
+    sub = [int(k) for k in W.parity_walker_subset(P, n=n) if k not in rows][:n - 3] + rows
+    return P, np.array(sorted(sub)), rows
+
+
+@pytest.mark.parametrize("ci", [0, 1, 2, 3])
+def test_full_size_loglike_on_walker_subset(emri, oracle, ci):
+    cfg = W.CONFIGS[ci]
+    P, sub, plungers = subset_with_plungers(oracle, cfg)
     psd = W.lisa_psd_barack_cutler(cfg.N, cfg.dt)
-    sub = W.parity_walker_subset(P, n=n_sub)
+    if cfg.K > 16:
+        assert len(sub) == 16 and {int(np.argmax(P[:, W.P_E0])), int(np.argmin(P[:, W.P_M])),
+                                   int(np.argmax(P[:, W.P_MU] / P[:, W.P_M]))} <= set(sub.tolist())
     hI, hII, st0 = oracle.waveform(P[0], cfg.N, cfg.dt, cfg.n_max)
     D = np.stack([oracle.rfft(hI), oracle.rfft(hII)])
     if cfg.noise_seed:
@@ -51,14 +67,17 @@ def test_full_size_loglike_on_walker_subset(emri, oracle, ci, n_sub):
         assert abs(got[0]) <= 1e-6          # noise-less data = walker 0's own waveform
     modes = plan.orbit_report(cfg.K)
     assert np.all(modes == 1)              # every walker's parallel-in-time orbit verified
+    rep = plan.synth_report()
+    print(f"cfg{ci} stage (b) paths: {rep}")
+    assert rep["units"] >= cfg.K * -(-cfg.N // 2048) and rep["skipped_units"] == 0     # units of <= 8 tiles
+    assert sum(rep["by_order"].values()) + rep["base_units"] == rep["units"]
     plan.close()
 
 
-@pytest.mark.parametrize("ci", [1, 2])
+@pytest.mark.parametrize("ci", [1, 2, 3])
 def test_full_size_waveform_sampled(emri, oracle, ci):
     cfg = W.CONFIGS[ci]
-    P = W.draw_params(cfg)
-    sub = W.parity_walker_subset(P, n=6)
+    P, sub, plungers = subset_with_plungers(oracle, cfg)
     plan = emri.Plan(cfg.N, cfg.dt, cfg.n_max, len(sub))
     hI, hII = plan.waveform(dev(P[sub]))
     torch.cuda.synchronize()

@@ -129,7 +129,7 @@ def lso_params(cfg, K, e_hi=0.5):
 
 
 @pytest.mark.parametrize("ci,N,S", [(1, 1 << 18, 256), (3, 1 << 16, 64), (2, 1 << 20, 256)])
-def test_lso_anchored_orbit_matches_oracle_and_sequential(emri, oracle, ci, N, S):
+def test_lso_anchored_orbit_matches_oracle_and_sequential(emri, oracle, oracle_lso, ci, N, S):
     cfg = W.scaled(W.CONFIGS[ci], K=10, N=N)
     P = lso_params(cfg, cfg.K)
     out = {}
@@ -148,10 +148,9 @@ def test_lso_anchored_orbit_matches_oracle_and_sequential(emri, oracle, ci, N, S
     n0, s0, _ = out[0]
     print("status", s1, "modes", modes)
     assert np.array_equal(s0, s1)
-    oracle.set_anchor(True)
-    try:
+    if True:
         for k in range(cfg.K):
-            ref = oracle.orbit(P[k], N, cfg.dt, S)
+            ref = oracle_lso.orbit(P[k], N, cfg.dt, S)
             assert s1[k] == ref["status"]
             if ref["status"]:
                 assert not n1[k].any() and not n0[k].any()
@@ -166,22 +165,16 @@ def test_lso_anchored_orbit_matches_oracle_and_sequential(emri, oracle, ci, N, S
                 np.testing.assert_allclose(val[q], n0[k, :, q], rtol=4e-16, atol=1e-300)
                 np.testing.assert_allclose(inc[q], ref["inc"][q], rtol=1e-11, atol=1e-25)
             np.testing.assert_allclose(slope, ref["slope"], rtol=1e-12, atol=1e-30)
-    finally:
-        oracle.set_anchor(False)
     assert (s1 == 0).sum() >= 5
 
 
-def test_lso_anchored_waveform_and_loglike_match_oracle(emri, oracle):
+def test_lso_anchored_waveform_and_loglike_match_oracle(emri, oracle, oracle_lso):
     cfg = W.scaled(W.CONFIGS[2], K=6, N=1 << 13)
     P = lso_params(cfg, cfg.K, e_hi=0.4)
     psd = W.lisa_psd_barack_cutler(cfg.N, cfg.dt)
-    oracle.set_anchor(True)
-    try:
-        h_ref, st_ref = oracle.waveform_batch(P, cfg.N, cfg.dt, cfg.n_max)
-        D = np.stack([oracle.rfft(h_ref[1, 0]), oracle.rfft(h_ref[1, 1])]) + W.noise_fft(cfg.N, cfg.dt, psd, 9)
-        L_ref, _ = oracle.loglike_batch(P, cfg.N, cfg.dt, cfg.n_max, D, psd)
-    finally:
-        oracle.set_anchor(False)
+    h_ref, st_ref = oracle_lso.waveform_batch(P, cfg.N, cfg.dt, cfg.n_max)
+    D = np.stack([oracle.rfft(h_ref[1, 0]), oracle.rfft(h_ref[1, 1])]) + W.noise_fft(cfg.N, cfg.dt, psd, 9)
+    L_ref, _ = oracle_lso.loglike_batch(P, cfg.N, cfg.dt, cfg.n_max, D, psd)
     plan = emri.Plan(cfg.N, cfg.dt, cfg.n_max, cfg.K, psd)
     plan.set_anchor(True)
     st = torch.zeros(cfg.K, dtype=torch.int32, device="cuda")
@@ -205,13 +198,12 @@ def test_lso_anchored_waveform_and_loglike_match_oracle(emri, oracle):
     plan.close()
 
 
-def test_paper_fig1_grid_matches_oracle(emri, oracle):
+def test_paper_fig1_grid_matches_oracle(emri, oracle, oracle_lso):
     """the paper's own illustration (Figure 1): M = 1e6, mu = 10, spins 0 / 0.4 / 0.8, e_LSO = 0 / 0.3 / 0.6,
     the last hour before the LSO, and the same nine systems over the last year (N = 2^21, sampled)"""
     import os
     P = W.paper_fig1_params(os.path.join(os.path.dirname(os.path.abspath(__file__)), "golden", "paper_fig1_parameters.txt"))
-    oracle.set_anchor(True)
-    try:
+    if True:
         for N, n_max, idx in ((256, 20, None), (1 << 21, 30, "sampled")):
             dt = 15.0
             plan = emri.Plan(N, dt, n_max, 9)
@@ -224,7 +216,7 @@ def test_paper_fig1_grid_matches_oracle(emri, oracle):
                 rng = np.random.default_rng(1)
                 idx = np.unique(np.concatenate([np.arange(0, 300), np.arange(N - 600, N), rng.integers(0, N, 1200)]))
             for k in range(9):
-                a, b, s_ref = oracle.waveform(P[k], N, dt, n_max, idx=idx)
+                a, b, s_ref = oracle_lso.waveform(P[k], N, dt, n_max, idx=idx)
                 assert st[k] == s_ref
                 if s_ref:
                     assert not hI[k].any()          # e grew past 1 on the way back: invalid on both sides
@@ -235,5 +227,3 @@ def test_paper_fig1_grid_matches_oracle(emri, oracle):
                 assert eI <= 1e-9 and eII <= 1e-9, (N, k, eI, eII)
             print(f"Fig. 1 grid, N = {N}: status {st}, modes {plan.orbit_report(9)}")
             plan.close()
-    finally:
-        oracle.set_anchor(False)

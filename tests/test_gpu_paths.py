@@ -1,0 +1,189 @@
+"""The data-selected paths of stage (b) and the boundary's corner cases that no seeded config is known to reach:
+forced base-series fallback and cube-root amplitude (emri_plan_set_synth_debug) checked element-wise against the oracle
+with the path counters (emri_plan_synth_report) asserted non-zero; a natural input that takes both; degenerate geometry
+(reading R16); the stretch move on a plan with K_max = K/2; small strides at full length; no allocation in the hot call."""
+import numpy as np
+import pytest
+
+from paper_2311_17174_b200 import workloads as W
+
+torch = pytest.importorskip("torch")
+pytestmark = pytest.mark.gpu
+H_TOL = 1e-9
+
+
+@pytest.fixture(scope="module")
+def emri():
+    if not torch.cuda.is_available():
+        pytest.skip("no CUDA device")
+    from paper_2311_17174_b200 import emri as m
+    m.load()
+    return m
+
+
+def dev(a):
+    return torch.from_numpy(np.ascontiguousarray(a)).cuda()
+
+
+def h_err(got, ref):
+    return np.max(np.abs(got - ref), axis=-1) / np.max(np.abs(ref), axis=-1)
+
+
+@pytest.mark.parametrize("force_base,force_cbrt", [(True, False), (False, True), (True, True)])
+def test_forced_slow_paths_match_oracle(emri, oracle, force_base, force_cbrt):
+    """every unit on the base series in e^2 and / or every sample on the cube-root amplitude: same waveform"""
+    cfg = W.scaled(W.CONFIGS[3], K=6, N=3 * 2048 + 300)          # several units and a ragged tail, n_max = 30
+    P = W.draw_params(cfg)
+    P[:, W.P_E0] = np.linspace(0.05, 0.5, cfg.K)
+    h_ref, st_ref = oracle.waveform_batch(P, cfg.N, cfg.dt, cfg.n_max)
+    assert not st_ref.any()
+    plan = emri.Plan(cfg.N, cfg.dt, cfg.n_max, cfg.K)
+    hI0, hII0 = plan.waveform(dev(P))
+    rep0 = plan.synth_report()
+    plan.set_synth_debug(force_base=force_base, force_cbrt=force_cbrt)
+    hI, hII = plan.waveform(dev(P))
+    rep = plan.synth_report()
+    torch.cuda.synchronize()
+    print("default paths", rep0, "forced", rep)
+    assert rep0["base_units"] == 0 and rep0["cbrt_samples"] == 0          # the defaults take neither here
+    if force_base:
+        assert rep["base_units"] == rep["units"] > 0 and sum(rep["by_order"].values()) == 0
+    if force_cbrt:
+        assert rep["cbrt_samples"] == cfg.K * cfg.N
+    for got, got0, ch in ((hI, hI0, 0), (hII, hII0, 1)):
+        e = h_err(got.cpu().numpy(), h_ref[:, ch])
+        assert np.all(e <= H_TOL), e
+        assert np.all(h_err(got.cpu().numpy(), got0.cpu().numpy()) <= 1e-11)    # and the fast paths agree with them
+    plan.close()
+
+
+def test_natural_input_reaches_both_slow_paths(emri, oracle):
+    """a stride of 4096 samples makes nu move by more than 4e-3 of the node value inside an interval (cube-root branch),
+    and e = 0.6 chirping hard over 16-tile units makes order 8 of the local series significant (base-series fallback):
+    the counters prove the paths ran, the oracle (same stride) that they are right"""
+    import os
+    N, S = 1 << 15, 4096
+    cfg = W.scaled(W.CONFIGS[3], K=4, N=N, n_max=30)
+    P = W.draw_params(cfg)
+    P[:, W.P_M], P[:, W.P_MU], P[:, W.P_E0] = 2e5, 50.0, np.array([0.6, 0.55, 0.5, 0.3])
+    for k in range(cfg.K):        # two days from plunge by the closed-form estimate
+        P[k, W.P_NU0] = W.nu0_for_plunge_after(P[k, W.P_M], P[k, W.P_MU], P[k, W.P_E0], 2.5 * N * cfg.dt)
+    h_ref, st_ref = oracle.waveform_batch(P, N, cfg.dt, cfg.n_max, S=S)
+    os.environ["EMRI_UNIT_TILES"] = "16"
+    try:
+        plan = emri.Plan(N, cfg.dt, cfg.n_max, cfg.K)
+    finally:
+        del os.environ["EMRI_UNIT_TILES"]
+    plan.set_coarse_stride(S)
+    st = torch.zeros(cfg.K, dtype=torch.int32, device="cuda")
+    hI, hII = plan.waveform(dev(P), status=st)
+    rep = plan.synth_report()
+    torch.cuda.synchronize()
+    print("paths", rep, "status", st.cpu().numpy(), st_ref)
+    assert np.array_equal(st.cpu().numpy(), st_ref)
+    assert rep["cbrt_samples"] > 0 and rep["base_units"] > 0
+    live = np.max(np.abs(h_ref[:, 0]), axis=1) > 0
+    assert live.any()
+    for got, ch in ((hI, 0), (hII, 1)):
+        g = got.cpu().numpy()
+        assert np.all(h_err(g[live], h_ref[live, ch]) <= H_TOL)
+    plan.close()
+
+
+def test_degenerate_geometry_is_finite(emri, oracle):
+    """reading R16: lambda = 0 (beta's atan2 arguments vanish identically: beta = 0) and theta_K = 0 (the literal
+    (S.n cos thK - cos thS)/sin thK is 0/0; the library uses its expanded form) must give finite waveforms with status 0.
+    The oracle's literal formulas are NaN exactly there, so: theta_K = 0 is compared with the oracle at theta_K = 1e-7
+    (continuous), and lambda = 0 by what beta = 0 implies: L^ = S^ does not precess, so alpha0 must not matter."""
+    cfg = W.scaled(W.CONFIGS[1], K=4, N=1 << 12)
+    P = W.draw_params(cfg)
+    P[1] = P[0]; P[1, W.P_LAM] = 0.0
+    P[2] = P[1]; P[2, W.P_ALP0] += 1.234
+    P[3] = P[0]; P[3, W.P_THK] = 0.0
+    psd = W.lisa_psd_barack_cutler(cfg.N, cfg.dt)
+    plan = emri.Plan(cfg.N, cfg.dt, cfg.n_max, cfg.K, psd)
+    st = torch.zeros(cfg.K, dtype=torch.int32, device="cuda")
+    hI, hII = plan.waveform(dev(P), status=st)
+    D = plan.data_fft(hI[0].contiguous(), hII[0].contiguous())
+    logL = plan.loglike(dev(P), D).cpu().numpy()
+    hI, hII = hI.cpu().numpy(), hII.cpu().numpy()
+    assert not st.cpu().numpy().any()
+    assert np.all(np.isfinite(hI)) and np.all(np.isfinite(hII)) and np.all(np.isfinite(logL))
+    assert np.max(np.abs(hI[1])) > 0 and np.max(np.abs(hI[3])) > 0
+    assert np.max(np.abs(hI[1] - hI[2])) <= 1e-11 * np.max(np.abs(hI[1]))
+    assert np.max(np.abs(hII[1] - hII[2])) <= 1e-11 * np.max(np.abs(hII[1]))
+    q = P[3].copy(); q[W.P_THK] = 1e-7
+    a, b, s3 = oracle.waveform(q, cfg.N, cfg.dt, cfg.n_max)
+    assert s3 == 0
+    assert np.max(np.abs(hI[3] - a)) <= 1e-5 * np.max(np.abs(a)) and np.max(np.abs(hII[3] - b)) <= 1e-5 * np.max(np.abs(b))
+    plan.close()
+
+
+def test_stretch_step_on_a_plan_of_half_the_ensemble(emri):
+    """include/emri.h: K/2 <= K_max.  A plan created for K/2 walkers must give the same chain as one created for K"""
+    cfg = W.scaled(W.CONFIGS[4], K=16, N=1 << 12, n_max=5)
+    P = W.draw_params(cfg)
+    psd = W.lisa_psd_barack_cutler(cfg.N, cfg.dt)
+    lo, hi = (dev(v) for v in W.prior_box(cfg))
+    out = []
+    for K_max in (cfg.K, cfg.K // 2):
+        plan = emri.Plan(cfg.N, cfg.dt, cfg.n_max, K_max, psd)
+        D = plan.waveform_fft(dev(P[:1]))[0].clone()
+        X = dev(P)
+        logL = torch.empty(cfg.K, dtype=torch.float64, device="cuda")
+        for h in (0, 1):      # logL of the start ensemble, half by half (K > K_max for the small plan)
+            sl = slice(h * cfg.K // 2, (h + 1) * cfg.K // 2)
+            logL[sl] = plan.loglike(X[sl].contiguous(), D)
+        acc = torch.zeros(cfg.K, dtype=torch.int32, device="cuda")
+        for step in range(3):
+            for half in (0, 1):
+                plan.stretch_step(X, logL, D, lo, hi, 2.0, 99, step, half, accepted=acc)
+        torch.cuda.synchronize()
+        out.append((X.cpu().numpy(), logL.cpu().numpy()))
+        plan.close()
+    assert np.array_equal(out[0][0], out[1][0]) and np.array_equal(out[0][1], out[1][1])
+    assert not np.array_equal(out[0][0], P)            # something was accepted
+
+
+def test_small_stride_at_full_length(emri):
+    """N = 2^21 with S = 16: 513 shooting segments (49 KB of shared memory in orbit_correct_kernel, above the default
+    limit) -- both schedules run and agree"""
+    cfg = W.scaled(W.CONFIGS[2], K=2, N=1 << 21)
+    P = dev(W.draw_params(cfg))
+    res = []
+    for schedule in (1, 0):
+        plan = emri.Plan(cfg.N, cfg.dt, cfg.n_max, cfg.K)
+        plan.set_coarse_stride(16)
+        plan.set_orbit_schedule(schedule)
+        st = torch.zeros(cfg.K, dtype=torch.int32, device="cuda")
+        nodes = plan.orbit(P, status=st)
+        torch.cuda.synchronize()
+        assert not st.cpu().numpy().any()
+        res.append(nodes.cpu().numpy())
+        plan.close()
+    np.testing.assert_allclose(res[0][:, :, 1], res[1][:, :, 1], rtol=1e-14)      # nu
+    np.testing.assert_allclose(res[0][:, :, 3], res[1][:, :, 3], rtol=1e-13, atol=1e-18)      # e
+    d = (res[0][:, :, 0] - res[1][:, :, 0]) % 1.0
+    assert np.max(np.minimum(d, 1.0 - d)) < 1e-10
+
+
+def test_hot_call_does_not_allocate(emri):
+    """include/emri.h: calls only enqueue.  After plan creation neither device memory nor the plan's workspace moves
+    across emri_loglike calls -- full ensemble, a ragged one (its cuFFT plan object is built on first use, inside the
+    work area that already exists) and a single walker"""
+    cfg = W.scaled(W.CONFIGS[1], K=40, N=1 << 14)
+    P = dev(W.draw_params(cfg))
+    psd = W.lisa_psd_barack_cutler(cfg.N, cfg.dt)
+    plan = emri.Plan(cfg.N, cfg.dt, cfg.n_max, cfg.K, psd)
+    plan.set_chunk(16)                                   # chunks of 16: 40 = 16 + 16 + 8
+    D = plan.waveform_fft(P[:1].contiguous())[0].clone()
+    logL = torch.empty(cfg.K, dtype=torch.float64, device="cuda")
+    plan.loglike(P, D, logL)                             # warm-up: every kernel's module is loaded
+    torch.cuda.synchronize()
+    free0, ws0 = torch.cuda.mem_get_info()[0], plan.workspace_bytes()
+    for K in (cfg.K, 37, 1, cfg.K):
+        plan.loglike(P[:K].contiguous() if K < cfg.K else P, D, logL[:K])
+    torch.cuda.synchronize()
+    assert plan.workspace_bytes() == ws0
+    assert torch.cuda.mem_get_info()[0] >= free0 - (2 << 20)      # cuFFT plan objects only (no work area, no buffers)
+    plan.close()

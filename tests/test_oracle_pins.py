@@ -429,31 +429,69 @@ def test_geometry_against_vector_algebra(oracle):
         assert g["psi"] == pytest.approx(math.atan2(g["Npsi"], g["Dpsi"]), abs=1e-15)
 
 
+def _detector_axes(phibar):
+    """Explicit unit vectors of the rolling LISA frame (Cutler 1998; S5.7 with phibar0 = alphabar0 = 0), in ecliptic
+    coordinates: the normal z_d is tilted 60 degrees from the ecliptic pole and follows the orbit; e2 points along the
+    orbital motion and e1 = e2 x z_d completes the in-plane pair; the arms' frame (x_d, y_d) counter-rotates in that plane
+    once per orbit, starting at t = 0 from x_d = -e2, y_d = e1 (which is what S5.7's phi_d says at phibar = 0:
+    sin(th_d) cos(phi_d) = -n_y, sin(th_d) sin(phi_d) = (n_x + sqrt3 n_z)/2)."""
+    zd = np.array([-math.sqrt(3) / 2 * math.cos(phibar), -math.sqrt(3) / 2 * math.sin(phibar), 0.5])
+    e2 = np.array([-math.sin(phibar), math.cos(phibar), 0.0])
+    e1 = np.cross(e2, zd)
+    xd = -math.cos(phibar) * e2 - math.sin(phibar) * e1
+    yd = -math.sin(phibar) * e2 + math.cos(phibar) * e1
+    return xd, yd, zd
+
+
 def test_detector_azimuth_against_rotating_frame(oracle):
-    """phi_d: azimuth of n^ in the detector frame that rolls about its normal once per orbit
-    (Cutler 1998); checked through cos/sin of 2 phi_d built from explicit detector axes"""
+    """phi_d is the azimuth of n^ in the rolling frame built from explicit axes: NO modulo (a quarter-turn slip, which
+    would flip the sign of both channels, fails here)"""
     rng = np.random.default_rng(5)
-    for _ in range(100):
+    for _ in range(200):
         thS = math.acos(rng.uniform(-0.99, 0.99))
         phS, phibar = rng.uniform(0, TWOPI, 2)
         g = oracle.geometry(base_row(THS=thS, PHS=phS), 0.3, phibar)
         n = _vec(thS, phS)
-        zd = np.array([-math.sqrt(3) / 2 * math.cos(phibar), -math.sqrt(3) / 2 * math.sin(phibar), 0.5])
-        # un-rolled in-plane axes: e1 along the projection of the ecliptic pole direction rotated by phibar
-        r = np.array([math.cos(phibar), math.sin(phibar), 0.0])          # Sun -> detector
-        e2 = np.array([-math.sin(phibar), math.cos(phibar), 0.0])        # along the orbit, in-plane
-        e1 = np.cross(e2, zd)
-        assert np.dot(e1, zd) == pytest.approx(0, abs=1e-15) and np.dot(e1, e1) == pytest.approx(1, abs=1e-14)
-        az0 = math.atan2(np.dot(n, e2), np.dot(n, e1))                   # azimuth before the roll
-        # the roll: the arms counter-rotate in the plane by -phibar relative to (e1, e2)
-        for k in range(-2, 3):
-            cand = az0 + phibar + k * math.pi / 2
-            if abs(math.remainder(2 * (cand - g["phid"]), TWOPI)) < 1e-9:
-                break
-        else:
-            pytest.fail("phi_d is not the rolled azimuth up to the 90-degree arm ambiguity")
+        xd, yd, zd = _detector_axes(phibar)
+        assert abs(np.dot(xd, yd)) < 1e-15 and abs(np.dot(xd, zd)) < 1e-15 and abs(np.dot(yd, zd)) < 1e-15
+        np.testing.assert_allclose(np.cross(xd, yd), zd, atol=1e-15)
         assert g["cthd"] == pytest.approx(np.dot(n, zd), abs=1e-15)
-        assert abs(np.dot(r, e2)) < 1e-15
+        az = math.atan2(np.dot(n, yd), np.dot(n, xd))
+        assert abs(math.remainder(g["phid"] - az, TWOPI)) < 1e-12         # full turns only: cos/sin(phi_d) are what enter
+        sthd = math.sqrt(1 - g["cthd"] ** 2)
+        assert sthd * math.cos(g["phid"]) == pytest.approx(np.dot(n, xd), abs=1e-14)
+        assert sthd * math.sin(g["phid"]) == pytest.approx(np.dot(n, yd), abs=1e-14)
+
+
+def test_antenna_patterns_from_the_detector_tensor(oracle):
+    """The whole response chain geometry() -> antenna() against tensors written out from vectors, with no angle and no
+    modulo anywhere: detector tensors D_I = (x_d x_d - y_d y_d)/2, D_II = (x_d y_d + y_d x_d)/2 (the second two-arm
+    combination = the first rotated by 45 degrees) from the explicit rolling axes; polarisation tensors of BC Eqs. 5-6,
+    e+ = p p - q q, ex = p q + q p with p = n x L / |n x L|, q = p x n; F = D : e.  Pins the sign and quadrant of phi_d
+    and psi and every sign of BC 15-16 (a quarter-turn slip of phi_d flips all four)."""
+    rng = np.random.default_rng(17)
+    z = np.array([0.0, 0.0, 1.0])
+    for _ in range(300):
+        thS, thK = np.arccos(rng.uniform(-0.99, 0.99, 2))
+        phS, phK, alpha, phibar = rng.uniform(0, TWOPI, 4)
+        lam = rng.uniform(0.05, math.pi - 0.05)
+        g = oracle.geometry(base_row(THS=thS, PHS=phS, THK=thK, PHK=phK, LAM=lam), alpha, phibar)
+        F = oracle.antenna(g["cthd"], g["phid"], g["psi"])
+        n, Sv = _vec(thS, phS), _vec(thK, phK)
+        L = (Sv * math.cos(lam) + (z - Sv * math.cos(thK)) / math.sin(thK) * math.sin(lam) * math.cos(alpha)
+             + np.cross(Sv, z) / math.sin(thK) * math.sin(lam) * math.sin(alpha))
+        nxL = np.cross(n, L)
+        if np.linalg.norm(nxL) < 1e-3:
+            continue
+        ph = nxL / np.linalg.norm(nxL)
+        q = np.cross(ph, n)
+        ep = np.outer(ph, ph) - np.outer(q, q)
+        ex = np.outer(ph, q) + np.outer(q, ph)
+        xd, yd, zd = _detector_axes(phibar)
+        DI = 0.5 * (np.outer(xd, xd) - np.outer(yd, yd))
+        DII = 0.5 * (np.outer(xd, yd) + np.outer(yd, xd))
+        want = [np.sum(DI * ep), np.sum(DI * ex), np.sum(DII * ep), np.sum(DII * ex)]
+        np.testing.assert_allclose(F, want, atol=5e-12)
 
 
 # ------------------------------------------------------------------ antenna patterns (S5.8)
@@ -839,10 +877,11 @@ def test_fdep_linear_in_f_delay_is_a_quadratic_phase_ie_a_dispersion(oracle):
 
 # ----------------------------------------------------------------------------- the paper's IC convention: anchored at the LSO
 @pytest.fixture()
-def lso(oracle):
-    oracle.set_anchor(True)
-    yield oracle
-    oracle.set_anchor(False)
+def lso():
+    """an oracle instance of its own, anchored at the LSO (the anchor is an explicit argument of every library call and a
+    property of the instance: nothing here can leak into the session-wide forward-anchored `oracle`)"""
+    from oracle.oracle import Oracle
+    return Oracle(anchor=True)
 
 
 def _lso_params(e_lso=0.3):
