@@ -113,9 +113,11 @@ int emri_plan_orbit_report(emri_plan* p, int K, int32_t* modes);
 /* Diagnostics of stage (b) over the last emri_waveform / emri_waveform_fft / emri_loglike* call (all chunks):
  * which evaluation path the data selected.  counts (HOST int64 [16]):
  *   [0] units (one walker x up to 8 tiles of 256 samples) synthesised, [1..8] of them by the local order kept in the
- *   re-summed harmonic series, [9] units that fell back to the base series in e^2 (local order 8 still significant),
+ *   re-summed harmonic series (first harmonic range), [9] units that fell back to the base series in e^2 (local order 8 still significant),
  *   [10] samples whose amplitude (2 pi M nu)^{2/3} took the cube root instead of the Taylor series about the coarse
- *   node (|nu/nu_j - 1| > 4e-3), [11] units of walkers with a fatal status (zero-filled), [12..15] 0.
+ *   node (|nu/nu_j - 1| > 4e-3), [11] units of walkers with a fatal status (zero-filled), [12] sum over units of the harmonics evaluated (the last
+ *   harmonic with a term above the truncation threshold, <= n_max), [13] of those, the harmonics of the first order range,
+ *   [14] sum over units of the second range's order, [15] 0.
  * Synchronises the device. */
 int emri_plan_synth_report(emri_plan* p, int64_t counts[16]);
 

@@ -50,7 +50,7 @@ struct emri_plan {
   int32_t* d_jpl = nullptr;
   int32_t* d_status = nullptr;
   // multiple-shooting orbit (orbit.cuh): segment records, per-walker mode / tail start / post-plunge row
-  int orbit_mode = 1, anchor_end = 0, seg_L = 0, seg_P = 0, unit_tiles_override = 0;
+  int orbit_mode = 1, anchor_end = 0, seg_L = 0, seg_P = 0, unit_tiles_override = 0, unit_tiles_cap = 8;
   int synth_debug = 0;                       // emri_plan_set_synth_debug
   int launches = 0;                          // kernels of this library enqueued by the last hot call
   unsigned long long* d_counts = nullptr;    // [SYN_COUNTS] path counters of stage (b), zeroed at the start of every call
@@ -294,10 +294,13 @@ int run_synth(emri_plan* p, int k0, int K, double* outI, double* outII, int64_t 
   while (ut > 1 && (int64_t)K * ((a.tiles_per_walker + ut - 1) / ut) < (int64_t)8 * p->synth_grid) ut >>= 1;
   if (p->unit_tiles_override > 0) ut = p->unit_tiles_override;
   a.unit_tiles = ut;
+  a.unit_tiles_cap = p->unit_tiles_cap;
   a.units_per_walker = (a.tiles_per_walker + ut - 1) / ut;
   int64_t total = (int64_t)K * a.units_per_walker;
   int grid = (int)std::min<int64_t>(total, p->synth_grid);
-  synth_kernel<<<grid, SYNTH_BLOCK, p->synth_smem, s>>>(a);
+  // S >= 256: every tile lies inside one coarse interval and the producer warp stages its cubics (the default)
+  if (p->S >= TILE) synth_kernel<true><<<grid, SYNTH_BLOCK, p->synth_smem, s>>>(a);
+  else synth_kernel<false><<<grid, SYNTH_BLOCK, p->synth_smem, s>>>(a);
   p->launches += 1;
   CK(cudaGetLastError());
   return EMRI_OK;
@@ -398,15 +401,18 @@ int emri_plan_create(emri_plan** out, int64_t N, double dt, int n_max, int K_max
     return fail(EMRI_ECUDA);
 
   // persistent grid for the synthesis kernel: resident CTAs per SM x SM count
-  p->synth_smem = (size_t)2 * (n_max + 1) * MLOC * sizeof(double4) + (size_t)SC_TAB * sizeof(double2) +
-                  (size_t)6 * 2 * SYNTH_THREADS * sizeof(double) + (size_t)2 * (WC_STRIDE + 2 * UNIT_TILES_MAX) * sizeof(double);
   if (const char* ev = std::getenv("EMRI_UNIT_TILES")) p->unit_tiles_override = std::max(1, std::min(UNIT_TILES_MAX, std::atoi(ev)));
-  if (cudaFuncSetAttribute(synth_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)p->synth_smem) != cudaSuccess)
+  p->unit_tiles_cap = std::max(UNIT_TILES_MAX / 2, p->unit_tiles_override);
+  p->synth_smem = synth_smem_doubles(n_max, p->unit_tiles_cap) * sizeof(double);
+  if (cudaFuncSetAttribute(synth_kernel<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)p->synth_smem) != cudaSuccess ||
+      cudaFuncSetAttribute(synth_kernel<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)p->synth_smem) != cudaSuccess)
     return fail(EMRI_ECUDA);
-  int per_sm = 0;
-  if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, synth_kernel, SYNTH_BLOCK, p->synth_smem) != cudaSuccess ||
-      per_sm < 1)
+  int per_sm = 0, per_sm_direct = 0;
+  if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, synth_kernel<true>, SYNTH_BLOCK, p->synth_smem) != cudaSuccess ||
+      cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm_direct, synth_kernel<false>, SYNTH_BLOCK, p->synth_smem) != cudaSuccess ||
+      per_sm < 1 || per_sm_direct < 1)
     return fail(EMRI_ECUDA);
+  per_sm = std::min(per_sm, per_sm_direct);
   p->synth_grid = per_sm * p->sm_count;
   if (cudaStreamCreateWithFlags(&p->s_copy, cudaStreamNonBlocking) != cudaSuccess ||
       cudaEventCreateWithFlags(&p->ev_call, cudaEventDisableTiming) != cudaSuccess ||

@@ -29,7 +29,10 @@ constexpr int SYNTH_THREADS = 128;        // consumer threads per CTA
 constexpr int SYNTH_BLOCK = SYNTH_THREADS + 32;   // + one producer warp
 constexpr int TILE = 2 * SYNTH_THREADS;   // samples per tile (2 adjacent samples per thread)
 constexpr int UNIT_TILES_MAX = 16;        // tiles per unit (one re-expansion per unit), chosen per launch
-constexpr int MLOC = 9;                   // local expansion orders 0..8
+constexpr int MLOC = 9;                   // local expansion orders 0..8 are computed ...
+constexpr int MKEEP = 6;                  // ... and a unit keeps at most 6 of them (more: base-series fallback)
+constexpr int HREC = 28;                  // doubles per harmonic record of the local table: orders 8..0 x {PA, PB, PC} + 1 pad
+constexpr int HERM = 24;                  // doubles per staged interval record (cubics of the 5 orbit functions + amplitude data)
 #ifndef SYNTH_MINBLOCKS
 #define SYNTH_MINBLOCKS 4
 #endif
@@ -52,7 +55,7 @@ struct SynthArgs {
   double* outII;
   int64_t pitch;
   double2* outZ;           // interleaved z = h_I + i h_II, row of walker k0+i at outZ + i*N
-  int unit_tiles;
+  int unit_tiles, unit_tiles_cap;   // tiles per unit of this launch; the plan's maximum (sizes the staging area)
   int64_t tiles_per_walker, units_per_walker;
   double tol;              // relative truncation of the harmonic series
   double cbrt_thr;         // |nu/nu_j - 1| above which the amplitude takes the cube root (4e-3; < 0 forces the branch)
@@ -60,25 +63,31 @@ struct SynthArgs {
   unsigned long long* counts;   // [SYN_COUNTS] path counters of the call (emri_plan_synth_report)
 };
 
-// counters: [0] units, [1..8] units by local order Mu, [9] units on the base-series fallback, [10] samples whose
-// amplitude took the cube-root branch, [11] units of walkers with a fatal status (zero-filled)
+// counters: [0] units, [1..8] units by local order of their first harmonic range, [9] units on the base-series fallback,
+// [10] samples whose amplitude took the cube-root branch, [11] units of walkers with a fatal status (zero-filled),
+// [12] sum over units of the harmonics evaluated (n2), [13] of those in the first range (n1), [14] sum of the second
+// range's order
 constexpr int SYN_COUNTS = 16;
-enum { SYC_UNITS = 0, SYC_BASE = 9, SYC_CBRT = 10, SYC_SKIP = 11 };
+enum { SYC_UNITS = 0, SYC_BASE = 9, SYC_CBRT = 10, SYC_SKIP = 11, SYC_NEVAL = 12, SYC_NFIRST = 13, SYC_M2 = 14 };
 
-constexpr int SC_TAB = 1024;              // entries of the shared cos/sin table (one per 1/1024 cycle)
+constexpr int SC_TAB = 128;               // entries of the shared cos/sin table (one per 1/128 cycle)
+constexpr int SC_REP = 8;                 // replicas of every entry, one per lane & 7
 
 // cos/sin(2 pi x) for x in cycles (|x| < 2^40): nearest table angle (round-to-nearest by the 1.5*2^52 trick, so the
-// remainder is exact) and a Taylor rotation by the remainder |z| <= pi/1024 (sin to z^5, cos to z^4: < 2e-18).
-DEVINL void sincos_cycles(const double2* __restrict__ tab, double x, double& sn, double& cs) {
+// remainder is exact) and a Taylor rotation by the remainder |z| <= pi/128 (sin to z^7, cos to z^6: < 4e-18).
+// The table is replicated 8 times, entry k of replica r at double2 index 8 k + r, and lane l reads replica l & 7: the
+// eight lanes of a quarter-warp then always hit eight different 16-byte bank groups, so the 128-bit lookup takes its
+// minimum of four wavefronts whatever the angles are (the single 1024-entry table cost ~9).
+DEVINL void sincos_cycles(const double2* __restrict__ tab_lane, double x, double& sn, double& cs) {
   const double magic = 6755399441055744.0;
   const double t = fma(x, (double)SC_TAB, magic);
   const int k = __double2loint(t) & (SC_TAB - 1);
   const double r = fma(x, (double)SC_TAB, -(t - magic));
   const double z = r * (kTwoPi / SC_TAB);
   const double z2 = z * z;
-  const double sz = fma(z * z2, fma(z2, 1.0 / 120.0, -1.0 / 6.0), z);
-  const double cz = fma(z2, fma(z2, 1.0 / 24.0, -0.5), 1.0);
-  const double2 e = tab[k];
+  const double sz = fma(z * z2, fma(z2, fma(z2, -1.0 / 5040.0, 1.0 / 120.0), -1.0 / 6.0), z);
+  const double cz = fma(z2, fma(z2, fma(z2, -1.0 / 720.0, 1.0 / 24.0), -0.5), 1.0);
+  const double2 e = tab_lane[k * SC_REP];
   cs = fma(e.x, cz, -e.y * sz);
   sn = fma(e.y, cz, e.x * sz);
 }
@@ -96,18 +105,21 @@ struct SampleOut {
   double x, ec, es, C2, S2;     // w - w0;  e cos/sin(Phi_tot);  cos/sin(2 Phi_tot)
 };
 
-// Everything of sample i that does not depend on the harmonic index.  (cpb, spb) = cos/sin of the detector phase
-// phibar = 2 pi t_i / T_yr.  fin[0..5] (stride fs) receive a_I, b_I, c_I, a_II, b_II, c_II.
-DEVINL void sample_setup(const double* __restrict__ w, const double2* __restrict__ sct, const double* __restrict__ nodes,
-                         const double2* __restrict__ aux, int64_t i, int S, int logS, double invS, double Delta, int32_t jpl, double cpb, double spb,
-                         double w0, double cbrt_thr, unsigned long long* __restrict__ counts, SampleOut& o,
-                         double* __restrict__ fin, int fs) {
-  // source-time split (reading D4)
+// Orbit functions of one sample (S4): cubic Hermite of (Phi_c, nu, gam_c, e, alp_c) at the source time, and the data of
+// the amplitude series.
+struct OrbitAt {
+  double Phic, nu, dnu, gamc, e, alpc;
+  double Aj, inv_nuj, amp;      // amplitude at the interval's first node (0 when the interval is past plunge), 1/nu_j, mu/(Xi D)
+};
+
+// Direct path (S < 256: a tile spans several coarse intervals): integer time split (reading D4), the two node rows from
+// global memory (L1-resident, uniform over most of the warp), Hermite basis.
+DEVINL void orbit_at_direct(const double* __restrict__ w, const double* __restrict__ nodes, const double2* __restrict__ aux,
+                            int64_t i, int S, int logS, double invS, double Delta, int32_t jpl, OrbitAt& o) {
   int64_t j = i >> logS;
   double s = (double)(i & (S - 1)) * invS - w[WC_SIGMA];
   if (s < 0.0) { s += 1.0; j -= 1; } else if (s >= 1.0) { s -= 1.0; j += 1; }
   const bool live = (j + 1 < (int64_t)jpl);
-  // cubic Hermite of (Phi_c, nu, gam_c, e, alp_c) on interval j (rows j+1, j+2)
   const double2* r0 = reinterpret_cast<const double2*>(nodes + (j + 1) * NODE_STRIDE);
   const double2* r1 = r0 + NODE_STRIDE / 2;
   const double2 v01 = __ldg(r0), v23 = __ldg(r0 + 1), v4m0 = __ldg(r0 + 2), m12 = __ldg(r0 + 3), m34 = __ldg(r0 + 4),
@@ -117,23 +129,50 @@ DEVINL void sample_setup(const double* __restrict__ w, const double2* __restrict
   const double s2 = s * s, s3 = s2 * s;
   const double hb = fma(-2.0, s3, 3.0 * s2);
   const double h0 = Delta * (s3 - 2.0 * s2 + s), h1 = Delta * (s3 - s2);
-  const double Phic = v01.x + fma(hb, d01.x, fma(h0, v4m0.y, h1 * n4m0.y));
-  const double dnu = fma(hb, d01.y, fma(h0, m12.x, h1 * n12.x));
-  const double nu = v01.y + dnu;
-  const double gamc = v23.x + fma(hb, d23.x, fma(h0, m12.y, h1 * n12.y));
-  const double e = v23.y + fma(hb, d23.y, fma(h0, m34.x, h1 * n34.x));
-  const double alpc = v4m0.x + fma(hb, d4.x, fma(h0, m34.y, h1 * n34.y));
+  o.Phic = v01.x + fma(hb, d01.x, fma(h0, v4m0.y, h1 * n4m0.y));
+  o.dnu = fma(hb, d01.y, fma(h0, m12.x, h1 * n12.x));
+  o.nu = v01.y + o.dnu;
+  o.gamc = v23.x + fma(hb, d23.x, fma(h0, m12.y, h1 * n12.y));
+  o.e = v23.y + fma(hb, d23.y, fma(h0, m34.x, h1 * n34.x));
+  o.alpc = v4m0.x + fma(hb, d4.x, fma(h0, m34.y, h1 * n34.y));
+  o.Aj = live ? ax.x : 0.0; o.inv_nuj = ax.y; o.amp = live ? w[WC_AMP] : 0.0;
+}
+
+// Staged path (S >= 256, the default): the producer warp has turned the (at most two) coarse intervals a tile touches
+// into cubics in s, y(s) = c0 + s (c1 + s (c2 + s c3)), in shared memory (stage_intervals).  `loc_s` = (i mod S)/S.
+DEVINL void orbit_at_staged(const double* __restrict__ w, const double2* __restrict__ herm, double loc_s, OrbitAt& o) {
+  double s = loc_s - w[WC_SIGMA];
+  int sel = 0;
+  if (s < 0.0) { s += 1.0; sel = HERM / 2; } else if (s >= 1.0) { s -= 1.0; sel = HERM / 2; }
+  const double2* h = herm + sel;
+  const double2 p01 = h[0], p23 = h[1], n01 = h[2], n23 = h[3], g01 = h[4], g23 = h[5], e01 = h[6], e23 = h[7],
+                a01 = h[8], a23 = h[9], ax = h[10];
+  o.Phic = fma(s, fma(s, fma(s, p23.y, p23.x), p01.y), p01.x);
+  o.dnu = s * fma(s, fma(s, n23.y, n23.x), n01.y);
+  o.nu = n01.x + o.dnu;
+  o.gamc = fma(s, fma(s, fma(s, g23.y, g23.x), g01.y), g01.x);
+  o.e = fma(s, fma(s, fma(s, e23.y, e23.x), e01.y), e01.x);
+  o.alpc = fma(s, fma(s, fma(s, a23.y, a23.x), a01.y), a01.x);
+  o.Aj = ax.x; o.inv_nuj = ax.y; o.amp = reinterpret_cast<const double*>(h)[22];
+}
+
+// Everything of a sample that does not depend on the harmonic index.  (cpb, spb) = cos/sin of the detector phase
+// phibar = 2 pi t_i / T_yr.  fin[0..5] (stride fs) receive a_I, b_I, c_I, a_II, b_II, c_II.
+DEVINL void sample_setup(const double* __restrict__ w, const double2* __restrict__ sct, const OrbitAt& ob, double cpb, double spb,
+                         double w0, double cbrt_thr, unsigned long long* __restrict__ counts, SampleOut& o,
+                         double* __restrict__ fin, int fs) {
+  const double Phic = ob.Phic, nu = ob.nu, gamc = ob.gamc, e = ob.e, alpc = ob.alpc;
   // amplitude A = (2 pi M nu)^{2/3} mu / (Xi D)  (BC 10 with Eqs. 4-6 folded in): Taylor of (1+d)^{2/3} about the
   // node value, d = (nu - nu_j)/nu_j; remainder 0.014 d^6 < 6e-17 for |d| <= 4e-3, else the cube root itself
   double A;
   {
-    const double d = dnu * ax.y;
+    const double d = ob.dnu * ob.inv_nuj;
     if (fabs(d) <= cbrt_thr) {
       const double p = fma(d, fma(d, fma(d, fma(d, 14.0 / 729.0, -7.0 / 243.0), 4.0 / 81.0), -1.0 / 9.0), 2.0 / 3.0);
-      A = fma(ax.x * d, p, ax.x);
+      A = fma(ob.Aj * d, p, ob.Aj);
     } else {
       const double cb = cbrt(w[WC_TWOPIMS] * nu);
-      A = cb * cb * w[WC_AMP];
+      A = cb * cb * ob.amp;
       atomicAdd(counts + SYC_CBRT, 1ULL);          // rare branch (counted for emri_plan_synth_report)
     }
   }
@@ -183,7 +222,7 @@ DEVINL void sample_setup(const double* __restrict__ w, const double2* __restrict
   // h_alpha = (sqrt3/2)(F+ A+ + Fx Ax) with A+ = A{(1+Ln^2)(c2g Sa - s2g sq Sb) + 2(1-Ln^2) Sc},
   // Ax = -2 A Ln (sq Sb c2g + Sa s2g)   (BC 7-9, 14 summed over n)  =>  h = a Sa + b Sb + c Sc
   const double sq = sqrt(fma(-e, e, 1.0));
-  const double kA = live ? kHalfSqrt3 * A : 0.0;
+  const double kA = kHalfSqrt3 * A;               // A is 0 past plunge (reading R8)
   const double Ln2 = Ln * Ln;
   const double P1 = kA * (1.0 + Ln2), P2 = 2.0 * kA * Ln, P3 = 2.0 * kA * (1.0 - Ln2);
   const double t1 = P1 * c2g, t2 = P2 * s2g, t3 = P1 * s2g, t4 = P2 * c2g;
@@ -207,18 +246,17 @@ DEVINL double4 ldg4(const double4* p) {
   return make_double4(lo.x, lo.y, hi.x, hi.y);
 }
 
-// Harmonic sum n = 1..n_max for the thread's two samples; returns S_a, S_b, S_c of each.  Coefficients are
-// warp-uniform.  Local version: M orders of the re-expanded series (compile-time M: fully unrolled Horner, the
-// coefficient loads of the next harmonic can be hoisted above the arithmetic of the current one).
+// ---- harmonic sum n = 1..n_max for the thread's two samples; returns S_a, S_b, S_c of each.
 #define EMRI_FMA(d, a, b, c) asm volatile("fma.rn.f64 %0, %1, %2, %3;" : "=d"(d) : "d"(a), "d"(b), "d"(c))
 #define EMRI_MUL(d, a, b) asm volatile("mul.rn.f64 %0, %1, %2;" : "=d"(d) : "d"(a), "d"(b))
+#define EMRI_LDS2(lo, hi, addr) asm volatile("ld.shared.v2.f64 {%0, %1}, [%2];" : "=d"(lo), "=d"(hi) : "r"(addr))
 #define EMRI_ACCUM_FIRST()                                                                       \
   double SaA = p[0] * A.ec, SbA = p[1] * A.es, ScA = p[2] * A.ec;                                \
   double SaB = p[3] * B.ec, SbB = p[4] * B.es, ScB = p[5] * B.ec;                                \
   double CA = A.C2, SA = A.S2, CB = B.C2, SB = B.S2;
 #define EMRI_ACCUM_NEXT()                                                                        \
   {                                                                                              \
-    /* issue order chosen so that consecutive instructions share an operand slot (see series_local) */ \
+    /* issue order chosen so that consecutive instructions share an operand slot (see horner_step) */ \
     double ta, ua, tb, ub;                                                                       \
     EMRI_FMA(SaA, p[0], CA, SaA); EMRI_FMA(ScA, p[2], CA, ScA); EMRI_FMA(SbA, p[1], SA, SbA);    \
     EMRI_MUL(ta, SA, A.es); EMRI_MUL(ua, CA, A.es);                                              \
@@ -228,37 +266,93 @@ DEVINL double4 ldg4(const double4* p) {
     EMRI_FMA(CB, CB, B.ec, -tb); EMRI_FMA(SB, SB, B.ec, ub);                                     \
   }
 
-// The six Horner chains of one harmonic (2 samples x 3 series) are issued in an order in which every consecutive
-// pair of DFMAs shares one operand in the same slot -- A_a, B_a (coefficient a), B_b (x_B), A_b (coefficient b), A_c (x_A),
-// B_c (coefficient c) -- so that the operand-reuse cache feeds it and each DFMA reads two fresh registers, not three.
-// Measured on B200 (section 7 of DESIGN.md): 28.9 TFLOP/s for this pattern against 20.9 in the compiler's own order.
-// `asm volatile` pins the order.
+// Local table (shared memory): record n holds the re-expanded series of harmonic n, orders 8..0, {PA, PB, PC} each:
+// coefficient (order m, series s) at double 3 (MLOC-1-m) + s of the record.  A thread that keeps M orders streams the
+// LAST 3 M doubles of a record, in the order the Horner evaluation consumes them, as 128-bit loads from the aligned
+// address below its first coefficient (LEAD = 1: the first double loaded is the tail of order M, unused).
 template <int M>
-DEVINL void series_local(const double4* __restrict__ t, double xa, double xb, double p[6]) {
-  double4 c = t[M - 1];
-  p[0] = c.x; p[1] = c.y; p[2] = c.z; p[3] = c.x; p[4] = c.y; p[5] = c.z;
-#pragma unroll
-  for (int m = M - 2; m >= 0; --m) {
-    c = t[m];
-    EMRI_FMA(p[0], p[0], xa, c.x); EMRI_FMA(p[3], p[3], xb, c.x);
-    EMRI_FMA(p[4], p[4], xb, c.y); EMRI_FMA(p[1], p[1], xa, c.y);
-    EMRI_FMA(p[2], p[2], xa, c.z); EMRI_FMA(p[5], p[5], xb, c.z);
-  }
-}
+struct CoefStream {
+  static constexpr int OFF = 3 * (MLOC - M);
+  static constexpr int LEAD = OFF & 1;
+  static constexpr int BASE = OFF - LEAD;
+  static constexpr int NCH = (3 * M + LEAD + 1) / 2;       // 128-bit chunks per harmonic
+};
 
-template <int M>
-DEVINL void harmonic_sum_local(const double4* __restrict__ tab, int n_max, const SampleOut& A, const SampleOut& B,
-                               double out[6]) {
+// One harmonic: the six Horner chains (2 samples x 3 series), the accumulation, the scaled rotation -- and the coefficient
+// loads of the NEXT harmonic, each 128-bit chunk re-issued as soon as the Horner step that consumed its last double has
+// been issued, so that a load has the rest of the harmonic (>= 20 FP64 instructions of this warp alone) to land and the
+// loop never waits on shared memory.  `asm volatile` pins this order (ptxas keeps it).
+// The Horner chains are issued so that every consecutive pair of DFMAs shares one operand in the same slot -- A_a, B_a
+// (coefficient a), B_b, A_b (coefficient b), A_c, B_c (coefficient c) -- which the operand-reuse cache turns into two
+// fresh register reads per DFMA instead of three (28.9 against 20.9 TFLOP/s).
+template <int M, bool FIRST>
+DEVINL void harmonic_step(double (&v)[2 * CoefStream<M>::NCH], unsigned nxt, const SampleOut& A, const SampleOut& B,
+                          double& SaA, double& SbA, double& ScA, double& SaB, double& SbB, double& ScB,
+                          double& CA, double& SA, double& CB, double& SB) {
+  using CS = CoefStream<M>;
+  constexpr int L = CS::LEAD;
   double p[6];
-  // n = 1: carrier e (cos, sin)(Phi);  n >= 2: carrier e^{n-2} (cos, sin)(n Phi), advanced by the scaled rotation
-  series_local<M>(tab + MLOC, A.x, B.x, p);
-  EMRI_ACCUM_FIRST()
-#pragma unroll 2
-  for (int n = 2; n <= n_max; ++n) {
-    series_local<M>(tab + n * MLOC, A.x, B.x, p);
+  int reloaded = 0;                 // compile-time after unrolling
+  if (M == 1) {
+    p[0] = v[L]; p[1] = v[L + 1]; p[2] = v[L + 2]; p[3] = v[L]; p[4] = v[L + 1]; p[5] = v[L + 2];
+  } else {
+#pragma unroll
+    for (int k = 1; k < M; ++k) {
+      const int hi = L + 3 * (k - 1), lo = L + 3 * k;
+      if (k == 1) {
+        EMRI_FMA(p[0], v[hi], A.x, v[lo]); EMRI_FMA(p[3], v[hi], B.x, v[lo]);
+        EMRI_FMA(p[4], v[hi + 1], B.x, v[lo + 1]); EMRI_FMA(p[1], v[hi + 1], A.x, v[lo + 1]);
+        EMRI_FMA(p[2], v[hi + 2], A.x, v[lo + 2]); EMRI_FMA(p[5], v[hi + 2], B.x, v[lo + 2]);
+      } else {
+        EMRI_FMA(p[0], p[0], A.x, v[lo]); EMRI_FMA(p[3], p[3], B.x, v[lo]);
+        EMRI_FMA(p[4], p[4], B.x, v[lo + 1]); EMRI_FMA(p[1], p[1], A.x, v[lo + 1]);
+        EMRI_FMA(p[2], p[2], A.x, v[lo + 2]); EMRI_FMA(p[5], p[5], B.x, v[lo + 2]);
+      }
+      const int freed = (lo + 3) / 2 < CS::NCH ? (lo + 3) / 2 : CS::NCH;     // chunks whose doubles are all consumed
+#pragma unroll
+      for (int j = 0; j < CS::NCH; ++j)
+        if (j >= reloaded && j < freed) EMRI_LDS2(v[2 * j], v[2 * j + 1], nxt + (unsigned)((CS::BASE + 2 * j) * 8));
+      reloaded = freed > reloaded ? freed : reloaded;
+    }
+  }
+  if (FIRST) {
+    // n = 1: carrier e (cos, sin)(Phi)
+    SaA = p[0] * A.ec; SbA = p[1] * A.es; ScA = p[2] * A.ec;
+    SaB = p[3] * B.ec; SbB = p[4] * B.es; ScB = p[5] * B.ec;
+    CA = A.C2; SA = A.S2; CB = B.C2; SB = B.S2;
+  } else {
+    // n >= 2: carrier e^{n-2} (cos, sin)(n Phi), advanced by the scaled rotation
     EMRI_ACCUM_NEXT()
   }
-  out[0] = SaA; out[1] = SbA; out[2] = ScA; out[3] = SaB; out[4] = SbB; out[5] = ScB;
+#pragma unroll
+  for (int j = 0; j < CS::NCH; ++j)
+    if (j >= reloaded) EMRI_LDS2(v[2 * j], v[2 * j + 1], nxt + (unsigned)((CS::BASE + 2 * j) * 8));
+}
+
+// carried between the two harmonic ranges of a unit
+struct HarmState {
+  double SaA, SbA, ScA, SaB, SbB, ScB, CA, SA, CB, SB;
+};
+
+// harmonics n_lo..n_hi (n_lo == 1 starts the sums) with M local orders
+template <int M>
+DEVINL void harmonic_range(unsigned tab, int n_lo, int n_hi, const SampleOut& A, const SampleOut& B, HarmState& h) {
+  using CS = CoefStream<M>;
+  double v[2 * CS::NCH];
+  unsigned rec = tab + (unsigned)(n_lo * HREC * 8);          // record of n_lo
+#pragma unroll
+  for (int j = 0; j < CS::NCH; ++j) EMRI_LDS2(v[2 * j], v[2 * j + 1], rec + (unsigned)((CS::BASE + 2 * j) * 8));
+  int n = n_lo;
+  if (n_lo == 1) {
+    rec += (unsigned)(HREC * 8);
+    harmonic_step<M, true>(v, rec, A, B, h.SaA, h.SbA, h.ScA, h.SaB, h.SbB, h.ScB, h.CA, h.SA, h.CB, h.SB);
+    n = 2;
+  }
+#pragma unroll 1
+  for (; n <= n_hi; ++n) {
+    rec += (unsigned)(HREC * 8);                             // the table has n_max + 2 records: the last prefetch stays inside
+    harmonic_step<M, false>(v, rec, A, B, h.SaA, h.SbA, h.ScA, h.SaB, h.SbB, h.ScB, h.CA, h.SA, h.CB, h.SB);
+  }
 }
 
 // Fallback version: the base series in w = e^2 straight from the global table, Mn[n] terms (rare, slow path)
@@ -287,10 +381,10 @@ __device__ __noinline__ void harmonic_sum_base(const double4* __restrict__ base,
 // ---- per-unit tables, prepared by the producer warp one unit ahead of the consumers (double-buffered)
 struct UnitMeta {
   double w0e;         // expansion point subtracted from e^2 (0 on the fallback path)
-  int Mu;             // local orders kept (maximum over the harmonics); >= MLOC: fallback to the base series
+  int M1, M2;         // local orders kept for harmonics 1..n1 and n1+1..n2; M1 >= MLOC: fallback to the base series
+  int n1, n2;         // n2 <= n_max: harmonics above n2 are below the truncation threshold over the whole unit
   int skip;           // walker has a fatal status: the unit is zero-filled
   int32_t jpl;
-  int pad;
 };
 
 DEVINL double warp_max(double v) {
@@ -299,20 +393,62 @@ DEVINL double warp_max(double v) {
   return v;
 }
 
+// Staged path: the (at most two) coarse intervals each tile of the unit touches, as cubics in s (executed by ONE warp;
+// lane = 2 tile + slot).  Slot 0 is the interval the tile lies in, j0; slot 1 the neighbour the time shift sigma =
+// Delta T / Delta (|sigma| < 1, one sign per walker) reaches: j0 - 1 for sigma > 0, j0 + 1 otherwise.  From the Hermite
+// data (value y, increment d, end slopes m0, m1):  c0 = y, c1 = Delta m0, c2 = 3 d - Delta (2 m0 + m1),
+// c3 = Delta (m0 + m1) - 2 d.  Record: {c0..c3} x (Phi_c, nu, gam_c, e, alp_c), then A_j, 1/nu_j, mu/(Xi D), pad; the two
+// amplitude entries are 0 for an interval past plunge (reading R8: the samples are 0).
+DEVINL void stage_intervals(const SynthArgs& a, int lane, const double* __restrict__ nodes, const double2* __restrict__ aux,
+                            int64_t i_begin, int64_t i_end, double Delta, double sigma, double amp, int32_t jpl,
+                            double* __restrict__ herm) {
+  for (int task = lane; task < 2 * a.unit_tiles; task += 32) {
+    const int t = task >> 1, slot = task & 1;
+    const int64_t i0 = i_begin + (int64_t)t * TILE;
+    if (i0 >= i_end) continue;
+    const int64_t j = (i0 >> a.logS) + (slot ? (sigma > 0.0 ? -1 : 1) : 0);
+    const double2* r0 = reinterpret_cast<const double2*>(nodes + (j + 1) * NODE_STRIDE);
+    const double2* r1 = r0 + NODE_STRIDE / 2;
+    const double2 v01 = __ldg(r0), v23 = __ldg(r0 + 1), v4m0 = __ldg(r0 + 2), m12 = __ldg(r0 + 3), m34 = __ldg(r0 + 4),
+                  d01 = __ldg(r0 + 5), d23 = __ldg(r0 + 6), d4 = __ldg(r0 + 7);
+    const double2 n4m0 = __ldg(r1 + 2), n12 = __ldg(r1 + 3), n34 = __ldg(r1 + 4);
+    const double2 ax = __ldg(aux + (j + 1));
+    const bool live = (j + 1 < (int64_t)jpl);
+    const double y[5] = {v01.x, v01.y, v23.x, v23.y, v4m0.x};
+    const double d[5] = {d01.x, d01.y, d23.x, d23.y, d4.x};
+    const double m0[5] = {v4m0.y, m12.x, m12.y, m34.x, m34.y};
+    const double m1[5] = {n4m0.y, n12.x, n12.y, n34.x, n34.y};
+    double* rec = herm + (size_t)task * HERM;
+#pragma unroll
+    for (int q = 0; q < 5; ++q) {
+      rec[4 * q] = y[q];
+      rec[4 * q + 1] = Delta * m0[q];
+      rec[4 * q + 2] = fma(-Delta, fma(2.0, m0[q], m1[q]), 3.0 * d[q]);
+      rec[4 * q + 3] = fma(Delta, m0[q] + m1[q], -2.0 * d[q]);
+    }
+    rec[20] = live ? ax.x : 0.0; rec[21] = ax.y; rec[22] = live ? amp : 0.0; rec[23] = 0.0;
+  }
+}
+
 // Executed by ONE warp: everything of unit (k, i_begin..i_end) that is shared by its samples.
+template <bool STAGED>
 DEVINL void prepare_unit(const SynthArgs& a, int lane, int k, int64_t i_begin, int64_t i_end, double Delta, double inv_year,
-                         double4* __restrict__ tab, double* __restrict__ s_wc, double* __restrict__ s_rot,
-                         int* __restrict__ s_Mb, UnitMeta* __restrict__ meta) {
+                         double* __restrict__ tab, double* __restrict__ s_wc, double* __restrict__ s_rot,
+                         double* __restrict__ s_herm, int* __restrict__ s_Mb, int* __restrict__ s_Ml, UnitMeta* __restrict__ meta) {
   for (int q = lane; q < WC_STRIDE; q += 32) s_wc[q] = a.wc[(size_t)k * WC_STRIDE + q];
   for (int q = lane; q <= a.n_max; q += 32) s_Mb[q] = 1;
   const int32_t st = a.status[k];
   const bool skip = (st & (EMRI_ST_BADPARAM | EMRI_ST_DELAY | EMRI_ST_STATE)) != 0;
+  const int32_t jpl = a.jpl[k];
   if (lane == 0) {
-    meta->skip = skip ? 1 : 0; meta->jpl = a.jpl[k];
+    meta->skip = skip ? 1 : 0; meta->jpl = jpl;
     atomicAdd(a.counts + (skip ? SYC_SKIP : SYC_UNITS), 1ULL);
   }
   if (skip) return;
   const double* nodes = a.nodes + (size_t)k * a.Nn * NODE_STRIDE;
+  if (STAGED)
+    stage_intervals(a, lane, nodes, a.nodeaux + (size_t)k * a.Nn, i_begin, i_end, Delta, a.wc[(size_t)k * WC_STRIDE + WC_SIGMA],
+                    a.wc[(size_t)k * WC_STRIDE + WC_AMP], jpl, s_herm);
   // range of e over the unit from the node rows it touches (the Hermite cubic stays within pad of the nodes)
   int64_t rlo = (i_begin >> a.logS), rhi = ((i_end - 1) >> a.logS) + 3;       // rows = node index + 1
   if (rlo < 0) rlo = 0;
@@ -331,8 +467,11 @@ DEVINL void prepare_unit(const SynthArgs& a, int lane, int k, int64_t i_begin, i
   const double w0 = 0.5 * fma(elo, elo, whi);
   const double xmax = 0.5 * (whi - elo * elo) * (1.0 + 1e-9);
   __syncwarp();
-  // re-expansion of the three series of every harmonic about w0 (task = (harmonic, series))
-  int Mu = 1;
+  // re-expansion of the three series of every harmonic about w0 (task = (harmonic, series)); T0 = size of the leading
+  // term of the harmonic INCLUDING its carrier e^{n-2} (n = 1: e), at the unit's mid-point
+  const double ebar = sqrt(w0);
+  const double l2e_mid = log2(fmax(ebar, 1e-300)), l2e_hi = log2(fmax(ehi, 1e-300));
+  double scale = 0.0;
   for (int task = lane; task < 3 * a.n_max; task += 32) {
     const int n = task / 3 + 1, si = task - 3 * (n - 1);
     const double* bp = reinterpret_cast<const double*>(a.base + (size_t)n * BASE_M) + si;
@@ -358,29 +497,62 @@ DEVINL void prepare_unit(const SynthArgs& a, int lane, int k, int64_t i_begin, i
       for (int j = MLOC - 1; j >= 1; --j) d[j] = fma(d[j], w0, d[j - 1]);
       d[0] = fma(d[0], w0, c);
     }
-    int Ml = 1;
-    {
-      double pw = 1.0, mx = 0.0;
+    double* dst = tab + (size_t)n * HREC + si;
 #pragma unroll
-      for (int j = 0; j < MLOC; ++j) {
-        const double t = fabs(d[j]) * pw;
-        mx = fmax(mx, t);
-        if (t >= a.tol * mx && t > 0.0) Ml = j + 1;
-        pw *= xmax;
-      }
-    }
-    double* dst = reinterpret_cast<double*>(tab + (size_t)n * MLOC) + si;
-#pragma unroll
-    for (int j = 0; j < MLOC; ++j) dst[4 * j] = d[j];
-    Mu = max(Mu, Ml);                          // Ml == MLOC: order MLOC-1 still significant, the tail is not bounded
+    for (int j = 0; j < MLOC; ++j) dst[3 * (MLOC - 1 - j)] = d[j];
+    const int pc = (n == 1) ? 1 : n - 2;                 // power of e the harmonic's carrier holds
+    scale = fmax(scale, fabs(d[0]) * (pc ? exp2(l2e_mid * (double)pc) : 1.0));
     atomicMax(&s_Mb[n], Mb);
   }
+  scale = warp_max(scale);
+  for (int q = lane; q <= a.n_max; q += 32) s_Ml[q] = 0;
+  __syncwarp();
+  // Orders kept per harmonic: a term of the local series is kept while it is above thr = tol/4 of the LARGEST harmonic
+  // of the unit, carriers included -- a weak overtone needs fewer orders than its own relative accuracy would ask for,
+  // and an overtone whose leading term is below thr over the whole unit is not evaluated at all (reading D13: the sum
+  // of everything dropped stays below ~n_max tol / 4 of the signal, nine orders inside the 1e-9 parity tolerance)
+  const double thr = 0.25 * a.tol * scale;
+  for (int task = lane; task < 3 * a.n_max; task += 32) {
+    const int n = task / 3 + 1, si = task - 3 * (n - 1);
+    const int pc = (n == 1) ? 1 : n - 2;
+    const double car = pc ? exp2(l2e_hi * (double)pc) : 1.0;      // upper bound of the carrier over the unit
+    const double* src = tab + (size_t)n * HREC + si;
+    int Ml = 0;
+    double pw = car;
 #pragma unroll
-  for (int off = 16; off > 0; off >>= 1) Mu = max(Mu, __shfl_xor_sync(0xffffffffu, Mu, off));
-  if (a.force_base) Mu = MLOC;
+    for (int j = 0; j < MLOC; ++j) {
+      if (fabs(src[3 * (MLOC - 1 - j)]) * pw >= thr && thr > 0.0) Ml = j + 1;
+      pw *= xmax;
+    }
+    atomicMax(&s_Ml[n], Ml);                   // Ml == MLOC: order MLOC-1 still significant, the tail is not bounded
+  }
+  __syncwarp();
   if (lane == 0) {
-    meta->Mu = Mu; meta->w0e = (Mu >= MLOC) ? 0.0 : w0;
-    atomicAdd(a.counts + (Mu >= MLOC ? SYC_BASE : Mu), 1ULL);
+    // n2 = last harmonic with a term above thr (at least 2: the quadrupole of a circular orbit); split 1..n1 | n1+1..n2
+    // at the point that minimises the FP64 instructions per sample, 7 + 3 (M - 1) per harmonic
+    int n2 = min(2, a.n_max), Mall = 1;
+    for (int n = 1; n <= a.n_max; ++n) { if (s_Ml[n] > 0) n2 = max(n2, n); Mall = max(Mall, s_Ml[n]); }
+    int M1 = Mall, M2 = 1, n1 = n2;
+    if (Mall < MLOC) {
+      int best = n2 * (4 + 3 * Mall), sfx = 1, run = 0;
+      // suffix maxima on the fly: walk n1 downwards
+      for (int c = n2 - 1; c >= 1; --c) {
+        sfx = max(sfx, s_Ml[c + 1]);
+        run = 0;
+        for (int n = 1; n <= c; ++n) run = max(run, s_Ml[n]);
+        run = max(run, 1);
+        const int cost = c * (4 + 3 * run) + (n2 - c) * (4 + 3 * sfx) + 6;      // + the second range's prologue
+        if (cost < best) { best = cost; n1 = c; M1 = run; M2 = sfx; }
+      }
+    }
+    if (a.force_base || M1 > MKEEP) M1 = MLOC;
+    if (M1 >= MLOC) { n1 = n2 = a.n_max; M2 = 1; }
+    meta->M1 = M1; meta->M2 = M2; meta->n1 = n1; meta->n2 = n2;
+    meta->w0e = (M1 >= MLOC) ? 0.0 : w0;
+    atomicAdd(a.counts + (M1 >= MLOC ? SYC_BASE : M1), 1ULL);
+    atomicAdd(a.counts + SYC_NEVAL, (unsigned long long)n2);
+    atomicAdd(a.counts + SYC_NFIRST, (unsigned long long)n1);
+    atomicAdd(a.counts + SYC_M2, (unsigned long long)(n2 > n1 ? M2 : 0));
   }
   // detector phase at the start of each tile of the unit
   if (lane < a.unit_tiles) {
@@ -390,27 +562,43 @@ DEVINL void prepare_unit(const SynthArgs& a, int lane, int k, int64_t i_begin, i
   }
 }
 
+// Shared memory of one CTA, in doubles (the host sizes the launch with the same function)
+__host__ __device__ inline size_t synth_smem_doubles(int n_max, int unit_tiles_cap) {
+  return (size_t)2 * (n_max + 2) * HREC                 // local series, double-buffered
+         + (size_t)2 * SC_TAB * SC_REP                  // cos/sin table (double2), replicated
+         + (size_t)6 * 2 * SYNTH_THREADS                // the six per-sample coefficients, parked during the harmonic loop
+         + (size_t)2 * WC_STRIDE + (size_t)2 * 2 * UNIT_TILES_MAX
+         + (size_t)2 * 2 * unit_tiles_cap * HERM;       // staged interval cubics, double-buffered
+}
+
 // Consumers (warps 0..3): 2 adjacent samples per thread per tile.  Producer (warp 4): tables of the NEXT unit.
+// STAGED: S >= 256, every tile lies inside one coarse interval (the default); otherwise node rows are read per sample.
+template <bool STAGED>
 __global__ void __launch_bounds__(SYNTH_BLOCK, SYNTH_MINBLOCKS) synth_kernel(SynthArgs a) {
   extern __shared__ __align__(16) unsigned char smem_raw[];
-  const size_t tab_elems = (size_t)(a.n_max + 1) * MLOC;
-  double4* s_tab = reinterpret_cast<double4*>(smem_raw);                               // [2][(n_max+1)][MLOC]
-  double2* s_sct = reinterpret_cast<double2*>(s_tab + 2 * tab_elems);                  // [SC_TAB] {cos, sin}
-  double* s_fin = reinterpret_cast<double*>(s_sct + SC_TAB);                           // [6][2][SYNTH_THREADS]
+  const size_t tab_elems = (size_t)(a.n_max + 2) * HREC;
+  double* s_tab = reinterpret_cast<double*>(smem_raw);                                 // [2][n_max+2][HREC]
+  double2* s_sct = reinterpret_cast<double2*>(s_tab + 2 * tab_elems);                  // [SC_TAB][SC_REP] {cos, sin}
+  double* s_fin = reinterpret_cast<double*>(s_sct + SC_TAB * SC_REP);                  // [6][2][SYNTH_THREADS]
   double* s_wc = s_fin + 6 * 2 * SYNTH_THREADS;                                        // [2][WC_STRIDE]
   double* s_rot = s_wc + 2 * WC_STRIDE;                                                // [2][2 UNIT_TILES_MAX]
+  double* s_herm = s_rot + 2 * 2 * UNIT_TILES_MAX;                                     // [2][2 unit_tiles_cap][HERM]
   __shared__ int s_Mb[2][EMRI_NMAX_CAP + 1];  // base-series terms per harmonic (fallback path)
+  __shared__ int s_Ml[EMRI_NMAX_CAP + 1];     // local orders per harmonic (producer scratch)
   __shared__ UnitMeta s_meta[2];
+  const size_t herm_elems = (size_t)2 * a.unit_tiles_cap * HERM;
 
   const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
   const bool producer = warp == SYNTH_THREADS / 32;
   const double Delta = a.S * a.dt, invS = 1.0 / (double)a.S;
   const double inv_year = 1.0 / kYearSec;
-  for (int q = tid; q < SC_TAB; q += SYNTH_BLOCK) {
+  for (int q = tid; q < SC_TAB * SC_REP; q += SYNTH_BLOCK) {
     double sv, cv;
-    sincospi(2.0 * (double)q / (double)SC_TAB, &sv, &cv);
+    sincospi(2.0 * (double)(q / SC_REP) / (double)SC_TAB, &sv, &cv);
     s_sct[q] = make_double2(cv, sv);
   }
+  for (int q = tid; q < 2 * (int)tab_elems; q += SYNTH_BLOCK) s_tab[q] = 0.0;      // pads and the prefetch-only last record
+  const double2* sct_lane = s_sct + (lane & (SC_REP - 1));
   // detector phase of the thread's first sample relative to the tile start, and of one sample step
   double so, co, s1s, c1s;
   sincospi(2.0 * ((double)(2 * tid) * a.dt * inv_year), &so, &co);
@@ -424,24 +612,21 @@ __global__ void __launch_bounds__(SYNTH_BLOCK, SYNTH_MINBLOCKS) synth_kernel(Syn
     ib = ug * unit_len;
     ie = min(a.N, ib + unit_len);
   };
-  if (producer && (int64_t)blockIdx.x < total) {
-    int kl; int64_t ib, ie;
-    unit_of(blockIdx.x, kl, ib, ie);
-    prepare_unit(a, lane, a.k0 + kl, ib, ie, Delta, inv_year, s_tab, s_wc, s_rot, s_Mb[0], &s_meta[0]);
-  }
   __syncthreads();
-  int buf = 0;
-  for (int64_t u = blockIdx.x; u < total; u += gridDim.x, buf ^= 1) {
+  // One loop, one call site of prepare_unit (its code is inlined once): in the pass of unit u the producer prepares
+  // unit u + gridDim.x while the consumers work on u; the first pass (u = first - gridDim.x) only prepares.
+  int buf = 1;
+  for (int64_t u = (int64_t)blockIdx.x - gridDim.x; u < total; u += gridDim.x, buf ^= 1) {
     if (producer) {
       const int64_t un = u + gridDim.x;
       if (un < total) {
         int kl; int64_t ib, ie;
         unit_of(un, kl, ib, ie);
         const int nb = buf ^ 1;
-        prepare_unit(a, lane, a.k0 + kl, ib, ie, Delta, inv_year, s_tab + nb * tab_elems, s_wc + nb * WC_STRIDE,
-                     s_rot + nb * 2 * UNIT_TILES_MAX, s_Mb[nb], &s_meta[nb]);
+        prepare_unit<STAGED>(a, lane, a.k0 + kl, ib, ie, Delta, inv_year, s_tab + nb * tab_elems, s_wc + nb * WC_STRIDE,
+                             s_rot + nb * 2 * UNIT_TILES_MAX, s_herm + nb * herm_elems, s_Mb[nb], s_Ml, &s_meta[nb]);
       }
-    } else {
+    } else if (u >= 0) {
       int kl; int64_t i_begin, i_end;
       unit_of(u, kl, i_begin, i_end);
       const int k = a.k0 + kl;
@@ -459,9 +644,10 @@ __global__ void __launch_bounds__(SYNTH_BLOCK, SYNTH_MINBLOCKS) synth_kernel(Syn
       } else {
         const double* nodes = a.nodes + (size_t)k * a.Nn * NODE_STRIDE;
         const double2* aux = a.nodeaux + (size_t)k * a.Nn;
-        const double4* tab = s_tab + buf * tab_elems;
+        const unsigned tab = (unsigned)__cvta_generic_to_shared(s_tab + buf * tab_elems);
         const double* wc = s_wc + buf * WC_STRIDE;
         const double* rot = s_rot + buf * 2 * UNIT_TILES_MAX;
+        const double2* herm = reinterpret_cast<const double2*>(s_herm + buf * herm_elems);
         for (int t = 0; t < a.unit_tiles; ++t) {
           const int64_t i0 = i_begin + (int64_t)t * TILE + 2 * tid;
           if (i0 >= i_end) break;
@@ -471,21 +657,37 @@ __global__ void __launch_bounds__(SYNTH_BLOCK, SYNTH_MINBLOCKS) synth_kernel(Syn
           const double cpb2 = fma(cpa, c1s, -spa * s1s), spb2 = fma(spa, c1s, cpa * s1s);
           SampleOut A, B;
           double* fin = s_fin + tid;
-          sample_setup(wc, s_sct, nodes, aux, i0, a.S, a.logS, invS, Delta, mt.jpl, cpa, spa, mt.w0e, a.cbrt_thr, a.counts, A, fin,
-                       2 * SYNTH_THREADS);
-          sample_setup(wc, s_sct, nodes, aux, i0 + 1, a.S, a.logS, invS, Delta, mt.jpl, cpb2, spb2, mt.w0e, a.cbrt_thr, a.counts, B,
-                       fin + SYNTH_THREADS, 2 * SYNTH_THREADS);
+          {
+            OrbitAt oa;
+            if (STAGED) orbit_at_staged(wc, herm + (size_t)t * HERM, (double)(int)(i0 & (a.S - 1)) * invS, oa);
+            else orbit_at_direct(wc, nodes, aux, i0, a.S, a.logS, invS, Delta, mt.jpl, oa);
+            sample_setup(wc, sct_lane, oa, cpa, spa, mt.w0e, a.cbrt_thr, a.counts, A, fin, 2 * SYNTH_THREADS);
+          }
+          {
+            OrbitAt ob;
+            if (STAGED) orbit_at_staged(wc, herm + (size_t)t * HERM, (double)(int)((i0 + 1) & (a.S - 1)) * invS, ob);
+            else orbit_at_direct(wc, nodes, aux, i0 + 1, a.S, a.logS, invS, Delta, mt.jpl, ob);
+            sample_setup(wc, sct_lane, ob, cpb2, spb2, mt.w0e, a.cbrt_thr, a.counts, B, fin + SYNTH_THREADS, 2 * SYNTH_THREADS);
+          }
           double S[6];
-          switch (mt.Mu) {
-            case 1: harmonic_sum_local<1>(tab, a.n_max, A, B, S); break;
-            case 2: harmonic_sum_local<2>(tab, a.n_max, A, B, S); break;
-            case 3: harmonic_sum_local<3>(tab, a.n_max, A, B, S); break;
-            case 4: harmonic_sum_local<4>(tab, a.n_max, A, B, S); break;
-            case 5: harmonic_sum_local<5>(tab, a.n_max, A, B, S); break;
-            case 6: harmonic_sum_local<6>(tab, a.n_max, A, B, S); break;
-            case 7: harmonic_sum_local<7>(tab, a.n_max, A, B, S); break;
-            case 8: harmonic_sum_local<8>(tab, a.n_max, A, B, S); break;
-            default: harmonic_sum_base(a.base, s_Mb[buf], a.n_max, A, B, S); break;
+          if (mt.M1 >= MLOC) {
+            harmonic_sum_base(a.base, s_Mb[buf], a.n_max, A, B, S);
+          } else {
+            HarmState hs;
+#pragma unroll 1
+            for (int ph = 0; ph < 2; ++ph) {
+              const int lo = ph ? mt.n1 + 1 : 1, hi = ph ? mt.n2 : mt.n1;
+              if (lo > hi) break;
+              switch (ph ? mt.M2 : mt.M1) {
+                case 1: harmonic_range<1>(tab, lo, hi, A, B, hs); break;
+                case 2: harmonic_range<2>(tab, lo, hi, A, B, hs); break;
+                case 3: harmonic_range<3>(tab, lo, hi, A, B, hs); break;
+                case 4: harmonic_range<4>(tab, lo, hi, A, B, hs); break;
+                case 5: harmonic_range<5>(tab, lo, hi, A, B, hs); break;
+                default: harmonic_range<6>(tab, lo, hi, A, B, hs); break;
+              }
+            }
+            S[0] = hs.SaA; S[1] = hs.SbA; S[2] = hs.ScA; S[3] = hs.SaB; S[4] = hs.SbB; S[5] = hs.ScB;
           }
           const double hIa = fma(fin[0], S[0], fma(fin[2 * SYNTH_THREADS], S[1], fin[4 * SYNTH_THREADS] * S[2]));
           const double hIIa = fma(fin[6 * SYNTH_THREADS], S[0], fma(fin[8 * SYNTH_THREADS], S[1], fin[10 * SYNTH_THREADS] * S[2]));

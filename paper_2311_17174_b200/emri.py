@@ -149,7 +149,8 @@ class Plan:
         c = np.zeros(16, dtype=np.int64)
         self._check(self._L.emri_plan_synth_report(self._h, c.ctypes.data_as(C.c_void_p)))
         return dict(units=int(c[0]), by_order={m: int(c[m]) for m in range(1, 9)}, base_units=int(c[9]),
-                    cbrt_samples=int(c[10]), skipped_units=int(c[11]))
+                    cbrt_samples=int(c[10]), skipped_units=int(c[11]), harmonics_evaluated=int(c[12]),
+                    harmonics_first_range=int(c[13]), second_range_orders=int(c[14]))
 
     def set_synth_debug(self, force_base=False, force_cbrt=False):
         """test hook: force the data-selected slow paths of stage (b)"""

@@ -38,7 +38,16 @@ def subset_with_plungers(oracle, cfg, n=16):
     P = with_plunging_walkers(oracle, P, cfg, rows)
     if cfg.K <= n:
         return P, np.arange(cfg.K), rows
-    sub = [int(k) for k in W.parity_walker_subset(P, n=n) if k not in rows][:n - 3] + rows
+    # parity_walker_subset keeps the extremes and 0-3 whatever n is; ask for n - 3 and add the plungers
+    P_rest = P.copy()
+    sub = [int(k) for k in W.parity_walker_subset(P_rest, n=n - 3)]
+    extra = [r for r in rows if r not in sub]
+    sub = sub + extra
+    rng = np.random.default_rng(7)
+    while len(sub) < n:                      # a plunger row was already picked: top up with seeded draws
+        k = int(rng.integers(0, cfg.K))
+        if k not in sub:
+            sub.append(k)
     return P, np.array(sorted(sub)), rows
 
 

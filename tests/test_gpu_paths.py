@@ -35,6 +35,8 @@ def test_forced_slow_paths_match_oracle(emri, oracle, force_base, force_cbrt):
     cfg = W.scaled(W.CONFIGS[3], K=6, N=3 * 2048 + 300)          # several units and a ragged tail, n_max = 30
     P = W.draw_params(cfg)
     P[:, W.P_E0] = np.linspace(0.05, 0.5, cfg.K)
+    for k in range(cfg.K):
+        P[k, W.P_NU0] = W.nu0_for_plunge_after(P[k, W.P_M], P[k, W.P_MU], P[k, W.P_E0], 1000.0 * cfg.T_obs)
     h_ref, st_ref = oracle.waveform_batch(P, cfg.N, cfg.dt, cfg.n_max)
     assert not st_ref.any()
     plan = emri.Plan(cfg.N, cfg.dt, cfg.n_max, cfg.K)
