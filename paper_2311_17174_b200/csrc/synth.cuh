@@ -388,9 +388,17 @@ struct UnitMeta {
 };
 
 DEVINL double warp_max(double v) {
-#pragma unroll
+#pragma unroll 1
   for (int off = 16; off > 0; off >>= 1) v = fmax(v, __shfl_xor_sync(0xffffffffu, v, off));
   return v;
+}
+
+// x^k, k >= 0, by repeated squaring (a bound on a harmonic's carrier e^{n-2}: a few ulps do not matter)
+DEVINL double ipow(double x, int k) {
+  double r = 1.0;
+#pragma unroll 1
+  for (; k > 0; k >>= 1) { if (k & 1) r *= x; x *= x; }
+  return r;
 }
 
 // Staged path: the (at most two) coarse intervals each tile of the unit touches, as cubics in s (executed by ONE warp;
@@ -402,6 +410,7 @@ DEVINL double warp_max(double v) {
 DEVINL void stage_intervals(const SynthArgs& a, int lane, const double* __restrict__ nodes, const double2* __restrict__ aux,
                             int64_t i_begin, int64_t i_end, double Delta, double sigma, double amp, int32_t jpl,
                             double* __restrict__ herm) {
+#pragma unroll 1
   for (int task = lane; task < 2 * a.unit_tiles; task += 32) {
     const int t = task >> 1, slot = task & 1;
     const int64_t i0 = i_begin + (int64_t)t * TILE;
@@ -434,8 +443,11 @@ DEVINL void stage_intervals(const SynthArgs& a, int lane, const double* __restri
 template <bool STAGED>
 DEVINL void prepare_unit(const SynthArgs& a, int lane, int k, int64_t i_begin, int64_t i_end, double Delta, double inv_year,
                          double* __restrict__ tab, double* __restrict__ s_wc, double* __restrict__ s_rot,
-                         double* __restrict__ s_herm, int* __restrict__ s_Mb, int* __restrict__ s_Ml, UnitMeta* __restrict__ meta) {
+                         double* __restrict__ s_herm, int* __restrict__ s_Mb, int* __restrict__ s_Ml, const double2* __restrict__ sct_lane,
+                         UnitMeta* __restrict__ meta) {
+#pragma unroll 1
   for (int q = lane; q < WC_STRIDE; q += 32) s_wc[q] = a.wc[(size_t)k * WC_STRIDE + q];
+#pragma unroll 1
   for (int q = lane; q <= a.n_max; q += 32) s_Mb[q] = 1;
   const int32_t st = a.status[k];
   const bool skip = (st & (EMRI_ST_BADPARAM | EMRI_ST_DELAY | EMRI_ST_STATE)) != 0;
@@ -454,13 +466,18 @@ DEVINL void prepare_unit(const SynthArgs& a, int lane, int k, int64_t i_begin, i
   if (rlo < 0) rlo = 0;
   if (rhi > a.Nn - 1) rhi = a.Nn - 1;
   double v0 = 0.0, v1 = -1.0, v2 = 0.0, v3 = 0.0;       // max e, max -e, max |e'|, max |increment of e|
+#pragma unroll 1
   for (int64_t r = rlo + lane; r <= rhi; r += 32) {
     const double* row = nodes + r * NODE_STRIDE;
     const double ev = __ldg(row + 3);
     v0 = fmax(v0, ev); v1 = fmax(v1, -ev);
     v2 = fmax(v2, fabs(__ldg(row + 8))); v3 = fmax(v3, fabs(__ldg(row + 13)));
   }
-  v0 = warp_max(v0); v1 = warp_max(v1); v2 = warp_max(v2); v3 = warp_max(v3);
+#pragma unroll 1
+  for (int off = 16; off > 0; off >>= 1) {          // rolled: the producer's code must stay small (instruction cache)
+    v0 = fmax(v0, __shfl_xor_sync(0xffffffffu, v0, off)); v1 = fmax(v1, __shfl_xor_sync(0xffffffffu, v1, off));
+    v2 = fmax(v2, __shfl_xor_sync(0xffffffffu, v2, off)); v3 = fmax(v3, __shfl_xor_sync(0xffffffffu, v3, off));
+  }
   const double pad = 0.3 * fma(Delta, v2, v3) + 1e-15;
   const double elo = fmax(-v1 - pad, 0.0), ehi = v0 + pad;
   const double whi = ehi * ehi;
@@ -470,8 +487,8 @@ DEVINL void prepare_unit(const SynthArgs& a, int lane, int k, int64_t i_begin, i
   // re-expansion of the three series of every harmonic about w0 (task = (harmonic, series)); T0 = size of the leading
   // term of the harmonic INCLUDING its carrier e^{n-2} (n = 1: e), at the unit's mid-point
   const double ebar = sqrt(w0);
-  const double l2e_mid = log2(fmax(ebar, 1e-300)), l2e_hi = log2(fmax(ehi, 1e-300));
   double scale = 0.0;
+#pragma unroll 1
   for (int task = lane; task < 3 * a.n_max; task += 32) {
     const int n = task / 3 + 1, si = task - 3 * (n - 1);
     const double* bp = reinterpret_cast<const double*>(a.base + (size_t)n * BASE_M) + si;
@@ -480,6 +497,7 @@ DEVINL void prepare_unit(const SynthArgs& a, int lane, int k, int64_t i_begin, i
     {
       double pw = 1.0, mx = 0.0;
       int below = 0;
+#pragma unroll 1
       for (int m = 0; m < BASE_M; ++m) {
         const double t = fabs(__ldg(bp + 4 * m)) * pw;
         mx = fmax(mx, t);
@@ -491,6 +509,7 @@ DEVINL void prepare_unit(const SynthArgs& a, int lane, int k, int64_t i_begin, i
     double d[MLOC];
 #pragma unroll
     for (int j = 0; j < MLOC; ++j) d[j] = 0.0;
+#pragma unroll 1
     for (int m = Mb - 1; m >= 0; --m) {
       const double c = __ldg(bp + 4 * m);
 #pragma unroll
@@ -501,10 +520,11 @@ DEVINL void prepare_unit(const SynthArgs& a, int lane, int k, int64_t i_begin, i
 #pragma unroll
     for (int j = 0; j < MLOC; ++j) dst[3 * (MLOC - 1 - j)] = d[j];
     const int pc = (n == 1) ? 1 : n - 2;                 // power of e the harmonic's carrier holds
-    scale = fmax(scale, fabs(d[0]) * (pc ? exp2(l2e_mid * (double)pc) : 1.0));
+    scale = fmax(scale, fabs(d[0]) * ipow(ebar, pc));
     atomicMax(&s_Mb[n], Mb);
   }
   scale = warp_max(scale);
+#pragma unroll 1
   for (int q = lane; q <= a.n_max; q += 32) s_Ml[q] = 0;
   __syncwarp();
   // Orders kept per harmonic: a term of the local series is kept while it is above thr = tol/4 of the LARGEST harmonic
@@ -512,10 +532,11 @@ DEVINL void prepare_unit(const SynthArgs& a, int lane, int k, int64_t i_begin, i
   // and an overtone whose leading term is below thr over the whole unit is not evaluated at all (reading D13: the sum
   // of everything dropped stays below ~n_max tol / 4 of the signal, nine orders inside the 1e-9 parity tolerance)
   const double thr = 0.25 * a.tol * scale;
+#pragma unroll 1
   for (int task = lane; task < 3 * a.n_max; task += 32) {
     const int n = task / 3 + 1, si = task - 3 * (n - 1);
     const int pc = (n == 1) ? 1 : n - 2;
-    const double car = pc ? exp2(l2e_hi * (double)pc) : 1.0;      // upper bound of the carrier over the unit
+    const double car = ipow(ehi, pc);                  // upper bound of the carrier over the unit
     const double* src = tab + (size_t)n * HREC + si;
     int Ml = 0;
     double pw = car;
@@ -531,14 +552,17 @@ DEVINL void prepare_unit(const SynthArgs& a, int lane, int k, int64_t i_begin, i
     // n2 = last harmonic with a term above thr (at least 2: the quadrupole of a circular orbit); split 1..n1 | n1+1..n2
     // at the point that minimises the FP64 instructions per sample, 7 + 3 (M - 1) per harmonic
     int n2 = min(2, a.n_max), Mall = 1;
+#pragma unroll 1
     for (int n = 1; n <= a.n_max; ++n) { if (s_Ml[n] > 0) n2 = max(n2, n); Mall = max(Mall, s_Ml[n]); }
     int M1 = Mall, M2 = 1, n1 = n2;
     if (Mall < MLOC) {
       int best = n2 * (4 + 3 * Mall), sfx = 1, run = 0;
       // suffix maxima on the fly: walk n1 downwards
+#pragma unroll 1
       for (int c = n2 - 1; c >= 1; --c) {
         sfx = max(sfx, s_Ml[c + 1]);
         run = 0;
+#pragma unroll 1
         for (int n = 1; n <= c; ++n) run = max(run, s_Ml[n]);
         run = max(run, 1);
         const int cost = c * (4 + 3 * run) + (n2 - c) * (4 + 3 * sfx) + 6;      // + the second range's prologue
@@ -557,7 +581,7 @@ DEVINL void prepare_unit(const SynthArgs& a, int lane, int k, int64_t i_begin, i
   // detector phase at the start of each tile of the unit
   if (lane < a.unit_tiles) {
     double sb, cb;
-    sincospi(2.0 * frac((double)(i_begin + (int64_t)lane * TILE) * a.dt * inv_year), &sb, &cb);
+    sincos_cycles(sct_lane, (double)(i_begin + (int64_t)lane * TILE) * a.dt * inv_year, sb, cb);
     s_rot[2 * lane] = cb; s_rot[2 * lane + 1] = sb;
   }
 }
@@ -624,7 +648,7 @@ __global__ void __launch_bounds__(SYNTH_BLOCK, SYNTH_MINBLOCKS) synth_kernel(Syn
         unit_of(un, kl, ib, ie);
         const int nb = buf ^ 1;
         prepare_unit<STAGED>(a, lane, a.k0 + kl, ib, ie, Delta, inv_year, s_tab + nb * tab_elems, s_wc + nb * WC_STRIDE,
-                             s_rot + nb * 2 * UNIT_TILES_MAX, s_herm + nb * herm_elems, s_Mb[nb], s_Ml, &s_meta[nb]);
+                             s_rot + nb * 2 * UNIT_TILES_MAX, s_herm + nb * herm_elems, s_Mb[nb], s_Ml, sct_lane, &s_meta[nb]);
       }
     } else if (u >= 0) {
       int kl; int64_t i_begin, i_end;
