@@ -121,6 +121,16 @@ int emri_plan_orbit_report(emri_plan* p, int K, int32_t* modes);
  * Synchronises the device. */
 int emri_plan_synth_report(emri_plan* p, int64_t counts[16]);
 
+/* How emri_loglike runs stages (c)+(d).  1 (default where available: N a power of two, 2^16 <= N <= 2^22): fused -- the
+ * synthesis writes the chunk walker-interleaved, ONE strided batched cuFFT pass does the first factor of N = N1 N2, and a
+ * kernel of this library does the last pass (N2 <= 1024 points per row, in registers and shared memory) and feeds its
+ * outputs straight into Eq. 8, so the spectrum is never written back nor read again (DESIGN.md
+ * section 6c).  0: the full cuFFT transform followed by the streaming reduction kernel (also used for every other N and by
+ * emri_loglike_fdep).  Both give logL within the parity tolerance of each other (not bit-identical: the fused path
+ * evaluates Eq. 8 as <d|d> - 2<d|h> + <h|h>).  emri_plan_transform_is_fused reports what the next emri_loglike will do. */
+int emri_plan_set_transform(emri_plan* p, int fused);
+int emri_plan_transform_is_fused(const emri_plan* p);
+
 /* Test hook: force the data-selected slow paths of stage (b) for every later call.  flags bit 0: every unit evaluates
  * the base series in e^2; bit 1: every sample takes the cube-root amplitude.  0 restores the defaults.  Results must
  * not change beyond rounding (tests/test_gpu_paths.py). */

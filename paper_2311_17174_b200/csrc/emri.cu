@@ -29,6 +29,7 @@
 #include "orbit.cuh"
 #include "synth.cuh"
 #include "loglike.cuh"
+#include "fftlike.cuh"
 #include "stretch.cuh"
 
 // =================================================================== host side
@@ -66,6 +67,16 @@ struct emri_plan {
   // stretch move scratch
   double* d_Y = nullptr; double* d_z = nullptr; double* d_lnu = nullptr; double* d_logLY = nullptr;
   int32_t* d_inbox = nullptr; int32_t* d_partner = nullptr;
+  // fused transform + reduction (fftlike.cuh): N = N1 N2; available for N = 2^16 .. 2^22
+  bool fused_ok = false, fused_on = true;
+  int N1 = 0, N2 = 0, log2N1 = 0, log2N2 = 0, n_cd = 0;
+  double2* d_twid = nullptr;
+  double2* d_twA = nullptr;
+  double2* d_twB = nullptr;
+  double* d_alpha = nullptr;
+  double2* d_gamma = nullptr;
+  double* d_cdpart = nullptr;
+  std::map<int, cufftHandle> fftA;     // strided pass-A plans, by walkers in the chunk
   // cuFFT
   std::map<int, cufftHandle> fft;
   void* d_fftwork = nullptr;
@@ -179,6 +190,7 @@ int alloc_workspace(emri_plan* p) {
 }
 
 int get_fft(emri_plan* p, int batch, cufftHandle* out);
+int get_fftA(emri_plan* p, int kc, cufftHandle* out);
 
 // (Re)allocates the chunk buffer and creates, up front, every cuFFT plan the hot calls of a full ensemble need: a full
 // chunk, the ragged last chunk of K_max walkers, and the single transform of emri_data_fft.  The work area is sized by
@@ -189,10 +201,16 @@ int alloc_chunk(emri_plan* p) {
   if ((rc = dev_alloc(p, &p->d_hbuf, (size_t)2 * p->chunk * p->N))) return rc;      // z = h_I + i h_II, [chunk][N] complex
   for (auto& kv : p->fft) cufftDestroy(kv.second);
   p->fft.clear();
+  for (auto& kv : p->fftA) cufftDestroy(kv.second);
+  p->fftA.clear();
   cufftHandle h;
   if ((rc = get_fft(p, p->chunk, &h))) return rc;
   if (p->K_max % p->chunk) { if ((rc = get_fft(p, p->K_max % p->chunk, &h))) return rc; }
   if ((rc = get_fft(p, 1, &h))) return rc;
+  if (p->fused_ok) {
+    if ((rc = get_fftA(p, p->chunk, &h))) return rc;
+    if (p->K_max % p->chunk) { if ((rc = get_fftA(p, p->K_max % p->chunk, &h))) return rc; }
+  }
   return EMRI_OK;
 }
 
@@ -220,9 +238,41 @@ int get_fft(emri_plan* p, int batch, cufftHandle* out) {
     p->fftwork_bytes = ws;
     p->bytes += (int64_t)ws;
     for (auto& kv : p->fft) cufftSetWorkArea(kv.second, p->d_fftwork);
+    for (auto& kv : p->fftA) cufftSetWorkArea(kv.second, p->d_fftwork);
   }
   if (p->d_fftwork) CKF(cufftSetWorkArea(h, p->d_fftwork));
   p->fft[batch] = h;
+  *out = h;
+  return EMRI_OK;
+}
+
+// pass A of the fused path: N2 strided transforms of length N1 per walker on the walker-interleaved chunk z[i1][k][i2]
+int get_fftA(emri_plan* p, int kc, cufftHandle* out) {
+  auto it = p->fftA.find(kc);
+  if (it != p->fftA.end()) { *out = it->second; return EMRI_OK; }
+  cufftHandle h;
+  CKF(cufftCreate(&h));
+  CKF(cufftSetAutoAllocation(h, 0));
+  long long n[1] = {(long long)p->N1};
+  long long embed[1] = {(long long)p->N1};
+  const long long stride = (long long)kc * p->N2;
+  size_t ws = 0;
+  cufftResult r = cufftMakePlanMany64(h, 1, n, embed, stride, 1, embed, stride, 1, CUFFT_Z2Z, stride, &ws);
+  if (r != CUFFT_SUCCESS) { p->last_err = (int)r; cufftDestroy(h); return EMRI_ECUFFT; }
+  if (ws > p->fftwork_bytes) {
+    // reached from alloc_chunk only (the full chunk is planned first)
+    cudaError_t e = cudaDeviceSynchronize();
+    if (e != cudaSuccess) { p->last_err = (int)e; cufftDestroy(h); return EMRI_ECUDA; }
+    if (p->d_fftwork) { cudaFree(p->d_fftwork); p->bytes -= (int64_t)p->fftwork_bytes; p->d_fftwork = nullptr; }
+    e = cudaMalloc(&p->d_fftwork, ws);
+    if (e != cudaSuccess) { p->last_err = (int)e; p->fftwork_bytes = 0; cufftDestroy(h); cudaGetLastError(); return EMRI_ENOMEM; }
+    p->fftwork_bytes = ws;
+    p->bytes += (int64_t)ws;
+    for (auto& kv : p->fft) cufftSetWorkArea(kv.second, p->d_fftwork);
+    for (auto& kv : p->fftA) cufftSetWorkArea(kv.second, p->d_fftwork);
+  }
+  if (p->d_fftwork) CKF(cufftSetWorkArea(h, p->d_fftwork));
+  p->fftA[kc] = h;
   *out = h;
   return EMRI_OK;
 }
@@ -279,8 +329,10 @@ int run_orbit(emri_plan* p, const double* params, int K, cudaStream_t s) {
   return EMRI_OK;
 }
 
-int run_synth(emri_plan* p, int k0, int K, double* outI, double* outII, int64_t pitch, double* outZ, cudaStream_t s) {
+int run_synth(emri_plan* p, int k0, int K, double* outI, double* outII, int64_t pitch, double* outZ, cudaStream_t s,
+              bool interleaved = false) {
   SynthArgs a;
+  a.z_log2n2 = interleaved ? p->log2N2 : 0;
   a.wc = p->d_wc; a.nodes = p->d_nodes; a.nodeaux = p->d_nodeaux; a.jpl = p->d_jpl; a.status = p->d_status;
   a.base = p->d_base; a.tol = 1e-16;
   a.cbrt_thr = (p->synth_debug & 2) ? -1.0 : 4e-3;
@@ -327,6 +379,26 @@ int run_like(emri_plan* p, int k0, int K, const double* Z, const double* data_ff
   dim3 grid((unsigned)p->n_part, (unsigned)((K + LL_GROUP - 1) / LL_GROUP));
   if (fcoef) loglike_kernel<true><<<grid, LL_THREADS, 0, s>>>(a);
   else loglike_kernel<false><<<grid, LL_THREADS, 0, s>>>(a);
+  p->launches += 1;
+  CK(cudaGetLastError());
+  return EMRI_OK;
+}
+
+int run_fft_like(emri_plan* p, int k0, int kc, const double* Y, cudaStream_t s) {
+  FftLikeArgs a;
+  a.Y = reinterpret_cast<const double2*>(Y); a.twid = p->d_twid; a.twA = p->d_twA; a.twB = p->d_twB; a.alpha = p->d_alpha; a.gamma = p->d_gamma;
+  a.partial = p->d_partial; a.k0 = k0; a.K = kc; a.n_part = p->N1; a.N1 = p->N1; a.N = p->N;
+  const int rows = FB_ELEMS / p->N2;
+  const int64_t groups = ((int64_t)p->N1 * kc + rows - 1) / rows;
+  const int grid = (int)std::min<int64_t>(groups, (int64_t)p->sm_count * 2 * 8);
+  const size_t smem = ((size_t)256 + p->N2 + (size_t)rows * (p->N2 + p->N2 / 16)) * sizeof(double2);
+  switch (p->log2N2) {
+    case 8: fft_like_kernel<8><<<grid, FB_THREADS, smem, s>>>(a); break;
+    case 9: fft_like_kernel<9><<<grid, FB_THREADS, smem, s>>>(a); break;
+    case 10: fft_like_kernel<10><<<grid, FB_THREADS, smem, s>>>(a); break;
+    case 11: fft_like_kernel<11><<<grid, FB_THREADS, smem, s>>>(a); break;
+    default: fft_like_kernel<12><<<grid, FB_THREADS, smem, s>>>(a); break;
+  }
   p->launches += 1;
   CK(cudaGetLastError());
   return EMRI_OK;
@@ -381,7 +453,66 @@ int emri_plan_create(emri_plan** out, int64_t N, double dt, int n_max, int K_max
   if ((rc = dev_alloc(p, &p->d_plrow, (size_t)K_max * NODE_STRIDE))) return fail(rc);
   if ((rc = dev_alloc(p, &p->d_base, base.size()))) return fail(rc);
   p->n_part = (int)((p->Nf + LL_RANGE - 1) / LL_RANGE);
-  if ((rc = dev_alloc(p, &p->d_partial, (size_t)K_max * p->n_part))) return fail(rc);
+  // fused transform + reduction: N = 2^16 .. 2^22 = N1 N2 with N1 = clamp(N / 1024, 256, 1024) (1024: the length cuFFT's
+  // strided batched kernel runs best at -- 4 TB/s against 2.8 TB/s at 2048, measured on B200) and N2 = N / N1 in 256 .. 4096
+  std::vector<double2> twid;
+  if ((N & (N - 1)) == 0 && N >= (1 << 16) && N <= (1 << 22)) {
+    int lg = 0;
+    while (((int64_t)1 << lg) < N) ++lg;
+    p->log2N1 = std::max(8, std::min(10, lg - 10)); p->log2N2 = lg - p->log2N1;
+    p->N2 = 1 << p->log2N2; p->N1 = 1 << p->log2N1;
+    p->fused_ok = true;
+    p->n_cd = (int)((p->Nf + 255) / 256);
+    {
+      // stage twiddles of the last pass, transposed (fftlike.cuh): W_256^{k t} at [16 t + k], W_N2^{jj t} at [t NSL + jj]
+      const long double tp = -2.0L * 3.14159265358979323846264338327950288L;
+      const int nfull = (p->log2N2 - 1) / 4, RL = p->N2 >> (4 * nfull), NSL = p->N2 / RL;
+      twid.resize((size_t)256 + p->N2);
+      for (int t = 0; t < 16; ++t)
+        for (int k = 0; k < 16; ++k) {
+          const long double ang = tp * (long double)(k * t) / 256.0L;
+          twid[16 * t + k] = make_double2((double)cosl(ang), (double)sinl(ang));
+        }
+      for (int t = 0; t < RL; ++t)
+        for (int jj = 0; jj < NSL; ++jj) {
+          const long double ang = tp * (long double)(((int64_t)jj * t) % p->N2) / (long double)p->N2;
+          twid[256 + (size_t)t * NSL + jj] = make_double2((double)cosl(ang), (double)sinl(ang));
+        }
+    }
+    if ((rc = dev_alloc(p, &p->d_twid, twid.size()))) return fail(rc);
+    if ((rc = dev_alloc(p, &p->d_alpha, (size_t)N))) return fail(rc);
+    if ((rc = dev_alloc(p, &p->d_gamma, (size_t)N))) return fail(rc);
+    if ((rc = dev_alloc(p, &p->d_cdpart, (size_t)p->n_cd))) return fail(rc);
+    if (cudaMemcpy(p->d_twid, twid.data(), twid.size() * sizeof(double2), cudaMemcpyHostToDevice) != cudaSuccess)
+      return fail(EMRI_ECUDA);
+    {
+      // two-level table of the inter-pass twiddle W_N^q = twA[q >> 10] twB[q & 1023]
+      const long double tp = -2.0L * 3.14159265358979323846264338327950288L;
+      std::vector<double2> tA((size_t)(N >> 10)), tB(1024);
+      for (size_t q = 0; q < tA.size(); ++q) {
+        const long double ang = tp * (long double)q / (long double)tA.size();
+        tA[q] = make_double2((double)cosl(ang), (double)sinl(ang));
+      }
+      for (int q = 0; q < 1024; ++q) {
+        const long double ang = tp * (long double)q / (long double)N;
+        tB[q] = make_double2((double)cosl(ang), (double)sinl(ang));
+      }
+      if ((rc = dev_alloc(p, &p->d_twA, tA.size()))) return fail(rc);
+      if ((rc = dev_alloc(p, &p->d_twB, tB.size()))) return fail(rc);
+      if (cudaMemcpy(p->d_twA, tA.data(), tA.size() * sizeof(double2), cudaMemcpyHostToDevice) != cudaSuccess ||
+          cudaMemcpy(p->d_twB, tB.data(), tB.size() * sizeof(double2), cudaMemcpyHostToDevice) != cudaSuccess)
+        return fail(EMRI_ECUDA);
+    }
+    const int rows = FB_ELEMS / p->N2;
+    const int smem = (int)(((size_t)256 + p->N2 + (size_t)rows * (p->N2 + p->N2 / 16)) * sizeof(double2));
+    if (cudaFuncSetAttribute(fft_like_kernel<8>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem) != cudaSuccess ||
+        cudaFuncSetAttribute(fft_like_kernel<9>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem) != cudaSuccess ||
+        cudaFuncSetAttribute(fft_like_kernel<10>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem) != cudaSuccess ||
+        cudaFuncSetAttribute(fft_like_kernel<11>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem) != cudaSuccess ||
+        cudaFuncSetAttribute(fft_like_kernel<12>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem) != cudaSuccess)
+      return fail(EMRI_ECUDA);
+  }
+  if ((rc = dev_alloc(p, &p->d_partial, (size_t)K_max * std::max(p->n_part, p->N1)))) return fail(rc);
   if ((rc = dev_alloc(p, &p->d_params, (size_t)K_max * EMRI_NPAR))) return fail(rc);
   if ((rc = dev_alloc(p, &p->d_data, (size_t)4 * p->Nf))) return fail(rc);
   if ((rc = dev_alloc(p, &p->d_logL, (size_t)K_max))) return fail(rc);
@@ -427,13 +558,15 @@ int emri_plan_destroy(emri_plan* p) {
   if (!p) return EMRI_EINVAL;
   cudaDeviceSynchronize();
   for (auto& kv : p->fft) cufftDestroy(kv.second);
+  for (auto& kv : p->fftA) cufftDestroy(kv.second);
   for (auto e : p->ev) cudaEventDestroy(e);
   if (p->ev_call) cudaEventDestroy(p->ev_call);
   if (p->ev_data) cudaEventDestroy(p->ev_data);
   if (p->s_copy) cudaStreamDestroy(p->s_copy);
   void* ptrs[] = {p->d_w, p->d_wc, p->d_nodes, p->d_hbuf, p->d_partial, p->d_base, p->d_nodeaux, p->d_jpl, p->d_status,
                   p->d_params, p->d_data, p->d_logL, p->d_Y, p->d_z, p->d_lnu, p->d_logLY, p->d_inbox,
-                  p->d_partner, p->d_fftwork, p->d_seg, p->d_plrow, p->d_mode, p->d_pclamp, p->d_counts};
+                  p->d_partner, p->d_fftwork, p->d_seg, p->d_plrow, p->d_mode, p->d_pclamp, p->d_counts,
+                  p->d_twid, p->d_twA, p->d_twB, p->d_alpha, p->d_gamma, p->d_cdpart};
   for (void* q : ptrs) if (q) cudaFree(q);
   delete p;
   return EMRI_OK;
@@ -484,6 +617,14 @@ int emri_plan_synth_report(emri_plan* p, int64_t counts[16]) {
   for (int i = 0; i < 16; ++i) counts[i] = i < SYN_COUNTS ? (int64_t)h[i] : 0;
   return EMRI_OK;
 }
+
+int emri_plan_set_transform(emri_plan* p, int fused) {
+  if (!p || (fused != 0 && fused != 1)) return EMRI_EINVAL;
+  p->fused_on = fused != 0;
+  return EMRI_OK;
+}
+
+int emri_plan_transform_is_fused(const emri_plan* p) { return (p && p->fused_ok && p->fused_on) ? 1 : 0; }
 
 int emri_plan_set_synth_debug(emri_plan* p, int flags) {
   if (!p || flags < 0 || flags > 3) return EMRI_EINVAL;
@@ -590,6 +731,38 @@ static int loglike_impl(emri_plan* p, const double* params, int K, const double*
   if (rc) return rc;
   mark(p, s);
   int nch = 0;
+  const double scale = 2.0 * p->dt / (double)p->N;
+  if (p->fused_ok && p->fused_on && !fcoef) {
+    // fused path (fftlike.cuh): walker-interleaved synthesis, one strided cuFFT pass, last pass + Eq. 8 in one kernel
+    for (int k0 = 0; k0 < K; k0 += p->chunk, ++nch) {
+      const int kc = std::min(p->chunk, K - k0);
+      mark(p, s);
+      if ((rc = run_synth(p, k0, kc, nullptr, nullptr, 0, p->d_hbuf, s, true))) return rc;
+      mark(p, s);
+      cufftHandle h;
+      if ((rc = get_fftA(p, kc, &h))) return rc;
+      CKF(cufftSetStream(h, s));
+      CKF(cufftExecZ2Z(h, reinterpret_cast<cufftDoubleComplex*>(p->d_hbuf), reinterpret_cast<cufftDoubleComplex*>(p->d_hbuf),
+                       CUFFT_FORWARD));
+      mark(p, s);
+      if (nch == 0) {
+        // the weights of Eq. 8 in pass-B order, from the caller's data spectrum (the only reader of data_fft)
+        if (p->wait_before_like) { CK(cudaStreamWaitEvent(s, p->wait_before_like, 0)); p->wait_before_like = nullptr; }
+        like_weights_kernel<<<p->n_cd, 256, 0, s>>>(reinterpret_cast<const double2*>(data_fft), p->d_w, p->N, p->Nf, p->N1,
+                                                    p->log2N1, p->N2, p->d_alpha, p->d_gamma, p->d_cdpart);
+        p->launches += 1;
+        CK(cudaGetLastError());
+      }
+      if ((rc = run_fft_like(p, k0, kc, p->d_hbuf, s))) return rc;
+      mark(p, s);
+    }
+    p->n_chunks_last = nch;
+    fftlike_final_kernel<<<(K + 3) / 4, 128, 0, s>>>(p->d_partial, p->N1, p->d_cdpart, p->n_cd, K, scale, p->d_status, logL,
+                                                     status);
+    p->launches += 1;
+    CK(cudaGetLastError());
+    return EMRI_OK;
+  }
   for (int k0 = 0; k0 < K; k0 += p->chunk, ++nch) {
     const int kc = std::min(p->chunk, K - k0);
     mark(p, s);
@@ -602,7 +775,6 @@ static int loglike_impl(emri_plan* p, const double* params, int K, const double*
     mark(p, s);
   }
   p->n_chunks_last = nch;
-  const double scale = 2.0 * p->dt / (double)p->N;
   loglike_final_kernel<<<(K + 3) / 4, 128, 0, s>>>(p->d_partial, p->n_part, K, scale, p->d_status, logL, status);
   p->launches += 1;
   CK(cudaGetLastError());

@@ -32,7 +32,7 @@ constexpr int UNIT_TILES_MAX = 16;        // tiles per unit (one re-expansion pe
 constexpr int MLOC = 9;                   // local expansion orders 0..8 are computed ...
 constexpr int MKEEP = 6;                  // ... and a unit keeps at most 6 of them (more: base-series fallback)
 constexpr int HREC = 28;                  // doubles per harmonic record of the local table: orders 8..0 x {PA, PB, PC} + 1 pad
-constexpr int HERM = 24;                  // doubles per staged interval record (cubics of the 5 orbit functions + amplitude data)
+constexpr int HERM = 26;                  // doubles per staged interval record (cubics of the 5 orbit functions + amplitude data)
 #ifndef SYNTH_MINBLOCKS
 #define SYNTH_MINBLOCKS 4
 #endif
@@ -54,7 +54,9 @@ struct SynthArgs {
   double* outI;            // separate channels: row of walker k0+i at outI + i*pitch (used when outZ == NULL)
   double* outII;
   int64_t pitch;
-  double2* outZ;           // interleaved z = h_I + i h_II, row of walker k0+i at outZ + i*N
+  double2* outZ;           // interleaved z = h_I + i h_II, row of walker k0+i at outZ + i*N ...
+  int z_log2n2;            // ... or, when > 0, walker-interleaved for the fused transform: sample i = N2 i1 + i2 of
+                           // walker i at ((i1 K + i) N2 + i2), N2 = 2^z_log2n2 (a multiple of the 256-sample tile)
   int unit_tiles, unit_tiles_cap;   // tiles per unit of this launch; the plan's maximum (sizes the staging area)
   int64_t tiles_per_walker, units_per_walker;
   double tol;              // relative truncation of the harmonic series
@@ -595,6 +597,13 @@ __host__ __device__ inline size_t synth_smem_doubles(int n_max, int unit_tiles_c
          + (size_t)2 * 2 * unit_tiles_cap * HERM;       // staged interval cubics, double-buffered
 }
 
+// position of sample i0 of chunk-walker kl in outZ (both layouts)
+DEVINL size_t z_index(const SynthArgs& a, int kl, int64_t i0) {
+  if (a.z_log2n2 == 0) return (size_t)kl * a.N + i0;
+  const int64_t i1 = i0 >> a.z_log2n2;
+  return (((size_t)i1 * a.K + kl) << a.z_log2n2) + (size_t)(i0 & ((1 << a.z_log2n2) - 1));
+}
+
 // Consumers (warps 0..3): 2 adjacent samples per thread per tile.  Producer (warp 4): tables of the NEXT unit.
 // STAGED: S >= 256, every tile lies inside one coarse interval (the default); otherwise node rows are read per sample.
 template <bool STAGED>
@@ -658,8 +667,9 @@ __global__ void __launch_bounds__(SYNTH_BLOCK, SYNTH_MINBLOCKS) synth_kernel(Syn
       if (mt.skip) {
         for (int64_t i0 = i_begin + 2 * tid; i0 < i_end; i0 += TILE) {
           if (a.outZ) {
-            a.outZ[(size_t)kl * a.N + i0] = make_double2(0.0, 0.0);
-            a.outZ[(size_t)kl * a.N + i0 + 1] = make_double2(0.0, 0.0);
+            const size_t zi = z_index(a, kl, i0);
+            a.outZ[zi] = make_double2(0.0, 0.0);
+            a.outZ[zi + 1] = make_double2(0.0, 0.0);
           } else {
             *reinterpret_cast<double2*>(a.outI + (size_t)kl * a.pitch + i0) = make_double2(0.0, 0.0);
             *reinterpret_cast<double2*>(a.outII + (size_t)kl * a.pitch + i0) = make_double2(0.0, 0.0);
@@ -719,8 +729,9 @@ __global__ void __launch_bounds__(SYNTH_BLOCK, SYNTH_MINBLOCKS) synth_kernel(Syn
           const double hIb = fma(fb[0], S[3], fma(fb[2 * SYNTH_THREADS], S[4], fb[4 * SYNTH_THREADS] * S[5]));
           const double hIIb = fma(fb[6 * SYNTH_THREADS], S[3], fma(fb[8 * SYNTH_THREADS], S[4], fb[10 * SYNTH_THREADS] * S[5]));
           if (a.outZ) {
-            a.outZ[(size_t)kl * a.N + i0] = make_double2(hIa, hIIa);
-            a.outZ[(size_t)kl * a.N + i0 + 1] = make_double2(hIb, hIIb);
+            const size_t zi = z_index(a, kl, i0);
+            a.outZ[zi] = make_double2(hIa, hIIa);
+            a.outZ[zi + 1] = make_double2(hIb, hIIb);
           } else {
             *reinterpret_cast<double2*>(a.outI + (size_t)kl * a.pitch + i0) = make_double2(hIa, hIb);
             *reinterpret_cast<double2*>(a.outII + (size_t)kl * a.pitch + i0) = make_double2(hIIa, hIIb);

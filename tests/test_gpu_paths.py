@@ -189,3 +189,43 @@ def test_hot_call_does_not_allocate(emri):
     assert plan.workspace_bytes() == ws0
     assert torch.cuda.mem_get_info()[0] >= free0 - (2 << 20)      # cuFFT plan objects only (no work area, no buffers)
     plan.close()
+
+
+@pytest.mark.parametrize("lgN,K,chunk", [(16, 5, 4), (17, 6, 6), (18, 9, 4), (19, 3, 2), (20, 5, 3), (21, 3, 2), (22, 3, 3)])
+def test_fused_transform_and_likelihood_match_the_cufft_path_and_the_oracle(emri, oracle, lgN, K, chunk):
+    """stages (c)+(d) fused (strided cuFFT pass + own last pass feeding Eq. 8) against the full cuFFT transform + streaming
+    reduction, for every row length of the last pass (256 .. 4096), ragged chunks, noisy data, a plunging walker and an
+    invalid one; and against the oracle's whole path at N = 2^16"""
+    N = 1 << lgN
+    cfg = W.scaled(W.CONFIGS[2], K=K, N=N, n_max=8)
+    P = W.draw_params(cfg)
+    P[1, W.P_NU0] = 0.9995 * W.nu_lso_hz(P[1, W.P_M], P[1, W.P_E0])      # about to plunge: truncated waveform
+    P[2, W.P_DL] = -1.0                                                  # invalid: logL = -inf
+    psd = W.lisa_psd_barack_cutler(N, cfg.dt)
+    plan = emri.Plan(N, cfg.dt, cfg.n_max, K, psd)
+    plan.set_chunk(chunk)
+    assert plan.transform_is_fused()
+    D = plan.waveform_fft(dev(P[:1]))[0].clone() + dev(W.noise_fft(N, cfg.dt, psd, 3))
+    st = torch.zeros(K, dtype=torch.int32, device="cuda")
+    fused = plan.loglike(dev(P), D, status=st).cpu().numpy()
+    again = plan.loglike(dev(P), D).cpu().numpy()
+    plan.set_chunk(K)
+    whole = plan.loglike(dev(P), D).cpu().numpy()
+    plan.set_transform(False)
+    assert not plan.transform_is_fused()
+    plain = plan.loglike(dev(P), D).cpu().numpy()
+    st = st.cpu().numpy()
+    print("fused", fused, "plain", plain, "status", st)
+    assert st[2] == 1 and fused[2] == -np.inf and plain[2] == -np.inf
+    ok = np.isfinite(plain)
+    assert np.array_equal(fused, again) and np.array_equal(fused[ok], whole[ok])           # reproducible, chunk-invariant
+    assert np.all(np.abs(fused[ok] - plain[ok]) <= 1e-9 * np.abs(plain[ok]) + 1e-6)
+    # noise-less data = walker 0's own waveform: logL[0] = 0 within the absolute floor of the tolerance
+    plan.set_transform(True)
+    D0 = plan.waveform_fft(dev(P[:1]))[0].clone()
+    z = plan.loglike(dev(P), D0).cpu().numpy()
+    assert abs(z[0]) <= 1e-6
+    if lgN == 16:
+        ref, _ = oracle.loglike_batch(P, N, cfg.dt, cfg.n_max, D.cpu().numpy(), psd)
+        assert np.all(np.abs(fused[ok] - ref[ok]) <= 1e-9 * np.abs(ref[ok]) + 1e-6)
+    plan.close()
