@@ -151,7 +151,7 @@ class OracleLeg:
         self.orc = Oracle(anchor=(cfg.index == 5))
         self.walkers = min(host_cores(), cfg.K)
         self.P = W.draw_params(cfg, K=self.walkers)
-        self.Np = cfg.N // ORACLE_DECIMATE.get(cfg.index, 4)
+        self.Np = 1 << ((cfg.N // ORACLE_DECIMATE.get(cfg.index, 4)).bit_length() - 1)      # a power of two (the oracle's FFT)
         self.psd = psd_of(args, self.Np, cfg.dt)
 
     def describe(self, seconds=None):

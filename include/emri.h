@@ -131,6 +131,16 @@ int emri_plan_synth_report(emri_plan* p, int64_t counts[16]);
 int emri_plan_set_transform(emri_plan* p, int fused);
 int emri_plan_transform_is_fused(const emri_plan* p);
 
+/* CUDA graphs.  1 (default): emri_loglike / emri_loglike_fdep (and the likelihood inside emri_stretch_step) capture their
+ * whole kernel sequence -- orbit, synthesis, transform, reduction, 15 to 30 launches -- into a CUDA graph the first time an
+ * argument set (pointers, K) is seen and replay it afterwards: one launch per call, which is what the small ensembles of
+ * the paper's own run shape (8 walkers) are bound by.  The plan keeps the graphs of the last 8 argument
+ * sets; any emri_plan_set_* call drops them.  Not used while stage timings are enabled nor by emri_loglike_host.
+ * 0: every call enqueues its kernels one by one.  Results are identical bit for bit.
+ * emri_plan_graph_stats: out[0] = graphs captured, out[1] = calls served by a replay, since plan creation. */
+int emri_plan_set_graphs(emri_plan* p, int on);
+int emri_plan_graph_stats(const emri_plan* p, int64_t out[2]);
+
 /* Test hook: force the data-selected slow paths of stage (b) for every later call.  flags bit 0: every unit evaluates
  * the base series in e^2; bit 1: every sample takes the cube-root amplitude.  0 restores the defaults.  Results must
  * not change beyond rounding (tests/test_gpu_paths.py). */

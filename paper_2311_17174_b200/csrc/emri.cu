@@ -54,6 +54,16 @@ struct emri_plan {
   int orbit_mode = 1, anchor_end = 0, seg_L = 0, seg_P = 0, unit_tiles_override = 0, unit_tiles_cap = 8;
   int synth_debug = 0;                       // emri_plan_set_synth_debug
   int launches = 0;                          // kernels of this library enqueued by the last hot call
+  // CUDA graphs of emri_loglike (one per distinct argument set, a few kept): the 15-30 launches of a call become one
+  struct GraphEntry {
+    const void *params, *data, *logL, *status, *fcoef;
+    int K; double fstar; cudaGraphExec_t exec; int launches, n_chunks; uint64_t used;
+  };
+  std::vector<GraphEntry> graphs;
+  bool graphs_on = true;
+  cudaStream_t s_cap = nullptr;              // capture stream (the caller's may be the legacy stream, which cannot capture)
+  int64_t graph_captures = 0, graph_replays = 0;
+  uint64_t graph_clock = 0;
   unsigned long long* d_counts = nullptr;    // [SYN_COUNTS] path counters of stage (b), zeroed at the start of every call
   double* d_seg = nullptr;
   double* d_plrow = nullptr;
@@ -122,6 +132,12 @@ int debug_sync(emri_plan* p, cudaStream_t s, const char* what) {
   return EMRI_OK;
 }
 #define DBG(what) do { int rc_ = debug_sync(p, s, what); if (rc_) return rc_; } while (0)
+
+// every setting that changes what a call enqueues invalidates the captured graphs
+void drop_graphs(emri_plan* p) {
+  for (auto& g : p->graphs) cudaGraphExecDestroy(g.exec);
+  p->graphs.clear();
+}
 
 template <class T> int dev_alloc(emri_plan* p, T** ptr, size_t count) {
   if (*ptr) { cudaFree(*ptr); *ptr = nullptr; }
@@ -311,7 +327,7 @@ int run_orbit(emri_plan* p, const double* params, int K, cudaStream_t s) {
   sa.round = 0; sa.last_round = 0;
   orbit_init_kernel<<<(K + 31) / 32, 32, 0, s>>>(sa);
   DBG("orbit_init_kernel");
-  p->launches += 1 + 2 * 3 + 3;
+  p->launches += 1 + 2 * 3 + 2;
   const int n_rounds = 3;
   for (int r = 0; r < n_rounds; ++r) {
     sa.round = r; sa.last_round = (r == n_rounds - 1);
@@ -323,8 +339,7 @@ int run_orbit(emri_plan* p, const double* params, int K, cudaStream_t s) {
   }
   orbit_tail_kernel<<<(K + 31) / 32, 32, 0, s>>>(sa);
   DBG("orbit_tail_kernel");
-  orbit_fixup_kernel<<<aux_grid, 128, 0, s>>>(sa);
-  orbit_aux_kernel<<<aux_grid, 128, 0, s>>>(a);
+  orbit_fixup_kernel<<<aux_grid, 128, 0, s>>>(sa);      // + the per-node amplitude pair (orbit_aux_kernel's work)
   CK(cudaGetLastError());
   return EMRI_OK;
 }
@@ -545,7 +560,8 @@ int emri_plan_create(emri_plan** out, int64_t N, double dt, int n_max, int K_max
     return fail(EMRI_ECUDA);
   per_sm = std::min(per_sm, per_sm_direct);
   p->synth_grid = per_sm * p->sm_count;
-  if (cudaStreamCreateWithFlags(&p->s_copy, cudaStreamNonBlocking) != cudaSuccess ||
+  if (cudaStreamCreateWithFlags(&p->s_cap, cudaStreamNonBlocking) != cudaSuccess ||
+      cudaStreamCreateWithFlags(&p->s_copy, cudaStreamNonBlocking) != cudaSuccess ||
       cudaEventCreateWithFlags(&p->ev_call, cudaEventDisableTiming) != cudaSuccess ||
       cudaEventCreateWithFlags(&p->ev_data, cudaEventDisableTiming) != cudaSuccess)
     return fail(EMRI_ECUDA);
@@ -562,6 +578,8 @@ int emri_plan_destroy(emri_plan* p) {
   for (auto e : p->ev) cudaEventDestroy(e);
   if (p->ev_call) cudaEventDestroy(p->ev_call);
   if (p->ev_data) cudaEventDestroy(p->ev_data);
+  drop_graphs(p);
+  if (p->s_cap) cudaStreamDestroy(p->s_cap);
   if (p->s_copy) cudaStreamDestroy(p->s_copy);
   void* ptrs[] = {p->d_w, p->d_wc, p->d_nodes, p->d_hbuf, p->d_partial, p->d_base, p->d_nodeaux, p->d_jpl, p->d_status,
                   p->d_params, p->d_data, p->d_logL, p->d_Y, p->d_z, p->d_lnu, p->d_logLY, p->d_inbox,
@@ -574,12 +592,14 @@ int emri_plan_destroy(emri_plan* p) {
 
 int emri_plan_set_cosmology(emri_plan* p, double H0, double Om) {
   if (!p || !(H0 > 0.0) || !(Om > 0.0) || !(Om <= 1.0) || !std::isfinite(H0)) return EMRI_EINVAL;
+  drop_graphs(p);
   p->H0 = H0; p->Om = Om;
   return EMRI_OK;
 }
 
 int emri_plan_set_coarse_stride(emri_plan* p, int S) {
   if (!p || S < 2 || S > 65536 || (S & (S - 1))) return EMRI_EINVAL;
+  drop_graphs(p);
   CK(cudaDeviceSynchronize());
   p->S = S;
   p->logS = 0;
@@ -592,12 +612,14 @@ int emri_plan_set_coarse_stride(emri_plan* p, int S) {
 
 int emri_plan_set_orbit_schedule(emri_plan* p, int schedule) {
   if (!p || (schedule != 0 && schedule != 1)) return EMRI_EINVAL;
+  drop_graphs(p);
   p->orbit_mode = schedule;
   return EMRI_OK;
 }
 
 int emri_plan_set_anchor(emri_plan* p, int at_lso) {
   if (!p || (at_lso != 0 && at_lso != 1)) return EMRI_EINVAL;
+  drop_graphs(p);
   p->anchor_end = at_lso;
   return EMRI_OK;
 }
@@ -620,6 +642,7 @@ int emri_plan_synth_report(emri_plan* p, int64_t counts[16]) {
 
 int emri_plan_set_transform(emri_plan* p, int fused) {
   if (!p || (fused != 0 && fused != 1)) return EMRI_EINVAL;
+  drop_graphs(p);
   p->fused_on = fused != 0;
   return EMRI_OK;
 }
@@ -628,12 +651,14 @@ int emri_plan_transform_is_fused(const emri_plan* p) { return (p && p->fused_ok 
 
 int emri_plan_set_synth_debug(emri_plan* p, int flags) {
   if (!p || flags < 0 || flags > 3) return EMRI_EINVAL;
+  drop_graphs(p);
   p->synth_debug = flags;
   return EMRI_OK;
 }
 
 int emri_plan_set_chunk(emri_plan* p, int c) {
   if (!p || c < 1) return EMRI_EINVAL;
+  drop_graphs(p);
   if (c > p->K_max) c = p->K_max;
   CK(cudaDeviceSynchronize());
   if (p->d_hbuf) p->bytes -= (int64_t)((size_t)2 * p->chunk * p->N * sizeof(double));
@@ -721,10 +746,68 @@ int emri_data_fft(emri_plan* p, const double* d_I, const double* d_II, double* d
   return EMRI_OK;
 }
 
+static int loglike_enqueue(emri_plan* p, const double* params, int K, const double* fcoef, double fstar, const double* data_fft,
+                           double* logL, int32_t* status, cudaStream_t s);
+
+// emri_loglike / emri_loglike_fdep: replay the CUDA graph of this argument set if the plan holds one, else capture it (on
+// the plan's own stream: the caller's may be the legacy default stream) and launch it into the caller's stream.  Plain
+// enqueueing when graphs are off, stage timings are on, the call is the host variant's (it waits on the copy stream), or
+// capture fails for any reason.
 static int loglike_impl(emri_plan* p, const double* params, int K, const double* fcoef, double fstar, const double* data_fft,
                         double* logL, int32_t* status, void* stream) {
   if (!valid_call(p, params, K) || !data_fft || !logL) return EMRI_EINVAL;
   cudaStream_t s = (cudaStream_t)stream;
+  static const bool dbg = std::getenv("EMRI_DEBUG_SYNC") != nullptr;
+  if (!p->graphs_on || p->timing || p->wait_before_like || dbg || !p->s_cap)
+    return loglike_enqueue(p, params, K, fcoef, fstar, data_fft, logL, status, s);
+  for (auto& g : p->graphs)
+    if (g.params == params && g.data == data_fft && g.logL == logL && g.status == status && g.fcoef == fcoef && g.K == K &&
+        g.fstar == fstar) {
+      CK(cudaGraphLaunch(g.exec, s));
+      g.used = ++p->graph_clock;
+      p->launches = g.launches; p->n_chunks_last = g.n_chunks; p->had_like = true; p->ev_used = 0;
+      ++p->graph_replays;
+      return EMRI_OK;
+    }
+  // every cuFFT plan the call needs must exist before the capture starts (plan creation cannot be captured)
+  {
+    const bool fused = p->fused_ok && p->fused_on && !fcoef;
+    cufftHandle h;
+    int rc;
+    for (int k0 = 0; k0 < K; k0 += p->chunk) {
+      const int kc = std::min(p->chunk, K - k0);
+      if ((rc = fused ? get_fftA(p, kc, &h) : get_fft(p, kc, &h))) return rc;
+    }
+  }
+  cudaGraph_t graph = nullptr;
+  if (cudaStreamBeginCapture(p->s_cap, cudaStreamCaptureModeThreadLocal) != cudaSuccess) {
+    cudaGetLastError();
+    return loglike_enqueue(p, params, K, fcoef, fstar, data_fft, logL, status, s);
+  }
+  const int rc = loglike_enqueue(p, params, K, fcoef, fstar, data_fft, logL, status, p->s_cap);
+  const cudaError_t ec = cudaStreamEndCapture(p->s_cap, &graph);
+  cudaGraphExec_t exec = nullptr;
+  if (rc != EMRI_OK || ec != cudaSuccess || !graph || cudaGraphInstantiate(&exec, graph, 0) != cudaSuccess) {
+    if (graph) cudaGraphDestroy(graph);
+    cudaGetLastError();
+    if (rc != EMRI_OK) return rc;
+    return loglike_enqueue(p, params, K, fcoef, fstar, data_fft, logL, status, s);
+  }
+  cudaGraphDestroy(graph);
+  if (p->graphs.size() >= 8) {            // keep a few: evict the least recently used
+    size_t lru = 0;
+    for (size_t i = 1; i < p->graphs.size(); ++i) if (p->graphs[i].used < p->graphs[lru].used) lru = i;
+    cudaGraphExecDestroy(p->graphs[lru].exec);
+    p->graphs.erase(p->graphs.begin() + (long)lru);
+  }
+  p->graphs.push_back({params, data_fft, logL, status, fcoef, K, fstar, exec, p->launches, p->n_chunks_last, ++p->graph_clock});
+  ++p->graph_captures;
+  CK(cudaGraphLaunch(exec, s));
+  return EMRI_OK;
+}
+
+static int loglike_enqueue(emri_plan* p, const double* params, int K, const double* fcoef, double fstar, const double* data_fft,
+                           double* logL, int32_t* status, cudaStream_t s) {
   p->ev_used = 0; p->had_like = true;
   mark(p, s);
   int rc = run_orbit(p, params, K, s);
@@ -814,6 +897,19 @@ int emri_loglike_host(emri_plan* p, const double* params, int K, const double* d
   CK(cudaMemcpyAsync(logL, p->d_logL, (size_t)K * sizeof(double), cudaMemcpyDeviceToHost, s));
   if (status) CK(cudaMemcpyAsync(status, p->d_status, (size_t)K * sizeof(int32_t), cudaMemcpyDeviceToHost, s));
   CK(cudaStreamSynchronize(s));
+  return EMRI_OK;
+}
+
+int emri_plan_set_graphs(emri_plan* p, int on) {
+  if (!p || (on != 0 && on != 1)) return EMRI_EINVAL;
+  p->graphs_on = on != 0;
+  if (!on) drop_graphs(p);
+  return EMRI_OK;
+}
+
+int emri_plan_graph_stats(const emri_plan* p, int64_t out[2]) {
+  if (!p || !out) return EMRI_EINVAL;
+  out[0] = p->graph_captures; out[1] = p->graph_replays;
   return EMRI_OK;
 }
 

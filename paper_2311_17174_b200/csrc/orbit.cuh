@@ -745,7 +745,14 @@ __global__ void __launch_bounds__(32) orbit_tail_kernel(ShootArgs s) {
   a.wc[(size_t)k * WC_STRIDE + WC_EMAX] = emax;
 }
 
-// ---- 5. node-parallel: global angles, post-plunge copies, zero rows
+// per-node amplitude data for stage (b): {(2 pi M nu_j)^{2/3} mu/(Xi D), 1/nu_j}
+DEVINL double2 node_aux(const double* __restrict__ wc, double nu) {
+  if (!(nu > 0.0) || !isfinite(nu)) return make_double2(0.0, 0.0);
+  const double cb = cbrt(wc[WC_TWOPIMS] * nu);
+  return make_double2(cb * cb * wc[WC_AMP], 1.0 / nu);
+}
+
+// ---- 5. node-parallel: global angles, post-plunge copies, zero rows, and the node's amplitude pair
 __global__ void __launch_bounds__(128) orbit_fixup_kernel(ShootArgs s) {
   const OrbitArgs& a = s.o;
   const int64_t idx = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
@@ -753,48 +760,46 @@ __global__ void __launch_bounds__(128) orbit_fixup_kernel(ShootArgs s) {
   const int k = (int)(idx / a.Nn);
   const int64_t m = idx - (int64_t)k * a.Nn;
   const int mode = s.mode[k];
+  const double* wc = a.wc + (size_t)k * WC_STRIDE;
   double2* row = reinterpret_cast<double2*>(a.nodes + ((size_t)k * a.Nn + m) * NODE_STRIDE);
   if (mode == OM_ZERO) {
 #pragma unroll
     for (int q = 0; q < NODE_STRIDE / 2; ++q) row[q] = make_double2(0.0, 0.0);
+    a.nodeaux[idx] = make_double2(0.0, 0.0);
     return;
   }
   // recursion index of this row's node: forward r = j = m - 1 (row 0 is the guard node, global angles already);
   // anchored at the LSO r = Nc - j = Nc + 1 - m (row Nc + 2 is the guard node)
   const int64_t r = a.anchor_end ? a.Nc + 1 - m : m - 1;
-  if (r < 0) return;
   const int32_t jpl = a.jpl[k];
-  if (!a.anchor_end && r >= (int64_t)jpl) {
+  if (r >= 0 && !a.anchor_end && r >= (int64_t)jpl) {
     const double2* src = reinterpret_cast<const double2*>(s.plrow + (size_t)k * NODE_STRIDE);
 #pragma unroll
     for (int q = 0; q < NODE_STRIDE / 2; ++q) row[q] = src[q];
+    a.nodeaux[idx] = node_aux(wc, src[0].y);
     return;
   }
+  double2 v01 = row[0];
+  a.nodeaux[idx] = node_aux(wc, v01.y);
+  if (r < 0) return;
   int64_t p = r / s.L;
   const int pc = s.pclamp[k];
   if (p > pc) p = pc;
   if (p == 0) return;
   const double* sg = s.seg + ((size_t)k * s.P + p) * SEG_STRIDE;
-  double2 v01 = row[0], v23 = row[1], v4 = row[2];
+  double2 v23 = row[1], v4 = row[2];
   v01.x = frac(v01.x + sg[SG_O0]);
   v23.x = frac(v23.x + sg[SG_O1]);
   v4.x = frac(v4.x + sg[SG_O2]);
   row[0] = v01; row[1] = v23; row[2] = v4;
 }
 
-// ---- node-parallel (both schedules): per-node amplitude data for stage (b), {(2 pi M nu_j)^{2/3} mu/(Xi D), 1/nu_j}
+// ---- node-parallel (sequential schedule; the parallel one does this in orbit_fixup_kernel): amplitude pair per node
 __global__ void __launch_bounds__(128) orbit_aux_kernel(OrbitArgs a) {
   const int64_t idx = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
   if (idx >= a.Nn * a.K) return;
   const int k = (int)(idx / a.Nn);
-  const double nu = a.nodes[(size_t)idx * NODE_STRIDE + 1];
-  const double* wc = a.wc + (size_t)k * WC_STRIDE;
-  double2 out = make_double2(0.0, 0.0);
-  if (nu > 0.0 && isfinite(nu)) {
-    const double cb = cbrt(wc[WC_TWOPIMS] * nu);
-    out = make_double2(cb * cb * wc[WC_AMP], 1.0 / nu);
-  }
-  a.nodeaux[idx] = out;
+  a.nodeaux[idx] = node_aux(a.wc + (size_t)k * WC_STRIDE, a.nodes[(size_t)idx * NODE_STRIDE + 1]);
 }
 
 }  // namespace

@@ -18,7 +18,7 @@ _lib = None
 EXPORTS = (
     "emri_strerror", "emri_plan_create", "emri_plan_destroy", "emri_plan_set_cosmology",
     "emri_plan_set_coarse_stride", "emri_plan_set_orbit_schedule", "emri_plan_set_anchor", "emri_plan_orbit_report",
-    "emri_plan_synth_report", "emri_plan_set_synth_debug", "emri_plan_set_transform", "emri_plan_transform_is_fused", "emri_plan_set_chunk", "emri_orbit", "emri_plan_num_nodes", "emri_waveform",
+    "emri_plan_synth_report", "emri_plan_set_synth_debug", "emri_plan_set_transform", "emri_plan_transform_is_fused", "emri_plan_set_graphs", "emri_plan_graph_stats", "emri_plan_set_chunk", "emri_orbit", "emri_plan_num_nodes", "emri_waveform",
     "emri_waveform_fft", "emri_data_fft", "emri_loglike", "emri_loglike_fdep", "emri_loglike_host", "emri_plan_enable_timings",
     "emri_plan_get_timings", "emri_plan_last_cuda_error", "emri_plan_last_launch_count", "emri_plan_workspace_bytes", "emri_stretch_step",
 )
@@ -51,6 +51,8 @@ def load():
     L.emri_plan_synth_report.argtypes = [vp, vp]
     L.emri_plan_set_synth_debug.argtypes = [vp, i32]
     L.emri_plan_set_transform.argtypes = [vp, i32]
+    L.emri_plan_set_graphs.argtypes = [vp, i32]
+    L.emri_plan_graph_stats.argtypes = [vp, vp]
     L.emri_plan_transform_is_fused.argtypes = [vp]
     L.emri_orbit.argtypes = [vp, vp, i32, vp, vp, vp]
     L.emri_plan_num_nodes.restype = i64
@@ -167,6 +169,16 @@ class Plan:
     def launch_count(self):
         """kernels of this library enqueued by the last hot call"""
         return int(self._L.emri_plan_last_launch_count(self._h))
+
+    def set_graphs(self, on):
+        """True (default): emri_loglike replays a captured CUDA graph per argument set"""
+        self._check(self._L.emri_plan_set_graphs(self._h, 1 if on else 0))
+
+    def graph_stats(self):
+        """(graphs captured, calls served by a replay)"""
+        c = np.zeros(2, dtype=np.int64)
+        self._check(self._L.emri_plan_graph_stats(self._h, c.ctypes.data_as(C.c_void_p)))
+        return int(c[0]), int(c[1])
 
     def set_transform(self, fused):
         """True: last transform pass fused with Eq. 8 (default where available); False: full cuFFT + reduction kernel"""

@@ -229,3 +229,51 @@ def test_fused_transform_and_likelihood_match_the_cufft_path_and_the_oracle(emri
         ref, _ = oracle.loglike_batch(P, N, cfg.dt, cfg.n_max, D.cpu().numpy(), psd)
         assert np.all(np.abs(fused[ok] - ref[ok]) <= 1e-9 * np.abs(ref[ok]) + 1e-6)
     plan.close()
+
+
+def test_graph_replay_gives_the_same_bits_and_follows_its_inputs(emri):
+    """emri_loglike through a captured CUDA graph: same bits as plain enqueueing; a replay reads the CURRENT contents of
+    the parameter and data buffers; a new argument set captures a new graph; settings drop the graphs"""
+    cfg = W.scaled(W.CONFIGS[1], K=12, N=1 << 16)
+    P = W.draw_params(cfg)
+    psd = W.lisa_psd_barack_cutler(cfg.N, cfg.dt)
+    plan = emri.Plan(cfg.N, cfg.dt, cfg.n_max, cfg.K, psd)
+    plan.set_chunk(8)
+    D = plan.waveform_fft(dev(P[:1]))[0].clone() + dev(W.noise_fft(cfg.N, cfg.dt, psd, 5))
+    p_d = dev(P)
+    logL = torch.empty(cfg.K, dtype=torch.float64, device="cuda")
+    st = torch.zeros(cfg.K, dtype=torch.int32, device="cuda")
+    plan.set_graphs(False)
+    ref = plan.loglike(p_d, D, logL, st).cpu().numpy().copy()
+    n_plain = plan.launch_count()
+    plan.set_graphs(True)
+    c0 = plan.graph_stats()
+    a = plan.loglike(p_d, D, logL, st).cpu().numpy().copy()          # captures
+    b = plan.loglike(p_d, D, logL, st).cpu().numpy().copy()          # replays
+    c1 = plan.graph_stats()
+    assert np.array_equal(a, ref) and np.array_equal(b, ref)
+    assert c1[0] == c0[0] + 1 and c1[1] == c0[1] + 1 and plan.launch_count() == n_plain
+    # the graph reads the buffers it was captured with: change their contents, replay, compare with plain enqueueing
+    P2 = P[::-1].copy()
+    p_d.copy_(dev(P2))
+    g = plan.loglike(p_d, D, logL, st).cpu().numpy().copy()
+    assert plan.graph_stats()[1] == c1[1] + 1
+    plan.set_graphs(False)
+    assert np.array_equal(g, plan.loglike(p_d, D, logL, st).cpu().numpy())
+    assert np.array_equal(g, ref[::-1])
+    # another K, another graph; a setting drops them all
+    plan.set_graphs(True)
+    plan.loglike(p_d[:5].contiguous(), D)
+    plan.loglike(p_d, D, logL, st)
+    caps = plan.graph_stats()[0]
+    plan.set_chunk(4)
+    plan.loglike(p_d, D, logL, st)
+    assert plan.graph_stats()[0] == caps + 1
+    assert np.array_equal(logL.cpu().numpy(), ref[::-1])
+    # with the data in the default stream's order: a legacy-stream caller and a side stream give the same result
+    side = torch.cuda.Stream()
+    torch.cuda.synchronize()
+    with torch.cuda.stream(side):
+        out = plan.loglike(p_d, D).cpu().numpy()
+    assert np.array_equal(out, ref[::-1])
+    plan.close()
