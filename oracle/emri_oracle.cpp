@@ -18,6 +18,10 @@
 //                                  PAPER.md:75-79 (Eq. 2), :118, Eq. 4-6 (:88-97)
 //   S6 un-normalised forward DFT
 //   S7 Gaussian log-likelihood     PAPER.md:112-116 (Eq. 8)
+//   S3' (next row f-3, reading D14) the paper's own kind of integrator instead of S3: an embedded Runge-Kutta pair with
+//       per-walker step control and dense output ("standard ODE methods ... Runge-Kutta scheme", solve_ivp; PAPER.md:120,
+//       :133) -- Dormand-Prince 5(4) with Hairer's step-size controller and Shampine's continuous extension, whose
+//       dense output is sampled at the coarse nodes; S4..S7 are unchanged
 // No blocking, fusion or reordering beyond what those passages state.  Bessel functions are the
 // ascending power series (the definition); cos(n Phi) is called directly for every n.
 //
@@ -295,8 +299,308 @@ Orbit integrate_orbit_from_lso(const Walker& w, int64_t N, real dt, int S, int p
   return o;
 }
 
+// ---------------------------------------------------------------- S3' adaptive embedded pair with dense output (f-3, D14)
+// Dormand & Prince 1980, RK5(4)7M: c, a_ij, b (5th order, = the 7th row: first-same-as-last), e = b - b^ (4th order
+// embedded), and the coefficients of Shampine's 4th-order continuous extension,
+//     y(t_n + theta h) = y_n + h sum_i K_i sum_{j=0..3} P_ij theta^{j+1}.
+const real DP_C[6] = {0, (real)1 / 5, (real)3 / 10, (real)4 / 5, (real)8 / 9, 1};
+const real DP_A[6][5] = {
+    {0, 0, 0, 0, 0},
+    {(real)1 / 5, 0, 0, 0, 0},
+    {(real)3 / 40, (real)9 / 40, 0, 0, 0},
+    {(real)44 / 45, (real)-56 / 15, (real)32 / 9, 0, 0},
+    {(real)19372 / 6561, (real)-25360 / 2187, (real)64448 / 6561, (real)-212 / 729, 0},
+    {(real)9017 / 3168, (real)-355 / 33, (real)46732 / 5247, (real)49 / 176, (real)-5103 / 18656}};
+const real DP_B[6] = {(real)35 / 384, 0, (real)500 / 1113, (real)125 / 192, (real)-2187 / 6784, (real)11 / 84};
+const real DP_E[7] = {(real)-71 / 57600, 0, (real)71 / 16695, (real)-71 / 1920, (real)17253 / 339200, (real)-22 / 525,
+                      (real)1 / 40};
+const real DP_P[7][4] = {
+    {1, (real)-8048581381.0L / 2820520608.0L, (real)8663915743.0L / 2820520608.0L, (real)-12715105075.0L / 11282082432.0L},
+    {0, 0, 0, 0},
+    {0, (real)131558114200.0L / 32700410799.0L, (real)-68118460800.0L / 10900136933.0L, (real)87487479700.0L / 32700410799.0L},
+    {0, (real)-1754552775.0L / 470086768.0L, (real)14199869525.0L / 1410260304.0L, (real)-10690763975.0L / 1880347072.0L},
+    {0, (real)127303824393.0L / 49829197408.0L, (real)-318862633887.0L / 49829197408.0L,
+     (real)701980252875.0L / 199316789632.0L},
+    {0, (real)-282668133.0L / 205662961.0L, (real)2019193451.0L / 616988883.0L, (real)-1453857185.0L / 822651844.0L},
+    {0, (real)40617522.0L / 29380423.0L, (real)-110615467.0L / 29380423.0L, (real)69997945.0L / 29380423.0L}};
+
+struct Dp5Step {
+  real t, h;          // start of the step and its signed size
+  real y[5];          // state at t: angles (0, 2, 4) in cycles wrapped to [0, 1), nu, e
+  real turns[3];      // whole cycles removed from the three angles so far (enters the error scale only)
+  real Q[5][4];       // dense output: y(t + theta h) = y + sum_j Q[q][j] theta^{j+1}  (already multiplied by h)
+  real D[5];          // the step's own increment h sum_i b_i K_i (unwrapped); Q(1) equals it up to the rounding of P
+};
+struct Dp5Branch {
+  std::vector<Dp5Step> steps;
+  real t_end;         // where the branch stops (the bound, or the end of the step after which the state is unusable)
+  int stop;           // 0 reached the bound; ST_PLUNGE / ST_STATE: stopped early after an accepted step
+};
+
+real rms5(const real v[5]) {
+  real s = 0;
+  for (int q = 0; q < 5; ++q) s += v[q] * v[q];
+  return std::sqrt(s / 5);
+}
+
+// Integrate dY/dt = f(Y) from (t0, y0) to t_bound with Dormand-Prince 5(4) and the step-size controller of Hairer,
+// Norsett & Wanner (Solving ODEs I, sec. II.4), in the form SciPy's solve_ivp(method="RK45") uses it (the paper's
+// integrator is solve_ivp): error norm = rms over the components of err_q / (atol_q + rtol max(|Y_q|,
+// |Y_q,new|)); accepted when < 1; new step = h min(10, 0.9 err^{-1/5}) (at most h after a rejection); rejected: h max(0.2,
+// 0.9 err^{-1/5}); first step from the two-evaluation estimate of the same section; the last step is cut to land on the
+// bound.  |Y| is the UNWRAPPED angle (turns + fraction) so that the scale is what an integration in plain cycles sees,
+// while the state itself is kept wrapped (only frac matters downstream, D2).  stop_at_plunge: forward integration of a
+// walker given at t = 0 ends after the first accepted step whose end state is past nu_LSO(e) (reading R8).
+Dp5Branch dp5_integrate(const Walker& w, const real y0[5], real t0, real t_bound, real rtol, const real atol[5], int pn_mask,
+                        bool stop_at_plunge) {
+  Dp5Branch br;
+  br.t_end = t0; br.stop = 0;
+  const real dir = (t_bound >= t0) ? 1 : -1;
+  if (t_bound == t0) return br;
+  real t = t0, y[5], turns[3] = {0, 0, 0}, f[5];
+  for (int q = 0; q < 5; ++q) y[q] = y0[q];
+  rhs(w, y, pn_mask, f);
+  auto unwrapped = [&](const real yy[5], const real tt[3], int q) -> real {
+    return (q == 0) ? tt[0] + yy[0] : (q == 2) ? tt[1] + yy[2] : (q == 4) ? tt[2] + yy[4] : yy[q];
+  };
+  // first step
+  real h_abs;
+  {
+    const real interval = std::fabs(t_bound - t0);
+    real sc[5], v0[5], v1[5];
+    for (int q = 0; q < 5; ++q) { sc[q] = atol[q] + std::fabs(unwrapped(y, turns, q)) * rtol; v0[q] = unwrapped(y, turns, q) / sc[q]; v1[q] = f[q] / sc[q]; }
+    const real d0 = rms5(v0), d1 = rms5(v1);
+    real h0 = (d0 < (real)1e-5 || d1 < (real)1e-5) ? (real)1e-6 : (real)0.01 * d0 / d1;
+    if (h0 > interval) h0 = interval;
+    real y1[5], f1[5], v2[5];
+    for (int q = 0; q < 5; ++q) y1[q] = y[q] + h0 * dir * f[q];
+    rhs(w, y1, pn_mask, f1);
+    for (int q = 0; q < 5; ++q) v2[q] = (f1[q] - f[q]) / sc[q];
+    const real d2 = rms5(v2) / h0;
+    const real dm = d1 > d2 ? d1 : d2;
+    real h1 = (d1 <= (real)1e-15 && d2 <= (real)1e-15) ? std::max((real)1e-6, h0 * (real)1e-3)
+                                                       : std::pow((real)0.01 / dm, (real)1 / 5);
+    h_abs = std::min(std::min(100 * h0, h1), interval);
+  }
+  const real expo = (real)-1 / 5;
+  for (int n_steps = 0; t != t_bound; ++n_steps) {
+    if (n_steps >= 1000000) { br.stop = ST_STATE; break; }
+    const real min_step = 10 * std::fabs(std::nextafter(t, dir * std::numeric_limits<real>::infinity()) - t);
+    if (h_abs < min_step) h_abs = min_step;
+    bool rejected = false;
+    real K[7][5], y_new[5], h = 0, t_new = t;
+    for (;;) {
+      if (h_abs < min_step) { br.stop = ST_STATE; br.t_end = t; return br; }
+      h = h_abs * dir;
+      t_new = t + h;
+      if (dir * (t_new - t_bound) > 0) t_new = t_bound;
+      h = t_new - t;
+      h_abs = std::fabs(h);
+      for (int q = 0; q < 5; ++q) K[0][q] = f[q];
+      for (int s = 1; s < 6; ++s) {
+        real ys[5];
+        for (int q = 0; q < 5; ++q) {
+          real dy = 0;
+          for (int j = 0; j < s; ++j) dy += DP_A[s][j] * K[j][q];
+          ys[q] = y[q] + dy * h;
+        }
+        rhs(w, ys, pn_mask, K[s]);
+      }
+      for (int q = 0; q < 5; ++q) {
+        real dy = 0;
+        for (int j = 0; j < 6; ++j) dy += DP_B[j] * K[j][q];
+        y_new[q] = y[q] + h * dy;
+      }
+      rhs(w, y_new, pn_mask, K[6]);
+      real en[5];
+      for (int q = 0; q < 5; ++q) {
+        real e = 0;
+        for (int j = 0; j < 7; ++j) e += DP_E[j] * K[j][q];
+        // |Y_new| unwrapped = |Y| + increment for the angles
+        const real Yo = unwrapped(y, turns, q), Yn = (q == 1 || q == 3) ? y_new[q] : Yo + (y_new[q] - y[q]);
+        const real sc = atol[q] + std::max(std::fabs(Yo), std::fabs(Yn)) * rtol;
+        en[q] = e * h / sc;
+      }
+      const real err = rms5(en);
+      if (err < 1) {
+        real factor = (err == 0) ? (real)10 : std::min((real)10, (real)0.9 * std::pow(err, expo));
+        if (rejected && factor > 1) factor = 1;
+        h_abs *= factor;
+        break;
+      }
+      h_abs *= std::max((real)0.2, (real)0.9 * std::pow(err, expo));
+      rejected = true;
+    }
+    // record the accepted step with its dense output
+    Dp5Step st;
+    st.t = t; st.h = h;
+    for (int q = 0; q < 5; ++q) st.y[q] = y[q];
+    for (int a = 0; a < 3; ++a) st.turns[a] = turns[a];
+    for (int q = 0; q < 5; ++q)
+      for (int j = 0; j < 4; ++j) {
+        real c = 0;
+        for (int i = 0; i < 7; ++i) c += K[i][q] * DP_P[i][j];
+        st.Q[q][j] = h * c;
+      }
+    for (int q = 0; q < 5; ++q) st.D[q] = y_new[q] - y[q];
+    br.steps.push_back(st);
+    // advance; the angles are wrapped and the whole cycles remembered
+    for (int q = 0; q < 5; ++q) y[q] = y_new[q];
+    for (int a = 0; a < 3; ++a) {
+      const int q = 2 * a;
+      const real fl = std::floor(y[q]);
+      turns[a] += fl; y[q] -= fl;
+    }
+    for (int q = 0; q < 5; ++q) f[q] = K[6][q];
+    t = t_new;
+    br.t_end = t;
+    if (!state_ok(y)) { br.stop = ST_STATE; break; }
+    if (stop_at_plunge && !(y[1] < nu_lso(w.Ms, y[3]))) { br.stop = ST_PLUNGE; break; }
+  }
+  return br;
+}
+
+// dense output of step st at fraction theta: offset from st.y (unwrapped for the angles)
+void dp5_offset(const Dp5Step& st, real theta, real off[5]) {
+  for (int q = 0; q < 5; ++q) off[q] = theta * (st.Q[q][0] + theta * (st.Q[q][1] + theta * (st.Q[q][2] + theta * st.Q[q][3])));
+}
+
+// The coarse orbit (same node table as S3) sampled from the dense output of the adaptive integration: from the anchor
+// (t = 0 forward convention, or the last node in the LSO convention) one branch runs forward to node Nc + 1 and one
+// backward to node -1.  Node values are y_n + offset(theta) (angles wrapped), node slopes the right-hand side AT the node,
+// interval increments the unwrapped offset differences, pieced together step by step so that no large number is ever
+// differenced.  Between nodes S4's cubic Hermite is kept: at the default stride its truncation error is below the rounding of
+// the phases (D3), so sampling the dense output at every sample instead would change nothing above 1e-14 cycles.
+Orbit integrate_orbit_adaptive(const Walker& w, int64_t N, real dt, int S, int pn_mask, int anchor, real rtol, const real atol[5]) {
+  Orbit o;
+  o.G = 1;
+  o.Nc = (N + S - 1) / S;
+  o.Nn = o.Nc + 1 + 2 * o.G;
+  o.Delta = S * dt;
+  o.jpl = o.Nn;
+  o.status = w.status;
+  for (int q = 0; q < 5; ++q) { o.val[q].assign(o.Nn, 0); o.slope[q].assign(o.Nn, 0); o.inc[q].assign(o.Nn, 0); }
+  if (w.status & ST_BADPARAM) return o;
+  const int G = o.G;
+  real y0[5];
+  for (int q = 0; q < 5; ++q) y0[q] = w.p0[q];
+  const int64_t ja = anchor ? o.Nc : 0;                 // anchor node
+  if (anchor) y0[1] = nu_lso(w.Ms, y0[3]);
+  else if (!(y0[1] < nu_lso(w.Ms, y0[3]))) { o.status |= ST_PLUNGE; o.jpl = 0; return o; }
+  const real ta = (real)ja * o.Delta;
+  Dp5Branch fwd = dp5_integrate(w, y0, ta, (real)(o.Nc + G) * o.Delta, rtol, atol, pn_mask, !anchor);
+  Dp5Branch bwd = dp5_integrate(w, y0, ta, (real)(-G) * o.Delta, rtol, atol, pn_mask, false);
+  auto zero_all = [&](int bit) {
+    for (int q = 0; q < 5; ++q) {
+      std::fill(o.val[q].begin(), o.val[q].end(), (real)0);
+      std::fill(o.slope[q].begin(), o.slope[q].end(), (real)0);
+      std::fill(o.inc[q].begin(), o.inc[q].end(), (real)0);
+    }
+    o.status |= bit;
+    return o;
+  };
+  if (bwd.stop || (anchor && fwd.stop)) return zero_all(ST_STATE);          // the guard side / the LSO convention must be clean
+  if (fwd.stop == ST_STATE && fwd.steps.empty()) return zero_all(ST_STATE);
+  // position of node j in its branch: step index and theta
+  struct Pos { const Dp5Branch* br; int64_t n; real theta; bool ok; };
+  auto locate = [&](int64_t j, int64_t hint, const Dp5Branch& br) -> Pos {
+    const real tj = (real)j * o.Delta;
+    const real dir = (br.steps.empty() || br.steps[0].h >= 0) ? 1 : -1;
+    if (br.steps.empty() || dir * (tj - br.t_end) > 0) return Pos{&br, 0, 0, false};
+    int64_t n = hint;
+    while (n + 1 < (int64_t)br.steps.size() && dir * (tj - (br.steps[n].t + br.steps[n].h)) > 0) ++n;
+    return Pos{&br, n, (tj - br.steps[n].t) / br.steps[n].h, true};
+  };
+  auto node_state = [&](const Pos& p, real y[5]) {
+    real off[5];
+    const Dp5Step& st = p.br->steps[p.n];
+    dp5_offset(st, p.theta, off);
+    for (int q = 0; q < 5; ++q) y[q] = st.y[q] + off[q];
+    y[0] = frac(y[0]); y[2] = frac(y[2]); y[4] = frac(y[4]);
+  };
+  // unwrapped change from position a to position b, b not before a in the branch's own order
+  auto change = [&](const Pos& a, const Pos& b, real d[5]) {
+    real oa[5], ob[5];
+    dp5_offset(a.br->steps[a.n], a.theta, oa);
+    dp5_offset(b.br->steps[b.n], b.theta, ob);
+    if (a.n == b.n) { for (int q = 0; q < 5; ++q) d[q] = ob[q] - oa[q]; return; }
+    // whole steps contribute their own increments D (what the state actually advanced by), so that the pieces add up
+    // to value(b) - value(a) exactly; every term is at most a step's increment in size
+    for (int q = 0; q < 5; ++q) d[q] = a.br->steps[a.n].D[q] - oa[q];
+    for (int64_t i = a.n + 1; i < b.n; ++i)
+      for (int q = 0; q < 5; ++q) d[q] += a.br->steps[i].D[q];
+    for (int q = 0; q < 5; ++q) d[q] += ob[q];
+  };
+  // forward side: nodes ja .. Nc + G in time order
+  {
+    int64_t hint = 0;
+    Pos prev{&fwd, 0, 0, false};
+    for (int64_t j = ja; j <= o.Nc + G; ++j) {
+      const int64_t jj = j + G;
+      Pos p = locate(j, hint, fwd);
+      real y[5];
+      bool bad = !p.ok;
+      if (p.ok) {
+        node_state(p, y);
+        if (!state_ok(y)) { bad = true; o.status |= ST_STATE; }
+        else if (!anchor && !(y[1] < nu_lso(w.Ms, y[3]))) { bad = true; o.status |= ST_PLUNGE; }
+      } else {
+        o.status |= (fwd.stop == ST_STATE) ? ST_STATE : ST_PLUNGE;
+      }
+      if (bad) {
+        if (anchor) return zero_all(ST_STATE);
+        o.jpl = j;
+        // nodes from j_pl on are copies of node j_pl - 1 with zero increments (as S3); the interval before them too
+        for (int64_t m = j; m <= o.Nc + G; ++m)
+          for (int q = 0; q < 5; ++q) {
+            o.val[q][m + G] = (j > ja) ? o.val[q][jj - 1] : (real)0;
+            o.slope[q][m + G] = (j > ja) ? o.slope[q][jj - 1] : (real)0;
+            o.inc[q][m + G] = 0;
+          }
+        if (j > ja) for (int q = 0; q < 5; ++q) o.inc[q][jj - 1] = 0;
+        break;
+      }
+      real f[5];
+      rhs(w, y, pn_mask, f);
+      for (int q = 0; q < 5; ++q) { o.val[q][jj] = y[q]; o.slope[q][jj] = f[q]; }
+      if (j > ja) {
+        real d[5];
+        change(prev, p, d);
+        for (int q = 0; q < 5; ++q) o.inc[q][jj - 1] = d[q];
+      }
+      prev = p; hint = p.n;
+    }
+  }
+  // backward side: nodes ja - 1 .. -G, in the branch's order (decreasing time); increments are stored in forward time
+  {
+    int64_t hint = 0;
+    Pos prev{&bwd, 0, 0, true};                       // the anchor node itself: step 0, theta 0
+    if (bwd.steps.empty()) return zero_all(ST_STATE);
+    for (int64_t j = ja - 1; j >= -G; --j) {
+      const int64_t jj = j + G;
+      Pos p = locate(j, hint, bwd);
+      if (!p.ok) return zero_all(ST_STATE);
+      real y[5], f[5], d[5];
+      node_state(p, y);
+      if (!state_ok(y)) return zero_all(ST_STATE);
+      rhs(w, y, pn_mask, f);
+      for (int q = 0; q < 5; ++q) { o.val[q][jj] = y[q]; o.slope[q][jj] = f[q]; }
+      change(prev, p, d);                              // from node j + 1 to node j
+      for (int q = 0; q < 5; ++q) o.inc[q][jj] = -d[q];
+      prev = p; hint = p.n;
+    }
+  }
+  return o;
+}
+
 // anchor: 0 = the parameter row is the state at the first sample (forward), 1 = at plunge, at the last coarse node (D12)
-Orbit integrate_orbit(const Walker& w, int64_t N, real dt, int S, int pn_mask, int anchor) {
+// adaptive: NULL = the fixed-step RK4 of S3; else {rtol, atol[5]} of the embedded pair of S3'
+Orbit integrate_orbit(const Walker& w, int64_t N, real dt, int S, int pn_mask, int anchor, const double* adaptive) {
+  if (adaptive) {
+    real at[5];
+    for (int q = 0; q < 5; ++q) at[q] = (real)adaptive[1 + q];
+    return integrate_orbit_adaptive(w, N, dt, S, pn_mask, anchor, (real)adaptive[0], at);
+  }
   if (anchor) return integrate_orbit_from_lso(w, N, dt, S, pn_mask);
   Orbit o;
   o.G = 1;
@@ -592,10 +896,10 @@ void emri_o_rhs(const double* params, const double* y, int pn_mask, double* f) {
 // coarse orbit.  Outputs (each may be NULL): val, slope, inc are [5][Nn] row-major with
 // Nn = ceil(N/S) + 3, node j at column j+1; info = {Nn, jpl (node index j, or Nn if none), status}
 int emri_o_orbit(const double* params, int64_t N, double dt, int S, int pn_mask, double H0, double Om,
-                 double* val, double* slope, double* inc, int64_t* info, int anchor) {
+                 double* val, double* slope, double* inc, int64_t* info, int anchor, const double* adaptive) {
   Cosmo c{(real)H0, (real)Om};
   Walker w = make_walker(params, c);
-  Orbit o = integrate_orbit(w, N, (real)dt, S, pn_mask, anchor);
+  Orbit o = integrate_orbit(w, N, (real)dt, S, pn_mask, anchor, adaptive);
   for (int q = 0; q < 5; ++q)
     for (int64_t m = 0; m < o.Nn; ++m) {
       if (val) val[q * o.Nn + m] = (double)o.val[q][m];
@@ -609,16 +913,39 @@ int emri_o_orbit(const double* params, int64_t N, double dt, int S, int pn_mask,
 // orbit interpolated at sample indices idx[0..n_idx): out[5][n_idx] (angles in cycles, unwrapped
 // relative to the wrapped node value)
 int emri_o_orbit_at(const double* params, int64_t N, double dt, int S, int pn_mask, double H0, double Om,
-                    const int64_t* idx, int64_t n_idx, double* out, int anchor) {
+                    const int64_t* idx, int64_t n_idx, double* out, int anchor, const double* adaptive) {
   Cosmo c{(real)H0, (real)Om};
   Walker w = make_walker(params, c);
-  Orbit o = integrate_orbit(w, N, (real)dt, S, pn_mask, anchor);
+  Orbit o = integrate_orbit(w, N, (real)dt, S, pn_mask, anchor, adaptive);
   for (int64_t m = 0; m < n_idx; ++m) {
     int64_t j; real s;
     split_time(idx[m], S, w.dT / o.Delta, &j, &s);
     for (int q = 0; q < 5; ++q) out[q * n_idx + m] = (double)hermite(o, q, j, s);
   }
   return 0;
+}
+
+// S3' for the pins: the accepted steps of the adaptive integration from the parameter row's state at t = 0 to t_end (either
+// sign).  Returns the number of steps (at most max_steps are written): t[n], h[n], y[n][5] (angles wrapped), turns[n][3],
+// Q[n][5][4]; info = {stop bit, t reached}.
+int64_t emri_o_dp5_steps(const double* params, double t_end, double rtol, const double* atol, int pn_mask, double H0, double Om,
+                         int stop_at_plunge, int64_t max_steps, double* t, double* h, double* y, double* turns, double* Q,
+                         double* info) {
+  Cosmo c{(real)H0, (real)Om};
+  Walker w = make_walker(params, c);
+  real at[5];
+  for (int q = 0; q < 5; ++q) at[q] = (real)atol[q];
+  Dp5Branch br = dp5_integrate(w, w.p0, 0, (real)t_end, (real)rtol, at, pn_mask, stop_at_plunge != 0);
+  const int64_t n = (int64_t)br.steps.size();
+  for (int64_t i = 0; i < n && i < max_steps; ++i) {
+    const Dp5Step& st = br.steps[i];
+    t[i] = (double)st.t; h[i] = (double)st.h;
+    for (int q = 0; q < 5; ++q) y[5 * i + q] = (double)st.y[q];
+    for (int a = 0; a < 3; ++a) turns[3 * i + a] = (double)st.turns[a];
+    for (int q = 0; q < 5; ++q) for (int j = 0; j < 4; ++j) Q[(5 * i + q) * 4 + j] = (double)st.Q[q][j];
+  }
+  if (info) { info[0] = br.stop; info[1] = (double)br.t_end; }
+  return n;
 }
 
 // Hermite basis check: interpolate a caller-supplied single interval
@@ -645,10 +972,11 @@ void emri_o_antenna(double cthd, double phid, double psi, double* F) {
 // waveform at selected sample indices (idx == NULL: all samples 0..N-1, n_idx = N).
 // hI, hII: [n_idx]; Apl, Acr (may be NULL): polarisation amplitudes A+, Ax.  Returns status bits.
 int emri_o_waveform(const double* params, int64_t N, double dt, int n_max, int S, double H0, double Om,
-                    const int64_t* idx, int64_t n_idx, double* hI, double* hII, double* Apl, double* Acr, int anchor) {
+                    const int64_t* idx, int64_t n_idx, double* hI, double* hII, double* Apl, double* Acr, int anchor,
+                    const double* adaptive) {
   Cosmo c{(real)H0, (real)Om};
   Walker w = make_walker(params, c);
-  Orbit o = integrate_orbit(w, N, (real)dt, S, 3, anchor);
+  Orbit o = integrate_orbit(w, N, (real)dt, S, 3, anchor, adaptive);
   o.status = finish_status(w, o);
   for (int64_t m = 0; m < n_idx; ++m) {
     int64_t i = idx ? idx[m] : m;
@@ -663,11 +991,11 @@ int emri_o_waveform(const double* params, int64_t N, double dt, int n_max, int S
 // batch of K walkers, all samples, OpenMP over walkers only.  h: [K][2][N] (channel I then II),
 // status: [K]
 int emri_o_waveform_batch(const double* params, int K, int64_t N, double dt, int n_max, int S, double H0,
-                          double Om, double* h, int32_t* status, int anchor) {
+                          double Om, double* h, int32_t* status, int anchor, const double* adaptive) {
 #pragma omp parallel for schedule(dynamic, 1)
   for (int k = 0; k < K; ++k)
     status[k] = emri_o_waveform(params + (size_t)k * NPAR, N, dt, n_max, S, H0, Om, nullptr, N,
-                                h + (size_t)k * 2 * N, h + (size_t)k * 2 * N + N, nullptr, nullptr, anchor);
+                                h + (size_t)k * 2 * N, h + (size_t)k * 2 * N + N, nullptr, nullptr, anchor, adaptive);
   return 0;
 }
 
@@ -757,14 +1085,14 @@ double emri_o_inner(const double* A, const double* B, const double* psd, int64_t
 // status-1/4/8 walkers get -inf.  spectra (may be NULL): [K][2][N/2+1] complex out.
 int emri_o_loglike_batch(const double* params, int K, int64_t N, double dt, int n_max, int S, double H0,
                          double Om, const double* D, const double* psd, double* logL, int32_t* status,
-                         double* spectra, int anchor) {
+                         double* spectra, int anchor, const double* adaptive) {
   const int64_t Nf = N / 2 + 1;
   int rc = 0;
 #pragma omp parallel for schedule(dynamic, 1)
   for (int k = 0; k < K; ++k) {
     std::vector<double> h(2 * (size_t)N), H(4 * (size_t)Nf);
     int st = emri_o_waveform(params + (size_t)k * NPAR, N, dt, n_max, S, H0, Om, nullptr, N, h.data(),
-                             h.data() + N, nullptr, nullptr, anchor);
+                             h.data() + N, nullptr, nullptr, anchor, adaptive);
     if (emri_o_rfft(h.data(), N, H.data()) || emri_o_rfft(h.data() + N, N, H.data() + 2 * Nf)) {
 #pragma omp atomic write
       rc = -1;

@@ -29,8 +29,9 @@ def _f64(a):
 
 
 class Oracle:
-    def __init__(self, long_double=False, anchor=False):
+    def __init__(self, long_double=False, anchor=False, adaptive=None):
         self.anchor = 1 if anchor else 0
+        self.set_adaptive(adaptive)
         lib, lib_ld = build_oracle.build()
         self.lib = L = C.CDLL(lib_ld if long_double else lib)
         L.emri_o_real_bits.restype = C.c_int
@@ -47,18 +48,18 @@ class Oracle:
         L.emri_o_walker_scalars.argtypes = [_dp, C.c_double, C.c_double, _dp]
         L.emri_o_rhs.argtypes = [_dp, _dp, C.c_int, _dp]
         L.emri_o_orbit.argtypes = [_dp, C.c_int64, C.c_double, C.c_int, C.c_int, C.c_double, C.c_double,
-                                   _dp, _dp, _dp, _ip, C.c_int]
+                                   _dp, _dp, _dp, _ip, C.c_int, _dp]
         L.emri_o_orbit_at.argtypes = [_dp, C.c_int64, C.c_double, C.c_int, C.c_int, C.c_double, C.c_double,
-                                      _ip, C.c_int64, _dp, C.c_int]
+                                      _ip, C.c_int64, _dp, C.c_int, _dp]
         L.emri_o_hermite1.restype = C.c_double
         L.emri_o_hermite1.argtypes = [C.c_double] * 6
         L.emri_o_geometry.argtypes = [_dp, C.c_double, C.c_double, _dp]
         L.emri_o_antenna.argtypes = [C.c_double, C.c_double, C.c_double, _dp]
         L.emri_o_waveform.restype = C.c_int
         L.emri_o_waveform.argtypes = [_dp, C.c_int64, C.c_double, C.c_int, C.c_int, C.c_double, C.c_double,
-                                      _ip, C.c_int64, _dp, _dp, _dp, _dp, C.c_int]
+                                      _ip, C.c_int64, _dp, _dp, _dp, _dp, C.c_int, _dp]
         L.emri_o_waveform_batch.argtypes = [_dp, C.c_int, C.c_int64, C.c_double, C.c_int, C.c_int,
-                                            C.c_double, C.c_double, _dp, _i32p, C.c_int]
+                                            C.c_double, C.c_double, _dp, _i32p, C.c_int, _dp]
         L.emri_o_rfft.restype = C.c_int
         L.emri_o_rfft.argtypes = [_dp, C.c_int64, _dp]
         L.emri_o_dft_naive.argtypes = [_dp, C.c_int64, _dp]
@@ -70,7 +71,32 @@ class Oracle:
         L.emri_o_inner.argtypes = [_dp, _dp, _dp, C.c_int64, C.c_double]
         L.emri_o_loglike_batch.restype = C.c_int
         L.emri_o_loglike_batch.argtypes = [_dp, C.c_int, C.c_int64, C.c_double, C.c_int, C.c_int, C.c_double,
-                                           C.c_double, _dp, _dp, _dp, _i32p, _dp, C.c_int]
+                                           C.c_double, _dp, _dp, _dp, _i32p, _dp, C.c_int, _dp]
+
+    def set_adaptive(self, adaptive):
+        """None: the fixed-step RK4 of S3.  (rtol, atol[5]): the embedded Dormand-Prince pair with dense output (S3', D14)"""
+        if adaptive is None:
+            self._adaptive, self._adp = None, None
+        else:
+            rtol, atol = adaptive
+            self._adaptive = np.ascontiguousarray(np.concatenate([[float(rtol)], np.broadcast_to(atol, (5,))]), dtype=np.float64)
+            self._adp = self._adaptive.ctypes.data_as(_dp)
+
+    def dp5_steps(self, params, t_end, rtol, atol, pn_mask=3, stop_at_plunge=False, max_steps=200000,
+                  H0=H0_DEFAULT, Om=OM_DEFAULT):
+        """accepted steps of the adaptive integration from t = 0 to t_end -> dict(t, h, y[n][5], turns[n][3], Q[n][5][4], stop, t_reached)"""
+        p = _f64(params)
+        at = np.ascontiguousarray(np.broadcast_to(atol, (5,)), dtype=np.float64)
+        t, h = np.zeros(max_steps), np.zeros(max_steps)
+        y, tu, Q = np.zeros((max_steps, 5)), np.zeros((max_steps, 3)), np.zeros((max_steps, 5, 4))
+        info = np.zeros(2)
+        self.lib.emri_o_dp5_steps.restype = C.c_int64
+        self.lib.emri_o_dp5_steps.argtypes = [_dp, C.c_double, C.c_double, _dp, C.c_int, C.c_double, C.c_double, C.c_int,
+                                              C.c_int64, _dp, _dp, _dp, _dp, _dp, _dp]
+        n = self.lib.emri_o_dp5_steps(_d(p), float(t_end), float(rtol), _d(at), pn_mask, H0, Om, 1 if stop_at_plunge else 0,
+                                      max_steps, _d(t), _d(h), _d(y), _d(tu), _d(Q), _d(info))
+        n = min(int(n), max_steps)
+        return dict(t=t[:n], h=h[:n], y=y[:n], turns=tu[:n], Q=Q[:n], stop=int(info[0]), t_reached=float(info[1]))
 
     def set_anchor(self, at_lso):
         """False (default): the parameter row is the state at t = 0; True: at plunge, at the last coarse node (D12).
@@ -127,14 +153,14 @@ class Oracle:
         val, slope, inc = (np.zeros((5, Nn)) for _ in range(3))
         info = np.zeros(3, dtype=np.int64)
         self.lib.emri_o_orbit(_d(p), N, dt, S, pn_mask, H0, Om, _d(val), _d(slope), _d(inc),
-                              info.ctypes.data_as(_ip), self.anchor)
+                              info.ctypes.data_as(_ip), self.anchor, self._adp)
         return dict(val=val, slope=slope, inc=inc, Nn=int(info[0]), jpl=int(info[1]), status=int(info[2]))
 
     def orbit_at(self, params, N, dt, idx, S=256, pn_mask=3, H0=H0_DEFAULT, Om=OM_DEFAULT):
         p = _f64(params)
         ii = np.ascontiguousarray(idx, dtype=np.int64)
         out = np.zeros((5, ii.size))
-        self.lib.emri_o_orbit_at(_d(p), N, dt, S, pn_mask, H0, Om, ii.ctypes.data_as(_ip), ii.size, _d(out), self.anchor)
+        self.lib.emri_o_orbit_at(_d(p), N, dt, S, pn_mask, H0, Om, ii.ctypes.data_as(_ip), ii.size, _d(out), self.anchor, self._adp)
         return out
 
     def hermite1(self, y0, inc, m0, m1, Delta, s):
@@ -164,7 +190,7 @@ class Oracle:
         hI, hII = np.zeros(n), np.zeros(n)
         Ap, Ax = (np.zeros(n), np.zeros(n)) if amplitudes else (None, None)
         st = self.lib.emri_o_waveform(_d(p), N, dt, n_max, S, H0, Om, ptr, n, _d(hI), _d(hII),
-                                      _d(Ap) if amplitudes else None, _d(Ax) if amplitudes else None, self.anchor)
+                                      _d(Ap) if amplitudes else None, _d(Ax) if amplitudes else None, self.anchor, self._adp)
         return (hI, hII, st, Ap, Ax) if amplitudes else (hI, hII, st)
 
     def waveform_batch(self, params, N, dt, n_max, S=256, H0=H0_DEFAULT, Om=OM_DEFAULT):
@@ -173,7 +199,7 @@ class Oracle:
         K = p.shape[0]
         h = np.zeros((K, 2, N))
         st = np.zeros(K, dtype=np.int32)
-        self.lib.emri_o_waveform_batch(_d(p), K, N, dt, n_max, S, H0, Om, _d(h), st.ctypes.data_as(_i32p), self.anchor)
+        self.lib.emri_o_waveform_batch(_d(p), K, N, dt, n_max, S, H0, Om, _d(h), st.ctypes.data_as(_i32p), self.anchor, self._adp)
         return h, st
 
     # ---- transform and likelihood
@@ -224,7 +250,7 @@ class Oracle:
         sp = np.zeros((K, 2, N // 2 + 1), dtype=np.complex128) if spectra else None
         rc = self.lib.emri_o_loglike_batch(_d(p), K, N, dt, n_max, S, H0, Om, _d(Dc.view(np.float64)), _d(s),
                                            _d(logL), st.ctypes.data_as(_i32p),
-                                           _d(sp.view(np.float64)) if spectra else None, self.anchor)
+                                           _d(sp.view(np.float64)) if spectra else None, self.anchor, self._adp)
         if rc:
             raise ValueError("oracle loglike_batch failed (N must be a power of two)")
         return (logL, st, sp) if spectra else (logL, st)

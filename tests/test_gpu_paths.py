@@ -277,3 +277,26 @@ def test_graph_replay_gives_the_same_bits_and_follows_its_inputs(emri):
         out = plan.loglike(p_d, D).cpu().numpy()
     assert np.array_equal(out, ref[::-1])
     plan.close()
+
+
+def test_second_noise_model_matches_oracle(emri, oracle):
+    """the paper's second noise curve (refs [51, 52]: Robson-Cornish-Liu with the galactic confusion fit,
+    a PSD with a sharp knee and 1e10 of dynamic range) through Eq. 8, both transform paths, against the oracle's whole path"""
+    cfg = W.scaled(W.CONFIGS[1], K=6, N=1 << 16)
+    P = W.draw_params(cfg)
+    psd = W.lisa_psd_robson(cfg.N, cfg.dt)
+    assert np.all(psd[1:-1] > 0) and np.isinf(psd[0]) and np.isinf(psd[-1])
+    h_ref, _ = oracle.waveform_batch(P[:1], cfg.N, cfg.dt, cfg.n_max)
+    D = np.stack([oracle.rfft(h_ref[0, 0]), oracle.rfft(h_ref[0, 1])]) + W.noise_fft(cfg.N, cfg.dt, psd, 11)
+    ref, st_ref = oracle.loglike_batch(P, cfg.N, cfg.dt, cfg.n_max, D, psd)
+    plan = emri.Plan(cfg.N, cfg.dt, cfg.n_max, cfg.K, psd)
+    for fused in (True, False):
+        plan.set_transform(fused)
+        got = plan.loglike(dev(P), dev(D)).cpu().numpy()
+        print("Robson PSD, fused" if fused else "Robson PSD, plain", np.abs(got - ref) / np.abs(ref))
+        assert np.all(np.abs(got - ref) <= 1e-9 * np.abs(ref) + 1e-6)
+    # and it is a different likelihood from the Barack-Cutler one
+    plan_bc = emri.Plan(cfg.N, cfg.dt, cfg.n_max, cfg.K, W.lisa_psd_barack_cutler(cfg.N, cfg.dt))
+    other = plan_bc.loglike(dev(P), dev(D)).cpu().numpy()
+    assert np.all(np.abs(other - ref) > 1e-3 * np.abs(ref))
+    plan.close(); plan_bc.close()

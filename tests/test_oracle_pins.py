@@ -987,3 +987,98 @@ def test_paper_fig1_grid_last_hour_before_plunge(lso):
         crossings = np.sum(np.signbit(hI[1:]) != np.signbit(hI[:-1]))
         # (with spin the precession of the orbital plane, alpha' ~ 0.1 nu at a = 0.8, shifts the observed phase by a few per cent)
         assert crossings == pytest.approx(2 * (2 * f_az) * N * dt, rel=0.10)
+
+
+# ----------------------------------------------------------------------------- S3': adaptive embedded pair with dense output (f-3, D14)
+DP_ATOL = np.array([1e-9, 1e-18, 1e-9, 1e-14, 1e-9])
+
+
+def _cycles_state(p):
+    return np.array([(p[W.P_PHI0] / TWOPI) % 1.0, p[W.P_NU0], (p[W.P_GAM0] / TWOPI) % 1.0, p[W.P_E0], (p[W.P_ALP0] / TWOPI) % 1.0])
+
+
+def _dense(r, tq):
+    """the oracle's dense output, unwrapped (turns + wrapped value + offset), at times tq"""
+    idx = np.clip(np.searchsorted(np.abs(r["t"]), np.abs(tq), side="right") - 1, 0, len(r["t"]) - 1)
+    th = (tq - r["t"][idx]) / r["h"][idx]
+    Y = r["y"][idx] + sum(r["Q"][idx][:, :, j] * th[:, None] ** (j + 1) for j in range(4))
+    for a, q in enumerate((0, 2, 4)):
+        Y[:, q] += r["turns"][idx, a]
+    return Y
+
+
+@pytest.mark.parametrize("T,rtol", [(2 ** 16 * 15.0, 1e-9), (2 ** 20 * 15.0, 1e-12), (-50 * 3840.0, 1e-11)])
+def test_adaptive_pair_takes_scipy_rk45_steps_and_dense_output(oracle, T, rtol):
+    """the paper integrates with SciPy's solve_ivp.  The oracle's Dormand-Prince 5(4) + step controller +
+    continuous extension against solve_ivp(method="RK45") on the same right-hand side (in cycles): the same number of
+    accepted steps at the same times, the same dense output -- forward over 11 days and half a year, and backwards.
+    (A wrong tableau entry, controller constant, exponent, first-step rule or dense-output coefficient fails this.)"""
+    P = W.draw_params(W.CONFIGS[1], K=3)
+    for k in range(3):
+        p = P[k]
+        r = oracle.dp5_steps(p, T, rtol, DP_ATOL)
+        sol = scipy.integrate.solve_ivp(lambda t, y: oracle.rhs(p, y), (0.0, T), _cycles_state(p), method="RK45", rtol=rtol,
+                                        atol=DP_ATOL, dense_output=True)
+        assert r["stop"] == 0 and r["t_reached"] == T
+        assert len(r["t"]) == len(sol.t) - 1
+        # SciPy carries the angles unwrapped (1e4 cycles: 2e-12 of rounding in its error estimate), hence not bit-equal
+        np.testing.assert_allclose(r["t"], sol.t[:-1], rtol=1e-5, atol=1e-9)
+        np.testing.assert_allclose(r["t"][:4], sol.t[:4], rtol=1e-12, atol=0)          # the first-step rule, exactly
+        tq = np.sort(np.random.default_rng(k).uniform(min(0.0, T), max(0.0, T), 300))
+        Y, S = _dense(r, tq), sol.sol(tq).T
+        for q in range(5):
+            assert np.max(np.abs(Y[:, q] - S[:, q])) <= 2e-15 * max(1.0, np.max(np.abs(S[:, q]))) + 1e-24
+
+
+def test_adaptive_orbit_nodes_are_consistent_and_converge_to_the_rk4_orbit(oracle):
+    """the node table sampled from the dense output: increments and values agree, slopes are the right-hand side at the
+    node, and with a tight tolerance it is the same orbit as the fixed-step scheme (both converge to the ODE solution)"""
+    from oracle.oracle import Oracle
+    p = W.draw_params(W.CONFIGS[1], K=1)[0]
+    N, dt, S = 1 << 18, 15.0, 256
+    ada = Oracle(adaptive=(1e-13, DP_ATOL * 1e-4))
+    a, f = ada.orbit(p, N, dt, S), oracle.orbit(p, N, dt, S)
+    assert a["status"] == 0 and a["Nn"] == f["Nn"] and a["jpl"] == a["Nn"]
+    v, inc, sl = a["val"], a["inc"], a["slope"]
+    for q in (0, 2, 4):
+        assert np.max(np.abs(circ_diff(v[q][:-1] + inc[q][:-1], v[q][1:]))) < 2e-14
+        assert np.max(np.abs(circ_diff(v[q], f["val"][q]))) < 1e-9            # 5th-order pair at 1e-13 against RK4 at 3840 s
+        np.testing.assert_allclose(inc[q][:-1], f["inc"][q][:-1], rtol=1e-10, atol=1e-12)
+    for q in (1, 3):
+        np.testing.assert_allclose(v[q][:-1] + inc[q][:-1], v[q][1:], rtol=1e-15)
+        np.testing.assert_allclose(v[q], f["val"][q], rtol=1e-12)
+    for jj in (0, 1, 500, a["Nn"] - 1):
+        np.testing.assert_array_equal(sl[:, jj], oracle.rhs(p, v[:, jj]))
+    # the initial state sits on node 0 exactly
+    np.testing.assert_array_equal(v[:, 1], _cycles_state(p))
+    # and the waveform through the same Hermite + harmonic sum agrees at the level the two orbits do
+    idx = np.arange(0, N, 997)
+    hA = ada.waveform(p, N, dt, 10, idx=idx)[0]
+    hF = oracle.waveform(p, N, dt, 10, idx=idx)[0]
+    assert np.max(np.abs(hA - hF)) < 1e-6 * np.max(np.abs(hF))
+
+
+def test_adaptive_orbit_plunge_and_lso_anchor(oracle):
+    from oracle.oracle import Oracle
+    p = W.draw_params(W.CONFIGS[1], K=1)[0].copy()
+    N, dt, S = 1 << 14, 15.0, 256
+    ada = Oracle(adaptive=(1e-12, DP_ATOL * 1e-3))
+    # forward convention, plunging inside the window: same truncation node as the fixed-step scheme (or its neighbour)
+    p[W.P_NU0] = 0.9995 * oracle.nu_lso(p[W.P_M], p[W.P_E0])
+    a, f = ada.orbit(p, N, dt, S), oracle.orbit(p, N, dt, S)
+    assert a["status"] == 2 and f["status"] == 2 and abs(a["jpl"] - f["jpl"]) <= 1 and 0 < a["jpl"] < a["Nn"] - 2
+    jj = a["jpl"] + 1                                      # column of node j_pl
+    np.testing.assert_array_equal(a["val"][:, jj], a["val"][:, jj - 1])      # copies of node j_pl - 1, zero increments
+    assert not a["inc"][:, jj - 1:].any()
+    # the LSO convention: anchored on nu_LSO at the last node, integrated backwards; agrees with the fixed-step LSO orbit
+    p[W.P_E0] = 0.3
+    adaL, fixL = Oracle(anchor=True, adaptive=(1e-13, DP_ATOL * 1e-4)), Oracle(anchor=True)
+    a, f = adaL.orbit(p, N, dt, S), fixL.orbit(p, N, dt, S)
+    assert a["status"] == 0 and f["status"] == 0
+    assert a["val"][1][-2] == f["val"][1][-2] == pytest.approx(oracle.nu_lso(p[W.P_M], 0.3), rel=1e-15)
+    np.testing.assert_allclose(a["val"][1], f["val"][1], rtol=1e-9)
+    np.testing.assert_allclose(a["val"][3], f["val"][3], rtol=1e-9)
+    assert np.max(np.abs(circ_diff(a["val"][0], f["val"][0]))) < 1e-6        # the last hours before plunge are stiff for RK4
+    # a bad parameter row stays bad
+    p[W.P_MU] = -1.0
+    assert adaL.orbit(p, N, dt, S)["status"] == 1
