@@ -135,7 +135,8 @@ def workload_config(cfg, args):
     return {"workload": f"configs[{cfg.index}]: K={cfg.K} walkers per GPU, N={cfg.N}, dt={cfg.dt} s, n_max={cfg.n_max}, "
                         f"data = injection{' + coloured noise' if cfg.noise_seed else ''}, "
                         f"PSD = {'Robson-Cornish-Liu' if args.psd == 'robson' else 'Barack-Cutler'}"
-                        + (", a step = one stretch-move update of the ensemble" if cfg.index in (4, 5) else ""),
+                        + (", a step = one stretch-move update of the ensemble" if cfg.index in (4, 5) else "")
+                        + (f", orbit by adaptive DP5(4) at rtol {args.adaptive:g}" if getattr(args, "adaptive", 0) else ""),
             "l2": f"per-step working set {16 * cfg.K * cfg.N / 1e6:.0f} MB > 126 MB L2: no flush needed"
                   if 16 * cfg.K * cfg.N > 126e6 else "per-step working set fits L2 (launch-bound case, reported as is)"}
 
@@ -227,6 +228,9 @@ def run_gpu(args, cfg):
     plan = emri.Plan(N, cfg.dt, cfg.n_max, K, psd)
     if cfg.index == 5:
         plan.set_anchor(True)            # the paper's convention: initial conditions at the LSO, integrated backwards
+    if args.adaptive:
+        # the paper's own kind of integrator: embedded pair, step control, dense output
+        plan.set_integrator((args.adaptive, args.adaptive * np.array([1.0, 1e-9, 1.0, 1e-5, 1.0])))
     p_d = torch.from_numpy(P).to(dev)
     # data = the library's own injection of walker 0 (+ seeded coloured noise when the config says so)
     spec = plan.waveform_fft(p_d[:1].contiguous())
@@ -369,6 +373,8 @@ def main():
                     help="index into BASELINE.json:configs (0-4; 4 = stretch-move steps); 5 = the paper's own run shape")
     ap.add_argument("--psd", default="bc", choices=["bc", "robson"],
                     help="noise curve: Barack-Cutler (the paper's example) or Robson-Cornish-Liu (its second model)")
+    ap.add_argument("--adaptive", type=float, default=0.0, metavar="RTOL",
+                    help="stage (a) by the adaptive Dormand-Prince 5(4) pair with this relative tolerance instead of fixed-step RK4")
     ap.add_argument("--impl", default="b200", choices=["b200", "reference"])
     args = ap.parse_args()
     cfg = W.CONFIGS[args.config]

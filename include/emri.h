@@ -96,6 +96,23 @@ int emri_plan_set_coarse_stride(emri_plan* p, int S);
  * the schedule and used by the tests).  Both evaluate the same scheme (S3). */
 int emri_plan_set_orbit_schedule(emri_plan* p, int schedule);
 
+/* Which integrator stage (a) uses.  kind 0 (default): the fixed-step RK4 of BASELINE.json's north_star (the two schedules
+ * above).  kind 1: the paper's own kind of integrator ("standard ODE methods, such as the 7th-order
+ * Runge-Kutta scheme", :133 solve_ivp, :157; reading D14) -- an embedded Runge-Kutta pair with per-walker step
+ * control and dense output on the device: Dormand-Prince 5(4), the step-size controller solve_ivp uses (error norm = rms
+ * over the five components of err / (atol + rtol max(|Y|, |Y_new|)), angles counted in unwrapped cycles), Shampine's
+ * continuous extension.  The dense output is sampled at the coarse nodes (value; slope = right-hand side at the node;
+ * unwrapped increment), so every later stage is unchanged.  rtol > 0; atol: HOST [5] for (Phi [cycles], nu [Hz],
+ * gamma~ [cycles], e, alpha [cycles]); max_steps: accepted steps kept per walker (>= 16; a walker that needs more gets
+ * EMRI_ST_STATE).  Allocates K_max (max_steps + 64) 256 B of step records; synchronises.  Works with both anchors. */
+int emri_plan_set_integrator(emri_plan* p, int kind, double rtol, const double* atol, int max_steps);
+
+/* Diagnostics of the last adaptive orbit (kind 1): the accepted steps of walker k's branch (0: forward from the anchor,
+ * 1: backward).  t, h: HOST [max_out] start and signed size of each step; y: HOST [max_out][5] state at the start (angles
+ * wrapped, cycles), any of them may be NULL; info: HOST int32 [2] = {steps taken, 0 / EMRI_ST_PLUNGE / EMRI_ST_STATE why
+ * the branch ended early}.  Synchronises. */
+int emri_plan_orbit_steps(emri_plan* p, int k, int branch, int max_out, double* t, double* h, double* y, int32_t* info);
+
 /* Where the orbital state of the parameter row is given.  0 (default): at the first sample, t = 0, integrated forward.
  * 1: the paper's own convention ("initial conditions at the LSO ... integrated backwards"): the row's
  * e0, Phi0, gam0, alp0 are the values AT PLUNGE, placed at the last coarse node t = ceil(N/S) S dt (the end of the window),

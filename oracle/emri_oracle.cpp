@@ -351,8 +351,11 @@ real rms5(const real v[5]) {
 // bound.  |Y| is the UNWRAPPED angle (turns + fraction) so that the scale is what an integration in plain cycles sees,
 // while the state itself is kept wrapped (only frac matters downstream, D2).  stop_at_plunge: forward integration of a
 // walker given at t = 0 ends after the first accepted step whose end state is past nu_LSO(e) (reading R8).
+// forced (may be NULL): n_forced prescribed step sizes taken one after the other instead of the controller's -- the
+// teacher-forced half of the parity protocol (D14): at tolerances near rounding the error estimate is dominated
+// by rounding noise, so two correct implementations choose different steps; given the SAME steps they must agree.
 Dp5Branch dp5_integrate(const Walker& w, const real y0[5], real t0, real t_bound, real rtol, const real atol[5], int pn_mask,
-                        bool stop_at_plunge) {
+                        bool stop_at_plunge, const double* forced = nullptr, int64_t n_forced = 0) {
   Dp5Branch br;
   br.t_end = t0; br.stop = 0;
   const real dir = (t_bound >= t0) ? 1 : -1;
@@ -383,18 +386,19 @@ Dp5Branch dp5_integrate(const Walker& w, const real y0[5], real t0, real t_bound
     h_abs = std::min(std::min(100 * h0, h1), interval);
   }
   const real expo = (real)-1 / 5;
-  for (int n_steps = 0; t != t_bound; ++n_steps) {
+  for (int n_steps = 0; forced ? n_steps < n_forced : t != t_bound; ++n_steps) {
     if (n_steps >= 1000000) { br.stop = ST_STATE; break; }
     const real min_step = 10 * std::fabs(std::nextafter(t, dir * std::numeric_limits<real>::infinity()) - t);
     if (h_abs < min_step) h_abs = min_step;
     bool rejected = false;
     real K[7][5], y_new[5], h = 0, t_new = t;
     for (;;) {
-      if (h_abs < min_step) { br.stop = ST_STATE; br.t_end = t; return br; }
+      if (h_abs < min_step && !forced) { br.stop = ST_STATE; br.t_end = t; return br; }
       h = h_abs * dir;
       t_new = t + h;
       if (dir * (t_new - t_bound) > 0) t_new = t_bound;
       h = t_new - t;
+      if (forced) { h = (real)forced[n_steps]; t_new = t + h; }
       h_abs = std::fabs(h);
       for (int q = 0; q < 5; ++q) K[0][q] = f[q];
       for (int s = 1; s < 6; ++s) {
@@ -422,6 +426,7 @@ Dp5Branch dp5_integrate(const Walker& w, const real y0[5], real t0, real t_bound
         en[q] = e * h / sc;
       }
       const real err = rms5(en);
+      if (forced) break;
       if (err < 1) {
         real factor = (err == 0) ? (real)10 : std::min((real)10, (real)0.9 * std::pow(err, expo));
         if (rejected && factor > 1) factor = 1;
@@ -471,7 +476,9 @@ void dp5_offset(const Dp5Step& st, real theta, real off[5]) {
 // interval increments the unwrapped offset differences, pieced together step by step so that no large number is ever
 // differenced.  Between nodes S4's cubic Hermite is kept: at the default stride its truncation error is below the rounding of
 // the phases (D3), so sampling the dense output at every sample instead would change nothing above 1e-14 cycles.
-Orbit integrate_orbit_adaptive(const Walker& w, int64_t N, real dt, int S, int pn_mask, int anchor, real rtol, const real atol[5]) {
+Orbit integrate_orbit_adaptive(const Walker& w, int64_t N, real dt, int S, int pn_mask, int anchor, real rtol, const real atol[5],
+                               const double* forced_fwd = nullptr, int64_t n_fwd = 0, const double* forced_bwd = nullptr,
+                               int64_t n_bwd = 0) {
   Orbit o;
   o.G = 1;
   o.Nc = (N + S - 1) / S;
@@ -488,8 +495,8 @@ Orbit integrate_orbit_adaptive(const Walker& w, int64_t N, real dt, int S, int p
   if (anchor) y0[1] = nu_lso(w.Ms, y0[3]);
   else if (!(y0[1] < nu_lso(w.Ms, y0[3]))) { o.status |= ST_PLUNGE; o.jpl = 0; return o; }
   const real ta = (real)ja * o.Delta;
-  Dp5Branch fwd = dp5_integrate(w, y0, ta, (real)(o.Nc + G) * o.Delta, rtol, atol, pn_mask, !anchor);
-  Dp5Branch bwd = dp5_integrate(w, y0, ta, (real)(-G) * o.Delta, rtol, atol, pn_mask, false);
+  Dp5Branch fwd = dp5_integrate(w, y0, ta, (real)(o.Nc + G) * o.Delta, rtol, atol, pn_mask, !anchor, forced_fwd, n_fwd);
+  Dp5Branch bwd = dp5_integrate(w, y0, ta, (real)(-G) * o.Delta, rtol, atol, pn_mask, false, forced_bwd, n_bwd);
   auto zero_all = [&](int bit) {
     for (int q = 0; q < 5; ++q) {
       std::fill(o.val[q].begin(), o.val[q].end(), (real)0);
@@ -594,12 +601,16 @@ Orbit integrate_orbit_adaptive(const Walker& w, int64_t N, real dt, int S, int p
 }
 
 // anchor: 0 = the parameter row is the state at the first sample (forward), 1 = at plunge, at the last coarse node (D12)
-// adaptive: NULL = the fixed-step RK4 of S3; else {rtol, atol[5]} of the embedded pair of S3'
+// adaptive: NULL = the fixed-step RK4 of S3; else {rtol, atol[5], n_fwd, n_bwd, forced steps ...} of the embedded pair of S3'
 Orbit integrate_orbit(const Walker& w, int64_t N, real dt, int S, int pn_mask, int anchor, const double* adaptive) {
   if (adaptive) {
     real at[5];
     for (int q = 0; q < 5; ++q) at[q] = (real)adaptive[1 + q];
-    return integrate_orbit_adaptive(w, N, dt, S, pn_mask, anchor, (real)adaptive[0], at);
+    // adaptive[6], adaptive[7]: numbers of prescribed steps of the forward / backward branch (0: the controller decides),
+    // followed by the step sizes themselves
+    const int64_t nf = (int64_t)adaptive[6], nb = (int64_t)adaptive[7];
+    return integrate_orbit_adaptive(w, N, dt, S, pn_mask, anchor, (real)adaptive[0], at, nf ? adaptive + 8 : nullptr, nf,
+                                    nb ? adaptive + 8 + nf : nullptr, nb);
   }
   if (anchor) return integrate_orbit_from_lso(w, N, dt, S, pn_mask);
   Orbit o;

@@ -73,13 +73,17 @@ class Oracle:
         L.emri_o_loglike_batch.argtypes = [_dp, C.c_int, C.c_int64, C.c_double, C.c_int, C.c_int, C.c_double,
                                            C.c_double, _dp, _dp, _dp, _i32p, _dp, C.c_int, _dp]
 
-    def set_adaptive(self, adaptive):
-        """None: the fixed-step RK4 of S3.  (rtol, atol[5]): the embedded Dormand-Prince pair with dense output (S3', D14)"""
+    def set_adaptive(self, adaptive, forced_fwd=None, forced_bwd=None):
+        """None: the fixed-step RK4 of S3.  (rtol, atol[5]): the embedded Dormand-Prince pair with dense output (S3', D14).
+        forced_fwd / forced_bwd: prescribed step sizes of the two branches (teacher-forced parity), else the controller's"""
         if adaptive is None:
             self._adaptive, self._adp = None, None
         else:
             rtol, atol = adaptive
-            self._adaptive = np.ascontiguousarray(np.concatenate([[float(rtol)], np.broadcast_to(atol, (5,))]), dtype=np.float64)
+            ff = np.zeros(0) if forced_fwd is None else np.asarray(forced_fwd, dtype=np.float64)
+            fb = np.zeros(0) if forced_bwd is None else np.asarray(forced_bwd, dtype=np.float64)
+            self._adaptive = np.ascontiguousarray(np.concatenate([[float(rtol)], np.broadcast_to(atol, (5,)),
+                                                                  [float(ff.size), float(fb.size)], ff, fb]), dtype=np.float64)
             self._adp = self._adaptive.ctypes.data_as(_dp)
 
     def dp5_steps(self, params, t_end, rtol, atol, pn_mask=3, stop_at_plunge=False, max_steps=200000,

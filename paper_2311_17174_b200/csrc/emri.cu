@@ -27,6 +27,7 @@
 
 #include "common.cuh"
 #include "orbit.cuh"
+#include "orbit_dp5.cuh"
 #include "synth.cuh"
 #include "loglike.cuh"
 #include "fftlike.cuh"
@@ -50,6 +51,11 @@ struct emri_plan {
   double2* d_nodeaux = nullptr;
   int32_t* d_jpl = nullptr;
   int32_t* d_status = nullptr;
+  // adaptive embedded pair (orbit_dp5.cuh): emri_plan_set_integrator
+  int integrator = 0, dp_cap = 0;
+  double dp_rtol = 1e-12, dp_atol[5] = {1e-12, 1e-21, 1e-12, 1e-17, 1e-12};
+  double* d_dpsteps = nullptr;
+  int32_t* d_dpn = nullptr; int32_t* d_dpstop = nullptr; int32_t* d_dpbad = nullptr; int32_t* d_dpzero = nullptr;
   // multiple-shooting orbit (orbit.cuh): segment records, per-walker mode / tail start / post-plunge row
   int orbit_mode = 1, anchor_end = 0, seg_L = 0, seg_P = 0, unit_tiles_override = 0, unit_tiles_cap = 8;
   int synth_debug = 0;                       // emri_plan_set_synth_debug
@@ -313,6 +319,22 @@ int run_orbit(emri_plan* p, const double* params, int K, cudaStream_t s) {
   a.tH = kMpcMetre / (p->H0 * 1000.0); a.Om = p->Om; a.anchor_end = p->anchor_end;
   a.wc = p->d_wc; a.nodes = p->d_nodes; a.jpl = p->d_jpl; a.status = p->d_status; a.nodeaux = p->d_nodeaux;
   const unsigned aux_grid = (unsigned)(((int64_t)K * p->Nn + 127) / 128);
+  if (p->integrator == 1) {
+    // the paper's own kind of integrator: adaptive embedded pair, dense output sampled at the coarse nodes
+    Dp5Args d;
+    d.o = a; d.rtol = p->dp_rtol;
+    for (int q = 0; q < 5; ++q) d.atol[q] = p->dp_atol[q];
+    d.steps = p->d_dpsteps; d.nsteps = p->d_dpn; d.stop = p->d_dpstop; d.first_bad = p->d_dpbad; d.zero_flag = p->d_dpzero;
+    d.cap_long = p->dp_cap;
+    orbit_dp5_kernel<<<(K + 31) / 32, 32, 0, s>>>(d);
+    DBG("orbit_dp5_kernel");
+    orbit_dp5_nodes_kernel<<<aux_grid, 128, 0, s>>>(d);
+    DBG("orbit_dp5_nodes_kernel");
+    orbit_dp5_finish_kernel<<<aux_grid, 128, 0, s>>>(d);
+    p->launches += 3;
+    CK(cudaGetLastError());
+    return EMRI_OK;
+  }
   if (p->orbit_mode == 0) {
     // reference schedule: the whole recursion in one thread per walker
     orbit_kernel<<<(K + 31) / 32, 32, 0, s>>>(a);
@@ -584,7 +606,8 @@ int emri_plan_destroy(emri_plan* p) {
   void* ptrs[] = {p->d_w, p->d_wc, p->d_nodes, p->d_hbuf, p->d_partial, p->d_base, p->d_nodeaux, p->d_jpl, p->d_status,
                   p->d_params, p->d_data, p->d_logL, p->d_Y, p->d_z, p->d_lnu, p->d_logLY, p->d_inbox,
                   p->d_partner, p->d_fftwork, p->d_seg, p->d_plrow, p->d_mode, p->d_pclamp, p->d_counts,
-                  p->d_twid, p->d_twA, p->d_twB, p->d_alpha, p->d_gamma, p->d_cdpart};
+                  p->d_twid, p->d_twA, p->d_twB, p->d_alpha, p->d_gamma, p->d_cdpart, p->d_dpsteps, p->d_dpn, p->d_dpstop,
+                  p->d_dpbad, p->d_dpzero};
   for (void* q : ptrs) if (q) cudaFree(q);
   delete p;
   return EMRI_OK;
@@ -637,6 +660,52 @@ int emri_plan_synth_report(emri_plan* p, int64_t counts[16]) {
   unsigned long long h[SYN_COUNTS];
   CK(cudaMemcpy(h, p->d_counts, sizeof(h), cudaMemcpyDeviceToHost));
   for (int i = 0; i < 16; ++i) counts[i] = i < SYN_COUNTS ? (int64_t)h[i] : 0;
+  return EMRI_OK;
+}
+
+int emri_plan_set_integrator(emri_plan* p, int kind, double rtol, const double* atol, int max_steps) {
+  if (!p || (kind != 0 && kind != 1)) return EMRI_EINVAL;
+  drop_graphs(p);
+  if (kind == 0) { p->integrator = 0; return EMRI_OK; }
+  if (!(rtol > 0.0) || !std::isfinite(rtol) || !atol || max_steps < 16) return EMRI_EINVAL;
+  for (int q = 0; q < 5; ++q) if (!(atol[q] >= 0.0) || !std::isfinite(atol[q])) return EMRI_EINVAL;
+  CK(cudaDeviceSynchronize());
+  int rc;
+  if (max_steps != p->dp_cap || !p->d_dpsteps) {
+    if (p->d_dpsteps) p->bytes -= (int64_t)((size_t)p->K_max * (p->dp_cap + DP_SHORT) * DP_REC * sizeof(double));
+    p->dp_cap = max_steps;
+    if ((rc = dev_alloc(p, &p->d_dpsteps, (size_t)p->K_max * (p->dp_cap + DP_SHORT) * DP_REC))) { p->dp_cap = 0; return rc; }
+  }
+  if (!p->d_dpn) {
+    if ((rc = dev_alloc(p, &p->d_dpn, (size_t)2 * p->K_max))) return rc;
+    if ((rc = dev_alloc(p, &p->d_dpstop, (size_t)2 * p->K_max))) return rc;
+    if ((rc = dev_alloc(p, &p->d_dpbad, (size_t)p->K_max))) return rc;
+    if ((rc = dev_alloc(p, &p->d_dpzero, (size_t)p->K_max))) return rc;
+  }
+  p->dp_rtol = rtol;
+  for (int q = 0; q < 5; ++q) p->dp_atol[q] = atol[q];
+  p->integrator = 1;
+  return EMRI_OK;
+}
+
+int emri_plan_orbit_steps(emri_plan* p, int k, int branch, int max_out, double* t, double* h, double* y, int32_t* info) {
+  if (!p || p->integrator != 1 || k < 0 || k >= p->K_max || (branch != 0 && branch != 1) || max_out < 0 || !info)
+    return EMRI_EINVAL;
+  CK(cudaDeviceSynchronize());
+  int32_t n[2], st[2];
+  CK(cudaMemcpy(n, p->d_dpn + 2 * k, sizeof(n), cudaMemcpyDeviceToHost));
+  CK(cudaMemcpy(st, p->d_dpstop + 2 * k, sizeof(st), cudaMemcpyDeviceToHost));
+  info[0] = n[branch]; info[1] = st[branch];
+  const bool is_long = (branch == 0) != (p->anchor_end != 0);
+  const size_t base = ((size_t)k * (p->dp_cap + DP_SHORT) + (is_long ? 0 : p->dp_cap)) * DP_REC;
+  const int cnt = std::min(max_out, (int)n[branch]);
+  std::vector<double> rec((size_t)cnt * DP_REC);
+  if (cnt > 0) CK(cudaMemcpy(rec.data(), p->d_dpsteps + base, rec.size() * sizeof(double), cudaMemcpyDeviceToHost));
+  for (int i = 0; i < cnt; ++i) {
+    if (t) t[i] = rec[(size_t)i * DP_REC];
+    if (h) h[i] = rec[(size_t)i * DP_REC + 1];
+    if (y) for (int q = 0; q < 5; ++q) y[5 * i + q] = rec[(size_t)i * DP_REC + 2 + q];
+  }
   return EMRI_OK;
 }
 

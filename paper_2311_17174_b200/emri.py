@@ -17,7 +17,7 @@ _lib = None
 
 EXPORTS = (
     "emri_strerror", "emri_plan_create", "emri_plan_destroy", "emri_plan_set_cosmology",
-    "emri_plan_set_coarse_stride", "emri_plan_set_orbit_schedule", "emri_plan_set_anchor", "emri_plan_orbit_report",
+    "emri_plan_set_coarse_stride", "emri_plan_set_orbit_schedule", "emri_plan_set_anchor", "emri_plan_set_integrator", "emri_plan_orbit_steps", "emri_plan_orbit_report",
     "emri_plan_synth_report", "emri_plan_set_synth_debug", "emri_plan_set_transform", "emri_plan_transform_is_fused", "emri_plan_set_graphs", "emri_plan_graph_stats", "emri_plan_set_chunk", "emri_orbit", "emri_plan_num_nodes", "emri_waveform",
     "emri_waveform_fft", "emri_data_fft", "emri_loglike", "emri_loglike_fdep", "emri_loglike_host", "emri_plan_enable_timings",
     "emri_plan_get_timings", "emri_plan_last_cuda_error", "emri_plan_last_launch_count", "emri_plan_workspace_bytes", "emri_stretch_step",
@@ -48,6 +48,8 @@ def load():
     L.emri_plan_set_orbit_schedule.argtypes = [vp, i32]
     L.emri_plan_orbit_report.argtypes = [vp, i32, vp]
     L.emri_plan_set_anchor.argtypes = [vp, i32]
+    L.emri_plan_set_integrator.argtypes = [vp, i32, dbl, vp, i32]
+    L.emri_plan_orbit_steps.argtypes = [vp, i32, i32, i32, vp, vp, vp, vp]
     L.emri_plan_synth_report.argtypes = [vp, vp]
     L.emri_plan_set_synth_debug.argtypes = [vp, i32]
     L.emri_plan_set_transform.argtypes = [vp, i32]
@@ -141,6 +143,25 @@ class Plan:
     def set_anchor(self, at_lso):
         """False: the parameter row is the state at t = 0 (default); True: at plunge, at the end of the window"""
         self._check(self._L.emri_plan_set_anchor(self._h, 1 if at_lso else 0))
+
+    def set_integrator(self, adaptive=None, max_steps=4096):
+        """None: fixed-step RK4 (default).  (rtol, atol[5]): the embedded Dormand-Prince pair with dense output"""
+        if adaptive is None:
+            self._check(self._L.emri_plan_set_integrator(self._h, 0, 0.0, None, 0))
+        else:
+            rtol, atol = adaptive
+            at = np.ascontiguousarray(np.broadcast_to(atol, (5,)), dtype=np.float64)
+            self._check(self._L.emri_plan_set_integrator(self._h, 1, float(rtol), at.ctypes.data_as(C.c_void_p), int(max_steps)))
+
+    def orbit_steps(self, k, branch=0, max_out=8192):
+        """accepted steps of walker k's adaptive orbit -> dict(t, h, y[n][5], stop)"""
+        t, h, y = np.zeros(max_out), np.zeros(max_out), np.zeros((max_out, 5))
+        info = np.zeros(2, dtype=np.int32)
+        self._check(self._L.emri_plan_orbit_steps(self._h, int(k), int(branch), max_out, t.ctypes.data_as(C.c_void_p),
+                                                   h.ctypes.data_as(C.c_void_p), y.ctypes.data_as(C.c_void_p),
+                                                   info.ctypes.data_as(C.c_void_p)))
+        n = min(int(info[0]), max_out)
+        return dict(t=t[:n], h=h[:n], y=y[:n], stop=int(info[1]), n=int(info[0]))
 
     def orbit_report(self, K):
         """modes of the last parallel-in-time orbit: 1 verified, 2 sequential tail, 3 zero rows"""

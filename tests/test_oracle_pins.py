@@ -1082,3 +1082,30 @@ def test_adaptive_orbit_plunge_and_lso_anchor(oracle):
     # a bad parameter row stays bad
     p[W.P_MU] = -1.0
     assert adaL.orbit(p, N, dt, S)["status"] == 1
+
+
+def test_adaptive_forced_steps_reproduce_the_free_run(oracle):
+    """teacher-forced mode: given its own accepted step sizes the integrator reproduces its own orbit bit for bit, and a
+    different (coarser) step sequence gives a different but close orbit -- the step sizes are really taken from the list"""
+    from oracle.oracle import Oracle
+    p = W.draw_params(W.CONFIGS[1], K=1)[0]
+    N, dt, S = 1 << 16, 15.0, 256
+    rtol, atol = 1e-10, DP_ATOL * 0.1
+    free = Oracle(adaptive=(rtol, atol))
+    a = free.orbit(p, N, dt, S)
+    Nc = N // S
+    fw = free.dp5_steps(p, (Nc + 1) * S * dt, rtol, atol, stop_at_plunge=True)
+    bw = free.dp5_steps(p, -S * dt, rtol, atol)
+    forced = Oracle()
+    forced.set_adaptive((rtol, atol), forced_fwd=fw["h"], forced_bwd=bw["h"])
+    b = forced.orbit(p, N, dt, S)
+    for key in ("val", "slope", "inc"):
+        np.testing.assert_array_equal(a[key], b[key])
+    # halve the number of forward steps (merge pairs): still an orbit, 5th order accurate, not the same bits
+    h2 = fw["h"][:len(fw["h"]) // 2 * 2].reshape(-1, 2).sum(axis=1)
+    if len(fw["h"]) % 2:
+        h2 = np.append(h2, fw["h"][-1])
+    forced.set_adaptive((rtol, atol), forced_fwd=h2, forced_bwd=bw["h"])
+    c = forced.orbit(p, N, dt, S)
+    assert c["status"] == 0 and not np.array_equal(a["val"], c["val"])
+    np.testing.assert_allclose(c["val"][1], a["val"][1], rtol=1e-9)
