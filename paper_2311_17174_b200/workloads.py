@@ -81,9 +81,11 @@ def nu0_for_plunge_after(M_msun, mu_msun, e0, t_plunge_sec):
 
     Closed-form estimate, not an integration: the leading-order circular chirp
     nu' = K nu^{11/3} reaches nu_LSO after (3/8K)(nu0^{-8/3} - nu_LSO^{-8/3}); eccentricity
-    shortens that by roughly (1-e^2)^{7/2}.  The PN and spin terms of the real model change the
-    plunge time by some tens of per cent, which the margin of `draw_params` (a factor >= 2.5)
-    covers; tests check that no walker of any config sets the plunge bit.
+    shortens that by roughly (1-e^2)^{7/2}.  The PN and spin terms of the real model make the true
+    plunge time 0.58-0.85 of this estimate (more for the heaviest systems; measured with the oracle),
+    so `draw_params` asks for 2.2-4.5 observation lengths to land on SURVEY 8(d)-1's strongly
+    chirping regime, plunge 1.3-4 T_obs after the window starts (median 2-2.8); tests check that no
+    walker of any config sets the plunge bit.
     """
     Ms, mus = M_msun * MSUN_SEC, mu_msun * MSUN_SEC
     Kc = 96.0 / (10.0 * np.pi) * mus / Ms ** 3 * (2.0 * np.pi * Ms) ** (11.0 / 3.0)
@@ -104,7 +106,7 @@ def _draw_row(rng, cfg):
         p[P_MU] = 10.0 ** _u(rng, cfg.log10_mu)
         p[P_A] = _u(rng, cfg.a)
         p[P_E0] = _u(rng, cfg.e0)
-        f_pl = rng.uniform(2.5, 6.0)               # estimated plunge time in units of T_obs
+        f_pl = rng.uniform(2.2, 4.5)               # ESTIMATED plunge time in units of T_obs (true: 0.58-0.85 of it)
         p[P_NU0] = nu0_for_plunge_after(p[P_M], p[P_MU], p[P_E0], f_pl * cfg.T_obs)
         p[P_PHI0], p[P_GAM0], p[P_ALP0] = rng.uniform(0.0, 2.0 * np.pi, 3)
         p[P_LAM] = rng.uniform(0.0, np.pi)
