@@ -29,9 +29,9 @@ constexpr int SYNTH_THREADS = 128;        // consumer threads per CTA
 constexpr int SYNTH_BLOCK = SYNTH_THREADS + 32;   // + one producer warp
 constexpr int TILE = 2 * SYNTH_THREADS;   // samples per tile (2 adjacent samples per thread)
 constexpr int UNIT_TILES_MAX = 16;        // tiles per unit (one re-expansion per unit), chosen per launch
-constexpr int MLOC = 9;                   // local expansion orders 0..8 are computed ...
-constexpr int MKEEP = 6;                  // ... and a unit keeps at most 6 of them (more: base-series fallback)
-constexpr int HREC = 28;                  // doubles per harmonic record of the local table: orders 8..0 x {PA, PB, PC} + 1 pad
+constexpr int MLOC = 7;                   // local expansion orders 0..6 are computed ...
+constexpr int MKEEP = 6;                  // ... and a unit keeps at most 6 of them (order 6 still significant: base-series fallback)
+constexpr int HREC = 22;                  // doubles per harmonic record of the local table: orders 6..0 x {PA, PB, PC} + 1 pad
 constexpr int HERM = 26;                  // doubles per staged interval record (cubics of the 5 orbit functions + amplitude data)
 #ifndef SYNTH_MINBLOCKS
 #define SYNTH_MINBLOCKS 4
@@ -268,7 +268,7 @@ DEVINL double4 ldg4(const double4* p) {
     EMRI_FMA(CB, CB, B.ec, -tb); EMRI_FMA(SB, SB, B.ec, ub);                                     \
   }
 
-// Local table (shared memory): record n holds the re-expanded series of harmonic n, orders 8..0, {PA, PB, PC} each:
+// Local table (shared memory): record n holds the re-expanded series of harmonic n, orders MLOC-1..0, {PA, PB, PC} each:
 // coefficient (order m, series s) at double 3 (MLOC-1-m) + s of the record.  A thread that keeps M orders streams the
 // LAST 3 M doubles of a record, in the order the Horner evaluation consumes them, as 128-bit loads from the aligned
 // address below its first coefficient (LEAD = 1: the first double loaded is the tail of order M, unused).
@@ -445,7 +445,8 @@ DEVINL void stage_intervals(const SynthArgs& a, int lane, const double* __restri
 template <bool STAGED>
 DEVINL void prepare_unit(const SynthArgs& a, int lane, int k, int64_t i_begin, int64_t i_end, double Delta, double inv_year,
                          double* __restrict__ tab, double* __restrict__ s_wc, double* __restrict__ s_rot,
-                         double* __restrict__ s_herm, int* __restrict__ s_Mb, int* __restrict__ s_Ml, const double2* __restrict__ sct_lane,
+                         double* __restrict__ s_herm, int* __restrict__ s_Mb, int* __restrict__ s_Ml, int* __restrict__ s_Pm,
+                         const double2* __restrict__ sct_lane,
                          UnitMeta* __restrict__ meta) {
 #pragma unroll 1
   for (int q = lane; q < WC_STRIDE; q += 32) s_wc[q] = a.wc[(size_t)k * WC_STRIDE + q];
@@ -558,17 +559,16 @@ DEVINL void prepare_unit(const SynthArgs& a, int lane, int k, int64_t i_begin, i
     for (int n = 1; n <= a.n_max; ++n) { if (s_Ml[n] > 0) n2 = max(n2, n); Mall = max(Mall, s_Ml[n]); }
     int M1 = Mall, M2 = 1, n1 = n2;
     if (Mall < MLOC) {
-      int best = n2 * (4 + 3 * Mall), sfx = 1, run = 0;
-      // suffix maxima on the fly: walk n1 downwards
+      // prefix maxima of the per-harmonic orders, then one walk of the split point downwards with the suffix maximum
+      int run = 1;
+#pragma unroll 1
+      for (int n = 1; n <= n2; ++n) { run = max(run, s_Ml[n]); s_Pm[n] = run; }
+      int best = n2 * (4 + 3 * Mall), sfx = 1;
 #pragma unroll 1
       for (int c = n2 - 1; c >= 1; --c) {
         sfx = max(sfx, s_Ml[c + 1]);
-        run = 0;
-#pragma unroll 1
-        for (int n = 1; n <= c; ++n) run = max(run, s_Ml[n]);
-        run = max(run, 1);
-        const int cost = c * (4 + 3 * run) + (n2 - c) * (4 + 3 * sfx) + 6;      // + the second range's prologue
-        if (cost < best) { best = cost; n1 = c; M1 = run; M2 = sfx; }
+        const int cost = c * (4 + 3 * s_Pm[c]) + (n2 - c) * (4 + 3 * sfx) + 6;      // + the second range's prologue
+        if (cost < best) { best = cost; n1 = c; M1 = s_Pm[c]; M2 = sfx; }
       }
     }
     if (a.force_base || M1 > MKEEP) M1 = MLOC;
@@ -618,6 +618,7 @@ __global__ void __launch_bounds__(SYNTH_BLOCK, SYNTH_MINBLOCKS) synth_kernel(Syn
   double* s_herm = s_rot + 2 * 2 * UNIT_TILES_MAX;                                     // [2][2 unit_tiles_cap][HERM]
   __shared__ int s_Mb[2][EMRI_NMAX_CAP + 1];  // base-series terms per harmonic (fallback path)
   __shared__ int s_Ml[EMRI_NMAX_CAP + 1];     // local orders per harmonic (producer scratch)
+  __shared__ int s_Pm[EMRI_NMAX_CAP + 1];     // their prefix maxima (producer scratch)
   __shared__ UnitMeta s_meta[2];
   const size_t herm_elems = (size_t)2 * a.unit_tiles_cap * HERM;
 
@@ -657,7 +658,7 @@ __global__ void __launch_bounds__(SYNTH_BLOCK, SYNTH_MINBLOCKS) synth_kernel(Syn
         unit_of(un, kl, ib, ie);
         const int nb = buf ^ 1;
         prepare_unit<STAGED>(a, lane, a.k0 + kl, ib, ie, Delta, inv_year, s_tab + nb * tab_elems, s_wc + nb * WC_STRIDE,
-                             s_rot + nb * 2 * UNIT_TILES_MAX, s_herm + nb * herm_elems, s_Mb[nb], s_Ml, sct_lane, &s_meta[nb]);
+                             s_rot + nb * 2 * UNIT_TILES_MAX, s_herm + nb * herm_elems, s_Mb[nb], s_Ml, s_Pm, sct_lane, &s_meta[nb]);
       }
     } else if (u >= 0) {
       int kl; int64_t i_begin, i_end;
