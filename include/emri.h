@@ -129,7 +129,7 @@ int emri_plan_orbit_report(emri_plan* p, int K, int32_t* modes);
 
 /* Diagnostics of stage (b) over the last emri_waveform / emri_waveform_fft / emri_loglike* call (all chunks):
  * which evaluation path the data selected.  counts (HOST int64 [16]):
- *   [0] units (one walker x up to 8 tiles of 256 samples) synthesised, [1..8] of them by the local order kept in the
+ *   [0] units (one walker x up to 16 tiles of 256 samples) synthesised, [1..8] of them by the local order kept in the
  *   re-summed harmonic series (first harmonic range), [9] units that fell back to the base series in e^2 (local order 8 still significant),
  *   [10] samples whose amplitude (2 pi M nu)^{2/3} took the cube root instead of the Taylor series about the coarse
  *   node (|nu/nu_j - 1| > 4e-3), [11] units of walkers with a fatal status (zero-filled), [12] sum over units of the harmonics evaluated (the last

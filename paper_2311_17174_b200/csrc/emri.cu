@@ -379,7 +379,7 @@ int run_synth(emri_plan* p, int k0, int K, double* outI, double* outII, int64_t 
   a.outI = outI; a.outII = outII; a.pitch = pitch; a.outZ = reinterpret_cast<double2*>(outZ);
   a.tiles_per_walker = (p->N + TILE - 1) / TILE;
   // tiles per unit: as many as leave >= 8 units per resident CTA (one series re-expansion per unit)
-  int ut = UNIT_TILES_MAX / 2;      // 8 tiles measured best on B200 (4: 3 % slower, 16: 1-2 % slower at n_max >= 20)
+  int ut = UNIT_TILES_MAX;          // 16 tiles measured best on B200 with the per-unit order selection (8: 2 % slower, 4: 8 %)
   while (ut > 1 && (int64_t)K * ((a.tiles_per_walker + ut - 1) / ut) < (int64_t)8 * p->synth_grid) ut >>= 1;
   if (p->unit_tiles_override > 0) ut = p->unit_tiles_override;
   a.unit_tiles = ut;
@@ -570,7 +570,7 @@ int emri_plan_create(emri_plan** out, int64_t N, double dt, int n_max, int K_max
 
   // persistent grid for the synthesis kernel: resident CTAs per SM x SM count
   if (const char* ev = std::getenv("EMRI_UNIT_TILES")) p->unit_tiles_override = std::max(1, std::min(UNIT_TILES_MAX, std::atoi(ev)));
-  p->unit_tiles_cap = std::max(UNIT_TILES_MAX / 2, p->unit_tiles_override);
+  p->unit_tiles_cap = UNIT_TILES_MAX;
   p->synth_smem = synth_smem_doubles(n_max, p->unit_tiles_cap) * sizeof(double);
   if (cudaFuncSetAttribute(synth_kernel<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)p->synth_smem) != cudaSuccess ||
       cudaFuncSetAttribute(synth_kernel<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)p->synth_smem) != cudaSuccess)

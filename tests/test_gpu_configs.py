@@ -78,7 +78,7 @@ def test_full_size_loglike_on_walker_subset(emri, oracle, ci):
     assert np.all(modes == 1)              # every walker's parallel-in-time orbit verified
     rep = plan.synth_report()
     print(f"cfg{ci} stage (b) paths: {rep}")
-    assert rep["units"] >= cfg.K * -(-cfg.N // 2048) and rep["skipped_units"] == 0     # units of <= 8 tiles
+    assert rep["units"] >= cfg.K * -(-cfg.N // 4096) and rep["skipped_units"] == 0     # units of <= 16 tiles
     assert sum(rep["by_order"].values()) + rep["base_units"] == rep["units"]
     plan.close()
 

@@ -32,7 +32,7 @@ def h_err(got, ref):
 @pytest.mark.parametrize("force_base,force_cbrt", [(True, False), (False, True), (True, True)])
 def test_forced_slow_paths_match_oracle(emri, oracle, force_base, force_cbrt):
     """every unit on the base series in e^2 and / or every sample on the cube-root amplitude: same waveform"""
-    cfg = W.scaled(W.CONFIGS[3], K=6, N=3 * 2048 + 300)          # several units and a ragged tail, n_max = 30
+    cfg = W.scaled(W.CONFIGS[3], K=6, N=3 * 4096 + 300)          # several units and a ragged tail, n_max = 30
     P = W.draw_params(cfg)
     P[:, W.P_E0] = np.linspace(0.05, 0.5, cfg.K)
     for k in range(cfg.K):
