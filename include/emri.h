@@ -51,7 +51,7 @@ extern "C" {
 #endif
 
 #define EMRI_NPAR 17
-#define EMRI_NMAX_CAP 48 /* largest n_max a plan accepts */
+#define EMRI_NMAX_CAP 128 /* largest n_max a plan accepts */
 
 enum {
   EMRI_OK = 0,

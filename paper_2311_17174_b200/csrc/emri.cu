@@ -48,6 +48,7 @@ struct emri_plan {
   double* d_hbuf = nullptr;
   double* d_partial = nullptr;
   double4* d_base = nullptr;      // Taylor coefficients of the harmonic brackets in e^2 (synth.cuh)
+  double* d_gtab = nullptr;       // n (n/2)^{n-2} / (n-2)!: bracket scale of the Bessel path (n_max > 48)
   double2* d_nodeaux = nullptr;
   int32_t* d_jpl = nullptr;
   int32_t* d_status = nullptr;
@@ -372,6 +373,7 @@ int run_synth(emri_plan* p, int k0, int K, double* outI, double* outII, int64_t 
   a.z_log2n2 = interleaved ? p->log2N2 : 0;
   a.wc = p->d_wc; a.nodes = p->d_nodes; a.nodeaux = p->d_nodeaux; a.jpl = p->d_jpl; a.status = p->d_status;
   a.base = p->d_base; a.tol = 1e-16;
+  a.gtab = p->d_gtab; a.bessel = p->n_max > 48 ? 1 : 0;
   a.cbrt_thr = (p->synth_debug & 2) ? -1.0 : 4e-3;
   a.force_base = (p->synth_debug & 1) ? 1 : 0;
   a.counts = p->d_counts;
@@ -388,8 +390,13 @@ int run_synth(emri_plan* p, int k0, int K, double* outI, double* outII, int64_t 
   int64_t total = (int64_t)K * a.units_per_walker;
   int grid = (int)std::min<int64_t>(total, p->synth_grid);
   // S >= 256: every tile lies inside one coarse interval and the producer warp stages its cubics (the default)
-  if (p->S >= TILE) synth_kernel<true><<<grid, SYNTH_BLOCK, p->synth_smem, s>>>(a);
-  else synth_kernel<false><<<grid, SYNTH_BLOCK, p->synth_smem, s>>>(a);
+  if (a.bessel) {
+    if (p->S >= TILE) synth_kernel<true, true><<<grid, SYNTH_BLOCK, p->synth_smem, s>>>(a);
+    else synth_kernel<false, true><<<grid, SYNTH_BLOCK, p->synth_smem, s>>>(a);
+  } else {
+    if (p->S >= TILE) synth_kernel<true, false><<<grid, SYNTH_BLOCK, p->synth_smem, s>>>(a);
+    else synth_kernel<false, false><<<grid, SYNTH_BLOCK, p->synth_smem, s>>>(a);
+  }
   p->launches += 1;
   CK(cudaGetLastError());
   return EMRI_OK;
@@ -489,6 +496,17 @@ int emri_plan_create(emri_plan** out, int64_t N, double dt, int n_max, int K_max
   if ((rc = dev_alloc(p, &p->d_pclamp, (size_t)K_max))) return fail(rc);
   if ((rc = dev_alloc(p, &p->d_plrow, (size_t)K_max * NODE_STRIDE))) return fail(rc);
   if ((rc = dev_alloc(p, &p->d_base, base.size()))) return fail(rc);
+  {
+    // bracket scale of the Bessel path: n (n/2)^{n-2} / (n-2)! as a running product in long double
+    std::vector<double> g((size_t)n_max + 1, 1.0);
+    for (int n = 2; n <= n_max; ++n) {
+      long double v = (long double)n;
+      for (int i = 1; i <= n - 2; ++i) v *= 0.5L * (long double)n / (long double)i;
+      g[n] = (double)v;
+    }
+    if ((rc = dev_alloc(p, &p->d_gtab, g.size()))) return fail(rc);
+    if (cudaMemcpy(p->d_gtab, g.data(), g.size() * sizeof(double), cudaMemcpyHostToDevice) != cudaSuccess) return fail(EMRI_ECUDA);
+  }
   p->n_part = (int)((p->Nf + LL_RANGE - 1) / LL_RANGE);
   // fused transform + reduction: N = 2^16 .. 2^22 = N1 N2 with N1 = clamp(N / 1024, 256, 1024) (1024: the length cuFFT's
   // strided batched kernel runs best at -- 4 TB/s against 2.8 TB/s at 2048, measured on B200) and N2 = N / N1 in 256 .. 4096
@@ -572,14 +590,21 @@ int emri_plan_create(emri_plan** out, int64_t N, double dt, int n_max, int K_max
   if (const char* ev = std::getenv("EMRI_UNIT_TILES")) p->unit_tiles_override = std::max(1, std::min(UNIT_TILES_MAX, std::atoi(ev)));
   p->unit_tiles_cap = UNIT_TILES_MAX;
   p->synth_smem = synth_smem_doubles(n_max, p->unit_tiles_cap) * sizeof(double);
-  if (cudaFuncSetAttribute(synth_kernel<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)p->synth_smem) != cudaSuccess ||
-      cudaFuncSetAttribute(synth_kernel<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)p->synth_smem) != cudaSuccess)
-    return fail(EMRI_ECUDA);
   int per_sm = 0, per_sm_direct = 0;
-  if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, synth_kernel<true>, SYNTH_BLOCK, p->synth_smem) != cudaSuccess ||
-      cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm_direct, synth_kernel<false>, SYNTH_BLOCK, p->synth_smem) != cudaSuccess ||
-      per_sm < 1 || per_sm_direct < 1)
-    return fail(EMRI_ECUDA);
+  if (n_max > 48) {
+    if (cudaFuncSetAttribute(synth_kernel<true, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)p->synth_smem) != cudaSuccess ||
+        cudaFuncSetAttribute(synth_kernel<false, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)p->synth_smem) != cudaSuccess ||
+        cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, synth_kernel<true, true>, SYNTH_BLOCK, p->synth_smem) != cudaSuccess ||
+        cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm_direct, synth_kernel<false, true>, SYNTH_BLOCK, p->synth_smem) != cudaSuccess)
+      return fail(EMRI_ECUDA);
+  } else {
+    if (cudaFuncSetAttribute(synth_kernel<true, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)p->synth_smem) != cudaSuccess ||
+        cudaFuncSetAttribute(synth_kernel<false, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)p->synth_smem) != cudaSuccess ||
+        cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, synth_kernel<true, false>, SYNTH_BLOCK, p->synth_smem) != cudaSuccess ||
+        cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm_direct, synth_kernel<false, false>, SYNTH_BLOCK, p->synth_smem) != cudaSuccess)
+      return fail(EMRI_ECUDA);
+  }
+  if (per_sm < 1 || per_sm_direct < 1) return fail(EMRI_ECUDA);
   per_sm = std::min(per_sm, per_sm_direct);
   p->synth_grid = per_sm * p->sm_count;
   if (cudaStreamCreateWithFlags(&p->s_cap, cudaStreamNonBlocking) != cudaSuccess ||
@@ -606,7 +631,7 @@ int emri_plan_destroy(emri_plan* p) {
   void* ptrs[] = {p->d_w, p->d_wc, p->d_nodes, p->d_hbuf, p->d_partial, p->d_base, p->d_nodeaux, p->d_jpl, p->d_status,
                   p->d_params, p->d_data, p->d_logL, p->d_Y, p->d_z, p->d_lnu, p->d_logLY, p->d_inbox,
                   p->d_partner, p->d_fftwork, p->d_seg, p->d_plrow, p->d_mode, p->d_pclamp, p->d_counts,
-                  p->d_twid, p->d_twA, p->d_twB, p->d_alpha, p->d_gamma, p->d_cdpart, p->d_dpsteps, p->d_dpn, p->d_dpstop,
+                  p->d_twid, p->d_twA, p->d_twB, p->d_alpha, p->d_gamma, p->d_cdpart, p->d_gtab, p->d_dpsteps, p->d_dpn, p->d_dpstop,
                   p->d_dpbad, p->d_dpzero};
   for (void* q : ptrs) if (q) cudaFree(q);
   delete p;

@@ -45,6 +45,9 @@ struct SynthArgs {
   const int32_t* jpl;
   const int32_t* status;
   const double4* base;     // [n_max+1][BASE_M] Taylor coefficients {PA, PB, PC, 0} in w = e^2
+  const double* gtab;      // [n_max+1] n (n/2)^{n-2} / (n-2)!  (n >= 2): scale of the brackets in the Bessel path
+  int bessel;              // 1: local series from Bessel recurrences (plans with n_max > 48, where the base series in e^2
+                           // would cancel); 0: from the tabulated base series
   int k0, K;               // walkers k0 .. k0+K-1
   int64_t N;
   double dt;
@@ -380,6 +383,149 @@ __device__ __noinline__ void harmonic_sum_base(const double4* __restrict__ base,
   out[0] = SaA; out[1] = SbA; out[2] = ScA; out[3] = SaB; out[4] = SbB; out[5] = ScB;
 }
 
+
+// ---- Bessel path (n_max > 48): local series of the brackets from recurrences instead of the base series in e^2.
+// With s_k(w) = sum_m (-n^2 w/4)^m / (m! (m+k)!) = J_k(n e) / (n e/2)^k one has d s_k/dw = -(n^2/4) s_{k+1}, so the Taylor
+// coefficients of s_k about w0 are (-n^2/4)^j s_{k+j}(w0) / j!, and the brackets are (BC Eqs. 7-9 divided by e^{n-2}):
+//   PA = G [s_{n-2} - n w s_{n-1} + (n/2) w s_n + (n^3/4) w^2 s_{n+1} - (n^4/16) w^2 s_{n+2}],
+//   PB = G [s_{n-2} - (n^2/2) w s_n + (n^4/16) w^2 s_{n+2}],   PC = G (n/4) w s_n,        G = n (n/2)^{n-2}
+// (n = 1, with J_{-1} = -J_1: PA = s_1/2 - 2 s_0 + w s_2/2 - w s_3/8, PB = -3 s_1/2 + w s_3/8, PC = s_1/2).
+// hat-s_k = k! s_k (= 1 at w = 0) obeys the division-free form of the three-term recurrence,
+//   hs_{k-1} = hs_k - y hs_{k+1} / (k (k+1)),   y = n^2 w0 / 4,
+// which is stable downwards.  Small y: the two highest orders from the series itself (terms fall from the start), then
+// down.  Otherwise Miller's algorithm: start far above from hs = 1, go down to order 0 and normalise with
+// J_0 + 2 sum_m J_2m = 1 (J_k = hs_k y^{k/2} / k!).  No cancellation at any n e (the base series in e^2 loses e^{n e} digits).
+constexpr int BES_NS = 5 + MLOC - 1;      // orders needed per harmonic: k = n-2 .. n+2+(MLOC-1)
+
+// hs[i] = hat-s_{k_lo + i}(y), i = 0 .. cnt-1
+DEVINL void bessel_hat_s(int k_lo, int cnt, double y, double* __restrict__ hs) {
+  const int K = k_lo + cnt - 1;
+  if (y <= 0.5 * (double)(K + 1)) {
+    double top[2];
+#pragma unroll 1
+    for (int which = 0; which < 2; ++which) {
+      const int k = K + 1 - which;
+      double t = 1.0, sum = 1.0;
+#pragma unroll 1
+      for (int m = 1; m <= 200; ++m) {
+        t *= -y / ((double)m * (double)(k + m));
+        sum += t;
+        if (fabs(t) < 1e-18 * fabs(sum)) break;
+      }
+      top[which] = sum;
+    }
+    double hp = top[0], h = top[1];       // orders K+1, K
+    hs[cnt - 1] = h;
+#pragma unroll 1
+    for (int k = K; k > k_lo; --k) {
+      const double hm = fma(-y / ((double)k * (double)(k + 1)), hp, h);
+      hp = h; h = hm;
+      hs[k - 1 - k_lo] = h;
+    }
+    return;
+  }
+  const double half = sqrt(y);
+  int M = K + 16 + (int)(2.0 * sqrt((double)K)) + (int)(2.0 * half);
+  M += M & 1;
+  double hp = 1.0, h = 1.0, S = 0.0;
+  // f_k = (z/2)^k / k!: tracked in logarithm until it is representable, then by its recurrence f_{k-1} = f_k k / (z/2)
+  const double lhalf = log(half);
+  double logf = (double)M * lhalf - lgamma((double)M + 1.0);
+  bool have_f = logf > -600.0;
+  double f = have_f ? exp(logf) : 0.0;
+#pragma unroll 1
+  for (int k = M; k >= 1; --k) {
+    if (k <= K && k >= k_lo) hs[k - k_lo] = h;
+    if (have_f && !(k & 1)) S = fma(2.0 * h, f, S);
+    const double hm = fma(-y / ((double)k * (double)(k + 1)), hp, h);
+    hp = h; h = hm;
+    if (have_f) f *= (double)k / half;
+    else {
+      logf += log((double)k) - lhalf;
+      if (logf > -600.0) { f = exp(logf); have_f = true; }
+    }
+  }
+  if (k_lo == 0) hs[0] = h;
+  S = fma(h, f, S);                         // k = 0 (f_0 = 1 up to rounding)
+  const double rS = 1.0 / S;
+#pragma unroll 1
+  for (int i = 0; i < cnt; ++i) hs[i] *= rS;
+}
+
+// coefficient j of (w0 + x) A(x) and of (w0 + x)^2 A(x)
+DEVINL double mulw1(const double* a, int j, double w0) { return fma(w0, a[j], j >= 1 ? a[j - 1] : 0.0); }
+DEVINL double mulw2(const double* a, int j, double w0) {
+  return fma(w0 * w0, a[j], fma(2.0 * w0, j >= 1 ? a[j - 1] : 0.0, j >= 2 ? a[j - 2] : 0.0));
+}
+
+// local series (NORD orders) of PA, PB, PC of harmonic n about w0
+template <int NORD>
+DEVINL void bessel_local_series(int n, double w0, double gn, double (&PA)[NORD], double (&PB)[NORD], double (&PC)[NORD]) {
+  constexpr int CNT = 5 + NORD - 1;
+  double hs[CNT], T[5][NORD];
+  const double nn = (double)n;
+  const double y = 0.25 * nn * nn * w0;
+  const int k_lo = (n == 1) ? 0 : n - 2;
+  bessel_hat_s(k_lo, (n == 1) ? CNT - 1 : CNT, y, hs);
+  // u_i = G s_{k_lo + i} = G hat-s / k!   (n >= 2: G / (n-2)! = gn;  n = 1: G = 1, 0! = 1)
+  double fac = (n == 1) ? 1.0 : gn;
+#pragma unroll
+  for (int i = 0; i < CNT; ++i) {
+    if (i > 0) fac /= (double)(k_lo + i);
+    hs[i] = (n == 1 && i == CNT - 1) ? 0.0 : hs[i] * fac;
+  }
+  const double c = -0.25 * nn * nn;
+#pragma unroll
+  for (int r = 0; r < 5; ++r) {
+    double cj = 1.0;
+#pragma unroll
+    for (int j = 0; j < NORD; ++j) {
+      T[r][j] = (n == 1 && r + j >= CNT - 1) ? 0.0 : cj * hs[r + j];
+      cj *= c / (double)(j + 1);
+    }
+  }
+  if (n == 1) {
+    // T[0..3] = series of s_0, s_1, s_2, s_3
+#pragma unroll
+    for (int j = 0; j < NORD; ++j) {
+      PA[j] = fma(0.5, T[1][j], fma(-2.0, T[0][j], fma(0.5, mulw1(T[2], j, w0), -0.125 * mulw1(T[3], j, w0))));
+      PB[j] = fma(-1.5, T[1][j], 0.125 * mulw1(T[3], j, w0));
+      PC[j] = 0.5 * T[1][j];
+    }
+    return;
+  }
+  const double n2 = nn * nn, n3 = n2 * nn, n4 = n2 * n2;
+#pragma unroll
+  for (int j = 0; j < NORD; ++j) {
+    const double w2 = mulw1(T[2], j, w0), w4 = mulw2(T[4], j, w0);
+    PA[j] = T[0][j] - nn * mulw1(T[1], j, w0) + 0.5 * nn * w2 + 0.25 * n3 * mulw2(T[3], j, w0) - 0.0625 * n4 * w4;
+    PB[j] = T[0][j] - 0.5 * n2 * w2 + 0.0625 * n4 * w4;
+    PC[j] = 0.25 * nn * w2;
+  }
+}
+
+// Fallback of the Bessel path (local order MKEEP not enough over the unit: the last hours before plunge at high n_max):
+// every sample evaluates the brackets of every harmonic at its own e^2 by the recurrences (slow, rare, exact)
+__device__ __noinline__ void harmonic_sum_bessel(const double* __restrict__ gtab, int n_max, const SampleOut& A, const SampleOut& B,
+                                                 double out[6]) {
+  double p[6];
+  {
+    double a1[1], b1[1], c1[1];
+    bessel_local_series<1>(1, A.x, 1.0, a1, b1, c1); p[0] = a1[0]; p[1] = b1[0]; p[2] = c1[0];
+    bessel_local_series<1>(1, B.x, 1.0, a1, b1, c1); p[3] = a1[0]; p[4] = b1[0]; p[5] = c1[0];
+  }
+  EMRI_ACCUM_FIRST()
+#pragma unroll 1
+  for (int n = 2; n <= n_max; ++n) {
+    double a1[1], b1[1], c1[1];
+    const double gn = __ldg(gtab + n);
+    bessel_local_series<1>(n, A.x, gn, a1, b1, c1); p[0] = a1[0]; p[1] = b1[0]; p[2] = c1[0];
+    bessel_local_series<1>(n, B.x, gn, a1, b1, c1); p[3] = a1[0]; p[4] = b1[0]; p[5] = c1[0];
+    EMRI_ACCUM_NEXT()
+  }
+  out[0] = SaA; out[1] = SbA; out[2] = ScA; out[3] = SaB; out[4] = SbB; out[5] = ScB;
+}
+
 // ---- per-unit tables, prepared by the producer warp one unit ahead of the consumers (double-buffered)
 struct UnitMeta {
   double w0e;         // expansion point subtracted from e^2 (0 on the fallback path)
@@ -442,7 +588,7 @@ DEVINL void stage_intervals(const SynthArgs& a, int lane, const double* __restri
 }
 
 // Executed by ONE warp: everything of unit (k, i_begin..i_end) that is shared by its samples.
-template <bool STAGED>
+template <bool STAGED, bool BES>
 DEVINL void prepare_unit(const SynthArgs& a, int lane, int k, int64_t i_begin, int64_t i_end, double Delta, double inv_year,
                          double* __restrict__ tab, double* __restrict__ s_wc, double* __restrict__ s_rot,
                          double* __restrict__ s_herm, int* __restrict__ s_Mb, int* __restrict__ s_Ml, int* __restrict__ s_Pm,
@@ -491,8 +637,23 @@ DEVINL void prepare_unit(const SynthArgs& a, int lane, int k, int64_t i_begin, i
   // term of the harmonic INCLUDING its carrier e^{n-2} (n = 1: e), at the unit's mid-point
   const double ebar = sqrt(w0);
   double scale = 0.0;
+  if (BES) {
+    // one lane per harmonic: the three local series from the Bessel recurrences
 #pragma unroll 1
-  for (int task = lane; task < 3 * a.n_max; task += 32) {
+    for (int n = 1 + lane; n <= a.n_max; n += 32) {
+      double PA[MLOC], PB[MLOC], PC[MLOC];
+      bessel_local_series<MLOC>(n, w0, __ldg(a.gtab + n), PA, PB, PC);
+      double* dst = tab + (size_t)n * HREC;
+#pragma unroll
+      for (int j = 0; j < MLOC; ++j) {
+        dst[3 * (MLOC - 1 - j)] = PA[j]; dst[3 * (MLOC - 1 - j) + 1] = PB[j]; dst[3 * (MLOC - 1 - j) + 2] = PC[j];
+      }
+      const int pc = (n == 1) ? 1 : n - 2;
+      scale = fmax(scale, fmax(fabs(PA[0]), fmax(fabs(PB[0]), fabs(PC[0]))) * ipow(ebar, pc));
+    }
+  }
+#pragma unroll 1
+  for (int task = BES ? 3 * a.n_max : lane; task < 3 * a.n_max; task += 32) {
     const int n = task / 3 + 1, si = task - 3 * (n - 1);
     const double* bp = reinterpret_cast<const double*>(a.base + (size_t)n * BASE_M) + si;
     // base terms that matter at w <= whi (terms rise, then fall: the running maximum is a safe scale)
@@ -606,7 +767,8 @@ DEVINL size_t z_index(const SynthArgs& a, int kl, int64_t i0) {
 
 // Consumers (warps 0..3): 2 adjacent samples per thread per tile.  Producer (warp 4): tables of the NEXT unit.
 // STAGED: S >= 256, every tile lies inside one coarse interval (the default); otherwise node rows are read per sample.
-template <bool STAGED>
+// BES: the Bessel path of plans with n_max > 48 (its code stays out of the kernels of the other plans: instruction cache).
+template <bool STAGED, bool BES>
 __global__ void __launch_bounds__(SYNTH_BLOCK, SYNTH_MINBLOCKS) synth_kernel(SynthArgs a) {
   extern __shared__ __align__(16) unsigned char smem_raw[];
   const size_t tab_elems = (size_t)(a.n_max + 2) * HREC;
@@ -657,7 +819,7 @@ __global__ void __launch_bounds__(SYNTH_BLOCK, SYNTH_MINBLOCKS) synth_kernel(Syn
         int kl; int64_t ib, ie;
         unit_of(un, kl, ib, ie);
         const int nb = buf ^ 1;
-        prepare_unit<STAGED>(a, lane, a.k0 + kl, ib, ie, Delta, inv_year, s_tab + nb * tab_elems, s_wc + nb * WC_STRIDE,
+        prepare_unit<STAGED, BES>(a, lane, a.k0 + kl, ib, ie, Delta, inv_year, s_tab + nb * tab_elems, s_wc + nb * WC_STRIDE,
                              s_rot + nb * 2 * UNIT_TILES_MAX, s_herm + nb * herm_elems, s_Mb[nb], s_Ml, s_Pm, sct_lane, &s_meta[nb]);
       }
     } else if (u >= 0) {
@@ -706,7 +868,8 @@ __global__ void __launch_bounds__(SYNTH_BLOCK, SYNTH_MINBLOCKS) synth_kernel(Syn
           }
           double S[6];
           if (mt.M1 >= MLOC) {
-            harmonic_sum_base(a.base, s_Mb[buf], a.n_max, A, B, S);
+            if (BES) harmonic_sum_bessel(a.gtab, a.n_max, A, B, S);
+            else harmonic_sum_base(a.base, s_Mb[buf], a.n_max, A, B, S);
           } else {
             HarmState hs;
 #pragma unroll 1

@@ -47,7 +47,7 @@ def test_strerror_and_argument_checks_need_no_gpu():
     assert L.emri_plan_create(C.byref(h), 7, 15.0, 5, 1, None) == -1      # N odd
     assert L.emri_plan_create(C.byref(h), 64, -1.0, 5, 1, None) == -1     # dt <= 0
     assert L.emri_plan_create(C.byref(h), 64, 15.0, 0, 1, None) == -1     # n_max < 1
-    assert L.emri_plan_create(C.byref(h), 64, 15.0, 49, 1, None) == -1    # n_max > cap
+    assert L.emri_plan_create(C.byref(h), 64, 15.0, 129, 1, None) == -1   # n_max > cap
     assert L.emri_plan_create(C.byref(h), 64, 15.0, 5, 0, None) == -1     # K_max < 1
     assert L.emri_plan_create(None, 64, 15.0, 5, 1, None) == -1
     assert L.emri_plan_destroy(None) == -1

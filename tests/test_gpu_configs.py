@@ -141,6 +141,42 @@ def test_harmonic_cap_and_eccentric_walkers(emri, oracle):
     plan.close()
 
 
+@pytest.mark.parametrize("n_max,e_hi,N", [(96, 0.6, 3 * 4096 + 2), (128, 0.7, 1 << 12), (64, 0.3, 1 << 13)])
+def test_many_harmonics_by_the_bessel_path(emri, oracle, n_max, e_hi, N):
+    """n_max beyond 48 (the overtone loop; SURVEY f-4): the local series come from Bessel recurrences instead of
+    the base series in e^2, whose terms would cancel by e^{n e}.  Element-wise against the oracle (power-series Bessel
+    functions of order > argument), eccentricities up to e_hi, including e = 0 and a walker close to plunge whose units
+    overflow the local orders and take the per-sample recurrence fallback"""
+    cfg = W.scaled(W.CONFIGS[3], K=6, N=N, n_max=n_max)
+    P = W.draw_params(cfg)
+    P[:, W.P_E0] = np.linspace(0.0, e_hi, cfg.K)
+    for k in range(cfg.K):
+        P[k, W.P_NU0] = W.nu0_for_plunge_after(P[k, W.P_M], P[k, W.P_MU], P[k, W.P_E0], 4.0 * 2 ** 21 * cfg.dt)
+    P[4, W.P_M], P[4, W.P_MU] = 2e5, 80.0
+    P[4, W.P_NU0] = 0.97 * W.nu_lso_hz(P[4, W.P_M], P[4, W.P_E0])            # hours from plunge: e^2 moves fast
+    plan = emri.Plan(cfg.N, cfg.dt, cfg.n_max, cfg.K)
+    st = torch.zeros(cfg.K, dtype=torch.int32, device="cuda")
+    hI, hII = plan.waveform(dev(P), status=st)
+    rep = plan.synth_report()
+    torch.cuda.synchronize()
+    h_ref, st_ref = oracle.waveform_batch(P, cfg.N, cfg.dt, cfg.n_max)
+    print(f"n_max={n_max}: paths {rep} status {st.cpu().numpy()} {st_ref}")
+    assert np.array_equal(st.cpu().numpy(), st_ref)
+    for ch, got in ((0, hI.cpu().numpy()), (1, hII.cpu().numpy())):
+        live = np.max(np.abs(h_ref[:, ch]), axis=1) > 0
+        err = np.max(np.abs(got[live] - h_ref[live, ch]), axis=1) / np.max(np.abs(h_ref[live, ch]), axis=1)
+        print("  err", err)
+        assert np.all(err <= H_TOL)
+    # the forced fallback (every unit evaluates the recurrences per sample) gives the same waveform
+    plan.set_synth_debug(force_base=True)
+    hI2, _ = plan.waveform(dev(P))
+    rep2 = plan.synth_report()
+    assert rep2["base_units"] == rep2["units"] > 0
+    g, g2 = hI.cpu().numpy(), hI2.cpu().numpy()
+    assert np.max(np.abs(g - g2)) <= 1e-11 * np.max(np.abs(g))
+    plan.close()
+
+
 def test_circular_orbit_has_only_the_quadrupole(emri, oracle):
     """e = 0 exactly (reading R18): e' = 0 keeps it there and only n = 2 survives: n_max = 2 and 30 agree"""
     cfg = W.scaled(W.CONFIGS[1], K=2, N=1 << 12)
