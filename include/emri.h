@@ -138,13 +138,14 @@ int emri_plan_orbit_report(emri_plan* p, int K, int32_t* modes);
  * Synchronises the device. */
 int emri_plan_synth_report(emri_plan* p, int64_t counts[16]);
 
-/* How emri_loglike runs stages (c)+(d).  1 (default where available: N a power of two, 2^16 <= N <= 2^22): fused -- the
- * synthesis writes the chunk walker-interleaved, ONE strided batched cuFFT pass does the first factor of N = N1 N2, and a
- * kernel of this library does the last pass (N2 <= 1024 points per row, in registers and shared memory) and feeds its
- * outputs straight into Eq. 8, so the spectrum is never written back nor read again (DESIGN.md
- * section 6c).  0: the full cuFFT transform followed by the streaming reduction kernel (also used for every other N and by
- * emri_loglike_fdep).  Both give logL within the parity tolerance of each other (not bit-identical: the fused path
- * evaluates Eq. 8 as <d|d> - 2<d|h> + <h|h>).  emri_plan_transform_is_fused reports what the next emri_loglike will do. */
+/* How emri_loglike runs stages (c)+(d).  1 (default where available: N a power of two, 2^16 <= N <= 2^22): fused -- ONE
+ * persistent kernel of this library does both passes of the transform, N = N1 N2 (N1-point transforms down the columns of
+ * the chunk the synthesis wrote, then N2 <= 4096 points per row, in registers and shared memory) and feeds the outputs of
+ * the last pass straight into Eq. 8, so the spectrum is never written back nor read again and cuFFT is not on the path
+ * (DESIGN.md section 6c).  Needs a second chunk-sized buffer.  0: the full cuFFT transform followed by
+ * the streaming reduction kernel (also used for every other N and by emri_loglike_fdep).  Both give logL within the parity
+ * tolerance of each other (not bit-identical: the fused path evaluates Eq. 8 as <d|d> - 2<d|h> + <h|h>).
+ * emri_plan_transform_is_fused reports what the next emri_loglike will do. */
 int emri_plan_set_transform(emri_plan* p, int fused);
 int emri_plan_transform_is_fused(const emri_plan* p);
 
@@ -164,8 +165,9 @@ int emri_plan_graph_stats(const emri_plan* p, int64_t out[2]);
 int emri_plan_set_synth_debug(emri_plan* p, int flags);
 
 /* Number of walkers processed per internal chunk (bounds the workspace: chunk*N complex128 for z = h_I + i h_II
- * plus the cuFFT work area).  Default min(K_max, 128).  Reallocates, re-creates the cuFFT plans (full chunk, ragged
- * last chunk of K_max, single transform) and their shared work area; synchronises. */
+ * plus the second buffer of the fused transform and the cuFFT work area).  Default min(K_max, 128).  Reallocates,
+ * re-creates the cuFFT plans (full chunk, ragged last chunk of K_max, single transform) and their shared work area;
+ * synchronises. */
 int emri_plan_set_chunk(emri_plan* p, int walkers_per_chunk);
 
 /* Stage (a): coarse orbit of Eq. 1 by fixed-step RK4 (S3).

@@ -85,15 +85,18 @@ struct emri_plan {
   double* d_Y = nullptr; double* d_z = nullptr; double* d_lnu = nullptr; double* d_logLY = nullptr;
   int32_t* d_inbox = nullptr; int32_t* d_partner = nullptr;
   // fused transform + reduction (fftlike.cuh): N = N1 N2; available for N = 2^16 .. 2^22
-  bool fused_ok = false, fused_on = true;
+  bool fused_ok = false;
+  bool fused_on = true;                // false: full cuFFT transform + loglike_kernel
   int N1 = 0, N2 = 0, log2N1 = 0, log2N2 = 0, n_cd = 0;
+  int fft2_g = 0;                      // walkers per group of fft2_like_kernel (0: the whole chunk)
+  double2* d_ring = nullptr;           // [slots][g][N] pass-A output
+  unsigned* d_fft2ctr = nullptr;       // ticket and completion counters of fft2_like_kernel
+  double2* d_twid1 = nullptr;          // stage twiddles of pass A (length N1)
+  double2* d_tw3 = nullptr;            // three-level inter-pass twiddle of fft2_like_kernel
   double2* d_twid = nullptr;
-  double2* d_twA = nullptr;
-  double2* d_twB = nullptr;
   double* d_alpha = nullptr;
   double2* d_gamma = nullptr;
   double* d_cdpart = nullptr;
-  std::map<int, cufftHandle> fftA;     // strided pass-A plans, by walkers in the chunk
   // cuFFT
   std::map<int, cufftHandle> fft;
   void* d_fftwork = nullptr;
@@ -213,7 +216,8 @@ int alloc_workspace(emri_plan* p) {
 }
 
 int get_fft(emri_plan* p, int batch, cufftHandle* out);
-int get_fftA(emri_plan* p, int kc, cufftHandle* out);
+cudaError_t fft2_set_smem();
+int fft2_group(const emri_plan* p) { return p->fft2_g > 0 ? std::min(p->fft2_g, p->chunk) : p->chunk; }
 
 // (Re)allocates the chunk buffer and creates, up front, every cuFFT plan the hot calls of a full ensemble need: a full
 // chunk, the ragged last chunk of K_max walkers, and the single transform of emri_data_fft.  The work area is sized by
@@ -222,18 +226,17 @@ int get_fftA(emri_plan* p, int kc, cufftHandle* out);
 int alloc_chunk(emri_plan* p) {
   int rc;
   if ((rc = dev_alloc(p, &p->d_hbuf, (size_t)2 * p->chunk * p->N))) return rc;      // z = h_I + i h_II, [chunk][N] complex
+  if (p->fused_ok) {
+    const int g = fft2_group(p), G = (p->chunk + g - 1) / g;
+    if ((rc = dev_alloc(p, &p->d_ring, (size_t)(G > 1 ? 2 : 1) * g * p->N))) return rc;
+    if ((rc = dev_alloc(p, &p->d_fft2ctr, (size_t)1 + 2 * G))) return rc;
+  }
   for (auto& kv : p->fft) cufftDestroy(kv.second);
   p->fft.clear();
-  for (auto& kv : p->fftA) cufftDestroy(kv.second);
-  p->fftA.clear();
   cufftHandle h;
   if ((rc = get_fft(p, p->chunk, &h))) return rc;
   if (p->K_max % p->chunk) { if ((rc = get_fft(p, p->K_max % p->chunk, &h))) return rc; }
   if ((rc = get_fft(p, 1, &h))) return rc;
-  if (p->fused_ok) {
-    if ((rc = get_fftA(p, p->chunk, &h))) return rc;
-    if (p->K_max % p->chunk) { if ((rc = get_fftA(p, p->K_max % p->chunk, &h))) return rc; }
-  }
   return EMRI_OK;
 }
 
@@ -261,41 +264,9 @@ int get_fft(emri_plan* p, int batch, cufftHandle* out) {
     p->fftwork_bytes = ws;
     p->bytes += (int64_t)ws;
     for (auto& kv : p->fft) cufftSetWorkArea(kv.second, p->d_fftwork);
-    for (auto& kv : p->fftA) cufftSetWorkArea(kv.second, p->d_fftwork);
   }
   if (p->d_fftwork) CKF(cufftSetWorkArea(h, p->d_fftwork));
   p->fft[batch] = h;
-  *out = h;
-  return EMRI_OK;
-}
-
-// pass A of the fused path: N2 strided transforms of length N1 per walker on the walker-interleaved chunk z[i1][k][i2]
-int get_fftA(emri_plan* p, int kc, cufftHandle* out) {
-  auto it = p->fftA.find(kc);
-  if (it != p->fftA.end()) { *out = it->second; return EMRI_OK; }
-  cufftHandle h;
-  CKF(cufftCreate(&h));
-  CKF(cufftSetAutoAllocation(h, 0));
-  long long n[1] = {(long long)p->N1};
-  long long embed[1] = {(long long)p->N1};
-  const long long stride = (long long)kc * p->N2;
-  size_t ws = 0;
-  cufftResult r = cufftMakePlanMany64(h, 1, n, embed, stride, 1, embed, stride, 1, CUFFT_Z2Z, stride, &ws);
-  if (r != CUFFT_SUCCESS) { p->last_err = (int)r; cufftDestroy(h); return EMRI_ECUFFT; }
-  if (ws > p->fftwork_bytes) {
-    // reached from alloc_chunk only (the full chunk is planned first)
-    cudaError_t e = cudaDeviceSynchronize();
-    if (e != cudaSuccess) { p->last_err = (int)e; cufftDestroy(h); return EMRI_ECUDA; }
-    if (p->d_fftwork) { cudaFree(p->d_fftwork); p->bytes -= (int64_t)p->fftwork_bytes; p->d_fftwork = nullptr; }
-    e = cudaMalloc(&p->d_fftwork, ws);
-    if (e != cudaSuccess) { p->last_err = (int)e; p->fftwork_bytes = 0; cufftDestroy(h); cudaGetLastError(); return EMRI_ENOMEM; }
-    p->fftwork_bytes = ws;
-    p->bytes += (int64_t)ws;
-    for (auto& kv : p->fft) cufftSetWorkArea(kv.second, p->d_fftwork);
-    for (auto& kv : p->fftA) cufftSetWorkArea(kv.second, p->d_fftwork);
-  }
-  if (p->d_fftwork) CKF(cufftSetWorkArea(h, p->d_fftwork));
-  p->fftA[kc] = h;
   *out = h;
   return EMRI_OK;
 }
@@ -367,10 +338,8 @@ int run_orbit(emri_plan* p, const double* params, int K, cudaStream_t s) {
   return EMRI_OK;
 }
 
-int run_synth(emri_plan* p, int k0, int K, double* outI, double* outII, int64_t pitch, double* outZ, cudaStream_t s,
-              bool interleaved = false) {
+int run_synth(emri_plan* p, int k0, int K, double* outI, double* outII, int64_t pitch, double* outZ, cudaStream_t s) {
   SynthArgs a;
-  a.z_log2n2 = interleaved ? p->log2N2 : 0;
   a.wc = p->d_wc; a.nodes = p->d_nodes; a.nodeaux = p->d_nodeaux; a.jpl = p->d_jpl; a.status = p->d_status;
   a.base = p->d_base; a.tol = 1e-16;
   a.gtab = p->d_gtab; a.bessel = p->n_max > 48 ? 1 : 0;
@@ -428,21 +397,45 @@ int run_like(emri_plan* p, int k0, int K, const double* Z, const double* data_ff
   return EMRI_OK;
 }
 
-int run_fft_like(emri_plan* p, int k0, int kc, const double* Y, cudaStream_t s) {
-  FftLikeArgs a;
-  a.Y = reinterpret_cast<const double2*>(Y); a.twid = p->d_twid; a.twA = p->d_twA; a.twB = p->d_twB; a.alpha = p->d_alpha; a.gamma = p->d_gamma;
-  a.partial = p->d_partial; a.k0 = k0; a.K = kc; a.n_part = p->N1; a.N1 = p->N1; a.N = p->N;
-  const int rows = FB_ELEMS / p->N2;
-  const int64_t groups = ((int64_t)p->N1 * kc + rows - 1) / rows;
-  const int grid = (int)std::min<int64_t>(groups, (int64_t)p->sm_count * 2 * 8);
-  const size_t smem = ((size_t)256 + p->N2 + (size_t)rows * (p->N2 + p->N2 / 16)) * sizeof(double2);
-  switch (p->log2N2) {
-    case 8: fft_like_kernel<8><<<grid, FB_THREADS, smem, s>>>(a); break;
-    case 9: fft_like_kernel<9><<<grid, FB_THREADS, smem, s>>>(a); break;
-    case 10: fft_like_kernel<10><<<grid, FB_THREADS, smem, s>>>(a); break;
-    case 11: fft_like_kernel<11><<<grid, FB_THREADS, smem, s>>>(a); break;
-    default: fft_like_kernel<12><<<grid, FB_THREADS, smem, s>>>(a); break;
+// both transform passes + Eq. 8 of a chunk in its natural layout z[kc][N] (fftlike.cuh: fft2_like_kernel)
+constexpr size_t FFT2_SMEM = ((size_t)256 + 512 + FB_ELEMS + FB_ELEMS / 16 + 16) * sizeof(double2);
+template <int LG1>
+cudaError_t fft2_set_smem_row() {
+  cudaError_t e;
+  if ((e = cudaFuncSetAttribute(fft2_like_kernel<LG1, 8>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)FFT2_SMEM))) return e;
+  if ((e = cudaFuncSetAttribute(fft2_like_kernel<LG1, 9>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)FFT2_SMEM))) return e;
+  if ((e = cudaFuncSetAttribute(fft2_like_kernel<LG1, 10>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)FFT2_SMEM))) return e;
+  if ((e = cudaFuncSetAttribute(fft2_like_kernel<LG1, 11>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)FFT2_SMEM))) return e;
+  return cudaFuncSetAttribute(fft2_like_kernel<LG1, 12>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)FFT2_SMEM);
+}
+cudaError_t fft2_set_smem() {
+  cudaError_t e;
+  if ((e = fft2_set_smem_row<8>())) return e;
+  if ((e = fft2_set_smem_row<9>())) return e;
+  return fft2_set_smem_row<10>();
+}
+template <int LG1>
+void fft2_launch_row(int lg2, int grid, cudaStream_t s, const Fft2Args& a) {
+  switch (lg2) {
+    case 8: fft2_like_kernel<LG1, 8><<<grid, FB_THREADS, FFT2_SMEM, s>>>(a); break;
+    case 9: fft2_like_kernel<LG1, 9><<<grid, FB_THREADS, FFT2_SMEM, s>>>(a); break;
+    case 10: fft2_like_kernel<LG1, 10><<<grid, FB_THREADS, FFT2_SMEM, s>>>(a); break;
+    case 11: fft2_like_kernel<LG1, 11><<<grid, FB_THREADS, FFT2_SMEM, s>>>(a); break;
+    default: fft2_like_kernel<LG1, 12><<<grid, FB_THREADS, FFT2_SMEM, s>>>(a); break;
   }
+}
+int run_fft2_like(emri_plan* p, int k0, int kc, const double* z, cudaStream_t s) {
+  Fft2Args a;
+  a.z = reinterpret_cast<const double2*>(z); a.ring = p->d_ring; a.twid1 = p->d_twid1; a.twid2 = p->d_twid;
+  a.tw3 = p->d_tw3; a.alpha = p->d_alpha; a.gamma = p->d_gamma; a.partial = p->d_partial; a.ctr = p->d_fft2ctr;
+  a.k0 = k0; a.kc = kc; a.g = fft2_group(p); a.G = (kc + a.g - 1) / a.g; a.n_part = p->N1; a.N1 = p->N1; a.N2 = p->N2;
+  a.N = p->N; a.items = (unsigned)(((int64_t)a.g * p->N) / FB_ELEMS);
+  CK(cudaMemsetAsync(p->d_fft2ctr, 0, ((size_t)1 + 2 * a.G) * sizeof(unsigned), s));
+  const int64_t total = (int64_t)2 * a.G * a.items;
+  const int grid = (int)std::min<int64_t>(total, (int64_t)p->sm_count * 2);
+  if (p->log2N1 == 8) fft2_launch_row<8>(p->log2N2, grid, s, a);
+  else if (p->log2N1 == 9) fft2_launch_row<9>(p->log2N2, grid, s, a);
+  else fft2_launch_row<10>(p->log2N2, grid, s, a);
   p->launches += 1;
   CK(cudaGetLastError());
   return EMRI_OK;
@@ -514,25 +507,38 @@ int emri_plan_create(emri_plan** out, int64_t N, double dt, int n_max, int K_max
   if ((N & (N - 1)) == 0 && N >= (1 << 16) && N <= (1 << 22)) {
     int lg = 0;
     while (((int64_t)1 << lg) < N) ++lg;
-    p->log2N1 = std::max(8, std::min(10, lg - 10)); p->log2N2 = lg - p->log2N1;
+    // split N = N1 N2 (N1 in 256 .. 1024, N2 in 256 .. 4096): N1 = 512 at one year of samples -- a pass-A ticket is then
+    // 8 adjacent columns (128-byte segments) and a pass-B ticket one 4096-point row (measured best on B200)
+    p->log2N1 = lg <= 19 ? 8 : (lg <= 21 ? 9 : 10);
+    if (const char* ev = std::getenv("EMRI_FFT_LOG2N1")) p->log2N1 = std::max(std::max(8, lg - 12), std::min(std::min(10, lg - 8), std::atoi(ev)));
+    p->log2N2 = lg - p->log2N1;
     p->N2 = 1 << p->log2N2; p->N1 = 1 << p->log2N1;
     p->fused_ok = true;
+    if (const char* ev = std::getenv("EMRI_FFT_GROUP")) p->fft2_g = std::max(0, std::atoi(ev));      // experiments (fftlike.cuh)
     p->n_cd = (int)((p->Nf + 255) / 256);
-    {
-      // stage twiddles of the last pass, transposed (fftlike.cuh): W_256^{k t} at [16 t + k], W_N2^{jj t} at [t NSL + jj]
+    // stage twiddles of an L-point pass, transposed (fftlike.cuh): W_256^{k t} at [16 t + k], W_L^{jj t} at [256 + t NSL + jj]
+    auto stage_twiddles = [](int log2L, std::vector<double2>& tw) {
       const long double tp = -2.0L * 3.14159265358979323846264338327950288L;
-      const int nfull = (p->log2N2 - 1) / 4, RL = p->N2 >> (4 * nfull), NSL = p->N2 / RL;
-      twid.resize((size_t)256 + p->N2);
+      const int L = 1 << log2L, nfull = (log2L - 1) / 4, RL = L >> (4 * nfull), NSL = L / RL;
+      tw.resize((size_t)256 + L);
       for (int t = 0; t < 16; ++t)
         for (int k = 0; k < 16; ++k) {
           const long double ang = tp * (long double)(k * t) / 256.0L;
-          twid[16 * t + k] = make_double2((double)cosl(ang), (double)sinl(ang));
+          tw[16 * t + k] = make_double2((double)cosl(ang), (double)sinl(ang));
         }
       for (int t = 0; t < RL; ++t)
         for (int jj = 0; jj < NSL; ++jj) {
-          const long double ang = tp * (long double)(((int64_t)jj * t) % p->N2) / (long double)p->N2;
-          twid[256 + (size_t)t * NSL + jj] = make_double2((double)cosl(ang), (double)sinl(ang));
+          const long double ang = tp * (long double)(((int64_t)jj * t) % L) / (long double)L;
+          tw[256 + (size_t)t * NSL + jj] = make_double2((double)cosl(ang), (double)sinl(ang));
         }
+    };
+    stage_twiddles(p->log2N2, twid);
+    {
+      std::vector<double2> tw1;
+      stage_twiddles(p->log2N1, tw1);
+      if ((rc = dev_alloc(p, &p->d_twid1, tw1.size()))) return fail(rc);
+      if (cudaMemcpy(p->d_twid1, tw1.data(), tw1.size() * sizeof(double2), cudaMemcpyHostToDevice) != cudaSuccess)
+        return fail(EMRI_ECUDA);
     }
     if ((rc = dev_alloc(p, &p->d_twid, twid.size()))) return fail(rc);
     if ((rc = dev_alloc(p, &p->d_alpha, (size_t)N))) return fail(rc);
@@ -541,31 +547,19 @@ int emri_plan_create(emri_plan** out, int64_t N, double dt, int n_max, int K_max
     if (cudaMemcpy(p->d_twid, twid.data(), twid.size() * sizeof(double2), cudaMemcpyHostToDevice) != cudaSuccess)
       return fail(EMRI_ECUDA);
     {
-      // two-level table of the inter-pass twiddle W_N^q = twA[q >> 10] twB[q & 1023]
+      // three-level table of the inter-pass twiddle: W_N^q, W_N^{128 q} (q < 128), W_N^{16384 q} (q < 256)
       const long double tp = -2.0L * 3.14159265358979323846264338327950288L;
-      std::vector<double2> tA((size_t)(N >> 10)), tB(1024);
-      for (size_t q = 0; q < tA.size(); ++q) {
-        const long double ang = tp * (long double)q / (long double)tA.size();
-        tA[q] = make_double2((double)cosl(ang), (double)sinl(ang));
+      std::vector<double2> t3(512, make_double2(1.0, 0.0));
+      for (int q = 0; q < 512; ++q) {
+        const int64_t e = q < 128 ? q : (q < 256 ? (int64_t)128 * (q - 128) : (int64_t)16384 * (q - 256));
+        if (e >= N) continue;
+        const long double ang = tp * (long double)e / (long double)N;
+        t3[q] = make_double2((double)cosl(ang), (double)sinl(ang));
       }
-      for (int q = 0; q < 1024; ++q) {
-        const long double ang = tp * (long double)q / (long double)N;
-        tB[q] = make_double2((double)cosl(ang), (double)sinl(ang));
-      }
-      if ((rc = dev_alloc(p, &p->d_twA, tA.size()))) return fail(rc);
-      if ((rc = dev_alloc(p, &p->d_twB, tB.size()))) return fail(rc);
-      if (cudaMemcpy(p->d_twA, tA.data(), tA.size() * sizeof(double2), cudaMemcpyHostToDevice) != cudaSuccess ||
-          cudaMemcpy(p->d_twB, tB.data(), tB.size() * sizeof(double2), cudaMemcpyHostToDevice) != cudaSuccess)
-        return fail(EMRI_ECUDA);
+      if ((rc = dev_alloc(p, &p->d_tw3, t3.size()))) return fail(rc);
+      if (cudaMemcpy(p->d_tw3, t3.data(), t3.size() * sizeof(double2), cudaMemcpyHostToDevice) != cudaSuccess) return fail(EMRI_ECUDA);
     }
-    const int rows = FB_ELEMS / p->N2;
-    const int smem = (int)(((size_t)256 + p->N2 + (size_t)rows * (p->N2 + p->N2 / 16)) * sizeof(double2));
-    if (cudaFuncSetAttribute(fft_like_kernel<8>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem) != cudaSuccess ||
-        cudaFuncSetAttribute(fft_like_kernel<9>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem) != cudaSuccess ||
-        cudaFuncSetAttribute(fft_like_kernel<10>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem) != cudaSuccess ||
-        cudaFuncSetAttribute(fft_like_kernel<11>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem) != cudaSuccess ||
-        cudaFuncSetAttribute(fft_like_kernel<12>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem) != cudaSuccess)
-      return fail(EMRI_ECUDA);
+    if (fft2_set_smem() != cudaSuccess) return fail(EMRI_ECUDA);
   }
   if ((rc = dev_alloc(p, &p->d_partial, (size_t)K_max * std::max(p->n_part, p->N1)))) return fail(rc);
   if ((rc = dev_alloc(p, &p->d_params, (size_t)K_max * EMRI_NPAR))) return fail(rc);
@@ -621,7 +615,6 @@ int emri_plan_destroy(emri_plan* p) {
   if (!p) return EMRI_EINVAL;
   cudaDeviceSynchronize();
   for (auto& kv : p->fft) cufftDestroy(kv.second);
-  for (auto& kv : p->fftA) cufftDestroy(kv.second);
   for (auto e : p->ev) cudaEventDestroy(e);
   if (p->ev_call) cudaEventDestroy(p->ev_call);
   if (p->ev_data) cudaEventDestroy(p->ev_data);
@@ -631,7 +624,7 @@ int emri_plan_destroy(emri_plan* p) {
   void* ptrs[] = {p->d_w, p->d_wc, p->d_nodes, p->d_hbuf, p->d_partial, p->d_base, p->d_nodeaux, p->d_jpl, p->d_status,
                   p->d_params, p->d_data, p->d_logL, p->d_Y, p->d_z, p->d_lnu, p->d_logLY, p->d_inbox,
                   p->d_partner, p->d_fftwork, p->d_seg, p->d_plrow, p->d_mode, p->d_pclamp, p->d_counts,
-                  p->d_twid, p->d_twA, p->d_twB, p->d_alpha, p->d_gamma, p->d_cdpart, p->d_gtab, p->d_dpsteps, p->d_dpn, p->d_dpstop,
+                  p->d_twid, p->d_twid1, p->d_tw3, p->d_ring, p->d_fft2ctr, p->d_alpha, p->d_gamma, p->d_cdpart, p->d_gtab, p->d_dpsteps, p->d_dpn, p->d_dpstop,
                   p->d_dpbad, p->d_dpzero};
   for (void* q : ptrs) if (q) cudaFree(q);
   delete p;
@@ -756,6 +749,10 @@ int emri_plan_set_chunk(emri_plan* p, int c) {
   if (c > p->K_max) c = p->K_max;
   CK(cudaDeviceSynchronize());
   if (p->d_hbuf) p->bytes -= (int64_t)((size_t)2 * p->chunk * p->N * sizeof(double));
+  if (p->d_ring) {
+    const int g = fft2_group(p), G = (p->chunk + g - 1) / g;
+    p->bytes -= (int64_t)((size_t)(G > 1 ? 2 : 1) * g * p->N * sizeof(double2) + ((size_t)1 + 2 * G) * sizeof(unsigned));
+  }
   p->chunk = c;
   return alloc_chunk(p);
 }
@@ -868,9 +865,9 @@ static int loglike_impl(emri_plan* p, const double* params, int K, const double*
     const bool fused = p->fused_ok && p->fused_on && !fcoef;
     cufftHandle h;
     int rc;
-    for (int k0 = 0; k0 < K; k0 += p->chunk) {
+    for (int k0 = 0; k0 < K && !fused; k0 += p->chunk) {
       const int kc = std::min(p->chunk, K - k0);
-      if ((rc = fused ? get_fftA(p, kc, &h) : get_fft(p, kc, &h))) return rc;
+      if ((rc = get_fft(p, kc, &h))) return rc;
     }
   }
   cudaGraph_t graph = nullptr;
@@ -910,17 +907,12 @@ static int loglike_enqueue(emri_plan* p, const double* params, int K, const doub
   int nch = 0;
   const double scale = 2.0 * p->dt / (double)p->N;
   if (p->fused_ok && p->fused_on && !fcoef) {
-    // fused path (fftlike.cuh): walker-interleaved synthesis, one strided cuFFT pass, last pass + Eq. 8 in one kernel
+    // fused path (fftlike.cuh): ONE kernel of this library does both transform passes and Eq. 8
     for (int k0 = 0; k0 < K; k0 += p->chunk, ++nch) {
       const int kc = std::min(p->chunk, K - k0);
       mark(p, s);
-      if ((rc = run_synth(p, k0, kc, nullptr, nullptr, 0, p->d_hbuf, s, true))) return rc;
+      if ((rc = run_synth(p, k0, kc, nullptr, nullptr, 0, p->d_hbuf, s))) return rc;
       mark(p, s);
-      cufftHandle h;
-      if ((rc = get_fftA(p, kc, &h))) return rc;
-      CKF(cufftSetStream(h, s));
-      CKF(cufftExecZ2Z(h, reinterpret_cast<cufftDoubleComplex*>(p->d_hbuf), reinterpret_cast<cufftDoubleComplex*>(p->d_hbuf),
-                       CUFFT_FORWARD));
       mark(p, s);
       if (nch == 0) {
         // the weights of Eq. 8 in pass-B order, from the caller's data spectrum (the only reader of data_fft)
@@ -930,7 +922,7 @@ static int loglike_enqueue(emri_plan* p, const double* params, int K, const doub
         p->launches += 1;
         CK(cudaGetLastError());
       }
-      if ((rc = run_fft_like(p, k0, kc, p->d_hbuf, s))) return rc;
+      if ((rc = run_fft2_like(p, k0, kc, p->d_hbuf, s))) return rc;
       mark(p, s);
     }
     p->n_chunks_last = nch;

@@ -1,17 +1,18 @@
-// fftlike.cuh -- stages (c)+(d) fused: the LAST pass of the transform and the reduction of Eq. 8
-// in one kernel, so that the spectrum is never written back nor read again (PAPER.md:43,
-// :134: waveform and FFT are one GPU stage).
+// fftlike.cuh -- stages (c)+(d) fused: BOTH passes of the transform and the reduction of Eq. 8
+// in one persistent kernel of this library, so that the spectrum is never written back nor read again
+// (waveform and FFT are one GPU stage).
 // Part of the sm_100a implementation of include/emri.h; included by emri.cu (one translation unit).
 //
-// N = N1 N2 (powers of two; N1 = 1024 for N >= 2^20 -- the length cuFFT's strided kernel is fastest at, measured -- and
-// N2 = N / N1 <= 4096).  With i = N2 i1 + i2 and m = m1 + N1 m2,
+// N = N1 N2 (powers of two, N1 in 256 .. 1024, N2 in 256 .. 4096; N1 = 512 at one year of samples).  With i = N2 i1 + i2
+// and m = m1 + N1 m2,
 //     Z[m1 + N1 m2] = sum_{i2} W_N^{i2 m1} W_N2^{i2 m2}  [ sum_{i1} z[N2 i1 + i2] W_N1^{i1 m1} ].
-//   pass A  the bracket: N2 strided transforms of length N1 per walker.  The synthesis writes the chunk walker-interleaved,
-//           z[i1][k][i2], so ONE strided batched cuFFT plan (stride K_c N2, distance 1, batch K_c N2) does all walkers of a
-//           chunk in place: Y[m1][k][i2].  (The one vendor call.)
-//   pass B  this file: one row (m1, k) of N2 contiguous elements per group of N2/16 threads: load, multiply by the
-//           twiddle W_N^{i2 m1}, N2-point transform (radix-16 stages in registers, padded shared-memory exchanges in
-//           between, last stage radix N2/256 or 16), and the outputs Z[m1 + N1 m2] go straight from registers into Eq. 8.
+//   pass A  the bracket: N2 strided transforms of length N1 per walker, read from the chunk z[k][N] the synthesis wrote
+//           (natural layout): a ticket is 4096/N1 adjacent columns (128-byte segments at N1 = 512); the result goes to
+//           a second buffer as Y[m1][k][i2].
+//   pass B  one row (m1, k) of N2 contiguous elements per group of N2/16 threads: load, multiply by the twiddle
+//           W_N^{i2 m1}, N2-point transform, and the outputs Z[m1 + N1 m2] go straight from registers into Eq. 8.
+// Both passes: 16 elements per thread, radix-16 stages in registers, padded shared-memory exchanges in between
+// (Stockham autosort), last stage radix L/256 (or 16).
 //
 // Eq. 8 without pairing.  With a = Z[m], b = conj Z[N-m] the two channels are H_I = (a+b)/2, H_II = (a-b)/(2i), and
 //     |D_I - H_I|^2 + |D_II - H_II|^2 = |D_I|^2 + |D_II|^2 - 2 Re(a P + b Q) + (|a|^2 + |b|^2)/2,
@@ -25,9 +26,9 @@
 
 namespace {
 
-constexpr int FB_THREADS = 256;           // threads per CTA of the pass-B kernel
+constexpr int FB_THREADS = 256;           // threads per CTA
 constexpr int FB_EPT = 16;                // elements per thread
-constexpr int FB_ELEMS = FB_THREADS * FB_EPT;   // elements per CTA pass = 4096: 4096 / N2 rows at once
+constexpr int FB_ELEMS = FB_THREADS * FB_EPT;   // elements per ticket = 4096
 
 DEVINL double2 cmul(const double2 a, const double2 b) {
   return make_double2(fma(a.x, b.x, -a.y * b.y), fma(a.x, b.y, a.y * b.x));
@@ -78,121 +79,242 @@ __host__ __device__ constexpr int bitrev(int q) {
 
 DEVINL int fb_pad(int a) { return a + (a >> 4); }      // one element of padding per 16: conflict-free exchanges
 
-struct FftLikeArgs {
-  const double2* Y;        // [N1][K][N2] after pass A
-  const double2* twid;     // [256 + N2]: W_256^{k t} at [16 t + k] (second radix-16 stage), then W_N2^{jj t} at
-                           // [t NSL + jj] (last stage) -- both transposed so that consecutive threads read consecutive entries
-  const double2* twA;      // [N / 1024] W_N^{1024 q}: with twB the inter-pass twiddle W_N^q = twA[q >> 10] twB[q & 1023]
-  const double2* twB;      // [1024] W_N^q
-  const double* alpha;     // [N1][N2] alpha of element (m1, m2), pass-B order
-  const double2* gamma;    // [N1][N2]
-  double* partial;         // [K_total][n_part]; this chunk's walker kl at row k0 + kl, entry m1
-  int k0, K, n_part;
-  int N1;
+// Pass B ticket: ROWS = FB_ELEMS / N2 consecutive rows of Y[N1][K][N2] starting at row r0 (row r = m1 K + k).
+// LOG2L = log2 N2 in {8 .. 12}.  Y is read with ld.global.cg (it was written by other CTAs of the same launch); the last
+// stage's twiddles `tw_last` [N2] and the weights come from global memory through L1.  s_tw3: three-level table of the
+// inter-pass twiddle in shared memory, W_N^q = t0[q & 127] t1[(q >> 7) & 127] t2[q >> 14].  Ends with the exchange
+// buffer free (barrier).
+template <int LOG2L>
+DEVINL void passB_rows(const double2* __restrict__ Ybuf, int64_t r0, int64_t n_rows, int K, int64_t N,
+                       const double2* s_tw3, const double2* s_tw2,
+                       const double2* __restrict__ tw_last, double2* s_x, double* s_red, const double* __restrict__ alpha,
+                       const double2* __restrict__ gamma, double* __restrict__ partial, int k_first, int n_part) {
+  constexpr int L = 1 << LOG2L, T = L / FB_EPT;                 // threads per row
+  constexpr int NFULL = (LOG2L - 1) / 4;                        // radix-16 stages that end in shared memory
+  constexpr int RL = L >> (4 * NFULL);                          // radix of the last stage (16, 2, 4, 8)
+  constexpr int U = FB_EPT / RL;                                // last-stage transforms per thread
+  constexpr int NSL = L / RL;                                   // their stride
+  const int tid = threadIdx.x, row_in = tid / T, j = tid % T;
+  double2* x = s_x + (size_t)row_in * (L + L / 16);
+  const int64_t r = r0 + row_in;
+  const bool live = r < n_rows;
+  const int m1 = live ? (int)(r / K) : 0, kl = live ? (int)(r - (int64_t)m1 * K) : 0;
+  double2 v[FB_EPT];
+  // ---- load (each element of Y is read exactly once) and inter-pass twiddle W_N^{c m1}, c = j + t T
+  {
+    const double2* src = Ybuf + (size_t)r * L + j;
+#pragma unroll
+    for (int t = 0; t < FB_EPT; ++t)
+      v[t] = live ? __ldcg(src + t * T) : make_double2(0.0, 0.0);
+    // W_N^{j m1} and W_N^{T m1} from the three-level table (exactly rounded entries, two complex products)
+    const int64_t q0 = ((int64_t)j * m1) & (N - 1), q1 = ((int64_t)T * m1) & (N - 1);
+    double2 w = cmul(cmul(s_tw3[q0 & 127], s_tw3[128 + ((q0 >> 7) & 127)]), s_tw3[256 + (q0 >> 14)]);
+    const double2 ws = cmul(cmul(s_tw3[q1 & 127], s_tw3[128 + ((q1 >> 7) & 127)]), s_tw3[256 + (q1 >> 14)]);
+    // running product: 15 complex multiplications, < 2e-15 relative on the last factor
+#pragma unroll
+    for (int t = 0; t < FB_EPT; ++t) {
+      v[t] = cmul(v[t], w);
+      w = cmul(w, ws);
+    }
+  }
+  // ---- radix-16 stages ending in shared memory (Stockham autosort)
+#pragma unroll
+  for (int s = 0; s < NFULL; ++s) {
+    const int Ns = 1 << (4 * s);
+    const int k = j & (Ns - 1);
+    if (s > 0) {
+#pragma unroll
+      for (int t = 0; t < FB_EPT; ++t) v[t] = x[fb_pad(j + t * T)];
+      // twiddle W_{16 Ns}^{k t}: Ns = 16 here (at most two such stages), table [t][k]
+#pragma unroll
+      for (int t = 1; t < FB_EPT; ++t) v[t] = cmul(v[t], s_tw2[16 * t + k]);
+      __syncthreads();                       // every thread holds its inputs: the buffer may be overwritten
+    }
+    fft_regs<16>(v);
+    const int base = (j - k) * 16 + k;
+#pragma unroll
+    for (int t = 0; t < FB_EPT; ++t) x[fb_pad(base + t * Ns)] = v[bitrev<16>(t)];
+    __syncthreads();
+  }
+  // ---- last stage in registers, outputs m2 = jj + t NSL go straight into Eq. 8
+  double acc = 0.0;
+  const double* al = alpha + (size_t)m1 * L;
+  const double2* ga = gamma + (size_t)m1 * L;
+#pragma unroll
+  for (int u = 0; u < U; ++u) {
+    const int jj = j + u * T;
+    double2 q[RL];
+#pragma unroll
+    for (int t = 0; t < RL; ++t) q[t] = x[fb_pad(jj + t * NSL)];
+#pragma unroll
+    for (int t = 1; t < RL; ++t) q[t] = cmul(q[t], __ldg(tw_last + t * NSL + jj));
+    fft_regs<RL>(q);
+#pragma unroll
+    for (int t = 0; t < RL; ++t) {
+      const double2 z = q[bitrev<RL>(t)];
+      const int m2 = jj + t * NSL;
+      const double alp = __ldg(al + m2);
+      const double2 g = __ldg(ga + m2);
+      acc = fma(alp, fma(z.x, z.x, z.y * z.y), acc);
+      acc = fma(-2.0, fma(z.x, g.x, -z.y * g.y), acc);
+    }
+  }
+  __syncthreads();                           // the exchange buffer is free for the next pass
+  // ---- fixed-order sum over the row's T threads: shuffle tree inside a warp, then across the row's warps
+  if (T >= 32) {
+#pragma unroll
+    for (int off = 16; off > 0; off >>= 1) acc += __shfl_xor_sync(0xffffffffu, acc, off);
+    if ((tid & 31) == 0) s_red[tid >> 5] = acc;
+    __syncthreads();
+    if (j == 0 && live) {
+      double sum = 0.0;
+#pragma unroll
+      for (int wq = 0; wq < T / 32; ++wq) sum += s_red[row_in * (T / 32) + wq];
+      partial[(size_t)(k_first + kl) * n_part + m1] = sum;
+    }
+    __syncthreads();
+  } else {
+#pragma unroll
+    for (int off = T / 2; off > 0; off >>= 1) acc += __shfl_xor_sync(0xffffffffu, acc, off);
+    if (j == 0 && live) partial[(size_t)(k_first + kl) * n_part + m1] = acc;
+  }
+}
+
+// ---- The kernel.  Walkers of a chunk are taken in groups of g (default: the whole chunk, one group).  Pass A of group q
+// writes slot q & 1 of the second buffer, pass B of group q reads it back and feeds Eq. 8.  One persistent kernel runs
+// everything as a dataflow: CTAs pop tickets from ONE counter in the order  A(0) | A(1) B(0) | A(2) B(1) | ... | B(G-1)
+// (`items` tickets per group and pass, 4096 elements each; inside a block the tickets of A(q+1) and B(q) alternate).
+// B(q) waits until all tickets of A(q) are done, A(q) until B(q-2) has released the slot: both point to SMALLER tickets,
+// which running CTAs hold, so the schedule cannot deadlock whatever the number of resident CTAs.  Measured on B200
+// (configs[3]): the larger the group the faster (the weights of a row m1 are shared by the g walkers of the group and
+// stay in L1/L2; keeping the intermediate of a small group inside the 126 MB L2 gained nothing because the kernel is
+// bound by instruction latency, not by HBM), hence g = chunk.
+struct Fft2Args {
+  const double2* z;        // [kc][N] chunk, natural layout
+  double2* ring;           // [slots][g][N], slots = 1 when there is a single group
+  const double2* twid1;    // [256 + N1] stage twiddles of pass A (same construction as twid2)
+  const double2* twid2;    // [256 + N2] of pass B
+  const double2* tw3;      // [512] inter-pass twiddle in three levels: W_N^q, W_N^{128 q} (q < 128), W_N^{16384 q} (q < 256)
+  const double* alpha;
+  const double2* gamma;
+  double* partial;
+  unsigned* ctr;           // [0] ticket counter, [1 + q] tickets of A(q) done, [1 + G + q] of B(q); zeroed before the launch
+  int k0, kc, g, G, n_part, N1, N2;
+  unsigned items;          // tickets per block = g N / 4096
   int64_t N;
 };
 
-// LOG2L = log2 N2 in {8 .. 12}.  CTA pass = FB_ELEMS / N2 consecutive rows of Y (same m1 for a chunk size that is a
-// multiple of that; any chunk size works, the row's (m1, k) are recomputed per row).
-template <int LOG2L>
-__global__ void __launch_bounds__(FB_THREADS, 2) fft_like_kernel(FftLikeArgs a) {
-  constexpr int L = 1 << LOG2L, T = L / FB_EPT;                 // threads per row
-  constexpr int ROWS = FB_ELEMS / L;                            // rows per CTA pass
-  constexpr int NFULL = (LOG2L - 1) / 4;                        // radix-16 stages that end in shared memory
-  constexpr int RL = L >> (4 * NFULL);                          // radix of the last stage (16, 2, 4)
-  constexpr int U = FB_EPT / RL;                                // last-stage transforms per thread
-  constexpr int NSL = L / RL;                                   // their stride
-  extern __shared__ __align__(16) unsigned char fb_smem[];
-  double2* s_tw2 = reinterpret_cast<double2*>(fb_smem);                      // [16][16]
-  double2* s_tw = s_tw2 + 256;                                               // [RL][NSL]
-  double2* s_x = s_tw + L;                                                   // [ROWS][L + L/16]
-  __shared__ double s_red[FB_THREADS / 32];
-  const int tid = threadIdx.x, row_in = tid / T, j = tid % T;
-  for (int q = tid; q < 256 + L; q += FB_THREADS) s_tw2[q] = a.twid[q];
-  double2* x = s_x + (size_t)row_in * (L + L / 16);
-  const int64_t n_rows = (int64_t)a.N1 * a.K;
+DEVINL void fft2_wait(const unsigned* ctr, unsigned target) {
+  if (threadIdx.x == 0) {
+    unsigned v;
+    for (;;) {
+      asm volatile("ld.acquire.gpu.global.u32 %0, [%1];" : "=r"(v) : "l"(ctr) : "memory");
+      if (v >= target) break;
+      __nanosleep(64);
+    }
+  }
   __syncthreads();
-  for (int64_t r0 = (int64_t)blockIdx.x * ROWS; r0 < n_rows; r0 += (int64_t)gridDim.x * ROWS) {
-    const int64_t r = r0 + row_in;
-    const bool live = r < n_rows;
-    const int m1 = live ? (int)(r / a.K) : 0, kl = live ? (int)(r - (int64_t)m1 * a.K) : 0;
-    double2 v[FB_EPT];
-    // ---- load (streaming: each element of Y is read exactly once) and inter-pass twiddle W_N^{c m1}, c = j + t T
-    {
-      const double2* src = a.Y + (size_t)r * L + j;
+}
+DEVINL void fft2_signal(unsigned* ctr) {
+  __syncthreads();                                  // every thread's global stores precede ...
+  if (threadIdx.x == 0) { __threadfence(); atomicAdd(ctr, 1u); }      // ... the release of the ticket
+}
+
+// Pass A ticket: COLS adjacent columns (col0 ..) of one walker: N1-point transforms along i1 (stride N2), output row m1
+// of the group's ring slot.  Lanes run over the columns first, so a warp touches 32 / COLS segments of COLS x 16 B.
+template <int LOG2L>
+DEVINL void passA_cols(const double2* __restrict__ zk, double2* __restrict__ Yslot, int gq, int kl, int col0, int N2,
+                       const double2* s_tw2, const double2* __restrict__ tw_last, double2* s_x) {
+  constexpr int L = 1 << LOG2L, T = L / FB_EPT, COLS = FB_ELEMS / L;
+  constexpr int NFULL = (LOG2L - 1) / 4, RL = L >> (4 * NFULL), U = FB_EPT / RL, NSL = L / RL;
+  constexpr int XS = L + L / 16 + (COLS >= 8 ? 1 : 8 / COLS);   // column stride: the COLS lanes of a quarter-warp hit different banks
+  const int tid = threadIdx.x, c = tid % COLS, j = tid / COLS;
+  double2* x = s_x + (size_t)c * XS;
+  double2 v[FB_EPT];
+  {
+    const double2* src = zk + (size_t)j * N2 + col0 + c;
 #pragma unroll
-      for (int t = 0; t < FB_EPT; ++t) v[t] = live ? __ldcs(src + t * T) : make_double2(0.0, 0.0);
-      // W_N^{j m1} and W_N^{T m1} from the two-level table (exactly rounded entries, one complex product)
-      const int64_t q0 = ((int64_t)j * m1) & (a.N - 1), q1 = ((int64_t)T * m1) & (a.N - 1);
-      double2 w = cmul(__ldg(a.twA + (q0 >> 10)), __ldg(a.twB + (q0 & 1023)));
-      const double2 ws = cmul(__ldg(a.twA + (q1 >> 10)), __ldg(a.twB + (q1 & 1023)));
-      // running product: 15 complex multiplications, < 2e-15 relative on the last factor
+    for (int t = 0; t < FB_EPT; ++t) v[t] = __ldcs(src + (size_t)t * T * N2);
+  }
 #pragma unroll
-      for (int t = 0; t < FB_EPT; ++t) {
-        v[t] = cmul(v[t], w);
-        w = cmul(w, ws);
-      }
-    }
-    // ---- radix-16 stages ending in shared memory (Stockham autosort)
+  for (int s = 0; s < NFULL; ++s) {
+    const int Ns = 1 << (4 * s);
+    const int k = j & (Ns - 1);
+    if (s > 0) {
 #pragma unroll
-    for (int s = 0; s < NFULL; ++s) {
-      const int Ns = 1 << (4 * s);
-      const int k = j & (Ns - 1);
-      if (s > 0) {
+      for (int t = 0; t < FB_EPT; ++t) v[t] = x[fb_pad(j + t * T)];
 #pragma unroll
-        for (int t = 0; t < FB_EPT; ++t) v[t] = x[fb_pad(j + t * T)];
-        // twiddle W_{16 Ns}^{k t}: Ns = 16 here (at most two such stages), table [t][k]
-#pragma unroll
-        for (int t = 1; t < FB_EPT; ++t) v[t] = cmul(v[t], s_tw2[16 * t + k]);
-        __syncthreads();                       // every thread holds its inputs: the buffer may be overwritten
-      }
-      fft_regs<16>(v);
-      const int base = (j - k) * 16 + k;
-#pragma unroll
-      for (int t = 0; t < FB_EPT; ++t) x[fb_pad(base + t * Ns)] = v[bitrev<16>(t)];
+      for (int t = 1; t < FB_EPT; ++t) v[t] = cmul(v[t], s_tw2[16 * t + k]);
       __syncthreads();
     }
-    // ---- last stage in registers, outputs m2 = jj + t NSL go straight into Eq. 8
-    double acc = 0.0;
-    const double* al = a.alpha + (size_t)m1 * L;
-    const double2* ga = a.gamma + (size_t)m1 * L;
+    fft_regs<16>(v);
+    const int base = (j - k) * 16 + k;
 #pragma unroll
-    for (int u = 0; u < U; ++u) {
-      const int jj = j + u * T;
-      double2 q[RL];
+    for (int t = 0; t < FB_EPT; ++t) x[fb_pad(base + t * Ns)] = v[bitrev<16>(t)];
+    __syncthreads();
+  }
 #pragma unroll
-      for (int t = 0; t < RL; ++t) q[t] = x[fb_pad(jj + t * NSL)];
+  for (int u = 0; u < U; ++u) {
+    const int jj = j + u * T;
+    double2 q[RL];
 #pragma unroll
-      for (int t = 1; t < RL; ++t) q[t] = cmul(q[t], s_tw[t * NSL + jj]);
-      fft_regs<RL>(q);
+    for (int t = 0; t < RL; ++t) q[t] = x[fb_pad(jj + t * NSL)];
 #pragma unroll
-      for (int t = 0; t < RL; ++t) {
-        const double2 z = q[bitrev<RL>(t)];
-        const int m2 = jj + t * NSL;
-        const double alp = __ldg(al + m2);
-        const double2 g = __ldg(ga + m2);
-        acc = fma(alp, fma(z.x, z.x, z.y * z.y), acc);
-        acc = fma(-2.0, fma(z.x, g.x, -z.y * g.y), acc);
-      }
+    for (int t = 1; t < RL; ++t) q[t] = cmul(q[t], __ldg(tw_last + t * NSL + jj));
+    fft_regs<RL>(q);
+#pragma unroll
+    for (int t = 0; t < RL; ++t) {
+      const int m1 = jj + t * NSL;
+      Yslot[((size_t)m1 * gq + kl) * N2 + col0 + c] = q[bitrev<RL>(t)];
     }
-    __syncthreads();                           // the exchange buffer is free for the next pass
-    // ---- fixed-order sum over the row's T threads: shuffle tree inside a warp, then across the row's warps
-    if (T >= 32) {
-#pragma unroll
-      for (int off = 16; off > 0; off >>= 1) acc += __shfl_xor_sync(0xffffffffu, acc, off);
-      if ((tid & 31) == 0) s_red[tid >> 5] = acc;
-      __syncthreads();
-      if (j == 0 && live) {
-        double sum = 0.0;
-#pragma unroll
-        for (int wq = 0; wq < T / 32; ++wq) sum += s_red[row_in * (T / 32) + wq];
-        a.partial[(size_t)(a.k0 + kl) * a.n_part + m1] = sum;
-      }
-      __syncthreads();
+  }
+  __syncthreads();                           // the exchange buffer is free for the next ticket
+}
+
+template <int LG1, int LG2>
+__global__ void __launch_bounds__(FB_THREADS, 2) fft2_like_kernel(Fft2Args a) {
+  constexpr int COLS = FB_ELEMS >> LG1, ROWS = FB_ELEMS >> LG2;
+  extern __shared__ __align__(16) unsigned char fb_smem[];
+  double2* s_tw2 = reinterpret_cast<double2*>(fb_smem);                      // [16][16] W_256^{k t}
+  double2* s_tw3 = s_tw2 + 256;                                              // [512] inter-pass twiddle levels
+  double2* s_x = s_tw3 + 512;                                                // exchange buffer of either pass
+  __shared__ double s_red[FB_THREADS / 32];
+  __shared__ unsigned s_ticket;
+  for (int q = threadIdx.x; q < 256; q += FB_THREADS) s_tw2[q] = a.twid2[q];
+  for (int q = threadIdx.x; q < 512; q += FB_THREADS) s_tw3[q] = a.tw3[q];
+  const unsigned total = 2u * (unsigned)a.G * a.items;
+  for (;;) {
+    __syncthreads();
+    if (threadIdx.x == 0) s_ticket = atomicAdd(a.ctr, 1u);
+    __syncthreads();
+    const unsigned tk = s_ticket;
+    if (tk >= total) break;
+    // ticket order: A(0) | A(1), B(0) alternating | A(2), B(1) alternating | ... | B(G-1)
+    int kind, q;
+    unsigned idx;
+    if (tk < a.items) { kind = 0; q = 0; idx = tk; }
+    else {
+      const unsigned t2 = tk - a.items, pb = t2 / (2u * a.items);
+      if (pb < (unsigned)a.G - 1u) {
+        const unsigned r = t2 - pb * 2u * a.items;
+        kind = (int)(r & 1u); q = kind ? (int)pb : (int)pb + 1; idx = r >> 1;
+      } else { kind = 1; q = a.G - 1; idx = t2 - ((unsigned)a.G - 1u) * 2u * a.items; }
+    }
+    const int gq = min(a.g, a.kc - q * a.g);
+    const unsigned nq = (unsigned)(((int64_t)gq * a.N) / FB_ELEMS);
+    if (idx >= nq) continue;                  // ragged last group
+    double2* slot = a.ring + (size_t)(q & 1) * a.g * a.N;
+    if (kind == 0) {
+      if (q >= 2) fft2_wait(a.ctr + 1 + a.G + (q - 2), a.items);
+      const int cbs = a.N2 / COLS;
+      const int kl = (int)idx / cbs, cb = (int)idx - kl * cbs;
+      passA_cols<LG1>(a.z + (size_t)(q * a.g + kl) * a.N, slot, gq, kl, cb * COLS, a.N2, s_tw2, a.twid1 + 256, s_x);
+      fft2_signal(a.ctr + 1 + q);
     } else {
-#pragma unroll
-      for (int off = T / 2; off > 0; off >>= 1) acc += __shfl_xor_sync(0xffffffffu, acc, off);
-      if (j == 0 && live) a.partial[(size_t)(a.k0 + kl) * a.n_part + m1] = acc;
+      fft2_wait(a.ctr + 1 + q, nq);
+      passB_rows<LG2>(slot, (int64_t)idx * ROWS, (int64_t)a.N1 * gq, gq, a.N, s_tw3, s_tw2, a.twid2 + 256, s_x,
+                                  s_red, a.alpha, a.gamma, a.partial, a.k0 + q * a.g, a.n_part);
+      fft2_signal(a.ctr + 1 + a.G + q);
     }
   }
 }

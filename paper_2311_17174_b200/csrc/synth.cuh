@@ -57,9 +57,7 @@ struct SynthArgs {
   double* outI;            // separate channels: row of walker k0+i at outI + i*pitch (used when outZ == NULL)
   double* outII;
   int64_t pitch;
-  double2* outZ;           // interleaved z = h_I + i h_II, row of walker k0+i at outZ + i*N ...
-  int z_log2n2;            // ... or, when > 0, walker-interleaved for the fused transform: sample i = N2 i1 + i2 of
-                           // walker i at ((i1 K + i) N2 + i2), N2 = 2^z_log2n2 (a multiple of the 256-sample tile)
+  double2* outZ;           // interleaved z = h_I + i h_II, row of walker k0+i at outZ + i*N
   int unit_tiles, unit_tiles_cap;   // tiles per unit of this launch; the plan's maximum (sizes the staging area)
   int64_t tiles_per_walker, units_per_walker;
   double tol;              // relative truncation of the harmonic series
@@ -758,13 +756,6 @@ __host__ __device__ inline size_t synth_smem_doubles(int n_max, int unit_tiles_c
          + (size_t)2 * 2 * unit_tiles_cap * HERM;       // staged interval cubics, double-buffered
 }
 
-// position of sample i0 of chunk-walker kl in outZ (both layouts)
-DEVINL size_t z_index(const SynthArgs& a, int kl, int64_t i0) {
-  if (a.z_log2n2 == 0) return (size_t)kl * a.N + i0;
-  const int64_t i1 = i0 >> a.z_log2n2;
-  return (((size_t)i1 * a.K + kl) << a.z_log2n2) + (size_t)(i0 & ((1 << a.z_log2n2) - 1));
-}
-
 // Consumers (warps 0..3): 2 adjacent samples per thread per tile.  Producer (warp 4): tables of the NEXT unit.
 // STAGED: S >= 256, every tile lies inside one coarse interval (the default); otherwise node rows are read per sample.
 // BES: the Bessel path of plans with n_max > 48 (its code stays out of the kernels of the other plans: instruction cache).
@@ -830,7 +821,7 @@ __global__ void __launch_bounds__(SYNTH_BLOCK, SYNTH_MINBLOCKS) synth_kernel(Syn
       if (mt.skip) {
         for (int64_t i0 = i_begin + 2 * tid; i0 < i_end; i0 += TILE) {
           if (a.outZ) {
-            const size_t zi = z_index(a, kl, i0);
+            const size_t zi = (size_t)kl * a.N + i0;
             a.outZ[zi] = make_double2(0.0, 0.0);
             a.outZ[zi + 1] = make_double2(0.0, 0.0);
           } else {
@@ -893,7 +884,7 @@ __global__ void __launch_bounds__(SYNTH_BLOCK, SYNTH_MINBLOCKS) synth_kernel(Syn
           const double hIb = fma(fb[0], S[3], fma(fb[2 * SYNTH_THREADS], S[4], fb[4 * SYNTH_THREADS] * S[5]));
           const double hIIb = fma(fb[6 * SYNTH_THREADS], S[3], fma(fb[8 * SYNTH_THREADS], S[4], fb[10 * SYNTH_THREADS] * S[5]));
           if (a.outZ) {
-            const size_t zi = z_index(a, kl, i0);
+            const size_t zi = (size_t)kl * a.N + i0;
             a.outZ[zi] = make_double2(hIa, hIIa);
             a.outZ[zi + 1] = make_double2(hIb, hIIb);
           } else {

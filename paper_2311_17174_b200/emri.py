@@ -202,14 +202,15 @@ class Plan:
         return int(c[0]), int(c[1])
 
     def set_transform(self, fused):
-        """True: last transform pass fused with Eq. 8 (default where available); False: full cuFFT + reduction kernel"""
+        """True (default where available): both transform passes and Eq. 8 in one kernel of the library; False: full cuFFT
+        transform + streaming reduction kernel"""
         self._check(self._L.emri_plan_set_transform(self._h, 1 if fused else 0))
 
     def transform_is_fused(self):
         return bool(self._L.emri_plan_transform_is_fused(self._h))
 
     def like_kernel_name(self):
-        return "fft_like_kernel" if self.transform_is_fused() else "loglike_kernel"
+        return "fft2_like_kernel" if self.transform_is_fused() else "loglike_kernel"
 
     def workspace_bytes(self):
         return int(self._L.emri_plan_workspace_bytes(self._h))

@@ -193,9 +193,9 @@ def test_hot_call_does_not_allocate(emri):
 
 @pytest.mark.parametrize("lgN,K,chunk", [(16, 5, 4), (17, 6, 6), (18, 9, 4), (19, 3, 2), (20, 5, 3), (21, 3, 2), (22, 3, 3)])
 def test_fused_transform_and_likelihood_match_the_cufft_path_and_the_oracle(emri, oracle, lgN, K, chunk):
-    """stages (c)+(d) fused (strided cuFFT pass + own last pass feeding Eq. 8) against the full cuFFT transform + streaming
-    reduction, for every row length of the last pass (256 .. 4096), ragged chunks, noisy data, a plunging walker and an
-    invalid one; and against the oracle's whole path at N = 2^16"""
+    """stages (c)+(d) fused (both transform passes and Eq. 8 in one kernel of the library) against the full cuFFT transform
+    + streaming reduction, for every split N = N1 N2 (N1 = 256 .. 1024, N2 = 256 .. 4096), ragged chunks, noisy data, a
+    plunging walker and an invalid one; and against the oracle's whole path at N = 2^16"""
     N = 1 << lgN
     cfg = W.scaled(W.CONFIGS[2], K=K, N=N, n_max=8)
     P = W.draw_params(cfg)
