@@ -302,8 +302,21 @@ def run_gpu(args, cfg):
         plan.loglike(p_d, D, logL, status)
         for k_, v in plan.timings().items():
             stage[k_] += v / args.steps
-    plan.enable_timings(False)
     paths = plan.synth_report()
+    # the plain path (full cuFFT transform + streaming reduction kernel) for comparison: a few steps, stage times only
+    fused = plan.transform_is_fused()
+    plain = None
+    if fused:
+        plan.set_transform(False)
+        plain = {"orbit": 0.0, "synth": 0.0, "fft": 0.0, "like": 0.0}
+        n_plain = min(args.steps, 3)
+        plan.loglike(p_d, D, logL, status)
+        for _ in range(n_plain):
+            plan.loglike(p_d, D, logL, status)
+            for k_, v in plan.timings().items():
+                plain[k_] += v / n_plain
+        plan.set_transform(True)
+    plan.enable_timings(False)
 
     if rank == 0:
         peaks, peaks_src = load_measured_peaks()
@@ -325,10 +338,13 @@ def run_gpu(args, cfg):
                     "flops_per_walker_sample": fpws, "flops_source": src,
                     "algorithmic_bytes_per_launch": 16.0 * min(K, CHUNK) * N,
                     "paths": paths}
-        # stages (c)+(d) read the series z[K][N] complex128 and write nothing the caller sees: 16 B per walker*sample is
-        # the algorithmic floor of each of them
-        like_gbs = (16.0 * K * N) / (stage["like"] * 1e-3) * 1e-9 if stage["like"] > 0 else None
+        # Stages (c)+(d).  Fused (fft2_like_kernel): z is read once, the intermediate of the two-pass transform is written
+        # and read once: 48 B per walker*sample through HBM, ~85 FP64 instructions per element beside it.  Plain path: the
+        # reduction kernel alone reads the spectrum once, 16 B per walker*sample.
+        bytes_ws = 48.0 if fused else 16.0
+        like_gbs = (bytes_ws * K * N) / (stage["like"] * 1e-3) * 1e-9 if stage["like"] > 0 else None
         cd_gbs = (16.0 * K * N) / ((stage["fft"] + stage["like"]) * 1e-3) * 1e-9
+        red_gbs = (16.0 * K * N) / (plain["like"] * 1e-3) * 1e-9 if plain and plain["like"] > 0 else None
         if world == 1:        # the oracle leg runs at N = 1 only (a scaling run does not repeat it on every N)
             leg = OracleLeg(cfg, args)
             cpu_t, cpu_units = leg.step()
@@ -351,8 +367,15 @@ def run_gpu(args, cfg):
             "stage_ms": stage,
             "roofline": roofline,
             "like_kernel": {"bound": "hbm", "kernel": plan.like_kernel_name(), "achieved_gbs": like_gbs,
+                            "bytes_per_walker_sample": bytes_ws,
                             "peak_gbs": peaks.get("hbm_gbs"), "frac": (like_gbs / peaks["hbm_gbs"]) if like_gbs else None,
                             "peak_source": f"MEASURED_PEAKS.json copy bandwidth ({peaks_src})"},
+            "plain_path": None if not plain else {
+                "note": "emri_plan_set_transform(0): full cuFFT transform + loglike_kernel, stage times of a few steps",
+                "stage_ms": plain,
+                "reduction_kernel": {"bound": "hbm", "kernel": "loglike_kernel", "achieved_gbs": red_gbs,
+                                     "bytes_per_walker_sample": 16.0, "peak_gbs": peaks.get("hbm_gbs"),
+                                     "frac": (red_gbs / peaks["hbm_gbs"]) if red_gbs else None}},
             "transform_and_likelihood": {"bound": "hbm", "achieved_gbs": cd_gbs, "frac": cd_gbs / peaks["hbm_gbs"],
                                          "note": "stages (c)+(d) together against one read of z (16 B per walker*sample)"},
             "cpu_baseline": cpu,

@@ -60,6 +60,7 @@ struct emri_plan {
   // multiple-shooting orbit (orbit.cuh): segment records, per-walker mode / tail start / post-plunge row
   int orbit_mode = 1, anchor_end = 0, seg_L = 0, seg_P = 0, unit_tiles_override = 0, unit_tiles_cap = 8;
   int synth_debug = 0;                       // emri_plan_set_synth_debug
+  double series_tol = 1e-16;                 // emri_plan_set_series_tolerance
   int launches = 0;                          // kernels of this library enqueued by the last hot call
   // CUDA graphs of emri_loglike (one per distinct argument set, a few kept): the 15-30 launches of a call become one
   struct GraphEntry {
@@ -341,7 +342,7 @@ int run_orbit(emri_plan* p, const double* params, int K, cudaStream_t s) {
 int run_synth(emri_plan* p, int k0, int K, double* outI, double* outII, int64_t pitch, double* outZ, cudaStream_t s) {
   SynthArgs a;
   a.wc = p->d_wc; a.nodes = p->d_nodes; a.nodeaux = p->d_nodeaux; a.jpl = p->d_jpl; a.status = p->d_status;
-  a.base = p->d_base; a.tol = 1e-16;
+  a.base = p->d_base; a.tol = p->series_tol;
   a.gtab = p->d_gtab; a.bessel = p->n_max > 48 ? 1 : 0;
   a.cbrt_thr = (p->synth_debug & 2) ? -1.0 : 4e-3;
   a.force_base = (p->synth_debug & 1) ? 1 : 0;
@@ -735,6 +736,13 @@ int emri_plan_set_transform(emri_plan* p, int fused) {
 }
 
 int emri_plan_transform_is_fused(const emri_plan* p) { return (p && p->fused_ok && p->fused_on) ? 1 : 0; }
+
+int emri_plan_set_series_tolerance(emri_plan* p, double tol) {
+  if (!p || !(tol >= 1e-17) || !(tol <= 1e-10)) return EMRI_EINVAL;
+  drop_graphs(p);
+  p->series_tol = tol;
+  return EMRI_OK;
+}
 
 int emri_plan_set_synth_debug(emri_plan* p, int flags) {
   if (!p || flags < 0 || flags > 3) return EMRI_EINVAL;

@@ -73,6 +73,14 @@ struct SynthArgs {
 constexpr int SYN_COUNTS = 16;
 enum { SYC_UNITS = 0, SYC_BASE = 9, SYC_CBRT = 10, SYC_SKIP = 11, SYC_NEVAL = 12, SYC_NFIRST = 13, SYC_M2 = 14 };
 
+// FP64 literals of the per-sample code whose low word is not zero.  As immediates ptxas builds each of them with two
+// UMOV / IMAD.MOV per use (~100 issue slots per thread and tile, measured); as entries of a __constant__ array with
+// literal indices they are constant-bank operands of the DFMA / DMUL itself.
+enum { KC_ZSCALE = 0, KC_S7, KC_S5, KC_S3, KC_C6, KC_C4, KC_A4, KC_A3, KC_A2, KC_A1, KC_A0, KC_HSQRT3, KC_SQRT3, KC_COUNT };
+__constant__ double kC[KC_COUNT] = {
+    kTwoPi / 128.0, -1.0 / 5040.0, 1.0 / 120.0, -1.0 / 6.0, -1.0 / 720.0, 1.0 / 24.0,
+    14.0 / 729.0, -7.0 / 243.0, 4.0 / 81.0, -1.0 / 9.0, 2.0 / 3.0, kHalfSqrt3, kSqrt3};
+
 constexpr int SC_TAB = 128;               // entries of the shared cos/sin table (one per 1/128 cycle)
 constexpr int SC_REP = 8;                 // replicas of every entry, one per lane & 7
 
@@ -86,10 +94,11 @@ DEVINL void sincos_cycles(const double2* __restrict__ tab_lane, double x, double
   const double t = fma(x, (double)SC_TAB, magic);
   const int k = __double2loint(t) & (SC_TAB - 1);
   const double r = fma(x, (double)SC_TAB, -(t - magic));
-  const double z = r * (kTwoPi / SC_TAB);
+  static_assert(SC_TAB == 128, "kC[KC_ZSCALE] is 2 pi / 128");
+  const double z = r * kC[KC_ZSCALE];
   const double z2 = z * z;
-  const double sz = fma(z * z2, fma(z2, fma(z2, -1.0 / 5040.0, 1.0 / 120.0), -1.0 / 6.0), z);
-  const double cz = fma(z2, fma(z2, fma(z2, -1.0 / 720.0, 1.0 / 24.0), -0.5), 1.0);
+  const double sz = fma(z * z2, fma(z2, fma(z2, kC[KC_S7], kC[KC_S5]), kC[KC_S3]), z);
+  const double cz = fma(z2, fma(z2, fma(z2, kC[KC_C6], kC[KC_C4]), -0.5), 1.0);
   const double2 e = tab_lane[k * SC_REP];
   cs = fma(e.x, cz, -e.y * sz);
   sn = fma(e.y, cz, e.x * sz);
@@ -171,7 +180,7 @@ DEVINL void sample_setup(const double* __restrict__ w, const double2* __restrict
   {
     const double d = ob.dnu * ob.inv_nuj;
     if (fabs(d) <= cbrt_thr) {
-      const double p = fma(d, fma(d, fma(d, fma(d, 14.0 / 729.0, -7.0 / 243.0), 4.0 / 81.0), -1.0 / 9.0), 2.0 / 3.0);
+      const double p = fma(d, fma(d, fma(d, fma(d, kC[KC_A4], kC[KC_A3]), kC[KC_A2]), kC[KC_A1]), kC[KC_A0]);
       A = fma(ob.Aj * d, p, ob.Aj);
     } else {
       const double cb = cbrt(w[WC_TWOPIMS] * nu);
@@ -194,25 +203,29 @@ DEVINL void sample_setup(const double* __restrict__ w, const double2* __restrict
   // detector-time quantities (BC 17-18)
   const double cphS = w[WC_CPHS], sphS = w[WC_SPHS], cS = w[WC_CS], sS = w[WC_SS];
   const double cd = fma(cpb, cphS, spb * sphS), sd = fma(spb, cphS, -cpb * sphS);
-  const double cthd = fma(-kHalfSqrt3 * sS, cd, 0.5 * cS);
-  const double Pq = fma(sS, cd, kSqrt3 * cS), Qq = 2.0 * sS * sd;
+  const double cthd = fma(-kC[KC_HSQRT3] * sS, cd, 0.5 * cS);
+  const double Pq = fma(sS, cd, kC[KC_SQRT3] * cS), Qq = 2.0 * sS * sd;
   const double den_a = fma(Pq, Pq, Qq * Qq);      // = 4 sin^2(theta_d): zero only for a source exactly on the detector normal
-  const double Npsi = fma(-cthd, Ln, fma(-kHalfSqrt3, fma(Lx, cpb, Ly * spb), 0.5 * Lz));
+  const double Npsi = fma(-cthd, Ln, fma(-kC[KC_HSQRT3], fma(Lx, cpb, Ly * spb), 0.5 * Lz));
   const double Dpsi = 0.5 * sS * fma(Ly, cphS, -Lx * sphS)
-                      - kHalfSqrt3 * (cpb * fma(Lz * sS, sphS, -cS * Ly) + spb * fma(cS, Lx, -Lz * sS * cphS));
+                      - kC[KC_HSQRT3] * (cpb * fma(Lz * sS, sphS, -cS * Ly) + spb * fma(cS, Lx, -Lz * sS * cphS));
   const double den_p0 = fma(Npsi, Npsi, Dpsi * Dpsi);
   // one division for the three normalisations.  Reading R16: an angle whose atan2 arguments both vanish is 0; its
   // denominator is replaced by 1 BEFORE the shared reciprocal so that the other two normalisations stay finite
+  // (a branch no sample of a generic walker takes, instead of a dozen selects on every sample)
   const bool ok_b = den_b0 > 0.0, ok_p = den_p0 > 0.0;
-  const double den_b = ok_b ? den_b0 : 1.0, den_p = ok_p ? den_p0 : 1.0;
+  double den_b = den_b0, den_p = den_p0;
+  if (!(ok_b && ok_p)) { den_b = ok_b ? den_b0 : 1.0; den_p = ok_p ? den_p0 : 1.0; }
   const double bp = den_b * den_p;
   const double inv = rcp_fast(bp * den_a);
   const double ib = inv * (den_a * den_p), ia = inv * bp, ip = inv * (den_a * den_b);
   double c2b = fma(Nc, Nc, -Ns * Ns) * ib, s2b = 2.0 * Ns * Nc * ib;
-  if (!ok_b) { c2b = 1.0; s2b = 0.0; }                              // beta = 0
   const double c2a = fma(Qq, Qq, -Pq * Pq) * ia, s2a = 2.0 * Pq * Qq * ia;
   double c2s = fma(Dpsi, Dpsi, -Npsi * Npsi) * ip, s2s = 2.0 * Npsi * Dpsi * ip;
-  if (!ok_p) { c2s = 1.0; s2s = 0.0; }                              // psi = 0
+  if (!(ok_b && ok_p)) {
+    if (!ok_b) { c2b = 1.0; s2b = 0.0; }                            // beta = 0
+    if (!ok_p) { c2s = 1.0; s2s = 0.0; }                            // psi = 0
+  }
   const double c2g = fma(c2gt, c2b, -s2gt * s2b), s2g = fma(s2gt, c2b, c2gt * s2b);
   const double c2pb = fma(cpb, cpb, -spb * spb), s2pb = 2.0 * cpb * spb;
   const double c2p = fma(c2pb, c2a, -s2pb * s2a), s2p = fma(s2pb, c2a, c2pb * s2a);
@@ -225,7 +238,7 @@ DEVINL void sample_setup(const double* __restrict__ w, const double2* __restrict
   // h_alpha = (sqrt3/2)(F+ A+ + Fx Ax) with A+ = A{(1+Ln^2)(c2g Sa - s2g sq Sb) + 2(1-Ln^2) Sc},
   // Ax = -2 A Ln (sq Sb c2g + Sa s2g)   (BC 7-9, 14 summed over n)  =>  h = a Sa + b Sb + c Sc
   const double sq = sqrt(fma(-e, e, 1.0));
-  const double kA = kHalfSqrt3 * A;               // A is 0 past plunge (reading R8)
+  const double kA = kC[KC_HSQRT3] * A;               // A is 0 past plunge (reading R8)
   const double Ln2 = Ln * Ln;
   const double P1 = kA * (1.0 + Ln2), P2 = 2.0 * kA * Ln, P3 = 2.0 * kA * (1.0 - Ln2);
   const double t1 = P1 * c2g, t2 = P2 * s2g, t3 = P1 * s2g, t4 = P2 * c2g;
@@ -859,8 +872,14 @@ __global__ void __launch_bounds__(SYNTH_BLOCK, SYNTH_MINBLOCKS) synth_kernel(Syn
           }
           double S[6];
           if (mt.M1 >= MLOC) {
-            if (BES) harmonic_sum_bessel(a.gtab, a.n_max, A, B, S);
-            else harmonic_sum_base(a.base, s_Mb[buf], a.n_max, A, B, S);
+            // copies: the noinline fallbacks take their arguments by reference, which must not force A and B of the
+            // common path into local memory
+            const SampleOut A2 = A, B2 = B;
+            double S2[6];
+            if (BES) harmonic_sum_bessel(a.gtab, a.n_max, A2, B2, S2);
+            else harmonic_sum_base(a.base, s_Mb[buf], a.n_max, A2, B2, S2);
+#pragma unroll
+            for (int q = 0; q < 6; ++q) S[q] = S2[q];
           } else {
             HarmState hs;
 #pragma unroll 1

@@ -18,7 +18,7 @@ _lib = None
 EXPORTS = (
     "emri_strerror", "emri_plan_create", "emri_plan_destroy", "emri_plan_set_cosmology",
     "emri_plan_set_coarse_stride", "emri_plan_set_orbit_schedule", "emri_plan_set_anchor", "emri_plan_set_integrator", "emri_plan_orbit_steps", "emri_plan_orbit_report",
-    "emri_plan_synth_report", "emri_plan_set_synth_debug", "emri_plan_set_transform", "emri_plan_transform_is_fused", "emri_plan_set_graphs", "emri_plan_graph_stats", "emri_plan_set_chunk", "emri_orbit", "emri_plan_num_nodes", "emri_waveform",
+    "emri_plan_synth_report", "emri_plan_set_synth_debug", "emri_plan_set_series_tolerance", "emri_plan_set_transform", "emri_plan_transform_is_fused", "emri_plan_set_graphs", "emri_plan_graph_stats", "emri_plan_set_chunk", "emri_orbit", "emri_plan_num_nodes", "emri_waveform",
     "emri_waveform_fft", "emri_data_fft", "emri_loglike", "emri_loglike_fdep", "emri_loglike_host", "emri_plan_enable_timings",
     "emri_plan_get_timings", "emri_plan_last_cuda_error", "emri_plan_last_launch_count", "emri_plan_workspace_bytes", "emri_stretch_step",
 )
@@ -52,6 +52,7 @@ def load():
     L.emri_plan_orbit_steps.argtypes = [vp, i32, i32, i32, vp, vp, vp, vp]
     L.emri_plan_synth_report.argtypes = [vp, vp]
     L.emri_plan_set_synth_debug.argtypes = [vp, i32]
+    L.emri_plan_set_series_tolerance.argtypes = [vp, C.c_double]
     L.emri_plan_set_transform.argtypes = [vp, i32]
     L.emri_plan_set_graphs.argtypes = [vp, i32]
     L.emri_plan_graph_stats.argtypes = [vp, vp]
@@ -200,6 +201,10 @@ class Plan:
         c = np.zeros(2, dtype=np.int64)
         self._check(self._L.emri_plan_graph_stats(self._h, c.ctypes.data_as(C.c_void_p)))
         return int(c[0]), int(c[1])
+
+    def set_series_tolerance(self, tol):
+        """relative truncation of the harmonic series of stage (b) (default 1e-16)"""
+        self._check(self._L.emri_plan_set_series_tolerance(self._h, float(tol)))
 
     def set_transform(self, fused):
         """True (default where available): both transform passes and Eq. 8 in one kernel of the library; False: full cuFFT

@@ -300,3 +300,33 @@ def test_second_noise_model_matches_oracle(emri, oracle):
     other = plan_bc.loglike(dev(P), dev(D)).cpu().numpy()
     assert np.all(np.abs(other - ref) > 1e-3 * np.abs(ref))
     plan.close(); plan_bc.close()
+
+
+def test_series_tolerance_bounds_the_truncation(emri, oracle):
+    """emri_plan_set_series_tolerance: the error of the truncated harmonic series stays below ~n_max tol of max |h|
+    (readings D8, D13), the default is below rounding, fewer orders and overtones are evaluated as tol grows, and even
+    the loosest setting accepted is inside the parity tolerance"""
+    cfg = W.scaled(W.CONFIGS[3], K=6, N=5 * 4096 + 78)
+    P = W.draw_params(cfg)
+    P[:, W.P_E0] = np.linspace(0.1, 0.5, cfg.K)
+    for k in range(cfg.K):
+        P[k, W.P_NU0] = W.nu0_for_plunge_after(P[k, W.P_M], P[k, W.P_MU], P[k, W.P_E0], 1000.0 * cfg.T_obs)
+    h_ref, st_ref = oracle.waveform_batch(P, cfg.N, cfg.dt, cfg.n_max)
+    assert not st_ref.any()
+    plan = emri.Plan(cfg.N, cfg.dt, cfg.n_max, cfg.K)
+    work, errs = [], []
+    for tol in (1e-16, 1e-13, 1e-10):
+        plan.set_series_tolerance(tol)
+        hI, hII = plan.waveform(dev(P))
+        rep = plan.synth_report()
+        e = max(h_err(hI.cpu().numpy(), h_ref[:, 0]).max(), h_err(hII.cpu().numpy(), h_ref[:, 1]).max())
+        orders = sum(int(m) * n for m, n in rep["by_order"].items())
+        print("tol", tol, "max error / max|h|", e, "harmonics", rep["harmonics_evaluated"], "order sum", orders)
+        assert e <= max(2e-12, 2.0 * cfg.n_max * tol) and e <= H_TOL
+        work.append((rep["harmonics_evaluated"], orders))
+        errs.append(e)
+    assert work[2][0] < work[0][0] and work[2][1] < work[0][1]
+    for bad in (0.0, 1e-18, 1e-9, float("nan")):
+        with pytest.raises(Exception):
+            plan.set_series_tolerance(bad)
+    plan.close()
