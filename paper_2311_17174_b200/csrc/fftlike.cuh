@@ -83,7 +83,7 @@ DEVINL int fb_pad(int a) { return a + (a >> 4); }      // one element of padding
 // LOG2L = log2 N2 in {8 .. 12}.  Y is read with ld.global.cg (it was written by other CTAs of the same launch); the last
 // stage's twiddles `tw_last` [N2] and the weights come from global memory through L1.  s_tw3: three-level table of the
 // inter-pass twiddle in shared memory, W_N^q = t0[q & 127] t1[(q >> 7) & 127] t2[q >> 14].  Ends with the exchange
-// buffer free (barrier).
+// buffer still in use by slower threads: the caller's next barrier frees it.
 template <int LOG2L>
 DEVINL void passB_rows(const double2* __restrict__ Ybuf, int64_t r0, int64_t n_rows, int K, int64_t N,
                        const double2* s_tw3, const double2* s_tw2,
@@ -159,8 +159,8 @@ DEVINL void passB_rows(const double2* __restrict__ Ybuf, int64_t r0, int64_t n_r
       acc = fma(-2.0, fma(z.x, g.x, -z.y * g.y), acc);
     }
   }
-  __syncthreads();                           // the exchange buffer is free for the next pass
   // ---- fixed-order sum over the row's T threads: shuffle tree inside a warp, then across the row's warps
+  // (no barrier of its own frees the exchange buffer or s_red: the one that releases the ticket follows)
   if (T >= 32) {
 #pragma unroll
     for (int off = 16; off > 0; off >>= 1) acc += __shfl_xor_sync(0xffffffffu, acc, off);
@@ -172,7 +172,6 @@ DEVINL void passB_rows(const double2* __restrict__ Ybuf, int64_t r0, int64_t n_r
       for (int wq = 0; wq < T / 32; ++wq) sum += s_red[row_in * (T / 32) + wq];
       partial[(size_t)(k_first + kl) * n_part + m1] = sum;
     }
-    __syncthreads();
   } else {
 #pragma unroll
     for (int off = T / 2; off > 0; off >>= 1) acc += __shfl_xor_sync(0xffffffffu, acc, off);
@@ -215,9 +214,15 @@ DEVINL void fft2_wait(const unsigned* ctr, unsigned target) {
   }
   __syncthreads();
 }
-DEVINL void fft2_signal(unsigned* ctr) {
-  __syncthreads();                                  // every thread's global stores precede ...
-  if (threadIdx.x == 0) { __threadfence(); atomicAdd(ctr, 1u); }      // ... the release of the ticket
+// end of a ticket: every thread's global stores and shared-memory reads precede the barrier; thread 0 then releases the
+// ticket (`done` may be NULL) and publishes the next one
+DEVINL void fft2_finish(unsigned* done, unsigned* s_ticket, unsigned next_tk) {
+  __syncthreads();
+  if (threadIdx.x == 0) {
+    if (done) { __threadfence(); atomicAdd(done, 1u); }
+    *s_ticket = next_tk;
+  }
+  __syncthreads();
 }
 
 // Pass A ticket: COLS adjacent columns (col0 ..) of one walker: N1-point transforms along i1 (stride N2), output row m1
@@ -268,8 +273,7 @@ DEVINL void passA_cols(const double2* __restrict__ zk, double2* __restrict__ Ysl
       Yslot[((size_t)m1 * gq + kl) * N2 + col0 + c] = q[bitrev<RL>(t)];
     }
   }
-  __syncthreads();                           // the exchange buffer is free for the next ticket
-}
+}                                            // (the barrier that releases the ticket frees the exchange buffer)
 
 template <int LG1, int LG2>
 __global__ void __launch_bounds__(FB_THREADS, 2) fft2_like_kernel(Fft2Args a) {
@@ -283,12 +287,17 @@ __global__ void __launch_bounds__(FB_THREADS, 2) fft2_like_kernel(Fft2Args a) {
   for (int q = threadIdx.x; q < 256; q += FB_THREADS) s_tw2[q] = a.twid2[q];
   for (int q = threadIdx.x; q < 512; q += FB_THREADS) s_tw3[q] = a.tw3[q];
   const unsigned total = 2u * (unsigned)a.G * a.items;
+  // thread 0 draws the NEXT ticket while the current one is being worked on (the round trip of the atomic is off the
+  // critical path); a CTA thus holds two tickets, which keeps the no-deadlock argument: the smallest unfinished ticket
+  // is running, or held by a CTA whose running ticket is smaller still
+  unsigned next_tk = 0;
+  if (threadIdx.x == 0) next_tk = atomicAdd(a.ctr, 1u);
+  if (threadIdx.x == 0) s_ticket = next_tk;
+  __syncthreads();
   for (;;) {
-    __syncthreads();
-    if (threadIdx.x == 0) s_ticket = atomicAdd(a.ctr, 1u);
-    __syncthreads();
     const unsigned tk = s_ticket;
     if (tk >= total) break;
+    if (threadIdx.x == 0) next_tk = atomicAdd(a.ctr, 1u);
     // ticket order: A(0) | A(1), B(0) alternating | A(2), B(1) alternating | ... | B(G-1)
     int kind, q;
     unsigned idx;
@@ -302,19 +311,19 @@ __global__ void __launch_bounds__(FB_THREADS, 2) fft2_like_kernel(Fft2Args a) {
     }
     const int gq = min(a.g, a.kc - q * a.g);
     const unsigned nq = (unsigned)(((int64_t)gq * a.N) / FB_ELEMS);
-    if (idx >= nq) continue;                  // ragged last group
+    if (idx >= nq) { fft2_finish(nullptr, &s_ticket, next_tk); continue; }      // ragged last group
     double2* slot = a.ring + (size_t)(q & 1) * a.g * a.N;
     if (kind == 0) {
       if (q >= 2) fft2_wait(a.ctr + 1 + a.G + (q - 2), a.items);
       const int cbs = a.N2 / COLS;
       const int kl = (int)idx / cbs, cb = (int)idx - kl * cbs;
       passA_cols<LG1>(a.z + (size_t)(q * a.g + kl) * a.N, slot, gq, kl, cb * COLS, a.N2, s_tw2, a.twid1 + 256, s_x);
-      fft2_signal(a.ctr + 1 + q);
+      fft2_finish(a.ctr + 1 + q, &s_ticket, next_tk);
     } else {
       fft2_wait(a.ctr + 1 + q, nq);
       passB_rows<LG2>(slot, (int64_t)idx * ROWS, (int64_t)a.N1 * gq, gq, a.N, s_tw3, s_tw2, a.twid2 + 256, s_x,
                                   s_red, a.alpha, a.gamma, a.partial, a.k0 + q * a.g, a.n_part);
-      fft2_signal(a.ctr + 1 + a.G + q);
+      fft2_finish(a.ctr + 1 + a.G + q, &s_ticket, next_tk);
     }
   }
 }
