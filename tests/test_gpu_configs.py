@@ -69,7 +69,9 @@ def test_full_size_loglike_on_walker_subset(emri, oracle, ci):
     got = plan.loglike(dev(P), dev(D), status=st)
     torch.cuda.synchronize()
     got, st = got.cpu().numpy(), st.cpu().numpy()
-    print(f"cfg{ci} K={cfg.K} N={cfg.N} n_max={cfg.n_max}: walkers {sub} logL ref {ref} |diff| {np.abs(got[sub] - ref)}")
+    diff = np.abs(got[sub] - ref)
+    print(f"cfg{ci} K={cfg.K} N={cfg.N} n_max={cfg.n_max}: {len(sub)} walkers, max |logL| {np.max(np.abs(ref)):.4e}, "
+          f"max |dlogL| {np.max(diff):.2e}, max |dlogL| / tolerance {np.max(diff / (1e-9 * np.abs(ref) + 1e-6)):.2e}")
     assert not st.any() and not st_ref.any()
     assert np.all(np.isfinite(got)) and logl_ok(got[sub], ref)
     if not cfg.noise_seed:
@@ -93,11 +95,14 @@ def test_full_size_waveform_sampled(emri, oracle, ci):
     hI, hII = hI.cpu().numpy(), hII.cpu().numpy()
     rng = np.random.default_rng(100 + ci)
     idx = np.unique(np.concatenate([np.arange(0, 520), np.arange(cfg.N - 520, cfg.N), rng.integers(0, cfg.N, 3000)]))
+    worst = 0.0
     for r, k in enumerate(sub):
         a, b, st = oracle.waveform(P[k], cfg.N, cfg.dt, cfg.n_max, idx=idx)
         eI = np.max(np.abs(hI[r, idx] - a)) / np.max(np.abs(hI[r]))
         eII = np.max(np.abs(hII[r, idx] - b)) / np.max(np.abs(hII[r]))
         assert st == 0 and eI <= H_TOL and eII <= H_TOL, (k, eI, eII)
+        worst = max(worst, eI, eII)
+    print(f"cfg{ci}: {len(sub)} walkers x {len(idx)} sampled outputs, max |dh| / max |h| = {worst:.2e}")
     plan.close()
 
 
