@@ -150,7 +150,7 @@ int emri_plan_set_transform(emri_plan* p, int fused);
 int emri_plan_transform_is_fused(const emri_plan* p);
 
 /* CUDA graphs.  1 (default): emri_loglike / emri_loglike_fdep (and the likelihood inside emri_stretch_step) capture their
- * whole kernel sequence -- orbit, synthesis, transform, reduction, 15 to 30 launches -- into a CUDA graph the first time an
+ * whole kernel sequence -- orbit, synthesis, transform, reduction, 13 to 30 launches -- into a CUDA graph the first time an
  * argument set (pointers, K) is seen and replay it afterwards: one launch per call, which is what the small ensembles of
  * the paper's own run shape (8 walkers) are bound by.  The plan keeps the graphs of the last 8 argument
  * sets; any emri_plan_set_* call drops them.  Not used while stage timings are enabled nor by emri_loglike_host.

@@ -62,7 +62,7 @@ struct emri_plan {
   int synth_debug = 0;                       // emri_plan_set_synth_debug
   double series_tol = 1e-16;                 // emri_plan_set_series_tolerance
   int launches = 0;                          // kernels of this library enqueued by the last hot call
-  // CUDA graphs of emri_loglike (one per distinct argument set, a few kept): the 15-30 launches of a call become one
+  // CUDA graphs of emri_loglike (one per distinct argument set, a few kept): the 13-27 launches of a call become one
   struct GraphEntry {
     const void *params, *data, *logL, *status, *fcoef;
     int K; double fstar; cudaGraphExec_t exec; int launches, n_chunks; uint64_t used;
@@ -502,8 +502,7 @@ int emri_plan_create(emri_plan** out, int64_t N, double dt, int n_max, int K_max
     if (cudaMemcpy(p->d_gtab, g.data(), g.size() * sizeof(double), cudaMemcpyHostToDevice) != cudaSuccess) return fail(EMRI_ECUDA);
   }
   p->n_part = (int)((p->Nf + LL_RANGE - 1) / LL_RANGE);
-  // fused transform + reduction: N = 2^16 .. 2^22 = N1 N2 with N1 = clamp(N / 1024, 256, 1024) (1024: the length cuFFT's
-  // strided batched kernel runs best at -- 4 TB/s against 2.8 TB/s at 2048, measured on B200) and N2 = N / N1 in 256 .. 4096
+  // fused transform + reduction (fftlike.cuh): N = 2^16 .. 2^22 = N1 N2
   std::vector<double2> twid;
   if ((N & (N - 1)) == 0 && N >= (1 << 16) && N <= (1 << 22)) {
     int lg = 0;
