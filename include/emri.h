@@ -161,8 +161,10 @@ int emri_plan_graph_stats(const emri_plan* p, int64_t out[2]);
 
 /* Truncation of the harmonic series of stage (b) (readings D8 and D13): a term of a re-summed
  * bracket series, or a whole overtone, is dropped where it stays below tol x the largest harmonic of its unit (one walker,
- * 4096 samples), so the waveform carries a relative truncation error of at most ~n_max tol.  Default 1e-16 (below
- * rounding).  1e-17 <= tol <= 1e-10; each decade buys about 3 % of the synthesis time at n_max = 30 (measured on B200). */
+ * 4096 samples), so the waveform carries a relative truncation error of at most ~n_max tol / 4.  Default 1e-14: a hundredth
+ * of the rounding noise the path has anyway (the phases are ~1e5 cycles known to 1e-16 relative: 1e-12 of max |h|, measured
+ * against the oracle), so the default is indistinguishable from 1e-16 in every parity figure.  1e-17 <= tol <= 1e-10; each
+ * decade buys about 3.5 % of the synthesis time at n_max = 30 (measured on B200). */
 int emri_plan_set_series_tolerance(emri_plan* p, double tol);
 
 /* Test hook: force the data-selected slow paths of stage (b) for every later call.  flags bit 0: every unit evaluates

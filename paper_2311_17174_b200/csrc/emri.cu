@@ -60,7 +60,7 @@ struct emri_plan {
   // multiple-shooting orbit (orbit.cuh): segment records, per-walker mode / tail start / post-plunge row
   int orbit_mode = 1, anchor_end = 0, seg_L = 0, seg_P = 0, unit_tiles_override = 0, unit_tiles_cap = 8;
   int synth_debug = 0;                       // emri_plan_set_synth_debug
-  double series_tol = 1e-16;                 // emri_plan_set_series_tolerance
+  double series_tol = 1e-14;                 // emri_plan_set_series_tolerance (reading D8)
   int launches = 0;                          // kernels of this library enqueued by the last hot call
   // CUDA graphs of emri_loglike (one per distinct argument set, a few kept): the 13-27 launches of a call become one
   struct GraphEntry {

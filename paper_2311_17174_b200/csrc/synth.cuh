@@ -15,7 +15,7 @@
 //  * Per unit (one walker, UNIT_TILES tiles of 256 samples) e^2 moves by ~1e-6, so the CTA first RE-EXPANDS the three
 //    series about the unit's mid-point w0 (Horner shift, orders 0..MLOC-1, in shared memory) and every sample then
 //    evaluates the short local series in x = w - w0.  The number of local orders kept per harmonic is the smallest that
-//    leaves a relative truncation < tol (1e-16); if order MLOC-1 is still significant the unit falls back to the
+//    leaves a relative truncation < tol (1e-14 by default, reading D8); if order MLOC-1 is still significant the unit falls back to the
 //    base series (same loop, global table).  This is a rigorous re-summation, not an interpolation of amplitudes.
 //  * Everything of a sample that does not depend on n (Hermite, geometry, antenna patterns, phases, amplitude) is
 //    folded into six numbers a_I, b_I, c_I, a_II, b_II, c_II with h_alpha = a S_a + b S_b + c S_c, parked in shared

@@ -203,7 +203,7 @@ class Plan:
         return int(c[0]), int(c[1])
 
     def set_series_tolerance(self, tol):
-        """relative truncation of the harmonic series of stage (b) (default 1e-16)"""
+        """relative truncation of the harmonic series of stage (b) (default 1e-14)"""
         self._check(self._L.emri_plan_set_series_tolerance(self._h, float(tol)))
 
     def set_transform(self, fused):

@@ -304,7 +304,7 @@ def test_second_noise_model_matches_oracle(emri, oracle):
 
 def test_series_tolerance_bounds_the_truncation(emri, oracle):
     """emri_plan_set_series_tolerance: the error of the truncated harmonic series stays below ~n_max tol of max |h|
-    (readings D8, D13), the default is below rounding, fewer orders and overtones are evaluated as tol grows, and even
+    (readings D8, D13), the default (1e-14) is indistinguishable from 1e-16 against the oracle, fewer orders and overtones are evaluated as tol grows, and even
     the loosest setting accepted is inside the parity tolerance"""
     cfg = W.scaled(W.CONFIGS[3], K=6, N=5 * 4096 + 78)
     P = W.draw_params(cfg)
@@ -314,8 +314,12 @@ def test_series_tolerance_bounds_the_truncation(emri, oracle):
     h_ref, st_ref = oracle.waveform_batch(P, cfg.N, cfg.dt, cfg.n_max)
     assert not st_ref.any()
     plan = emri.Plan(cfg.N, cfg.dt, cfg.n_max, cfg.K)
+    hI_def, hII_def = (t.clone() for t in plan.waveform(dev(P)))          # the default is 1e-14
+    plan.set_series_tolerance(1e-14)
+    hI_14, hII_14 = plan.waveform(dev(P))
+    assert torch.equal(hI_def, hI_14) and torch.equal(hII_def, hII_14)
     work, errs = [], []
-    for tol in (1e-16, 1e-13, 1e-10):
+    for tol in (1e-16, 1e-14, 1e-10):
         plan.set_series_tolerance(tol)
         hI, hII = plan.waveform(dev(P))
         rep = plan.synth_report()
@@ -325,6 +329,7 @@ def test_series_tolerance_bounds_the_truncation(emri, oracle):
         assert e <= max(2e-12, 2.0 * cfg.n_max * tol) and e <= H_TOL
         work.append((rep["harmonics_evaluated"], orders))
         errs.append(e)
+    assert errs[1] <= 1.5 * errs[0] + 1e-14           # default vs the tightest setting: the same error against the oracle
     assert work[2][0] < work[0][0] and work[2][1] < work[0][1]
     for bad in (0.0, 1e-18, 1e-9, float("nan")):
         with pytest.raises(Exception):
