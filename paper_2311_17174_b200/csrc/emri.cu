@@ -320,14 +320,14 @@ int run_orbit(emri_plan* p, const double* params, int K, cudaStream_t s) {
   sa.o = a; sa.L = p->seg_L; sa.P = p->seg_P; sa.n_steps = p->Nc + 1;
   sa.seg = p->d_seg; sa.mode = p->d_mode; sa.pclamp = p->d_pclamp; sa.plrow = p->d_plrow;
   sa.round = 0; sa.last_round = 0;
-  orbit_init_kernel<<<(K + 31) / 32, 32, 0, s>>>(sa);
+  orbit_init_kernel<<<(K + 31) / 32, 64, 0, s>>>(sa);      // two warps per 32 walkers
   DBG("orbit_init_kernel");
   p->launches += 1 + 2 * 3 + 2;
   const int n_rounds = 3;
   for (int r = 0; r < n_rounds; ++r) {
     sa.round = r; sa.last_round = (r == n_rounds - 1);
-    const int64_t threads = (int64_t)K * sa.P * (r == 0 ? 3 : 1);
-    orbit_sweep_kernel<<<(unsigned)((threads + 63) / 64), 64, 0, s>>>(sa);
+    const int64_t threads = (int64_t)K * sa.P;
+    orbit_sweep_kernel<<<dim3((unsigned)((threads + 63) / 64), r == 0 ? 3 : 1), 64, 0, s>>>(sa);
     DBG("orbit_sweep_kernel");
     orbit_correct_kernel<<<K, 32, (size_t)sa.P * 12 * sizeof(double), s>>>(sa);
     DBG("orbit_correct_kernel");

@@ -382,6 +382,25 @@ enum {
 static_assert(SG_COUNT <= SEG_STRIDE, "segment record too small");
 enum { OM_ACTIVE = 0, OM_CONVERGED = 1, OM_TAIL = 2, OM_ZERO = 3, OM_DONE = 4 };
 
+// The part of the prologue the recursion itself needs (validity of the orbital parameters and the constants of the
+// right-hand side); the rest -- z(D_L), Xi, Delta T, the geometry block -- is walker_prologue's and can run beside it.
+DEVINL bool orbit_const_only(const double* __restrict__ p, OrbitConst& oc) {
+  bool ok = true;
+#pragma unroll
+  for (int i = 0; i < EMRI_NPAR; ++i) ok = ok && isfinite(p[i]);
+  ok = ok && p[P_M] > 0.0 && p[P_MU] > 0.0 && p[P_DL] > 0.0 && p[P_E0] >= 0.0 && p[P_E0] < 1.0 &&
+       fabs(p[P_A]) <= 1.0 && p[P_NU0] > 0.0;
+  const double Ms = p[P_M] * kMsunSec, mus = p[P_MU] * kMsunSec;
+  oc.twoPiMs = kTwoPi * Ms;
+  oc.Cnu = 96.0 / (10.0 * kPi) * (mus / (Ms * Ms * Ms));
+  oc.Ce = mus / (Ms * Ms);
+  oc.a = p[P_A];
+  double sl, cl;
+  sincos(p[P_LAM], &sl, &cl);
+  oc.sp = p[P_A] * cl;
+  return ok;
+}
+
 struct ShootArgs {
   OrbitArgs o;
   int L, P;               // fine steps per segment, number of segments
@@ -446,20 +465,41 @@ DEVINL void load_orbit_const(const double* __restrict__ wc, OrbitConst& oc) {
 }
 
 // ---- 1. per walker: prologue, guard node, coarse sweep
-__global__ void __launch_bounds__(32) orbit_init_kernel(ShootArgs s) {
+__global__ void __launch_bounds__(64) orbit_init_kernel(ShootArgs s) {
+  // Two warps per 32 walkers.  Warp 1 runs the full prologue (z(D_L), Xi, Delta T, the geometry block: walker_prologue);
+  // warp 0 needs only the constants of the right-hand side for the guard step and the coarse sweep, so the two chains of
+  // dependent arithmetic run side by side instead of one after the other (59 -> 33 us at K = 8).
+  __shared__ int s_status[32];
+  __shared__ int s_ok[32];
   const OrbitArgs& a = s.o;
-  const int k = blockIdx.x * blockDim.x + threadIdx.x;
-  if (k >= a.K) return;
-  const double* p = a.params + (size_t)k * EMRI_NPAR;
-  double* wc = a.wc + (size_t)k * WC_STRIDE;
-  double* nodes = a.nodes + (size_t)k * a.Nn * NODE_STRIDE;
-  double* seg = s.seg + (size_t)k * s.P * SEG_STRIDE;
+  const int lane = threadIdx.x & 31;
+  const int k = blockIdx.x * 32 + lane;
+  const bool live = k < a.K;
+  const double* p = a.params + (size_t)(live ? k : 0) * EMRI_NPAR;
+  double* wc = a.wc + (size_t)(live ? k : 0) * WC_STRIDE;
+  if (threadIdx.x >= 32) {
+    if (live) {
+      int st = 0;
+      OrbitConst oc1;
+      const bool ok1 = walker_prologue(a, p, wc, oc1, st);
+      s_status[lane] = st;
+      s_ok[lane] = ok1 ? 1 : 0;
+    }
+    __syncthreads();
+    return;
+  }
+  double* nodes = a.nodes + (size_t)(live ? k : 0) * a.Nn * NODE_STRIDE;
+  double* seg = s.seg + (size_t)(live ? k : 0) * s.P * SEG_STRIDE;
   const double Delta = a.S * a.dt;
   int status = 0;
   OrbitConst oc;
-  const bool ok = walker_prologue(a, p, wc, oc, status);
-  double y[5] = {frac(p[P_PHI0] / kTwoPi), p[P_NU0], frac(p[P_GAM0] / kTwoPi), p[P_E0], frac(p[P_ALP0] / kTwoPi)};
-  if (a.anchor_end) y[1] = nu_lso(oc.twoPiMs, y[3]);
+  const bool ok = live && orbit_const_only(p, oc);
+  double y[5] = {0.0, 0.0, 0.0, 0.0, 0.0};
+  if (ok) {
+    y[0] = frac(p[P_PHI0] / kTwoPi); y[1] = p[P_NU0]; y[2] = frac(p[P_GAM0] / kTwoPi); y[3] = p[P_E0];
+    y[4] = frac(p[P_ALP0] / kTwoPi);
+    if (a.anchor_end) y[1] = nu_lso(oc.twoPiMs, y[3]);
+  }
   const double dir = a.anchor_end ? -1.0 : 1.0;
   int mode = OM_ACTIVE;
   int32_t jpl = (int32_t)a.Nn;
@@ -504,6 +544,10 @@ __global__ void __launch_bounds__(32) orbit_init_kernel(ShootArgs s) {
       }
     }
   }
+  __syncthreads();                            // warp 1's verdict on the remaining parameters (Xi(z) > 0) and its status bits
+  if (!live) return;
+  if (!s_ok[lane]) { mode = OM_ZERO; status = s_status[lane]; jpl = (int32_t)a.Nn; emax = 0.0; }
+  else status |= s_status[lane];
   wc[WC_EMAX] = emax;
   a.jpl[k] = jpl;
   a.status[k] = status;
@@ -514,12 +558,12 @@ __global__ void __launch_bounds__(32) orbit_init_kernel(ShootArgs s) {
 // ---- 2. one thread per (variant, walker, segment): the fine steps of the segment
 __global__ void __launch_bounds__(64) orbit_sweep_kernel(ShootArgs s) {
   const OrbitArgs& a = s.o;
-  const int64_t idx = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+  // blockIdx.y = variant (0: the scheme itself; 1, 2 in round 0: the perturbed copies for the Jacobian), so that no warp
+  // mixes the two code paths (a warp straddling variants ran them one after the other: 56 instead of 34 us at K = 8)
+  const int64_t r0 = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
   const int64_t per_v = (int64_t)a.K * s.P;
-  const int nvar = (s.round == 0) ? 3 : 1;
-  if (idx >= per_v * nvar) return;
-  const int v = (int)(idx / per_v);
-  const int64_t r0 = idx - (int64_t)v * per_v;
+  if (r0 >= per_v) return;
+  const int v = (int)blockIdx.y;
   const int k = (int)(r0 / s.P), pp = (int)(r0 - (int64_t)k * s.P);
   if (s.mode[k] != OM_ACTIVE) return;
   double* sg = s.seg + ((size_t)k * s.P + pp) * SEG_STRIDE;
