@@ -33,7 +33,7 @@ METRIC = "AK waveform+logL evaluations/sec (walkers x samples/s)"
 UNIT = "walker*samples/s"
 CHUNK = 128                 # walkers per synth / transform / loglike launch (emri_plan_set_chunk default)
 COUNTS_FILE = os.path.join(ROOT, "profiles", "counts_r2.json")
-COUNTED_SOURCES = ("paper_2311_17174_b200/csrc/synth.cuh",)
+COUNTED_SOURCES = ("paper_2311_17174_b200/csrc/synth.cuh", "paper_2311_17174_b200/csrc/emri.cu")   # kernel + its launch heuristics
 # The oracle leg covers the first N / ORACLE_DECIMATE[i] samples of the window (same dt, n_max, parameters): a bounded
 # sample of the workload sized to a few seconds of host time per step.
 ORACLE_DECIMATE = {0: 1, 1: 1, 2: 4, 3: 4, 4: 4, 5: 4}

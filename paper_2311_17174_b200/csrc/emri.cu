@@ -350,9 +350,11 @@ int run_synth(emri_plan* p, int k0, int K, double* outI, double* outII, int64_t 
   a.k0 = k0; a.K = K; a.N = p->N; a.dt = p->dt; a.S = p->S; a.logS = p->logS; a.Nn = p->Nn; a.n_max = p->n_max;
   a.outI = outI; a.outII = outII; a.pitch = pitch; a.outZ = reinterpret_cast<double2*>(outZ);
   a.tiles_per_walker = (p->N + TILE - 1) / TILE;
-  // tiles per unit: as many as leave >= 8 units per resident CTA (one series re-expansion per unit)
-  int ut = UNIT_TILES_MAX;          // 16 tiles measured best on B200 with the per-unit order selection (8: 2 % slower, 4: 8 %)
-  while (ut > 1 && (int64_t)K * ((a.tiles_per_walker + ut - 1) / ut) < (int64_t)8 * p->synth_grid) ut >>= 1;
+  // tiles per unit: 16 measured best on B200 with the per-unit order selection (8: 2-3 % slower, 4: 8 %); fewer only while
+  // there is not one unit per resident CTA (tiny calls: one re-expansion per tile makes the producer warp the bottleneck,
+  // configs[0]: 39 us at 1 tile per unit, 33 at 2 or 4)
+  int ut = UNIT_TILES_MAX;
+  while (ut > 1 && (int64_t)K * ((a.tiles_per_walker + ut - 1) / ut) < (int64_t)p->synth_grid) ut >>= 1;
   if (p->unit_tiles_override > 0) ut = p->unit_tiles_override;
   a.unit_tiles = ut;
   a.unit_tiles_cap = p->unit_tiles_cap;
