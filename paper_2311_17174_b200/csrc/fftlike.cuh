@@ -8,7 +8,7 @@
 //     Z[m1 + N1 m2] = sum_{i2} W_N^{i2 m1} W_N2^{i2 m2}  [ sum_{i1} z[N2 i1 + i2] W_N1^{i1 m1} ].
 //   pass A  the bracket: N2 strided transforms of length N1 per walker, read from the chunk z[k][N] the synthesis wrote
 //           (natural layout): a ticket is 4096/N1 adjacent columns (128-byte segments at N1 = 512); the result goes to
-//           a second buffer as Y[m1][k][i2].
+//           a second buffer as Y[k][m1][i2] (per walker N1 rows of N2: pass A's stores stay within 32 MB per ticket).
 //   pass B  one row (m1, k) of N2 contiguous elements per group of N2/16 threads: load, multiply by the twiddle
 //           W_N^{i2 m1}, N2-point transform, and the outputs Z[m1 + N1 m2] go straight from registers into Eq. 8.
 // Both passes: 16 elements per thread, radix-16 stages in registers, padded shared-memory exchanges in between
@@ -79,7 +79,8 @@ __host__ __device__ constexpr int bitrev(int q) {
 
 DEVINL int fb_pad(int a) { return a + (a >> 4); }      // one element of padding per 16: conflict-free exchanges
 
-// Pass B ticket: ROWS = FB_ELEMS / N2 consecutive rows of Y[N1][K][N2] starting at row r0 (row r = m1 K + k).
+// Pass B ticket: ROWS = FB_ELEMS / N2 consecutive rows (m1, k) of Y[K][N1][N2] in the order r = m1 K + k (the K walkers of
+// a row m1 share its weights), starting at r0.
 // LOG2L = log2 N2 in {8 .. 12}.  Y is read with ld.global.cg (it was written by other CTAs of the same launch); the last
 // stage's twiddles `tw_last` [N2] and the weights come from global memory through L1.  s_tw3: three-level table of the
 // inter-pass twiddle in shared memory, W_N^q = t0[q & 127] t1[(q >> 7) & 127] t2[q >> 14].  Ends with the exchange
@@ -102,7 +103,8 @@ DEVINL void passB_rows(const double2* __restrict__ Ybuf, int64_t r0, int64_t n_r
   double2 v[FB_EPT];
   // ---- load (each element of Y is read exactly once) and inter-pass twiddle W_N^{c m1}, c = j + t T
   {
-    const double2* src = Ybuf + (size_t)r * L + j;
+    const int N1 = (int)(n_rows / K);
+    const double2* src = Ybuf + ((size_t)kl * N1 + m1) * L + j;      // Y[k][m1][i2]
 #pragma unroll
     for (int t = 0; t < FB_EPT; ++t)
       v[t] = live ? __ldcg(src + t * T) : make_double2(0.0, 0.0);
@@ -270,7 +272,7 @@ DEVINL void passA_cols(const double2* __restrict__ zk, double2* __restrict__ Ysl
 #pragma unroll
     for (int t = 0; t < RL; ++t) {
       const int m1 = jj + t * NSL;
-      Yslot[((size_t)m1 * gq + kl) * N2 + col0 + c] = q[bitrev<RL>(t)];
+      Yslot[((size_t)kl * L + m1) * N2 + col0 + c] = q[bitrev<RL>(t)];      // Y[k][m1][i2], L = N1
     }
   }
 }                                            // (the barrier that releases the ticket frees the exchange buffer)
