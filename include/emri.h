@@ -58,7 +58,8 @@ enum {
   EMRI_EINVAL = -1, /* bad argument (NULL pointer, K > K_max, N odd or < 4, n_max out of range ...) */
   EMRI_ENOMEM = -2, /* host or device allocation failed */
   EMRI_ECUDA = -3,  /* a CUDA runtime call failed; see emri_plan_last_cuda_error */
-  EMRI_ECUFFT = -4  /* a cuFFT call failed; see emri_plan_last_cuda_error */
+  EMRI_ECUFFT = -4, /* a cuFFT call failed; see emri_plan_last_cuda_error */
+  EMRI_ELIMIT = -5  /* the problem is larger than the library's built-in scratch array (emri_spectra_loglike_static) */
 };
 
 enum { EMRI_ST_BADPARAM = 1, EMRI_ST_PLUNGE = 2, EMRI_ST_DELAY = 4, EMRI_ST_STATE = 8 };
@@ -264,6 +265,49 @@ int emri_stretch_step(emri_plan* p, double* X, double* logL, int K, const double
                       const double* lo, const double* hi, double a_stretch, uint64_t seed,
                       int64_t step, int half, int32_t* accepted, double* log_buf,
                       void* cuda_stream);
+
+/* ---- Eq. 8 without any device allocation (csrc/loglike_static.cu)
+ *
+ * For callers that cannot allocate device memory and therefore cannot own an emri_plan (a plan cudaMallocs its
+ * workspace): a process that gave the whole card to one memory pool at start-up, a client running under a fixed memory
+ * quota that may refuse the request, or a latency-critical host thread that must keep clear of cudaMalloc / cudaFree
+ * because both synchronise the entire device and stall every other stream.  Such a caller keeps the model spectra in a
+ * buffer of its own (layout of emri_waveform_fft) and gets the noise-weighted residual sum of PAPER.md:112-116 from
+ *
+ *   logL[k] = -(2 dt / N) sum_{chan I,II} sum_{m=0..N/2} |data_fft[chan][m] - spectra[k][chan][m]|^2 / psd[m]
+ *
+ * spectra: DEV [K][2][N/2+1] complex128; data_fft: DEV [2][N/2+1] complex128; psd: DEV [N/2+1] one-sided S_n(f_m), masked
+ * exactly as in emri_plan_create (an entry that is <= 0, NaN or +inf gives its bin weight 0); logL: DEV [K].  The caller
+ * owns all four and nothing else is touched except the scratch described next.  No per-walker status enters: a walker
+ * whose rows are all zero gets -(1/2)<d|d>, not -inf.  Enqueues two kernels on cuda_stream and returns without
+ * synchronising.  The call itself performs no cudaMalloc, cudaFree or other allocating call, ever.
+ *
+ * Scratch and its limit.  The per-(walker, bin range) partial sums of the two-pass reduction live in an array that is part
+ * of the library image: EMRI_STATIC_SCRATCH_DOUBLES doubles = 512 KiB, held by every GPU on which the library is loaded
+ * until the process exits.  One partial covers EMRI_STATIC_BINS_PER_PART bins, so the call needs
+ * emri_static_scratch_need(K, N) = K ceil((N/2+1)/8192) doubles (K <= 508 at N = 2^21, K <= 13107 at N = 2^16) and returns
+ * EMRI_ELIMIT, before touching the CUDA runtime, when that exceeds the array.  Split a larger ensemble into several
+ * calls on ONE stream.
+ *
+ * Sharing.  There is one array per GPU and every call on that GPU uses it from offset 0.  Calls that may overlap on the
+ * device (different streams, different host threads without ordering between their streams) race on it and give
+ * wrong logL; calls on one stream are ordered and safe.  The array keeps the previous call's partials; that is harmless
+ * because the first kernel writes every cell the second one reads, so nothing needs to start at zero.
+ *
+ * First call on a device.  With that device current, the first call looks up the array's device address
+ * (cudaGetSymbolAddress) and remembers it; this can make the runtime load the library's kernels onto the device.  Make
+ * that first call during start-up, before any stream capture you intend to do.  Later calls on the same device only
+ * launch.  The stream must belong to the current device.
+ *
+ * Errors: EMRI_EINVAL (NULL pointer, K < 1, N odd or < 4, dt <= 0, device ordinal >= 64), EMRI_ELIMIT (see above),
+ * EMRI_ECUDA (a runtime call or launch failed; emri_static_last_cuda_error() returns the raw cudaError_t of the last
+ * such failure in this process). */
+#define EMRI_STATIC_SCRATCH_DOUBLES 65536
+#define EMRI_STATIC_BINS_PER_PART 8192
+int emri_spectra_loglike_static(const double* spectra, int K, int64_t N, double dt, const double* data_fft,
+                                const double* psd, double* logL, void* cuda_stream);
+int64_t emri_static_scratch_need(int K, int64_t N); /* doubles of scratch a (K, N) call needs; -1 for invalid K, N */
+int emri_static_last_cuda_error(void);
 
 #ifdef __cplusplus
 }

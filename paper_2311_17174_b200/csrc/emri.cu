@@ -457,6 +457,7 @@ const char* emri_strerror(int code) {
     case EMRI_ENOMEM: return "out of memory";
     case EMRI_ECUDA: return "CUDA runtime error (see emri_plan_last_cuda_error)";
     case EMRI_ECUFFT: return "cuFFT error (see emri_plan_last_cuda_error)";
+    case EMRI_ELIMIT: return "problem larger than the built-in scratch array (EMRI_STATIC_SCRATCH_DOUBLES)";
     default: return "unknown error code";
   }
 }

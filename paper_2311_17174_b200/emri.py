@@ -21,6 +21,7 @@ EXPORTS = (
     "emri_plan_synth_report", "emri_plan_set_synth_debug", "emri_plan_set_series_tolerance", "emri_plan_set_transform", "emri_plan_transform_is_fused", "emri_plan_set_graphs", "emri_plan_graph_stats", "emri_plan_set_chunk", "emri_orbit", "emri_plan_num_nodes", "emri_waveform",
     "emri_waveform_fft", "emri_data_fft", "emri_loglike", "emri_loglike_fdep", "emri_loglike_host", "emri_plan_enable_timings",
     "emri_plan_get_timings", "emri_plan_last_cuda_error", "emri_plan_last_launch_count", "emri_plan_workspace_bytes", "emri_stretch_step",
+    "emri_spectra_loglike_static", "emri_static_scratch_need", "emri_static_last_cuda_error",
 )
 
 
@@ -73,8 +74,12 @@ def load():
     L.emri_plan_workspace_bytes.restype = i64
     L.emri_plan_workspace_bytes.argtypes = [vp]
     L.emri_stretch_step.argtypes = [vp, vp, vp, i32, vp, vp, vp, dbl, u64, i64, i32, vp, vp, vp]
+    L.emri_spectra_loglike_static.argtypes = [vp, i32, i64, dbl, vp, vp, vp, vp]
+    L.emri_static_scratch_need.restype = i64
+    L.emri_static_scratch_need.argtypes = [i32, i64]
+    L.emri_static_last_cuda_error.argtypes = []
     for name in EXPORTS:
-        if name not in ("emri_strerror", "emri_plan_num_nodes", "emri_plan_workspace_bytes"):
+        if name not in ("emri_strerror", "emri_plan_num_nodes", "emri_plan_workspace_bytes", "emri_static_scratch_need"):
             getattr(L, name).restype = i32
     _lib = L
     return L
@@ -97,6 +102,29 @@ def _ptr(t, dtype=None, shape=None):
     if shape is not None and tuple(t.shape) != tuple(shape):
         raise TypeError(f"expected shape {tuple(shape)}, got {tuple(t.shape)}")
     return C.c_void_p(t.data_ptr())
+
+
+STATIC_SCRATCH_DOUBLES = 65536
+
+
+def spectra_loglike_static(spectra, data_fft, psd, N, dt, logL):
+    """emri_spectra_loglike_static: Eq. 8 from spectra the caller already holds, for code that must not allocate device
+    memory (the whole card belongs to another pool, a fixed memory quota, or a host thread that cannot afford the
+    device-wide synchronisation of cudaMalloc / cudaFree).  No plan is involved and this wrapper allocates nothing either,
+    which is why `logL` is a required argument.  All tensors are contiguous CUDA tensors on the current device:
+    spectra complex128 [K][2][N/2+1], data_fft complex128 [2][N/2+1], psd float64 [N/2+1] (masked like the `psd` of Plan),
+    logL float64 [K].  Raises EmriError with the library's message when K ceil((N/2+1)/8192) > STATIC_SCRATCH_DOUBLES.
+    Calls share one built-in scratch array per GPU: keep them on one stream.  The first call on a device also looks up that
+    array's address; make it before any stream capture."""
+    import torch
+    L = load()
+    K, Nf = spectra.shape[0], int(N) // 2 + 1
+    rc = L.emri_spectra_loglike_static(_ptr(spectra, torch.complex128, (K, 2, Nf)), K, int(N), float(dt),
+                                       _ptr(data_fft, torch.complex128, (2, Nf)), _ptr(psd, torch.float64, (Nf,)),
+                                       _ptr(logL, torch.float64, (K,)), _stream())
+    if rc != 0:
+        raise EmriError(f"{L.emri_strerror(rc).decode()} (code {rc}, raw {L.emri_static_last_cuda_error()})")
+    return logL
 
 
 class Plan:
