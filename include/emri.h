@@ -111,7 +111,8 @@ int emri_plan_set_integrator(emri_plan* p, int kind, double rtol, const double* 
 /* Diagnostics of the last adaptive orbit (kind 1): the accepted steps of walker k's branch (0: forward from the anchor,
  * 1: backward).  t, h: HOST [max_out] start and signed size of each step; y: HOST [max_out][5] state at the start (angles
  * wrapped, cycles), any of them may be NULL; info: HOST int32 [2] = {steps taken, 0 / EMRI_ST_PLUNGE / EMRI_ST_STATE why
- * the branch ended early}.  Synchronises. */
+ * the branch ended early}.  Synchronises.  EMRI_EINVAL unless the adaptive integrator is selected and stage (a) has run since
+ * it was selected. */
 int emri_plan_orbit_steps(emri_plan* p, int k, int branch, int max_out, double* t, double* h, double* y, int32_t* info);
 
 /* Where the orbital state of the parameter row is given.  0 (default): at the first sample, t = 0, integrated forward.
@@ -125,7 +126,8 @@ int emri_plan_set_anchor(emri_plan* p, int at_lso);
 /* Diagnostics of the last parallel-in-time orbit evaluation: modes[k] (HOST int32 [K]) is 1 if
  * walker k's segments were all verified after a Newton round, 2 if a sequential tail was needed
  * from the first unverified boundary, 3 if its node rows are zero (invalid parameters, plunge at
- * t = 0, bad guard step).  Synchronises the device. */
+ * t = 0, bad guard step).  Synchronises the device.  EMRI_EINVAL unless the plan is on the fixed-step integrator with
+ * schedule 1 and stage (a) has run since that was last set (the modes of another configuration would be leftovers). */
 int emri_plan_orbit_report(emri_plan* p, int K, int32_t* modes);
 
 /* Diagnostics of stage (b) over the last emri_waveform / emri_waveform_fft / emri_loglike* call (all chunks):
@@ -172,6 +174,13 @@ int emri_plan_set_series_tolerance(emri_plan* p, double tol);
  * the base series in e^2; bit 1: every sample takes the cube-root amplitude.  0 restores the defaults.  Results must
  * not change beyond rounding (tests/test_gpu_paths.py). */
 int emri_plan_set_synth_debug(emri_plan* p, int flags);
+
+/* Test hook: tiles (of 256 samples) per synthesis unit, the stretch of one walker over which stage (b) re-expands the
+ * harmonic series and picks its order.  0 (default): chosen per call -- 16, fewer while a small call would otherwise leave
+ * CTAs idle.  1, 2, 4, 8 or 16 fixes it for every later call, so that a test can put a short, strongly chirping series
+ * into 16-tile units and reach the base-series fallback (tests/test_gpu_paths.py).  Results must not change beyond
+ * rounding. */
+int emri_plan_set_unit_tiles(emri_plan* p, int tiles);
 
 /* Number of walkers processed per internal chunk (bounds the workspace: chunk*N complex128 for z = h_I + i h_II
  * plus the second buffer of the fused transform and the cuFFT work area).  Default min(K_max, 128).  Reallocates,

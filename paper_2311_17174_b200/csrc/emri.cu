@@ -54,6 +54,7 @@ struct emri_plan {
   int32_t* d_status = nullptr;
   // adaptive embedded pair (orbit_dp5.cuh): emri_plan_set_integrator
   int integrator = 0, dp_cap = 0;
+  bool orbit_ran = false;                    // stage (a) has run since the last change of integrator / schedule
   double dp_rtol = 1e-12, dp_atol[5] = {1e-12, 1e-21, 1e-12, 1e-17, 1e-12};
   double* d_dpsteps = nullptr;
   int32_t* d_dpn = nullptr; int32_t* d_dpstop = nullptr; int32_t* d_dpbad = nullptr; int32_t* d_dpzero = nullptr;
@@ -89,8 +90,7 @@ struct emri_plan {
   bool fused_ok = false;
   bool fused_on = true;                // false: full cuFFT transform + loglike_kernel
   int N1 = 0, N2 = 0, log2N1 = 0, log2N2 = 0, n_cd = 0;
-  int fft2_g = 0;                      // walkers per group of fft2_like_kernel (0: the whole chunk)
-  double2* d_ring = nullptr;           // [slots][g][N] pass-A output
+  double2* d_ring = nullptr;           // [chunk][N] pass-A output
   unsigned* d_fft2ctr = nullptr;       // ticket and completion counters of fft2_like_kernel
   double2* d_twid1 = nullptr;          // stage twiddles of pass A (length N1)
   double2* d_tw3 = nullptr;            // three-level inter-pass twiddle of fft2_like_kernel
@@ -218,8 +218,6 @@ int alloc_workspace(emri_plan* p) {
 
 int get_fft(emri_plan* p, int batch, cufftHandle* out);
 cudaError_t fft2_set_smem();
-int fft2_group(const emri_plan* p) { return p->fft2_g > 0 ? std::min(p->fft2_g, p->chunk) : p->chunk; }
-
 // (Re)allocates the chunk buffer and creates, up front, every cuFFT plan the hot calls of a full ensemble need: a full
 // chunk, the ragged last chunk of K_max walkers, and the single transform of emri_data_fft.  The work area is sized by
 // the largest of them (the full chunk), so a later call with another ragged K only builds its plan object on first use
@@ -228,9 +226,8 @@ int alloc_chunk(emri_plan* p) {
   int rc;
   if ((rc = dev_alloc(p, &p->d_hbuf, (size_t)2 * p->chunk * p->N))) return rc;      // z = h_I + i h_II, [chunk][N] complex
   if (p->fused_ok) {
-    const int g = fft2_group(p), G = (p->chunk + g - 1) / g;
-    if ((rc = dev_alloc(p, &p->d_ring, (size_t)(G > 1 ? 2 : 1) * g * p->N))) return rc;
-    if ((rc = dev_alloc(p, &p->d_fft2ctr, (size_t)1 + 2 * G))) return rc;
+    if ((rc = dev_alloc(p, &p->d_ring, (size_t)p->chunk * p->N))) return rc;          // pass A -> pass B intermediate
+    if ((rc = dev_alloc(p, &p->d_fft2ctr, (size_t)2))) return rc;                       // ticket counter, pass-A tickets done
   }
   for (auto& kv : p->fft) cufftDestroy(kv.second);
   p->fft.clear();
@@ -256,7 +253,9 @@ int get_fft(emri_plan* p, int batch, cufftHandle* out) {
   if (r != CUFFT_SUCCESS) { p->last_err = (int)r; cufftDestroy(h); return EMRI_ECUFFT; }
   if (ws > p->fftwork_bytes) {
     // grow the shared work area; every cached plan is re-pointed at it.  Reached from alloc_chunk (plan creation,
-    // emri_plan_set_chunk) only: the full chunk is planned first and no smaller batch needs more
+    // emri_plan_set_chunk) only: the full chunk is planned first and no smaller batch is expected to need more.  Should
+    // cuFFT ever ask for more for a smaller batch, the captured graphs still hold the old work-area pointer: drop them
+    drop_graphs(p);
     cudaError_t e = cudaDeviceSynchronize();
     if (e != cudaSuccess) { p->last_err = (int)e; cufftDestroy(h); return EMRI_ECUDA; }
     if (p->d_fftwork) { cudaFree(p->d_fftwork); p->bytes -= (int64_t)p->fftwork_bytes; p->d_fftwork = nullptr; }
@@ -286,6 +285,7 @@ void mark(emri_plan* p, cudaStream_t s) {
 
 int run_orbit(emri_plan* p, const double* params, int K, cudaStream_t s) {
   p->launches = 0;
+  p->orbit_ran = true;     // (a graph replay re-runs what a capture enqueued here under the same settings)
   CK(cudaMemsetAsync(p->d_counts, 0, SYN_COUNTS * sizeof(unsigned long long), s));
   OrbitArgs a;
   a.params = params; a.K = K; a.N = p->N; a.dt = p->dt; a.S = p->S; a.Nc = p->Nc; a.Nn = p->Nn; a.n_max = p->n_max;
@@ -431,10 +431,10 @@ int run_fft2_like(emri_plan* p, int k0, int kc, const double* z, cudaStream_t s)
   Fft2Args a;
   a.z = reinterpret_cast<const double2*>(z); a.ring = p->d_ring; a.twid1 = p->d_twid1; a.twid2 = p->d_twid;
   a.tw3 = p->d_tw3; a.alpha = p->d_alpha; a.gamma = p->d_gamma; a.partial = p->d_partial; a.ctr = p->d_fft2ctr;
-  a.k0 = k0; a.kc = kc; a.g = fft2_group(p); a.G = (kc + a.g - 1) / a.g; a.n_part = p->N1; a.N1 = p->N1; a.N2 = p->N2;
-  a.N = p->N; a.items = (unsigned)(((int64_t)a.g * p->N) / FB_ELEMS);
-  CK(cudaMemsetAsync(p->d_fft2ctr, 0, ((size_t)1 + 2 * a.G) * sizeof(unsigned), s));
-  const int64_t total = (int64_t)2 * a.G * a.items;
+  a.k0 = k0; a.kc = kc; a.n_part = p->N1; a.N1 = p->N1; a.N2 = p->N2;
+  a.N = p->N; a.items = (unsigned)(((int64_t)kc * p->N) / FB_ELEMS);
+  CK(cudaMemsetAsync(p->d_fft2ctr, 0, (size_t)2 * sizeof(unsigned), s));
+  const int64_t total = (int64_t)2 * a.items;
   const int grid = (int)std::min<int64_t>(total, (int64_t)p->sm_count * 2);
   if (p->log2N1 == 8) fft2_launch_row<8>(p->log2N2, grid, s, a);
   else if (p->log2N1 == 9) fft2_launch_row<9>(p->log2N2, grid, s, a);
@@ -513,11 +513,9 @@ int emri_plan_create(emri_plan** out, int64_t N, double dt, int n_max, int K_max
     // split N = N1 N2 (N1 in 256 .. 1024, N2 in 256 .. 4096): N1 = 512 at one year of samples -- a pass-A ticket is then
     // 8 adjacent columns (128-byte segments) and a pass-B ticket one 4096-point row (measured best on B200)
     p->log2N1 = lg <= 19 ? 8 : (lg <= 21 ? 9 : 10);
-    if (const char* ev = std::getenv("EMRI_FFT_LOG2N1")) p->log2N1 = std::max(std::max(8, lg - 12), std::min(std::min(10, lg - 8), std::atoi(ev)));
     p->log2N2 = lg - p->log2N1;
     p->N2 = 1 << p->log2N2; p->N1 = 1 << p->log2N1;
     p->fused_ok = true;
-    if (const char* ev = std::getenv("EMRI_FFT_GROUP")) p->fft2_g = std::max(0, std::atoi(ev));      // experiments (fftlike.cuh)
     p->n_cd = (int)((p->Nf + 255) / 256);
     // stage twiddles of an L-point pass, transposed (fftlike.cuh): W_256^{k t} at [16 t + k], W_L^{jj t} at [256 + t NSL + jj]
     auto stage_twiddles = [](int log2L, std::vector<double2>& tw) {
@@ -584,7 +582,6 @@ int emri_plan_create(emri_plan** out, int64_t N, double dt, int n_max, int K_max
     return fail(EMRI_ECUDA);
 
   // persistent grid for the synthesis kernel: resident CTAs per SM x SM count
-  if (const char* ev = std::getenv("EMRI_UNIT_TILES")) p->unit_tiles_override = std::max(1, std::min(UNIT_TILES_MAX, std::atoi(ev)));
   p->unit_tiles_cap = UNIT_TILES_MAX;
   p->synth_smem = synth_smem_doubles(n_max, p->unit_tiles_cap) * sizeof(double);
   int per_sm = 0, per_sm_direct = 0;
@@ -658,6 +655,7 @@ int emri_plan_set_orbit_schedule(emri_plan* p, int schedule) {
   if (!p || (schedule != 0 && schedule != 1)) return EMRI_EINVAL;
   drop_graphs(p);
   p->orbit_mode = schedule;
+  p->orbit_ran = false;
   return EMRI_OK;
 }
 
@@ -670,6 +668,8 @@ int emri_plan_set_anchor(emri_plan* p, int at_lso) {
 
 int emri_plan_orbit_report(emri_plan* p, int K, int32_t* modes) {
   if (!p || !modes || K < 1 || K > p->K_max) return EMRI_EINVAL;
+  // d_mode is written by the parallel-in-time RK4 schedule only: refuse to hand out leftovers of another configuration
+  if (p->integrator != 0 || p->orbit_mode != 1 || !p->orbit_ran) return EMRI_EINVAL;
   CK(cudaDeviceSynchronize());
   CK(cudaMemcpy(modes, p->d_mode, (size_t)K * sizeof(int32_t), cudaMemcpyDeviceToHost));
   return EMRI_OK;
@@ -687,6 +687,7 @@ int emri_plan_synth_report(emri_plan* p, int64_t counts[16]) {
 int emri_plan_set_integrator(emri_plan* p, int kind, double rtol, const double* atol, int max_steps) {
   if (!p || (kind != 0 && kind != 1)) return EMRI_EINVAL;
   drop_graphs(p);
+  p->orbit_ran = false;
   if (kind == 0) { p->integrator = 0; return EMRI_OK; }
   if (!(rtol > 0.0) || !std::isfinite(rtol) || !atol || max_steps < 16) return EMRI_EINVAL;
   for (int q = 0; q < 5; ++q) if (!(atol[q] >= 0.0) || !std::isfinite(atol[q])) return EMRI_EINVAL;
@@ -710,7 +711,7 @@ int emri_plan_set_integrator(emri_plan* p, int kind, double rtol, const double* 
 }
 
 int emri_plan_orbit_steps(emri_plan* p, int k, int branch, int max_out, double* t, double* h, double* y, int32_t* info) {
-  if (!p || p->integrator != 1 || k < 0 || k >= p->K_max || (branch != 0 && branch != 1) || max_out < 0 || !info)
+  if (!p || p->integrator != 1 || !p->orbit_ran || k < 0 || k >= p->K_max || (branch != 0 && branch != 1) || max_out < 0 || !info)
     return EMRI_EINVAL;
   CK(cudaDeviceSynchronize());
   int32_t n[2], st[2];
@@ -727,6 +728,13 @@ int emri_plan_orbit_steps(emri_plan* p, int k, int branch, int max_out, double* 
     if (h) h[i] = rec[(size_t)i * DP_REC + 1];
     if (y) for (int q = 0; q < 5; ++q) y[5 * i + q] = rec[(size_t)i * DP_REC + 2 + q];
   }
+  return EMRI_OK;
+}
+
+int emri_plan_set_unit_tiles(emri_plan* p, int tiles) {
+  if (!p || tiles < 0 || tiles > UNIT_TILES_MAX || (tiles & (tiles - 1))) return EMRI_EINVAL;
+  drop_graphs(p);
+  p->unit_tiles_override = tiles;
   return EMRI_OK;
 }
 
@@ -759,10 +767,7 @@ int emri_plan_set_chunk(emri_plan* p, int c) {
   if (c > p->K_max) c = p->K_max;
   CK(cudaDeviceSynchronize());
   if (p->d_hbuf) p->bytes -= (int64_t)((size_t)2 * p->chunk * p->N * sizeof(double));
-  if (p->d_ring) {
-    const int g = fft2_group(p), G = (p->chunk + g - 1) / g;
-    p->bytes -= (int64_t)((size_t)(G > 1 ? 2 : 1) * g * p->N * sizeof(double2) + ((size_t)1 + 2 * G) * sizeof(unsigned));
-  }
+  if (p->d_ring) p->bytes -= (int64_t)((size_t)p->chunk * p->N * sizeof(double2) + (size_t)2 * sizeof(unsigned));
   p->chunk = c;
   return alloc_chunk(p);
 }

@@ -181,27 +181,26 @@ DEVINL void passB_rows(const double2* __restrict__ Ybuf, int64_t r0, int64_t n_r
   }
 }
 
-// ---- The kernel.  Walkers of a chunk are taken in groups of g (default: the whole chunk, one group).  Pass A of group q
-// writes slot q & 1 of the second buffer, pass B of group q reads it back and feeds Eq. 8.  One persistent kernel runs
-// everything as a dataflow: CTAs pop tickets from ONE counter in the order  A(0) | A(1) B(0) | A(2) B(1) | ... | B(G-1)
-// (`items` tickets per group and pass, 4096 elements each; inside a block the tickets of A(q+1) and B(q) alternate).
-// B(q) waits until all tickets of A(q) are done, A(q) until B(q-2) has released the slot: both point to SMALLER tickets,
-// which running CTAs hold, so the schedule cannot deadlock whatever the number of resident CTAs.  Measured on B200
-// (configs[3]): the larger the group the faster (the weights of a row m1 are shared by the g walkers of the group and
-// stay in L1/L2; keeping the intermediate of a small group inside the 126 MB L2 gained nothing because the kernel is
-// bound by instruction latency, not by HBM), hence g = chunk.
+// ---- The kernel.  Pass A of the chunk writes the second buffer, pass B reads it back and feeds Eq. 8.  One persistent
+// kernel runs both as a dataflow: CTAs pop tickets (4096 elements each) from ONE counter, first the `items` tickets of
+// pass A, then the `items` tickets of pass B.  A pass-B ticket waits until every pass-A ticket is done; those are SMALLER
+// tickets, which running CTAs hold, so the schedule cannot deadlock whatever the number of resident CTAs.
+// (Round 2 also measured splitting the chunk into groups of g walkers with a two-slot ring, A(q+1) interleaved with B(q):
+// on B200 at configs[3] the larger the group the faster -- the weights of a row m1 are shared by all walkers and stay in
+// L1/L2, and keeping the intermediate of a small group inside the 126 MB L2 gained nothing because the kernel is bound by
+// instruction latency, not by HBM -- so only the single-group schedule is kept; DESIGN.md section 6c has the numbers.)
 struct Fft2Args {
   const double2* z;        // [kc][N] chunk, natural layout
-  double2* ring;           // [slots][g][N], slots = 1 when there is a single group
+  double2* ring;           // [kc][N] intermediate Y[k][m1][i2]
   const double2* twid1;    // [256 + N1] stage twiddles of pass A (same construction as twid2)
   const double2* twid2;    // [256 + N2] of pass B
   const double2* tw3;      // [512] inter-pass twiddle in three levels: W_N^q, W_N^{128 q} (q < 128), W_N^{16384 q} (q < 256)
   const double* alpha;
   const double2* gamma;
   double* partial;
-  unsigned* ctr;           // [0] ticket counter, [1 + q] tickets of A(q) done, [1 + G + q] of B(q); zeroed before the launch
-  int k0, kc, g, G, n_part, N1, N2;
-  unsigned items;          // tickets per block = g N / 4096
+  unsigned* ctr;           // [0] ticket counter, [1] tickets of pass A done; zeroed before the launch
+  int k0, kc, n_part, N1, N2;
+  unsigned items;          // tickets per pass = kc N / 4096
   int64_t N;
 };
 
@@ -288,7 +287,7 @@ __global__ void __launch_bounds__(FB_THREADS, 2) fft2_like_kernel(Fft2Args a) {
   __shared__ unsigned s_ticket;
   for (int q = threadIdx.x; q < 256; q += FB_THREADS) s_tw2[q] = a.twid2[q];
   for (int q = threadIdx.x; q < 512; q += FB_THREADS) s_tw3[q] = a.tw3[q];
-  const unsigned total = 2u * (unsigned)a.G * a.items;
+  const unsigned total = 2u * a.items;
   // thread 0 draws the NEXT ticket while the current one is being worked on (the round trip of the atomic is off the
   // critical path); a CTA thus holds two tickets, which keeps the no-deadlock argument: the smallest unfinished ticket
   // is running, or held by a CTA whose running ticket is smaller still
@@ -300,32 +299,19 @@ __global__ void __launch_bounds__(FB_THREADS, 2) fft2_like_kernel(Fft2Args a) {
     const unsigned tk = s_ticket;
     if (tk >= total) break;
     if (threadIdx.x == 0) next_tk = atomicAdd(a.ctr, 1u);
-    // ticket order: A(0) | A(1), B(0) alternating | A(2), B(1) alternating | ... | B(G-1)
-    int kind, q;
-    unsigned idx;
-    if (tk < a.items) { kind = 0; q = 0; idx = tk; }
-    else {
-      const unsigned t2 = tk - a.items, pb = t2 / (2u * a.items);
-      if (pb < (unsigned)a.G - 1u) {
-        const unsigned r = t2 - pb * 2u * a.items;
-        kind = (int)(r & 1u); q = kind ? (int)pb : (int)pb + 1; idx = r >> 1;
-      } else { kind = 1; q = a.G - 1; idx = t2 - ((unsigned)a.G - 1u) * 2u * a.items; }
-    }
-    const int gq = min(a.g, a.kc - q * a.g);
-    const unsigned nq = (unsigned)(((int64_t)gq * a.N) / FB_ELEMS);
-    if (idx >= nq) { fft2_finish(nullptr, &s_ticket, next_tk); continue; }      // ragged last group
-    double2* slot = a.ring + (size_t)(q & 1) * a.g * a.N;
+    // ticket order: the `items` tickets of pass A, then the `items` tickets of pass B
+    const int kind = tk >= a.items ? 1 : 0;
+    const unsigned idx = tk - (kind ? a.items : 0u);
     if (kind == 0) {
-      if (q >= 2) fft2_wait(a.ctr + 1 + a.G + (q - 2), a.items);
       const int cbs = a.N2 / COLS;
       const int kl = (int)idx / cbs, cb = (int)idx - kl * cbs;
-      passA_cols<LG1>(a.z + (size_t)(q * a.g + kl) * a.N, slot, gq, kl, cb * COLS, a.N2, s_tw2, a.twid1 + 256, s_x);
-      fft2_finish(a.ctr + 1 + q, &s_ticket, next_tk);
+      passA_cols<LG1>(a.z + (size_t)kl * a.N, a.ring, a.kc, kl, cb * COLS, a.N2, s_tw2, a.twid1 + 256, s_x);
+      fft2_finish(a.ctr + 1, &s_ticket, next_tk);
     } else {
-      fft2_wait(a.ctr + 1 + q, nq);
-      passB_rows<LG2>(slot, (int64_t)idx * ROWS, (int64_t)a.N1 * gq, gq, a.N, s_tw3, s_tw2, a.twid2 + 256, s_x,
-                                  s_red, a.alpha, a.gamma, a.partial, a.k0 + q * a.g, a.n_part);
-      fft2_finish(a.ctr + 1 + a.G + q, &s_ticket, next_tk);
+      fft2_wait(a.ctr + 1, a.items);
+      passB_rows<LG2>(a.ring, (int64_t)idx * ROWS, (int64_t)a.N1 * a.kc, a.kc, a.N, s_tw3, s_tw2, a.twid2 + 256, s_x,
+                      s_red, a.alpha, a.gamma, a.partial, a.k0, a.n_part);
+      fft2_finish(nullptr, &s_ticket, next_tk);
     }
   }
 }

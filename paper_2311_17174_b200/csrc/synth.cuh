@@ -185,7 +185,11 @@ DEVINL void sample_setup(const double* __restrict__ w, const double2* __restrict
     } else {
       const double cb = cbrt(w[WC_TWOPIMS] * nu);
       A = cb * cb * ob.amp;
-      atomicAdd(counts + SYC_CBRT, 1ULL);          // rare branch (counted for emri_plan_synth_report)
+      // rare branch, counted for emri_plan_synth_report: one atomic per converged group of lanes, not one per sample
+      // (near plunge whole tiles come here, and a per-sample atomic on one address would serialise them)
+      const unsigned act = __activemask();
+      if ((threadIdx.x & 31u) == (unsigned)(__ffs((int)act) - 1))
+        atomicAdd(counts + SYC_CBRT, (unsigned long long)__popc(act));
     }
   }
   double sa, ca, s2gt, c2gt;

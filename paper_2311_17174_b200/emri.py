@@ -18,7 +18,7 @@ _lib = None
 EXPORTS = (
     "emri_strerror", "emri_plan_create", "emri_plan_destroy", "emri_plan_set_cosmology",
     "emri_plan_set_coarse_stride", "emri_plan_set_orbit_schedule", "emri_plan_set_anchor", "emri_plan_set_integrator", "emri_plan_orbit_steps", "emri_plan_orbit_report",
-    "emri_plan_synth_report", "emri_plan_set_synth_debug", "emri_plan_set_series_tolerance", "emri_plan_set_transform", "emri_plan_transform_is_fused", "emri_plan_set_graphs", "emri_plan_graph_stats", "emri_plan_set_chunk", "emri_orbit", "emri_plan_num_nodes", "emri_waveform",
+    "emri_plan_synth_report", "emri_plan_set_synth_debug", "emri_plan_set_unit_tiles", "emri_plan_set_series_tolerance", "emri_plan_set_transform", "emri_plan_transform_is_fused", "emri_plan_set_graphs", "emri_plan_graph_stats", "emri_plan_set_chunk", "emri_orbit", "emri_plan_num_nodes", "emri_waveform",
     "emri_waveform_fft", "emri_data_fft", "emri_loglike", "emri_loglike_fdep", "emri_loglike_host", "emri_plan_enable_timings",
     "emri_plan_get_timings", "emri_plan_last_cuda_error", "emri_plan_last_launch_count", "emri_plan_workspace_bytes", "emri_stretch_step",
     "emri_spectra_loglike_static", "emri_static_scratch_need", "emri_static_last_cuda_error",
@@ -53,6 +53,7 @@ def load():
     L.emri_plan_orbit_steps.argtypes = [vp, i32, i32, i32, vp, vp, vp, vp]
     L.emri_plan_synth_report.argtypes = [vp, vp]
     L.emri_plan_set_synth_debug.argtypes = [vp, i32]
+    L.emri_plan_set_unit_tiles.argtypes = [vp, i32]
     L.emri_plan_set_series_tolerance.argtypes = [vp, C.c_double]
     L.emri_plan_set_transform.argtypes = [vp, i32]
     L.emri_plan_set_graphs.argtypes = [vp, i32]
@@ -209,6 +210,10 @@ class Plan:
     def set_synth_debug(self, force_base=False, force_cbrt=False):
         """test hook: force the data-selected slow paths of stage (b)"""
         self._check(self._L.emri_plan_set_synth_debug(self._h, (1 if force_base else 0) | (2 if force_cbrt else 0)))
+
+    def set_unit_tiles(self, tiles):
+        """test hook: tiles of 256 samples per synthesis unit (0 = chosen per call)"""
+        self._check(self._L.emri_plan_set_unit_tiles(self._h, int(tiles)))
 
     def set_chunk(self, c):
         self._check(self._L.emri_plan_set_chunk(self._h, c))

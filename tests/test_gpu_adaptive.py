@@ -147,3 +147,33 @@ def test_adaptive_orbit_from_the_lso_matches_oracle(emri):
         assert s_ref == 0 and np.max(np.abs(hI[k, idx] - a)) <= 1e-9 * np.max(np.abs(hI[k]))
         assert b["n"] > 10 and b["h"][0] < 0 and b["stop"] == 0 and f["n"] >= 1         # the long branch runs backwards
     plan.close()
+
+
+def test_reports_refuse_leftovers_of_another_integrator(emri):
+    """emri_plan_orbit_report belongs to the parallel-in-time RK4 schedule and emri_plan_orbit_steps to the adaptive pair:
+    each returns EMRI_EINVAL when the plan is configured for the other, or before stage (a) has run in that configuration,
+    instead of handing out whatever an earlier call left in the buffers"""
+    cfg = W.scaled(W.CONFIGS[0], K=4, N=1 << 14)
+    P = dev(W.draw_params(cfg))
+    plan = emri.Plan(cfg.N, cfg.dt, cfg.n_max, cfg.K)
+    with pytest.raises(emri.EmriError):
+        plan.orbit_report(cfg.K)                        # nothing has run yet
+    plan.orbit(P)
+    assert set(plan.orbit_report(cfg.K).tolist()) <= {1, 2}
+    plan.set_integrator((1e-9, ATOL))
+    with pytest.raises(emri.EmriError):
+        plan.orbit_report(cfg.K)                        # modes of the RK4 call would be leftovers now
+    with pytest.raises(emri.EmriError):
+        plan.orbit_steps(0, 0)                          # the adaptive integrator has not run yet
+    plan.orbit(P)
+    assert plan.orbit_steps(0, 0)["n"] > 0
+    with pytest.raises(emri.EmriError):
+        plan.orbit_report(cfg.K)
+    plan.set_integrator(None)
+    with pytest.raises(emri.EmriError):
+        plan.orbit_steps(0, 0)
+    plan.set_orbit_schedule(0)
+    plan.orbit(P)
+    with pytest.raises(emri.EmriError):
+        plan.orbit_report(cfg.K)                        # the sequential schedule writes no modes
+    plan.close()

@@ -63,7 +63,6 @@ def test_natural_input_reaches_both_slow_paths(emri, oracle):
     """a stride of 4096 samples makes nu move by more than 4e-3 of the node value inside an interval (cube-root branch),
     and e = 0.6 chirping hard over 16-tile units makes order 8 of the local series significant (base-series fallback):
     the counters prove the paths ran, the oracle (same stride) that they are right"""
-    import os
     N, S = 1 << 15, 4096
     cfg = W.scaled(W.CONFIGS[3], K=4, N=N, n_max=30)
     P = W.draw_params(cfg)
@@ -71,11 +70,8 @@ def test_natural_input_reaches_both_slow_paths(emri, oracle):
     for k in range(cfg.K):        # two days from plunge by the closed-form estimate
         P[k, W.P_NU0] = W.nu0_for_plunge_after(P[k, W.P_M], P[k, W.P_MU], P[k, W.P_E0], 2.5 * N * cfg.dt)
     h_ref, st_ref = oracle.waveform_batch(P, N, cfg.dt, cfg.n_max, S=S)
-    os.environ["EMRI_UNIT_TILES"] = "16"
-    try:
-        plan = emri.Plan(N, cfg.dt, cfg.n_max, cfg.K)
-    finally:
-        del os.environ["EMRI_UNIT_TILES"]
+    plan = emri.Plan(N, cfg.dt, cfg.n_max, cfg.K)
+    plan.set_unit_tiles(16)
     plan.set_coarse_stride(S)
     st = torch.zeros(cfg.K, dtype=torch.int32, device="cuda")
     hI, hII = plan.waveform(dev(P), status=st)
