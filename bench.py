@@ -32,7 +32,7 @@ from paper_2311_17174_b200 import sharding, workloads as W  # noqa: E402
 METRIC = "AK waveform+logL evaluations/sec (walkers x samples/s)"
 UNIT = "walker*samples/s"
 CHUNK = 128                 # walkers per synth / transform / loglike launch (emri_plan_set_chunk default)
-COUNTS_FILE = os.path.join(ROOT, "profiles", "counts_r2.json")
+COUNTS_FILE = os.path.join(ROOT, "profiles", "counts_r3.json")
 COUNTED_SOURCES = ("paper_2311_17174_b200/csrc/synth.cuh", "paper_2311_17174_b200/csrc/emri.cu")   # kernel + its launch heuristics
 # The oracle leg covers the first N / ORACLE_DECIMATE[i] samples of the window (same dt, n_max, parameters): a bounded
 # sample of the workload sized to a few seconds of host time per step.
@@ -46,9 +46,10 @@ def git_blob_sha(path):
 
 
 def counted_work(cfg_index, n_max):
-    """Algorithmic work of synth_kernel per (walker, sample): FP64 flops EXECUTED by the kernel as built (2 dfma + dmul +
-    dadd, ncu thread-instruction counters) and its DRAM bytes per launch, from profiles/counts_r2.json.  The file records
-    the git blob hash of the kernel source it was counted on: a different source gives (None, None, 'stale')."""
+    """Algorithmic work of synth_kernel per (walker, sample): FP64 flops EXECUTED by the kernel as built, 2 dfma + dmul +
+    dadd, formed HERE from the raw ncu thread-instruction counters of one launch that profiles/counts_r3.json records
+    (the same rows are in profiles/counts_r3.md with the command), and the launch's DRAM bytes.  The file also records the
+    git blob hash of the kernel source it was counted on: a different source gives (None, None, 'stale')."""
     try:
         with open(COUNTS_FILE) as f:
             c = json.load(f)
@@ -57,11 +58,12 @@ def counted_work(cfg_index, n_max):
     for rel in COUNTED_SOURCES:
         if c.get("sources", {}).get(rel) != git_blob_sha(os.path.join(ROOT, rel)):
             return None, None, "stale"
-    entry = c.get("configs", {}).get(str(cfg_index))
-    if not entry or entry.get("n_max") != n_max:
+    e = c.get("configs", {}).get(str(cfg_index))
+    if not e or e.get("n_max") != n_max:
         return None, None, "not counted for this config"
-    return float(entry["flops_per_walker_sample"]), entry.get("dram_bytes_per_launch"), \
-        f"counted by ncu on the configs' own inputs ({os.path.relpath(COUNTS_FILE, ROOT)}, source hash verified)"
+    flops = (2.0 * e["dfma"] + e["dmul"] + e["dadd"]) / (float(e["walkers_per_launch"]) * float(e["samples"]))
+    return flops, float(e["dram_bytes_read"]) + float(e["dram_bytes_write"]), \
+        f"2 dfma + dmul + dadd of one launch, ncu counters on the configs' own inputs ({os.path.relpath(COUNTS_FILE, ROOT)}, source hash verified)"
 
 
 def load_measured_peaks():
@@ -329,10 +331,14 @@ def run_gpu(args, cfg):
         # configs[4] runs the kernel of configs[2] on a ball of walkers around one injection: counted on its own inputs
         fpws, traffic, src = counted_work(cfg.index, cfg.n_max)
         achieved = fpws * K * N / (stage["synth"] * 1e-3) * 1e-12 if fpws else None
-        roofline = {"bound": "alu", "kernel": "synth_kernel", "achieved": achieved, "peak": fp64_nominal,
-                    "unit": "TFLOP/s", "frac": (achieved / fp64_nominal) if achieved else None, "traffic": traffic,
-                    "peak_source": f"derived: {sms} SMs x 64 FP64 lanes x 2 x {sm_max:.0f} MHz (DESIGN.md section 7)",
-                    "peak_dfma_probe": fp64_probe, "frac_of_probe": (achieved / fp64_probe) if achieved else None,
+        # peak = the dependent-free DFMA probe of THIS run (probe.cu: 2 register operands reused, all SMs), the derived
+        # figure beside it (they agree to ~2 % at 1965 MHz; MEASURED_PEAKS.json has no FP64 entry)
+        roofline = {"bound": "alu", "kernel": "synth_kernel", "achieved": achieved, "peak": fp64_probe,
+                    "unit": "TFLOP/s", "frac": (achieved / fp64_probe) if achieved else None, "traffic": traffic,
+                    "peak_source": "measured in this run: DFMA probe on all SMs (paper_2311_17174_b200/csrc/probe.cu)",
+                    "peak_derived": fp64_nominal,
+                    "peak_derived_from": f"{sms} SMs x 64 FP64 lanes x 2 x {sm_max:.0f} MHz (DESIGN.md section 7)",
+                    "frac_of_derived": (achieved / fp64_nominal) if achieved else None,
                     "peak_dfma_probe_3_register_operands": fp64_probe3,
                     "launches_per_step": n_chunks, "ms_per_launch": stage["synth"] / n_chunks,
                     "flops_per_walker_sample": fpws, "flops_source": src,

@@ -147,7 +147,8 @@ int emri_plan_synth_report(emri_plan* p, int64_t counts[16]);
  * the last pass straight into Eq. 8, so the spectrum is never written back nor read again and cuFFT is not on the path
  * (DESIGN.md section 6c).  Needs a second chunk-sized buffer.  0: the full cuFFT transform followed by
  * the streaming reduction kernel (also used for every other N and by emri_loglike_fdep).  Both give logL within the parity
- * tolerance of each other (not bit-identical: the fused path evaluates Eq. 8 as <d|d> - 2<d|h> + <h|h>).
+ * tolerance of each other (not bit-identical: the fused path sums alpha_j |Z_j - ZD_j|^2 over the single elements of the
+ * packed transform, the same squared residuals in another order; both give logL = 0 at a noise-free injection).
  * emri_plan_transform_is_fused reports what the next emri_loglike will do. */
 int emri_plan_set_transform(emri_plan* p, int fused);
 int emri_plan_transform_is_fused(const emri_plan* p);

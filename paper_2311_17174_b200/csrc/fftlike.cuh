@@ -14,13 +14,17 @@
 // Both passes: 16 elements per thread, radix-16 stages in registers, padded shared-memory exchanges in between
 // (Stockham autosort), last stage radix L/256 (or 16).
 //
-// Eq. 8 without pairing.  With a = Z[m], b = conj Z[N-m] the two channels are H_I = (a+b)/2, H_II = (a-b)/(2i), and
-//     |D_I - H_I|^2 + |D_II - H_II|^2 = |D_I|^2 + |D_II|^2 - 2 Re(a P + b Q) + (|a|^2 + |b|^2)/2,
-//     P = (conj D_I - i conj D_II)/2,  Q = (conj D_I + i conj D_II)/2,
-// which is a sum over single elements of Z: logL = -(2 dt/N) [ C_D + sum_j ( alpha_j |Z_j|^2 - 2 Re(Z_j gamma_j) ) ],
-// alpha_j = w_m / 2, gamma_m = w_m P_m, gamma_{N-m} = w_m conj(Q_m) (the self-paired bins m = 0, N/2 carry both halves),
-// C_D = sum_m w_m (|D_I|^2 + |D_II|^2).  like_weights_kernel builds alpha, gamma (in pass-B order) and C_D from the
-// caller's data spectrum once per call; every partial sum has a fixed place and order (bitwise reproducible).
+// Eq. 8 without pairing, on the residual itself.  Z = DFT(h_I + i h_II) holds Z[m] = H_I[m] + i H_II[m] and
+// Z[N-m] = conj H_I[m] + i conj H_II[m].  Pack the data the same way, ZD[m] = D_I[m] + i D_II[m],
+// ZD[N-m] = conj D_I[m] + i conj D_II[m]; with R = D - H per channel, ZD[m] - Z[m] = R_I + i R_II and
+// ZD[N-m] - Z[N-m] = conj R_I + i conj R_II, whose squared moduli add up to 2 (|R_I|^2 + |R_II|^2) (the cross terms
+// cancel).  Hence a sum over single elements of Z:
+//     logL = -(2 dt/N) [ C_self + sum_j alpha_j |Z_j - ZD_j|^2 ],   alpha_m = alpha_{N-m} = w_m / 2.
+// The self-paired bins m = 0, N/2 take alpha = w_m and ZD = Re D_I + i Re D_II; what the definition adds there for data
+// whose DC / Nyquist entries are not real, w_m (Im D_I^2 + Im D_II^2), is the constant C_self (0 for the transform of a
+// real series).  No <d|d> - 2<d|h> + <h|h> cancellation: at the injection every term is a small square and logL -> 0
+// like the plain path's.  like_weights_kernel builds alpha, ZD (in pass-B order) and C_self from the caller's data
+// spectrum once per call; every partial sum has a fixed place and order (bitwise reproducible).
 #pragma once
 #include "common.cuh"
 
@@ -156,9 +160,9 @@ DEVINL void passB_rows(const double2* __restrict__ Ybuf, int64_t r0, int64_t n_r
       const double2 z = q[bitrev<RL>(t)];
       const int m2 = jj + t * NSL;
       const double alp = __ldg(al + m2);
-      const double2 g = __ldg(ga + m2);
-      acc = fma(alp, fma(z.x, z.x, z.y * z.y), acc);
-      acc = fma(-2.0, fma(z.x, g.x, -z.y * g.y), acc);
+      const double2 g = __ldg(ga + m2);                       // packed data spectrum ZD at this element
+      const double rx = z.x - g.x, ry = z.y - g.y;
+      acc = fma(alp, fma(rx, rx, ry * ry), acc);
     }
   }
   // ---- fixed-order sum over the row's T threads: shuffle tree inside a warp, then across the row's warps
@@ -316,8 +320,9 @@ __global__ void __launch_bounds__(FB_THREADS, 2) fft2_like_kernel(Fft2Args a) {
   }
 }
 
-// alpha, gamma (pass-B order: element j = m1 + N1 m2 at m1 N2 + m2) and the partial sums of C_D, from the data spectrum
-// D[2][Nf] and the weights w[Nf].  One thread per bin m = 0..N/2; block b writes cd_part[b].
+// alpha and the packed data spectrum ZD (`gamma`; pass-B order: element j = m1 + N1 m2 at m1 N2 + m2) and the partial
+// sums of C_self, from the data spectrum D[2][Nf] and the weights w[Nf].  One thread per bin m = 0..N/2; block b writes
+// cd_part[b].
 __global__ void __launch_bounds__(256) like_weights_kernel(const double2* __restrict__ D, const double* __restrict__ w,
                                                            int64_t N, int64_t Nf, int N1, int log2N1, int N2,
                                                            double* __restrict__ alpha, double2* __restrict__ gamma,
@@ -327,18 +332,15 @@ __global__ void __launch_bounds__(256) like_weights_kernel(const double2* __rest
   if (m < Nf) {
     const double wt = w[m];
     const double2 dI = D[m], dII = D[Nf + m];
-    cd = wt * (fma(dI.x, dI.x, dI.y * dI.y) + fma(dII.x, dII.x, dII.y * dII.y));
-    // P = (conj D_I - i conj D_II)/2,  conj Q = (D_I - i D_II)/2
-    const double2 P = make_double2(0.5 * (dI.x - dII.y), 0.5 * (-dI.y - dII.x));
-    const double2 cQ = make_double2(0.5 * (dI.x + dII.y), 0.5 * (dI.y - dII.x));
     const int64_t jn = (m == 0) ? 0 : N - m;
     const int64_t pa = (m & (N1 - 1)) * N2 + (m >> log2N1), pb = (jn & (N1 - 1)) * N2 + (jn >> log2N1);
-    if (jn == m) {            // m = 0 or N/2: the element pairs with itself
+    if (jn == m) {            // m = 0 or N/2: the element pairs with itself; Z is H_I + i H_II with both real
       alpha[pa] = wt;
-      gamma[pa] = make_double2(wt * (P.x + cQ.x), wt * (P.y + cQ.y));
+      gamma[pa] = make_double2(dI.x, dII.x);
+      cd = wt * fma(dI.y, dI.y, dII.y * dII.y);               // 0 for the transform of a real series
     } else {
-      alpha[pa] = 0.5 * wt; gamma[pa] = make_double2(wt * P.x, wt * P.y);
-      alpha[pb] = 0.5 * wt; gamma[pb] = make_double2(wt * cQ.x, wt * cQ.y);
+      alpha[pa] = 0.5 * wt; gamma[pa] = make_double2(dI.x - dII.y, dI.y + dII.x);      // D_I + i D_II
+      alpha[pb] = 0.5 * wt; gamma[pb] = make_double2(dI.x + dII.y, dII.x - dI.y);      // conj D_I + i conj D_II
     }
   }
   __shared__ double s[8];
@@ -354,7 +356,7 @@ __global__ void __launch_bounds__(256) like_weights_kernel(const double2* __rest
   }
 }
 
-// fixed-order final sum of the fused path: logL_k = -scale (C_D + sum_m1 partial[k][m1]); one warp per walker
+// fixed-order final sum of the fused path: logL_k = -scale (C_self + sum_m1 partial[k][m1]); one warp per walker
 __global__ void fftlike_final_kernel(const double* partial, int n_part, const double* cd_part, int n_cd, int K, double scale,
                                      const int32_t* status, double* logL, int32_t* status_out) {
   const int k = blockIdx.x * (blockDim.x >> 5) + (threadIdx.x >> 5);

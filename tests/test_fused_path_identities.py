@@ -27,14 +27,14 @@ def test_two_pass_split_of_the_dft(N1, N2):
 
 
 def test_eq8_without_pairing():
-    """-(2 dt/N) sum_m w_m (|D_I - H_I|^2 + |D_II - H_II|^2) = -(2 dt/N) [ C_D + sum_j (alpha_j |Z_j|^2 - 2 Re(Z_j gamma_j)) ]
-    with H_I = (Z[m] + conj Z[N-m])/2, H_II = (Z[m] - conj Z[N-m])/(2i), alpha = w/2, gamma_m = w P, gamma_{N-m} = w conj Q,
-    P = (conj D_I - i conj D_II)/2, Q = (conj D_I + i conj D_II)/2; the self-paired bins m = 0, N/2 carry both halves"""
+    """-(2 dt/N) sum_m w_m (|D_I - H_I|^2 + |D_II - H_II|^2) = -(2 dt/N) [ C_self + sum_j alpha_j |Z_j - ZD_j|^2 ]
+    with Z = DFT(h_I + i h_II), ZD[m] = D_I[m] + i D_II[m], ZD[N-m] = conj D_I[m] + i conj D_II[m], alpha = w/2; the
+    self-paired bins m = 0, N/2 carry alpha = w, ZD = Re D_I + i Re D_II and C_self = w (Im D_I^2 + Im D_II^2)"""
     rng = np.random.default_rng(8)
     N, dt = 64, 15.0
     Nf = N // 2 + 1
     hI, hII = rng.standard_normal(N), rng.standard_normal(N)
-    D = rng.standard_normal((2, Nf)) + 1j * rng.standard_normal((2, Nf))
+    D = rng.standard_normal((2, Nf)) + 1j * rng.standard_normal((2, Nf))       # DC / Nyquist deliberately not real
     w = rng.uniform(0.5, 2.0, Nf)
     w[3] = 0.0                                                    # a masked bin
     # the definition, bin by bin (what the plain path and the oracle evaluate)
@@ -45,18 +45,26 @@ def test_eq8_without_pairing():
     m = np.arange(Nf)
     assert np.allclose((Z[m] + np.conj(Z[(N - m) % N])) / 2, HI) and np.allclose((Z[m] - np.conj(Z[(N - m) % N])) / 2j, HII)
     alpha = np.zeros(N)
-    gamma = np.zeros(N, dtype=complex)
-    P = (np.conj(D[0]) - 1j * np.conj(D[1])) / 2
-    Q = (np.conj(D[0]) + 1j * np.conj(D[1])) / 2
+    ZD = np.zeros(N, dtype=complex)
+    c_self = 0.0
     for k in range(Nf):
         j = (N - k) % N
         if j == k:
             alpha[k] = w[k]
-            gamma[k] = w[k] * (P[k] + np.conj(Q[k]))
+            ZD[k] = D[0, k].real + 1j * D[1, k].real
+            c_self += w[k] * (D[0, k].imag ** 2 + D[1, k].imag ** 2)
         else:
             alpha[k] = alpha[j] = 0.5 * w[k]
-            gamma[k] = w[k] * P[k]
-            gamma[j] = w[k] * np.conj(Q[k])
-    CD = np.sum(w * (np.abs(D[0]) ** 2 + np.abs(D[1]) ** 2))
-    fused = -(2 * dt / N) * (CD + np.sum(alpha * np.abs(Z) ** 2 - 2 * np.real(Z * gamma)))
-    assert fused == pytest.approx(direct, rel=1e-12)
+            ZD[k] = D[0, k] + 1j * D[1, k]
+            ZD[j] = np.conj(D[0, k]) + 1j * np.conj(D[1, k])
+    fused = -(2 * dt / N) * (c_self + np.sum(alpha * np.abs(Z - ZD) ** 2))
+    assert fused == pytest.approx(direct, rel=1e-13)
+    # and no cancellation: data = the model itself gives exactly 0
+    D0 = np.stack([HI, HII])
+    ZD0 = np.zeros(N, dtype=complex)
+    for k in range(Nf):
+        j = (N - k) % N
+        ZD0[k] = D0[0, k] + 1j * D0[1, k] if j != k else D0[0, k].real + 1j * D0[1, k].real
+        if j != k:
+            ZD0[j] = np.conj(D0[0, k]) + 1j * np.conj(D0[1, k])
+    assert np.sum(alpha * np.abs(Z - ZD0) ** 2) <= 1e-24 * np.sum(alpha * np.abs(Z) ** 2)

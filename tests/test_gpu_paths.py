@@ -220,10 +220,39 @@ def test_fused_transform_and_likelihood_match_the_cufft_path_and_the_oracle(emri
     plan.set_transform(True)
     D0 = plan.waveform_fft(dev(P[:1]))[0].clone()
     z = plan.loglike(dev(P), D0).cpu().numpy()
-    assert abs(z[0]) <= 1e-6
+    hh = 2.0 * np.max(np.abs(z[np.isfinite(z)]))                  # the scale of <h|h>
+    assert z[0] <= 0.0 and abs(z[0]) <= 1e-12 * hh                # a sum of squared residuals: no cancellation (D16)
     if lgN == 16:
         ref, _ = oracle.loglike_batch(P, N, cfg.dt, cfg.n_max, D.cpu().numpy(), psd)
         assert np.all(np.abs(fused[ok] - ref[ok]) <= 1e-9 * np.abs(ref[ok]) + 1e-6)
+    plan.close()
+
+
+@pytest.mark.parametrize("lgN", [16, 20])
+def test_loud_noise_free_injection_on_the_fused_path(emri, oracle, lgN):
+    """the mock data are the noise-less fiducial waveform, so the residual vanishes at the injection.
+    A loud source (D_L = 0.01 Gpc: <h|h> ~ 1e7 and more) is where a likelihood assembled from <d|d> - 2<d|h> + <h|h>
+    would lose the north-star tolerance 1e-9 |logL_ref| + 1e-6 at walker 0 (logL_ref = 0); the fused path sums squared
+    residuals (reading D16) and must hold it, for the injection and for the walkers away from it, against the oracle"""
+    N = 1 << lgN
+    cfg = W.scaled(W.CONFIGS[1], K=4, N=N, n_max=10 if lgN == 16 else 6)
+    P = W.draw_params(cfg)
+    P[:, W.P_DL] = 0.01
+    psd = W.lisa_psd_barack_cutler(N, cfg.dt)
+    h_ref, st_ref = oracle.waveform_batch(P[:1], N, cfg.dt, cfg.n_max)
+    assert not st_ref.any()
+    D = np.stack([oracle.rfft(h_ref[0, 0]), oracle.rfft(h_ref[0, 1])])
+    ref, _ = oracle.loglike_batch(P, N, cfg.dt, cfg.n_max, D, psd)
+    plan = emri.Plan(N, cfg.dt, cfg.n_max, cfg.K, psd)
+    assert plan.transform_is_fused()
+    got = plan.loglike(dev(P), dev(D)).cpu().numpy()
+    plan.set_transform(False)
+    plain = plan.loglike(dev(P), dev(D)).cpu().numpy()
+    print("N", N, "fused", got, "plain", plain, "oracle", ref)
+    assert ref[0] == 0.0 and np.min(np.abs(ref[1:])) > 1e6        # loud indeed
+    for a in (got, plain):
+        assert a[0] <= 0.0 and abs(a[0]) <= 1e-6
+        assert np.all(np.abs(a - ref) <= 1e-9 * np.abs(ref) + 1e-6)
     plan.close()
 
 
