@@ -16,6 +16,11 @@ LIB = os.path.join(HERE, "libemri_oracle.so")
 LIB_LD = os.path.join(HERE, "libemri_oracle_ld.so")
 # -ffp-contract=off: no FMA contraction, so the arithmetic is what the source says
 FLAGS = ["-O2", "-ffp-contract=off", "-fopenmp", "-shared", "-fPIC", "-std=c++17"]
+# EMRI_ORACLE_SANITIZE=1: AddressSanitizer + UndefinedBehaviorSanitizer build; load it with
+#   LD_PRELOAD=$(gcc -print-file-name=libasan.so) ASAN_OPTIONS=detect_leaks=0 python -m pytest tests/test_oracle_pins.py
+# and rebuild with --force afterwards (profiles/sanitizers_r3.md records the run)
+if os.environ.get("EMRI_ORACLE_SANITIZE"):
+    FLAGS += ["-g", "-fno-omit-frame-pointer", "-fsanitize=address,undefined", "-fno-sanitize-recover=undefined"]
 
 
 def _stale(lib):

@@ -330,6 +330,7 @@ struct Dp5Step {
   real turns[3];      // whole cycles removed from the three angles so far (enters the error scale only)
   real Q[5][4];       // dense output: y(t + theta h) = y + sum_j Q[q][j] theta^{j+1}  (already multiplied by h)
   real D[5];          // the step's own increment h sum_i b_i K_i (unwrapped); Q(1) equals it up to the rounding of P
+  real err;           // the controller's error norm of this step (also evaluated, but not acted on, for a forced step)
 };
 struct Dp5Branch {
   std::vector<Dp5Step> steps;
@@ -391,7 +392,7 @@ Dp5Branch dp5_integrate(const Walker& w, const real y0[5], real t0, real t_bound
     const real min_step = 10 * std::fabs(std::nextafter(t, dir * std::numeric_limits<real>::infinity()) - t);
     if (h_abs < min_step) h_abs = min_step;
     bool rejected = false;
-    real K[7][5], y_new[5], h = 0, t_new = t;
+    real K[7][5], y_new[5], h = 0, t_new = t, err_acc = 0;
     for (;;) {
       if (h_abs < min_step && !forced) { br.stop = ST_STATE; br.t_end = t; return br; }
       h = h_abs * dir;
@@ -426,6 +427,7 @@ Dp5Branch dp5_integrate(const Walker& w, const real y0[5], real t0, real t_bound
         en[q] = e * h / sc;
       }
       const real err = rms5(en);
+      err_acc = err;
       if (forced) break;
       if (err < 1) {
         real factor = (err == 0) ? (real)10 : std::min((real)10, (real)0.9 * std::pow(err, expo));
@@ -438,7 +440,7 @@ Dp5Branch dp5_integrate(const Walker& w, const real y0[5], real t0, real t_bound
     }
     // record the accepted step with its dense output
     Dp5Step st;
-    st.t = t; st.h = h;
+    st.t = t; st.h = h; st.err = err_acc;
     for (int q = 0; q < 5; ++q) st.y[q] = y[q];
     for (int a = 0; a < 3; ++a) st.turns[a] = turns[a];
     for (int q = 0; q < 5; ++q)
@@ -957,6 +959,26 @@ int64_t emri_o_dp5_steps(const double* params, double t_end, double rtol, const 
   }
   if (info) { info[0] = br.stop; info[1] = (double)br.t_end; }
   return n;
+}
+
+// S3', validity half of the teacher-forced protocol (D14): the controller's error norm, as THIS implementation
+// evaluates it, of every step of a prescribed sequence h[0..n) taken from the parameter row's state at t = 0 (steps of
+// either sign, all of one sign).  A step another implementation accepted must have norm < 1 here, and where the norm is
+// above rounding the next step it chose must be h min(10, 0.9 norm^{-1/5}) (or smaller, after a rejection).
+// Returns the number of norms written.
+int64_t emri_o_dp5_forced_errors(const double* params, double rtol, const double* atol, int pn_mask, double H0, double Om,
+                                 const double* h, int64_t n, double* err) {
+  Cosmo c{(real)H0, (real)Om};
+  Walker w = make_walker(params, c);
+  real at[5];
+  for (int q = 0; q < 5; ++q) at[q] = (real)atol[q];
+  real t_end = 0;
+  for (int64_t i = 0; i < n; ++i) t_end += (real)h[i];
+  if (n < 1 || t_end == 0) return 0;
+  Dp5Branch br = dp5_integrate(w, w.p0, 0, t_end, (real)rtol, at, pn_mask, false, h, n);
+  const int64_t m = (int64_t)br.steps.size();
+  for (int64_t i = 0; i < m; ++i) err[i] = (double)br.steps[i].err;
+  return m;
 }
 
 // Hermite basis check: interpolate a caller-supplied single interval

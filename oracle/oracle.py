@@ -86,6 +86,18 @@ class Oracle:
                                                                   [float(ff.size), float(fb.size)], ff, fb]), dtype=np.float64)
             self._adp = self._adaptive.ctypes.data_as(_dp)
 
+    def dp5_forced_errors(self, params, rtol, atol, h, pn_mask=3, H0=H0_DEFAULT, Om=OM_DEFAULT):
+        """the controller's error norm (this implementation's) of each step of the prescribed sequence h taken from the
+        row's state at t = 0 -- the validity half of the teacher-forced protocol (D14)"""
+        p = _f64(params)
+        at = np.ascontiguousarray(np.broadcast_to(atol, (5,)), dtype=np.float64)
+        h = np.ascontiguousarray(h, dtype=np.float64)
+        err = np.zeros(len(h))
+        self.lib.emri_o_dp5_forced_errors.restype = C.c_int64
+        self.lib.emri_o_dp5_forced_errors.argtypes = [_dp, C.c_double, _dp, C.c_int, C.c_double, C.c_double, _dp, C.c_int64, _dp]
+        n = self.lib.emri_o_dp5_forced_errors(_d(p), float(rtol), _d(at), pn_mask, H0, Om, _d(h), len(h), _d(err))
+        return err[:n]
+
     def dp5_steps(self, params, t_end, rtol, atol, pn_mask=3, stop_at_plunge=False, max_steps=200000,
                   H0=H0_DEFAULT, Om=OM_DEFAULT):
         """accepted steps of the adaptive integration from t = 0 to t_end -> dict(t, h, y[n][5], turns[n][3], Q[n][5][4], stop, t_reached)"""

@@ -1040,6 +1040,45 @@ def test_adaptive_pair_takes_scipy_rk45_steps_and_dense_output(oracle, T, rtol):
                 assert np.max(np.abs(Y[:, q] - S[:, q])) <= 100 * rtol * max(1.0, np.max(np.abs(S[:, q])))
 
 
+def test_forced_error_norms_are_scipys_and_the_free_run_obeys_the_controller(oracle):
+    """dp5_forced_errors (the validity half of the teacher-forced protocol, D14) returns, for a prescribed step
+    sequence, the norm the controller would have judged each step by.  Pins: (1) SciPy's own RK45 machinery (`rk_step` and
+    the rms of K^T E h / scale, the code path of solve_ivp) gives the same number for arbitrary -- not controller-chosen --
+    step sizes, good steps and bad ones alike; (2) the oracle's free run satisfies its own rule exactly: every accepted
+    norm is below 1 and the next step is h min(10, 0.9 norm^-1/5)."""
+    from scipy.integrate._ivp.rk import RK45, rk_step
+    P = W.draw_params(W.CONFIGS[1], K=2)
+    for k in range(2):
+        p = P[k]
+        fun = lambda t, y: oracle.rhs(p, y)                                     # noqa: E731
+        for rtol, sign in ((1e-8, 1.0), (1e-11, -1.0)):
+            atol = DP_ATOL * (rtol / 1e-9)
+            # arbitrary multiples of the largest step the controller itself takes, so that the norms straddle 1
+            h_star = np.max(np.abs(oracle.dp5_steps(p, sign * 2 ** 20 * 15.0, rtol, atol)["h"][:-1]))
+            hs = [sign * c * h_star for c in (0.3, 1.5, 0.6, 1.0)]
+            got = oracle.dp5_forced_errors(p, rtol, atol, hs)
+            t, y = 0.0, _cycles_state(p)
+            f = fun(t, y)
+            want = []
+            Kbuf = np.empty((7, 5))
+            for h in hs:
+                y_new, f_new = rk_step(fun, t, y, f, h, RK45.A, RK45.B, RK45.C, Kbuf)
+                scale = atol + np.maximum(np.abs(y), np.abs(y_new)) * rtol
+                want.append(np.linalg.norm(np.dot(Kbuf.T, RK45.E) * h / scale) / 5 ** 0.5)
+                t, y, f = t + h, y_new, f_new
+            assert len(got) == len(hs)
+            np.testing.assert_allclose(got, want, rtol=1e-6, atol=1e-8)         # (SciPy's state is unwrapped: rounding noise)
+            assert max(want) > 1.0 > min(want)                                  # both verdicts occur in the sample
+        for rtol in (1e-8, 1e-11):
+            atol = DP_ATOL * (rtol / 1e-9)
+            r = oracle.dp5_steps(p, 2 ** 18 * 15.0, rtol, atol)
+            err = oracle.dp5_forced_errors(p, rtol, atol, r["h"])
+            assert len(err) == len(r["h"]) and np.all(err < 1.0)
+            # (a step after a rejection is smaller than the rule allows, and the last one is cut to the bound)
+            ratio, fac = r["h"][1:-1] / r["h"][:-2], np.minimum(10.0, 0.9 * err[:-2] ** -0.2)
+            assert np.all(ratio <= fac * (1 + 1e-12)) and np.mean(np.abs(ratio / fac - 1) < 1e-12) > 0.9
+
+
 def test_adaptive_orbit_nodes_are_consistent_and_converge_to_the_rk4_orbit(oracle):
     """the node table sampled from the dense output: increments and values agree, slopes are the right-hand side at the
     node, and with a tight tolerance it is the same orbit as the fixed-step scheme (both converge to the ODE solution)"""
